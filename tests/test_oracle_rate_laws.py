@@ -1,0 +1,158 @@
+"""P10: each rate law reduces to a textbook special case (CPU only)."""
+import math
+
+import numpy as np
+import pytest
+
+import mechgen as mg
+from mechgen import MechBuilder
+from oracle import Oracle
+
+R = 8314.46261815324
+PATM = 101325.0
+CP = lambda a0, a5, a6: [a0, 0, 0, 0, 0, a5, a6]
+
+
+def _three(**rx):
+    """A <=> B + C style test bed: species A, B, C, bath N (last)."""
+    mb = MechBuilder()
+    mb.add_species(30.0, CP(4.0, 1000.0, 5.0)); mb.add_species(10.0, CP(3.0, 9000.0, 4.0))
+    mb.add_species(20.0, CP(3.5, 4000.0, 6.0)); mb.add_species(28.0, CP(3.5, -1000.0, 6.5))
+    mb.add_reaction({0: 1}, {1: 1, 2: 1}, **rx)
+    return mb.build()
+
+
+def _state(T=1300.0, P=3 * PATM, V=0.05, X=(0.3, 0.2, 0.1, 0.4)):
+    n = np.array(X) * P * V / (R * T)
+    return np.concatenate([[T, V], n[:3]]), P
+
+
+def _run(m, **kw):
+    o = Oracle(m)
+    phi, P = _state(**kw)
+    return o, o.intermediates(mg.CONP, phi, P), o.source(mg.CONP, phi, [P])[0], o.jacobian_dense(mg.CONP, phi, [P])[0]
+
+
+ARR = dict(A=4e13, beta=0.3, Ta=22000.0)
+LOW = (6e15, -1.0, 20000.0)
+
+
+def test_constant_cp_gibbs_closed_form():
+    _, it, _, _ = _run(_three(**ARR))
+    T = 1300.0
+    for k, (a0, a5, a6) in enumerate([(4.0, 1000.0, 5.0), (3.0, 9000.0, 4.0), (3.5, 4000.0, 6.0), (3.5, -1000.0, 6.5)]):
+        assert it["g"][k] == pytest.approx(a0 * (1 - math.log(T)) + a5 / T - a6, rel=1e-14)
+        assert it["h"][k] == pytest.approx(R * (a0 * T + a5), rel=1e-14)
+        assert it["cp"][k] == pytest.approx(R * a0, rel=1e-15)
+
+
+def test_nasa_full_polynomial_against_numpy():
+    m = mg.config_mechanism(1)
+    o = Oracle(m)
+    for T in (650.0, 1000.0, 1000.0001, 2400.0):
+        phi = np.concatenate([[T, 1.0], np.full(12, 1e-4)])
+        it = o.intermediates(mg.CONP, phi, 1e5)
+        for k in range(13):
+            a = m["nasa_lo"][7 * k:7 * k + 7] if T <= 1000.0 else m["nasa_hi"][7 * k:7 * k + 7]
+            cp = np.polyval(a[4::-1], T)
+            hint = np.polyval(np.concatenate([(a[:5] / np.arange(1, 6))[::-1], [a[5]]]), T) / T
+            assert it["cp"][k] == pytest.approx(R * cp, rel=1e-13)
+            assert it["h"][k] == pytest.approx(R * T * hint, rel=1e-12)
+    # continuity at T_mid (generator property) seen through the oracle
+    lo = o.intermediates(mg.CONP, np.concatenate([[1000.0, 1.0], np.full(12, 1e-4)]), 1e5)
+    hi = o.intermediates(mg.CONP, np.concatenate([[1000.0 + 1e-9, 1.0], np.full(12, 1e-4)]), 1e5)
+    np.testing.assert_allclose(lo["g"], hi["g"], rtol=1e-9)
+
+
+def test_equilibrium_constant_sum_nu_term():
+    _, it, _, _ = _run(_three(**ARR))
+    T = 1300.0
+    dg = it["g"][1] + it["g"][2] - it["g"][0]
+    assert it["Kc"][0] == pytest.approx(math.exp(-dg) * (PATM / (R * T)) ** 1, rel=1e-13)
+    assert it["kr"][0] == pytest.approx(it["kf"][0] / it["Kc"][0], rel=1e-15)
+
+
+def test_troe_reduces_to_lindemann():
+    lind = _run(_three(type=mg.FALLOFF_LINDEMANN, low=LOW, **ARR))
+    troe = _run(_three(type=mg.FALLOFF_TROE, low=LOW, troe=(1.0, 123.0, 1e300, None), **ARR))
+    assert troe[1]["F"][0] == pytest.approx(1.0, abs=1e-15)
+    np.testing.assert_allclose(troe[2], lind[2], rtol=1e-14)
+    np.testing.assert_allclose(troe[3], lind[3], rtol=1e-12, atol=1e-300)
+
+
+def test_sri_reduces_to_lindemann():
+    lind = _run(_three(type=mg.FALLOFF_LINDEMANN, low=LOW, **ARR))
+    sri = _run(_three(type=mg.FALLOFF_SRI, low=LOW, sri=(0.0, 500.0, 1e300, 1.0, 0.0), **ARR))
+    assert sri[1]["F"][0] == pytest.approx(1.0, abs=1e-15)
+    np.testing.assert_allclose(sri[2], lind[2], rtol=1e-14)
+    np.testing.assert_allclose(sri[3], lind[3], rtol=1e-12, atol=1e-300)
+
+
+def test_falloff_limits():
+    elem = _run(_three(**ARR))
+    hi = _run(_three(type=mg.FALLOFF_LINDEMANN, low=(6e45, -1.0, 20000.0), **ARR))       # Pr -> inf: k -> k_inf
+    np.testing.assert_allclose(hi[2], elem[2], rtol=1e-12)
+    lo = _run(_three(type=mg.FALLOFF_LINDEMANN, low=(6e-15, -1.0, 20000.0), **ARR))      # Pr -> 0: c k_inf -> k0 [M]
+    T = 1300.0
+    k0 = 6e-15 * T ** -1.0 * math.exp(-20000.0 / T)
+    Ctot = 3 * PATM / (R * T)
+    assert lo[1]["c"][0] * lo[1]["kf"][0] == pytest.approx(k0 * Ctot, rel=1e-12)
+
+
+def test_third_body_all_default_efficiencies_is_total_concentration():
+    _, it, _, _ = _run(_three(type=mg.THIRD_BODY, **ARR))
+    assert it["M"][0] == pytest.approx(3 * PATM / (R * 1300.0), rel=1e-14)
+    _, it2, _, _ = _run(_three(type=mg.THIRD_BODY, eff={1: 2.5, 3: 0.0}, **ARR))
+    C = it2["C"]
+    assert it2["M"][0] == pytest.approx(C[0] + 2.5 * C[1] + C[2], rel=1e-14)
+
+
+def test_plog_identical_points_is_arrhenius_and_node_values():
+    elem = _run(_three(**ARR))
+    pts = [(p * PATM, ARR["A"], ARR["beta"], ARR["Ta"]) for p in (0.1, 1.0, 10.0)]
+    pl = _run(_three(type=mg.PLOG, plog=pts))
+    np.testing.assert_allclose(pl[2], elem[2], rtol=1e-13)
+    np.testing.assert_allclose(pl[3], elem[3], rtol=1e-11, atol=1e-300)
+    # on a node and outside the table the value is that node's Arrhenius (reading S4)
+    pts = [(1.0 * PATM, 1e10, 0.0, 5000.0), (10.0 * PATM, 1e12, 0.5, 8000.0)]
+    m = _three(type=mg.PLOG, plog=pts)
+    for P, (A, b, Ta) in ((1.0 * PATM, (1e10, 0.0, 5000.0)), (0.2 * PATM, (1e10, 0.0, 5000.0)),
+                         (10.0 * PATM, (1e12, 0.5, 8000.0)), (80.0 * PATM, (1e12, 0.5, 8000.0))):
+        _, it, _, _ = _run(m, P=P)
+        assert it["kf"][0] == pytest.approx(A * 1300.0 ** b * math.exp(-Ta / 1300.0), rel=1e-13)
+    # geometric mean of pressures -> geometric mean of rates
+    _, it, _, _ = _run(m, P=math.sqrt(10.0) * PATM)
+    k1 = 1e10 * math.exp(-5000.0 / 1300.0); k2 = 1e12 * 1300.0 ** 0.5 * math.exp(-8000.0 / 1300.0)
+    assert it["kf"][0] == pytest.approx(math.sqrt(k1 * k2), rel=1e-12)
+
+
+def test_chebyshev_special_cases():
+    lim = dict(Tmin=300.0, Tmax=3000.0, Pmin=0.01 * PATM, Pmax=100.0 * PATM)
+    _, it, _, J = _run(_three(type=mg.CHEBYSHEV, cheb=dict(coef=[[7.25]], **lim)))
+    assert it["kf"][0] == pytest.approx(10 ** 7.25, rel=1e-13)
+    # linear in T~ and P~: log10 k = e00 + e10 T~ + e01 P~
+    coef = [[6.0, 0.3], [-0.7, 0.0]]
+    _, it, _, _ = _run(_three(type=mg.CHEBYSHEV, cheb=dict(coef=coef, **lim)))
+    T, P = 1300.0, 3 * PATM
+    Tt = (2 / T - 1 / 300.0 - 1 / 3000.0) / (1 / 3000.0 - 1 / 300.0)
+    Pt = (2 * math.log10(P) - math.log10(0.01 * PATM) - math.log10(100 * PATM)) / (math.log10(100 * PATM) - math.log10(0.01 * PATM))
+    assert it["kf"][0] == pytest.approx(10 ** (6.0 + 0.3 * Pt - 0.7 * Tt), rel=1e-12)
+    # against numpy's Chebyshev evaluation for a full grid
+    rng = np.random.default_rng(0)
+    c = rng.uniform(-1, 1, (7, 3)); c[0, 0] = 8.0
+    _, it, _, _ = _run(_three(type=mg.CHEBYSHEV, cheb=dict(coef=c, **lim)))
+    assert it["kf"][0] == pytest.approx(10 ** np.polynomial.chebyshev.chebval2d(Tt, Pt, c), rel=1e-11)
+
+
+def test_zero_concentration_is_safe():
+    """Reading S7: C_k = 0 gives finite values and the Jacobian still equals the complex step."""
+    m = mg.hand_all_types(True, True)
+    o = Oracle(m)
+    st = mg.make_states(6, 1, 99)
+    phi, par = o.pack(st, mg.CONP)
+    phi[0, 2] = 0.0
+    J = o.jacobian_dense(mg.CONP, phi, par)[0]
+    Jc = o.cs_jacobian(mg.CONP, phi[0], par[0])
+    assert np.isfinite(J).all()
+    rowmax = np.abs(Jc).max(axis=1, keepdims=True)
+    assert np.all(np.abs(J - Jc) <= np.maximum(1e-8 * np.abs(Jc), 1e-12 * rowmax))
