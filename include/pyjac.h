@@ -1,0 +1,133 @@
+/* pyjac.h -- C ABI of pyjac-b200: batched chemical-kinetic source terms and analytical Jacobians
+ * (sparse CSR/CSC and dense) on one NVIDIA B200 (sm_100a), after pyJac v2, arXiv:1809.01029.
+ *
+ * Citations "PAPER.md Lnnn" refer to the paper text; "DESIGN.md Rn" to the readings listed there
+ * for everything the paper defers to its (unavailable) supplement.
+ *
+ * State vector (Eq. 1):  phi = [T, E, n_1 .. n_{Ns-1}],  E = V (CONP) or P (CONV).
+ * The other thermodynamic variable is the per-state PARAMETER: P for CONP, V for CONV.
+ * n_var = Ns + 1.  The last species' concentration follows from the ideal-gas law and its rate from
+ * mass conservation.
+ * Source terms f = dphi/dt: PAPER.md Eqs. 2-8 (L128-164).  Jacobian J(i,j) = d f_i / d phi_j
+ * (Eq. 9), 0-based: index 0 = T, 1 = E, 2+k = n_{k+1}.
+ *
+ * Units: T [K], P [Pa], V [m^3], n [kmol], concentrations [kmol/m^3], W [kg/kmol],
+ * R = 8314.46261815324 J/(kmol K), P_atm = 101325 Pa.  Rate parameters in SI kmol-m^3-s, Ta = Ea/R [K].
+ *
+ * LAYOUT of every per-state device array (phi, dphi, sparse values, dense Jacobian):
+ * element e (0 <= e < n_e) of state s (0 <= s < n_states) lives at
+ *        (s / tile) * (n_e * tile)  +  e * tile  +  (s % tile)
+ * with n_e = n_var (phi, dphi), nnz (sparse values), n_var^2 (dense; e = r*n_var + c for order 'C',
+ * c*n_var + r for order 'F').  tile == ld is the pure structure-of-arrays / state-fastest layout (the
+ * paper's "F" order); a small power-of-two tile is the paper's chunked "vectorised"
+ * order (Fig. 3); tile == 1 is the state-major "C" order.
+ * Constraints: ld >= n_states, ld % tile == 0, tile >= 1; tile is a power of two or tile == ld.
+ * d_param is a plain [ld] array.  Base pointers must be 16-byte aligned.  Slots of states
+ * s >= n_states are never read or written.
+ *
+ * OWNERSHIP: desc arrays are caller-owned HOST memory, copied by pyjac_mech_create.  The handle owns
+ * its host and device tables.  State and output buffers are caller-owned DEVICE memory on the
+ * handle's device.  The compute calls enqueue work on `stream` (a cudaStream_t passed as void*,
+ * NULL = default stream) and return without synchronising; they allocate nothing and copy nothing
+ * between host and device.  The *_host convenience calls take HOST buffers and do the copies
+ * themselves (synchronous).
+ *
+ * ERRORS: every int-returning call returns PYJAC_OK or a nonzero status; pyjac_last_error() gives a
+ * thread-local message.  State VALUES are not validated on the device (garbage in, NaN out).
+ */
+#ifndef PYJAC_H
+#define PYJAC_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct pyjac_mech pyjac_mech; /* opaque */
+
+enum { PYJAC_OK = 0, PYJAC_EINVAL = 1, PYJAC_EMECH = 2, PYJAC_ECUDA = 3, PYJAC_ENOMEM = 4 };
+enum { PYJAC_CONP = 0, PYJAC_CONV = 1 };                 /* mode */
+enum { PYJAC_CSR = 0, PYJAC_CSC = 1 };                   /* sparse format */
+enum { PYJAC_ELEMENTARY = 0, PYJAC_THIRD_BODY = 1, PYJAC_FALLOFF_LINDEMANN = 2, PYJAC_FALLOFF_TROE = 3,
+       PYJAC_FALLOFF_SRI = 4, PYJAC_PLOG = 5, PYJAC_CHEBYSHEV = 6 };   /* reaction type */
+
+/* Mechanism description ("all modern reaction types"; rate laws: DESIGN.md R2).
+ * All pointers are HOST memory.  Ragged lists use CSR-style pointer arrays of length Nr+1. */
+typedef struct {
+  int32_t n_species, n_reactions;
+  const double *mol_weight;                          /* [Ns] W_k, > 0                                  */
+  const double *nasa_tmid, *nasa_lo, *nasa_hi;       /* [Ns], [Ns*7], [Ns*7]: a0..a6; low iff T<=tmid  */
+  const int32_t *reac_ptr, *reac_species, *reac_nu;  /* reactants: <= 3 entries, integer nu' in 1..3   */
+  const int32_t *prod_ptr, *prod_species, *prod_nu;  /* products, nu''                                 */
+  const uint8_t *reversible;                         /* [Nr] 1: k_r = k_f / K_c, 0: k_r = 0            */
+  const int32_t *type;                               /* [Nr] PYJAC_ELEMENTARY ..                       */
+  const double *A, *beta, *Ta;                       /* [Nr] Arrhenius (k_inf for falloff), A > 0      */
+  const int32_t *eff_ptr, *eff_species;              /* non-default third-body efficiencies, >= 0      */
+  const double *eff_value;
+  const int32_t *collider;                           /* [Nr] -1: mixture [M]; k: single collider (+X_k) */
+  const double *low_A, *low_beta, *low_Ta;           /* [Nr] falloff low-pressure limit k_0            */
+  const double *troe;                                /* [Nr*4] a, T3, T1, T2                           */
+  const uint8_t *troe_has_T2;                        /* [Nr]                                           */
+  const double *sri;                                 /* [Nr*5] a, b, c, d, e                           */
+  const int32_t *plog_ptr;                           /* P-Log points, pressures strictly ascending [Pa] */
+  const double *plog_P, *plog_A, *plog_beta, *plog_Ta;
+  const int32_t *cheb_ptr, *cheb_nT, *cheb_nP;       /* Chebyshev: coefficient offset, grid sizes      */
+  const double *cheb_Tmin, *cheb_Tmax, *cheb_Pmin, *cheb_Pmax; /* [Nr]                                 */
+  const double *cheb_coef;                           /* row-major nT x nP, log10 of k in SI            */
+} pyjac_mech_desc;
+
+/* Step a0 (one-time, host): validate, sort reactions by type, pack device tables, build the exact
+ * sparsity pattern in CSR and CSC and the static gather maps that replace the
+ * paper's run-time index search.  Uploads the tables to `cuda_device`.
+ * PYJAC_EMECH: Ns < 2, Nr < 1, index out of range, nu outside 1..3, more than 3 species per side,
+ * A <= 0, W <= 0, tmid <= 0, negative efficiency, P-Log with < 2 points or non-ascending pressures,
+ * empty Chebyshev grid or Tmin >= Tmax or Pmin >= Pmax, unknown type.  PYJAC_ECUDA: no such device.
+ * cuda_device = -1 builds a HOST-ONLY handle (pyjac_mech_dims / pyjac_sparsity work; every compute
+ * call fails with PYJAC_ECUDA) -- there is no CPU compute path.  The compute calls launch on the
+ * caller's current device, which must be the handle's device. */
+int pyjac_mech_create(const pyjac_mech_desc *desc, int cuda_device, pyjac_mech **out);
+void pyjac_mech_destroy(pyjac_mech *mech);
+
+int pyjac_mech_dims(const pyjac_mech *mech, int32_t *ns, int32_t *nr, int32_t *nvar, int64_t *nnz);
+
+/* Sparsity pattern of the n_var x n_var Jacobian (one pattern for CONP and CONV).  ptr has n_var+1
+ * entries, idx has nnz entries, ascending inside each row (CSR) or column (CSC); CSC is the exact
+ * transpose view of CSR.  The returned HOST pointers are owned by the handle.  Rule (R5):
+ * rows and columns T, E dense; species block = union over reactions of
+ * {k: nu_ki != 0} x {j: rate of i depends on C_j or on C_Ns, or alpha_ij != alpha_i,Ns}. */
+int pyjac_sparsity(const pyjac_mech *mech, int fmt, const int32_t **ptr, const int32_t **idx);
+
+/* Steps a1-a7: d_dphi = f(phi; param).  PAPER.md Eqs. 3-8. */
+int pyjac_source_terms(const pyjac_mech *mech, int mode, int64_t n_states, int64_t ld, int64_t tile,
+                       const double *d_phi, const double *d_param, double *d_dphi, void *stream);
+
+/* Steps a1-a11: the nnz values of J per state, in the value order of `fmt`.  Every nonzero is
+ * accumulated on chip and stored exactly once. */
+int pyjac_jacobian_sparse(const pyjac_mech *mech, int mode, int fmt, int64_t n_states, int64_t ld,
+                          int64_t tile, const double *d_phi, const double *d_param, double *d_vals,
+                          void *stream);
+
+/* Steps a1-a11: all n_var^2 entries per state (structural zeros written as 0.0, each entry stored
+ * exactly once; no memset pass).  order 'C': e = r*n_var + c, 'F': e = c*n_var + r. */
+int pyjac_jacobian_dense(const pyjac_mech *mech, int mode, char order, int64_t n_states, int64_t ld,
+                         int64_t tile, const double *d_phi, const double *d_param, double *d_J,
+                         void *stream);
+
+/* End-to-end convenience calls on HOST buffers (same layouts): allocate device scratch, copy in,
+ * run, copy out, synchronise.  what: 0 = source terms, 1 = sparse Jacobian (fmt), 2 = dense Jacobian
+ * (fmt = 'C' or 'F').  h_out must hold n_e * ld doubles. */
+int pyjac_eval_host(const pyjac_mech *mech, int what, int mode, int fmt, int64_t n_states, int64_t ld,
+                    int64_t tile, const double *h_phi, const double *h_param, double *h_out);
+
+/* Launch geometry chosen for a call (for DESIGN/bench reporting): states per CTA, threads per CTA,
+ * dynamic shared memory bytes.  what as in pyjac_eval_host. */
+int pyjac_launch_info(const pyjac_mech *mech, int what, int32_t *states_per_cta, int32_t *threads,
+                      int64_t *smem_bytes);
+
+const char *pyjac_last_error(void); /* thread-local, never NULL */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PYJAC_H */

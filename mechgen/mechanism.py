@@ -126,16 +126,16 @@ class MechBuilder:
 # configs (BASELINE.json configs[0..4] == C1..C5)
 # ------------------------------------------------------------------------------------------------
 CONFIGS = {
-    1: dict(ns=13, nr=27, n_states=1024, mode=CONP, max_atoms=4, zipf=0.3, T=(800.0, 2000.0),
+    1: dict(ns=13, nr=27, n_states=1024, mode=CONP, max_atoms=4, zipf=2.0, n_eff=(1, 2), T=(800.0, 2000.0),
             P_atm=(1.0, 50.0), sparse_X=False, bath_reacts=False,
             mix=dict(arr_rev=20, arr_irr=0, third=4, troe=3, lind=0, sri=0, plog=0, cheb=0)),
-    2: dict(ns=53, nr=325, n_states=1 << 17, mode=CONP, max_atoms=8, zipf=0.8, T=(800.0, 2000.0),
+    2: dict(ns=53, nr=325, n_states=1 << 17, mode=CONP, max_atoms=8, zipf=1.1, T=(800.0, 2000.0),
             P_atm=(1.0, 50.0), sparse_X=False, bath_reacts=False, mix="std"),
-    3: dict(ns=111, nr=784, n_states=1 << 17, mode=CONP, max_atoms=12, zipf=1.0, T=(800.0, 2000.0),
+    3: dict(ns=111, nr=784, n_states=1 << 17, mode=CONP, max_atoms=12, zipf=2.0, T=(800.0, 2000.0),
             P_atm=(1.0, 50.0), sparse_X=False, bath_reacts=True, mix="full"),
-    4: dict(ns=360, nr=2172, n_states=1 << 14, mode=CONV, max_atoms=20, zipf=1.1, T=(600.0, 2500.0),
+    4: dict(ns=360, nr=2172, n_states=1 << 14, mode=CONV, max_atoms=20, zipf=1.3, T=(600.0, 2500.0),
             P_atm=(1.0, 100.0), sparse_X=False, bath_reacts=False, mix="full"),
-    5: dict(ns=360, nr=2172, n_states=1 << 18, mode=CONP, max_atoms=20, zipf=1.1, T=(800.0, 2000.0),
+    5: dict(ns=360, nr=2172, n_states=1 << 18, mode=CONP, max_atoms=20, zipf=1.3, T=(800.0, 2000.0),
             P_atm=(1.0, 50.0), sparse_X=True, bath_reacts=False, mix="full"),
 }
 
@@ -329,7 +329,7 @@ def _efficiencies(rng, sampler, n_lo=3, n_hi=6, lo=0.5, hi=5.0, extra=None):
     return eff
 
 
-def make_mechanism(ns, nr, mix, seed, max_atoms=8, zipf=1.0, bath_reacts=False):
+def make_mechanism(ns, nr, mix, seed, max_atoms=8, zipf=1.0, bath_reacts=False, n_eff=(3, 6)):
     rng = np.random.Generator(np.random.PCG64(seed))
     counts = _mix_counts(nr, mix)
     assert sum(counts.values()) == nr, counts
@@ -337,13 +337,13 @@ def make_mechanism(ns, nr, mix, seed, max_atoms=8, zipf=1.0, bath_reacts=False):
         comp = _draw_compositions(rng, ns, max_atoms, with_n_species=bath_reacts)
         sampler = _ReactionSampler(rng, comp, zipf, bath_reacts)
         try:
-            return _build(rng, comp, sampler, counts, bath_reacts)
+            return _build(rng, comp, sampler, counts, bath_reacts, n_eff)
         except RuntimeError:
             continue
     raise RuntimeError("mechanism generation failed")
 
 
-def _build(rng, comp, sampler, counts, bath_reacts):
+def _build(rng, comp, sampler, counts, bath_reacts, n_eff=(3, 6)):
     ns = len(comp)
     mb = MechBuilder()
     for k in range(ns):
@@ -384,12 +384,12 @@ def _build(rng, comp, sampler, counts, bath_reacts):
                 extra = bath if (n_bath_eff > 0) else None
                 n_bath_eff -= 1 if extra is not None else 0
                 mb.add_reaction(reac, prod, A, b, Ta, rev=rng.random() < 0.8, type=THIRD_BODY,
-                                eff=_efficiencies(rng, sampler, extra=extra))
+                                eff=_efficiencies(rng, sampler, n_eff[0], n_eff[1], extra=extra))
             elif kind in ("troe", "lind", "sri"):
                 A, b, Ta = _arrhenius(rng, order)
                 low = (A * 10.0 ** rng.uniform(3.0, 8.0) * 1e-3, rng.uniform(-2.0, 2.0),
                        rng.uniform(0.0, 50.0) * 1000.0 * 4.184 / 8.31446261815324)
-                kw = dict(rev=rng.random() < 0.8, eff=_efficiencies(rng, sampler), low=low)
+                kw = dict(rev=rng.random() < 0.8, eff=_efficiencies(rng, sampler, n_eff[0], n_eff[1]), low=low)
                 if kind == "troe":
                     t = [rng.uniform(0.2, 0.9), rng.uniform(50.0, 1000.0), rng.uniform(500.0, 5000.0),
                          rng.uniform(1000.0, 8000.0) if rng.random() < 0.5 else None]
@@ -434,7 +434,7 @@ def config_mechanism(c):
     if key not in _MECH_CACHE:
         cfg = CONFIGS[key]
         _MECH_CACHE[key] = make_mechanism(cfg["ns"], cfg["nr"], cfg["mix"], 18090100 + key,
-                                          cfg["max_atoms"], cfg["zipf"], cfg["bath_reacts"])
+                                          cfg["max_atoms"], cfg["zipf"], cfg["bath_reacts"], cfg.get("n_eff", (3, 6)))
     return _MECH_CACHE[key]
 
 

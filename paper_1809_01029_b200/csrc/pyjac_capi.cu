@@ -1,0 +1,225 @@
+// C ABI of pyjac-b200 (include/pyjac.h): handle management, argument checking, table upload,
+// kernel dispatch.  No torch types; plain pointers and sizes only.
+#include <cuda_runtime.h>
+
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "pyjac_internal.h"
+
+using namespace pyjac;
+
+namespace {
+thread_local std::string g_err;
+int fail(int code, const std::string& msg) { g_err = msg; return code; }
+int cuda_fail(cudaError_t e, const char* what) {
+  g_err = std::string(what) + ": " + cudaGetErrorString(e);
+  return PYJAC_ECUDA;
+}
+#define CK(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return cuda_fail(e_, #call); } while (0)
+}  // namespace
+
+struct pyjac_mech {
+  int device = 0;
+  HostTables h;
+  DevMech dm{};
+  DevPlan plan[4]{};
+  std::vector<void*> allocs;
+  ~pyjac_mech() {
+    for (void* p : allocs) cudaFree(p);
+  }
+  template <class T> int upload(const std::vector<T>& v, const T** out) {
+    void* p = nullptr;
+    const size_t bytes = (v.size() ? v.size() : 1) * sizeof(T) + 32;   // +32: vector loads may touch padding
+    CK(cudaMalloc(&p, bytes));
+    allocs.push_back(p);
+    CK(cudaMemset(p, 0, bytes));
+    if (!v.empty()) CK(cudaMemcpy(p, v.data(), v.size() * sizeof(T), cudaMemcpyHostToDevice));
+    *out = (const T*)p;
+    return PYJAC_OK;
+  }
+};
+
+extern "C" {
+
+const char* pyjac_last_error(void) { return g_err.c_str(); }
+
+int pyjac_mech_create(const pyjac_mech_desc* desc, int cuda_device, pyjac_mech** out) {
+  if (!desc || !out) return fail(PYJAC_EINVAL, "pyjac_mech_create: null argument");
+  *out = nullptr;
+  pyjac_mech* m = new (std::nothrow) pyjac_mech();
+  if (!m) return fail(PYJAC_ENOMEM, "out of host memory");
+  std::string err;
+  int rc = build_host_tables(desc, m->h, err);
+  if (rc != PYJAC_OK) { delete m; return fail(rc, err); }
+  if (cuda_device == -1) { m->device = -1; *out = m; return PYJAC_OK; }   // host-only handle: pattern and dims only
+  int ndev = 0;
+  cudaError_t e = cudaGetDeviceCount(&ndev);
+  if (e != cudaSuccess || cuda_device < 0 || cuda_device >= ndev) {
+    delete m;
+    return fail(PYJAC_ECUDA, "pyjac_mech_create: no CUDA device " + std::to_string(cuda_device) +
+                                 (e != cudaSuccess ? std::string(" (") + cudaGetErrorString(e) + ")" : std::string()));
+  }
+  m->device = cuda_device;
+  int prev = 0;
+  cudaGetDevice(&prev);
+  auto body = [&]() -> int {
+    CK(cudaSetDevice(cuda_device));
+    if (int ea = set_kernel_attributes()) return cuda_fail((cudaError_t)ea, "cudaFuncSetAttribute");
+    HostTables& h = m->h;
+    DevMech& d = m->dm;
+    d.ns = h.ns; d.nr = h.nr; d.nvar = h.nvar; d.nslots = h.nslots;
+#define UP(field) if (int r_ = m->upload(h.field, &d.field)) return r_;
+    UP(nasa) UP(wr) UP(lnA) UP(beta) UP(Ta) UP(dn) UP(info) UP(aux) UP(sp) UP(eff_ptr) UP(eff_sp) UP(eff_d)
+    UP(slot_base) UP(fall) UP(plog_ptr) UP(plog_P) UP(plog_lnP) UP(plog_lnA) UP(plog_b) UP(plog_Ta)
+    UP(cheb_meta) UP(cheb_lim) UP(cheb_coef) UP(b_ptr) UP(b_ent) UP(bq_ent) UP(c_ptr) UP(c_ent)
+#undef UP
+    const int32_t *a_ptr[2], *a_ent[2];
+    const uint32_t* mask[2];
+    for (int p = 0; p < 2; ++p) {
+      if (int r_ = m->upload(h.a_ptr[p], &a_ptr[p])) return r_;
+      if (int r_ = m->upload(h.a_ent[p], &a_ent[p])) return r_;
+      if (int r_ = m->upload(h.nzmask[p], &mask[p])) return r_;
+    }
+    for (int f = 0; f < 4; ++f) {
+      DevPlan& pl = m->plan[f];
+      pl.nA = h.nA;
+      pl.n_e = f < 2 ? h.nnz : (int64_t)h.nvar * h.nvar;
+      pl.a_ptr = a_ptr[f & 1]; pl.a_ent = a_ent[f & 1];
+      if (int r_ = m->upload(h.a_pos[f], &pl.a_pos)) return r_;
+      if (int r_ = m->upload(h.b_pos[f], &pl.b_pos)) return r_;
+      if (int r_ = m->upload(h.c_pos[f], &pl.c_pos)) return r_;
+      for (int j = 0; j < 4; ++j) pl.d_pos[j] = h.d_pos[f][j];
+      pl.nzmask = f < 2 ? nullptr : mask[f & 1];
+    }
+    CK(cudaDeviceSynchronize());
+    return PYJAC_OK;
+  };
+  rc = body();
+  cudaSetDevice(prev);
+  if (rc != PYJAC_OK) { delete m; return rc; }
+  *out = m;
+  return PYJAC_OK;
+}
+
+void pyjac_mech_destroy(pyjac_mech* mech) {
+  if (!mech) return;
+  if (mech->device < 0) { delete mech; return; }
+  int prev = 0;
+  cudaGetDevice(&prev);
+  cudaSetDevice(mech->device);
+  delete mech;
+  cudaSetDevice(prev);
+}
+
+int pyjac_mech_dims(const pyjac_mech* mech, int32_t* ns, int32_t* nr, int32_t* nvar, int64_t* nnz) {
+  if (!mech) return fail(PYJAC_EINVAL, "pyjac_mech_dims: null handle");
+  if (ns) *ns = mech->h.ns;
+  if (nr) *nr = mech->h.nr;
+  if (nvar) *nvar = mech->h.nvar;
+  if (nnz) *nnz = mech->h.nnz;
+  return PYJAC_OK;
+}
+
+int pyjac_sparsity(const pyjac_mech* mech, int fmt, const int32_t** ptr, const int32_t** idx) {
+  if (!mech || !ptr || !idx) return fail(PYJAC_EINVAL, "pyjac_sparsity: null argument");
+  if (fmt != PYJAC_CSR && fmt != PYJAC_CSC) return fail(PYJAC_EINVAL, "pyjac_sparsity: fmt must be PYJAC_CSR or PYJAC_CSC");
+  *ptr = fmt == PYJAC_CSR ? mech->h.csr_ptr.data() : mech->h.csc_ptr.data();
+  *idx = fmt == PYJAC_CSR ? mech->h.csr_idx.data() : mech->h.csc_idx.data();
+  return PYJAC_OK;
+}
+
+static int check_common(const char* fn, const pyjac_mech* mech, int mode, int64_t n_states, int64_t ld, int64_t tile,
+                        const void* phi, const void* param, const void* out) {
+  if (!mech) return fail(PYJAC_EINVAL, std::string(fn) + ": null handle");
+  if (mech->device < 0) return fail(PYJAC_ECUDA, std::string(fn) + ": host-only handle (created with cuda_device = -1) cannot compute");
+  if (mode != PYJAC_CONP && mode != PYJAC_CONV) return fail(PYJAC_EINVAL, std::string(fn) + ": mode must be PYJAC_CONP or PYJAC_CONV");
+  if (n_states < 0) return fail(PYJAC_EINVAL, std::string(fn) + ": n_states < 0");
+  if (ld < n_states) return fail(PYJAC_EINVAL, std::string(fn) + ": ld < n_states");
+  if (tile < 1 || (tile != ld && (tile & (tile - 1)) != 0)) return fail(PYJAC_EINVAL, std::string(fn) + ": tile must be a power of two or equal to ld");
+  if (n_states > 0 && ld % tile != 0) return fail(PYJAC_EINVAL, std::string(fn) + ": ld must be a multiple of tile");
+  if (n_states > 0 && (!phi || !param || !out)) return fail(PYJAC_EINVAL, std::string(fn) + ": null buffer");
+  if (((uintptr_t)phi | (uintptr_t)param | (uintptr_t)out) & 15) return fail(PYJAC_EINVAL, std::string(fn) + ": buffers must be 16-byte aligned");
+  return PYJAC_OK;
+}
+
+int pyjac_source_terms(const pyjac_mech* mech, int mode, int64_t n_states, int64_t ld, int64_t tile, const double* d_phi,
+                       const double* d_param, double* d_dphi, void* stream) {
+  if (int rc = check_common("pyjac_source_terms", mech, mode, n_states, ld, tile, d_phi, d_param, d_dphi)) return rc;
+  if (n_states == 0) return PYJAC_OK;
+  const LaunchCfg cfg = choose_cfg(mech->h, false, tile, n_states);
+  if (cfg.smem > 227 * 1024) return fail(PYJAC_ENOMEM, "pyjac_source_terms: mechanism too large for shared memory");
+  int e = launch_source(mech->dm, cfg, mode, n_states, ld, tile, d_phi, d_param, d_dphi, stream);
+  if (e) return cuda_fail((cudaError_t)e, "source_kernel launch");
+  return PYJAC_OK;
+}
+
+static int run_jac(const char* fn, const pyjac_mech* mech, int mode, int ofmt, int64_t n_states, int64_t ld, int64_t tile,
+                   const double* d_phi, const double* d_param, double* d_out, void* stream) {
+  if (int rc = check_common(fn, mech, mode, n_states, ld, tile, d_phi, d_param, d_out)) return rc;
+  if (n_states == 0) return PYJAC_OK;
+  const LaunchCfg cfg = choose_cfg(mech->h, true, tile, n_states);
+  if (cfg.smem > 227 * 1024) return fail(PYJAC_ENOMEM, std::string(fn) + ": mechanism too large for shared memory");
+  int e = launch_jacobian(mech->dm, mech->plan[ofmt], cfg, mode, n_states, ld, tile, d_phi, d_param, d_out, stream);
+  if (e) return cuda_fail((cudaError_t)e, "jacobian_kernel launch");
+  return PYJAC_OK;
+}
+
+int pyjac_jacobian_sparse(const pyjac_mech* mech, int mode, int fmt, int64_t n_states, int64_t ld, int64_t tile,
+                          const double* d_phi, const double* d_param, double* d_vals, void* stream) {
+  if (fmt != PYJAC_CSR && fmt != PYJAC_CSC) return fail(PYJAC_EINVAL, "pyjac_jacobian_sparse: fmt must be PYJAC_CSR or PYJAC_CSC");
+  return run_jac("pyjac_jacobian_sparse", mech, mode, fmt == PYJAC_CSR ? OUT_CSR : OUT_CSC, n_states, ld, tile, d_phi, d_param, d_vals, stream);
+}
+
+int pyjac_jacobian_dense(const pyjac_mech* mech, int mode, char order, int64_t n_states, int64_t ld, int64_t tile,
+                         const double* d_phi, const double* d_param, double* d_J, void* stream) {
+  if (order != 'C' && order != 'F') return fail(PYJAC_EINVAL, "pyjac_jacobian_dense: order must be 'C' or 'F'");
+  return run_jac("pyjac_jacobian_dense", mech, mode, order == 'C' ? OUT_DENSE_C : OUT_DENSE_F, n_states, ld, tile, d_phi, d_param, d_J, stream);
+}
+
+int pyjac_launch_info(const pyjac_mech* mech, int what, int32_t* states_per_cta, int32_t* threads, int64_t* smem_bytes) {
+  if (!mech) return fail(PYJAC_EINVAL, "pyjac_launch_info: null handle");
+  const LaunchCfg cfg = choose_cfg(mech->h, what != 0, (int64_t)1 << 40, (int64_t)1 << 40);
+  if (states_per_cta) *states_per_cta = cfg.S;
+  if (threads) *threads = cfg.threads;
+  if (smem_bytes) *smem_bytes = (int64_t)cfg.smem;
+  return PYJAC_OK;
+}
+
+int pyjac_eval_host(const pyjac_mech* mech, int what, int mode, int fmt, int64_t n_states, int64_t ld, int64_t tile,
+                    const double* h_phi, const double* h_param, double* h_out) {
+  if (!mech) return fail(PYJAC_EINVAL, "pyjac_eval_host: null handle");
+  if (what < 0 || what > 2) return fail(PYJAC_EINVAL, "pyjac_eval_host: what must be 0, 1 or 2");
+  if (n_states < 0 || ld < n_states) return fail(PYJAC_EINVAL, "pyjac_eval_host: bad n_states / ld");
+  if (mech->device < 0) return fail(PYJAC_ECUDA, "pyjac_eval_host: host-only handle cannot compute");
+  if (n_states == 0) return PYJAC_OK;
+  if (!h_phi || !h_param || !h_out) return fail(PYJAC_EINVAL, "pyjac_eval_host: null buffer");
+  const int64_t n_e = what == 0 ? mech->h.nvar : (what == 1 ? mech->h.nnz : (int64_t)mech->h.nvar * mech->h.nvar);
+  int prev = 0;
+  cudaGetDevice(&prev);
+  double *d_phi = nullptr, *d_param = nullptr, *d_out = nullptr;
+  auto body = [&]() -> int {
+    CK(cudaSetDevice(mech->device));
+    CK(cudaMalloc(&d_phi, sizeof(double) * mech->h.nvar * ld));
+    CK(cudaMalloc(&d_param, sizeof(double) * ld));
+    CK(cudaMalloc(&d_out, sizeof(double) * n_e * ld));
+    CK(cudaMemcpy(d_phi, h_phi, sizeof(double) * mech->h.nvar * ld, cudaMemcpyHostToDevice));
+    CK(cudaMemcpy(d_param, h_param, sizeof(double) * ld, cudaMemcpyHostToDevice));
+    int rc;
+    if (what == 0) rc = pyjac_source_terms(mech, mode, n_states, ld, tile, d_phi, d_param, d_out, nullptr);
+    else if (what == 1) rc = pyjac_jacobian_sparse(mech, mode, fmt, n_states, ld, tile, d_phi, d_param, d_out, nullptr);
+    else rc = pyjac_jacobian_dense(mech, mode, (char)fmt, n_states, ld, tile, d_phi, d_param, d_out, nullptr);
+    if (rc) return rc;
+    CK(cudaMemcpy(h_out, d_out, sizeof(double) * n_e * ld, cudaMemcpyDeviceToHost));
+    return PYJAC_OK;
+  };
+  int rc = body();
+  cudaFree(d_phi); cudaFree(d_param); cudaFree(d_out);
+  cudaSetDevice(prev);
+  return rc;
+}
+
+}  // extern "C"

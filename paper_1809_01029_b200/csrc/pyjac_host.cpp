@@ -1,0 +1,315 @@
+// Step a0 of the hot path (one-time, host): mechanism description -> packed tables, sparsity
+// pattern and static gather maps.  The paper bakes this information into generated code
+// and searches the CRS/CCS index arrays at run time; here the
+// kernels are mechanism-agnostic and read tables, and the run-time search is replaced by static
+// maps, as the paper itself proposes.
+#include <algorithm>
+#include <cmath>
+#include <map>
+#include <numeric>
+#include <sstream>
+
+#include "pyjac_internal.h"
+
+namespace pyjac {
+
+namespace {
+
+struct Role { int species; int slot; };   // a Jacobian slot holding  dQ_i/dC_species  (one role)
+
+#define MECH_FAIL(msg) do { std::ostringstream os_; os_ << msg; err = os_.str(); return PYJAC_EMECH; } while (0)
+
+int validate(const pyjac_mech_desc* d, std::string& err) {
+  const int ns = d->n_species, nr = d->n_reactions;
+  if (ns < 2) MECH_FAIL("n_species must be >= 2, got " << ns);
+  if (nr < 1) MECH_FAIL("n_reactions must be >= 1, got " << nr);
+  if (ns > 32767) MECH_FAIL("n_species > 32767 unsupported");
+  for (int k = 0; k < ns; ++k) {
+    if (!(d->mol_weight[k] > 0.0)) MECH_FAIL("species " << k << ": molecular weight must be > 0");
+    if (!(d->nasa_tmid[k] > 0.0)) MECH_FAIL("species " << k << ": T_mid must be > 0");
+  }
+  for (int i = 0; i < nr; ++i) {
+    const int ty = d->type[i];
+    if (ty < PYJAC_ELEMENTARY || ty > PYJAC_CHEBYSHEV) MECH_FAIL("reaction " << i << ": unknown type " << ty);
+    for (int side = 0; side < 2; ++side) {
+      const int32_t* ptr = side ? d->prod_ptr : d->reac_ptr;
+      const int32_t* sp = side ? d->prod_species : d->reac_species;
+      const int32_t* nu = side ? d->prod_nu : d->reac_nu;
+      const int n = ptr[i + 1] - ptr[i];
+      if (n < 1 || n > 3) MECH_FAIL("reaction " << i << ": " << (side ? "products" : "reactants") << " must have 1..3 species, got " << n);
+      for (int j = ptr[i]; j < ptr[i + 1]; ++j) {
+        if (sp[j] < 0 || sp[j] >= ns) MECH_FAIL("reaction " << i << ": species index " << sp[j] << " out of range");
+        if (nu[j] < 1 || nu[j] > 3) MECH_FAIL("reaction " << i << ": stoichiometric coefficient " << nu[j] << " outside 1..3");
+        for (int l = ptr[i]; l < j; ++l)
+          if (sp[l] == sp[j]) MECH_FAIL("reaction " << i << ": species " << sp[j] << " listed twice on one side");
+      }
+    }
+    if (ty <= PYJAC_FALLOFF_SRI && !(d->A[i] > 0.0)) MECH_FAIL("reaction " << i << ": A must be > 0 (ln A is tabulated)");
+    if (ty >= PYJAC_FALLOFF_LINDEMANN && ty <= PYJAC_FALLOFF_SRI && !(d->low_A[i] > 0.0))
+      MECH_FAIL("reaction " << i << ": low-pressure A must be > 0");
+    if (d->collider[i] < -1 || d->collider[i] >= ns) MECH_FAIL("reaction " << i << ": collider index out of range");
+    for (int j = d->eff_ptr[i]; j < d->eff_ptr[i + 1]; ++j) {
+      if (d->eff_species[j] < 0 || d->eff_species[j] >= ns) MECH_FAIL("reaction " << i << ": efficiency species out of range");
+      if (!(d->eff_value[j] >= 0.0)) MECH_FAIL("reaction " << i << ": negative third-body efficiency");
+    }
+    if (ty == PYJAC_PLOG) {
+      const int n = d->plog_ptr[i + 1] - d->plog_ptr[i];
+      if (n < 2) MECH_FAIL("reaction " << i << ": P-Log needs >= 2 pressure points");
+      for (int j = d->plog_ptr[i]; j < d->plog_ptr[i + 1]; ++j) {
+        if (!(d->plog_P[j] > 0.0) || !(d->plog_A[j] > 0.0)) MECH_FAIL("reaction " << i << ": P-Log P and A must be > 0");
+        if (j > d->plog_ptr[i] && !(d->plog_P[j] > d->plog_P[j - 1])) MECH_FAIL("reaction " << i << ": P-Log pressures must be strictly ascending");
+      }
+    }
+    if (ty == PYJAC_CHEBYSHEV) {
+      if (d->cheb_nT[i] < 1 || d->cheb_nP[i] < 1) MECH_FAIL("reaction " << i << ": empty Chebyshev grid");
+      if (!(d->cheb_Tmin[i] > 0.0) || !(d->cheb_Tmin[i] < d->cheb_Tmax[i])) MECH_FAIL("reaction " << i << ": Chebyshev needs 0 < Tmin < Tmax");
+      if (!(d->cheb_Pmin[i] > 0.0) || !(d->cheb_Pmin[i] < d->cheb_Pmax[i])) MECH_FAIL("reaction " << i << ": Chebyshev needs 0 < Pmin < Pmax");
+    }
+  }
+  return PYJAC_OK;
+}
+
+}  // namespace
+
+int build_host_tables(const pyjac_mech_desc* d, HostTables& h, std::string& err) {
+  if (int rc = validate(d, err)) return rc;
+  const int ns = d->n_species, nr = d->n_reactions, nvar = ns + 1, L = ns - 1;
+  h.ns = ns; h.nr = nr; h.nvar = nvar;
+
+  // ---- species tables ---------------------------------------------------------------------------
+  h.nasa.assign((size_t)ns * 16, 0.0);
+  h.wr.resize(ns);
+  for (int k = 0; k < ns; ++k) {
+    h.nasa[16 * k] = d->nasa_tmid[k];
+    for (int j = 0; j < 7; ++j) { h.nasa[16 * k + 1 + j] = d->nasa_lo[7 * k + j]; h.nasa[16 * k + 8 + j] = d->nasa_hi[7 * k + j]; }
+    h.wr[k] = d->mol_weight[k] / d->mol_weight[L];
+  }
+
+  // ---- sort reactions by (type, reversible): warps become type-uniform ------------
+  h.perm.resize(nr);
+  std::iota(h.perm.begin(), h.perm.end(), 0);
+  std::stable_sort(h.perm.begin(), h.perm.end(), [&](int a, int b) {
+    const int ka = d->type[a] * 2 + (d->reversible[a] ? 1 : 0), kb = d->type[b] * 2 + (d->reversible[b] ? 1 : 0);
+    return ka < kb;
+  });
+
+  h.lnA.resize(nr); h.beta.resize(nr); h.Ta.resize(nr); h.dn.resize(nr);
+  h.info.resize(nr); h.aux.assign(nr, -1); h.sp.assign((size_t)nr * 8, 0u);
+  h.eff_ptr.assign(1, 0); h.slot_base.assign(1, 0);
+  std::vector<std::vector<Role>> roles(nr);
+  std::vector<std::vector<std::pair<int, int>>> net(nr);   // (species k < Ns-1... incl. last, net nu != 0)
+
+  for (int r = 0; r < nr; ++r) {
+    const int i = h.perm[r];
+    const int ty = d->type[i];
+    const bool rev = d->reversible[i] != 0;
+    const bool tb = ty >= PYJAC_THIRD_BODY && ty <= PYJAC_FALLOFF_SRI;
+    const bool falloff = ty >= PYJAC_FALLOFF_LINDEMANN && ty <= PYJAC_FALLOFF_SRI;
+    h.lnA[r] = (ty <= PYJAC_FALLOFF_SRI) ? std::log(d->A[i]) : 0.0;
+    h.beta[r] = d->beta[i]; h.Ta[r] = d->Ta[i];
+    const int nre = d->reac_ptr[i + 1] - d->reac_ptr[i], npr = d->prod_ptr[i + 1] - d->prod_ptr[i];
+    int snu = 0;
+    std::map<int, int> netnu;
+    for (int a = 0; a < nre; ++a) {
+      const int j = d->reac_ptr[i] + a;
+      h.sp[8 * r + a] = (uint32_t)d->reac_species[j] | ((uint32_t)d->reac_nu[j] << 16);
+      snu -= d->reac_nu[j]; netnu[d->reac_species[j]] -= d->reac_nu[j];
+    }
+    for (int b = 0; b < npr; ++b) {
+      const int j = d->prod_ptr[i] + b;
+      h.sp[8 * r + 3 + b] = (uint32_t)d->prod_species[j] | ((uint32_t)d->prod_nu[j] << 16);
+      snu += d->prod_nu[j]; netnu[d->prod_species[j]] += d->prod_nu[j];
+    }
+    double dn = 0.0;
+    for (auto& kv : netnu)
+      if (kv.second != 0) { net[r].push_back(kv); if (kv.first != L) dn += kv.second * (1.0 - h.wr[kv.first]); }
+    h.dn[r] = dn;
+    const bool adef = tb && d->collider[i] < 0;
+    int info = ty | (rev ? INFO_REV : 0) | (adef ? INFO_ADEF : 0) | ((snu + 8) << INFO_SNU_SHIFT) |
+               (nre << INFO_NREAC_SHIFT) | (npr << INFO_NPROD_SHIFT);
+    if (ty == PYJAC_FALLOFF_TROE && d->troe_has_T2[i]) info |= INFO_T2;
+    h.info[r] = info;
+    // slots: 0 = T column, 1 = E column, then one per role
+    int slot = h.slot_base[r] + 2;
+    for (int a = 0; a < nre; ++a) roles[r].push_back({d->reac_species[d->reac_ptr[i] + a], slot++});
+    if (rev) for (int b = 0; b < npr; ++b) roles[r].push_back({d->prod_species[d->prod_ptr[i] + b], slot++});
+    if (tb) {
+      if (d->collider[i] >= 0) {           // [M] = C_collider: default 0, one efficiency of 1
+        h.eff_sp.push_back(d->collider[i]); h.eff_d.push_back(1.0);
+        roles[r].push_back({d->collider[i], slot++});
+      } else {
+        for (int j = d->eff_ptr[i]; j < d->eff_ptr[i + 1]; ++j) {
+          if (d->eff_value[j] == 1.0) continue;
+          bool dup = false;
+          for (int l = d->eff_ptr[i]; l < j; ++l) dup |= d->eff_species[l] == d->eff_species[j];
+          if (dup) MECH_FAIL("reaction " << i << ": efficiency of species " << d->eff_species[j] << " given twice");
+          h.eff_sp.push_back(d->eff_species[j]); h.eff_d.push_back(d->eff_value[j] - 1.0);
+          roles[r].push_back({d->eff_species[j], slot++});
+        }
+      }
+    }
+    h.eff_ptr.push_back((int)h.eff_sp.size());
+    h.max_eff = std::max(h.max_eff, h.eff_ptr[r + 1] - h.eff_ptr[r]);
+    h.slot_base.push_back(slot);
+    if (falloff) {
+      h.aux[r] = (int)(h.fall.size() / 12);
+      double f[12] = {std::log(d->low_A[i]), d->low_beta[i], d->low_Ta[i], 0, 0, 0, 0, 0, 0, 0, 0, 0};
+      if (ty == PYJAC_FALLOFF_TROE) for (int j = 0; j < 4; ++j) f[4 + j] = d->troe[4 * i + j];
+      if (ty == PYJAC_FALLOFF_SRI) for (int j = 0; j < 5; ++j) f[4 + j] = d->sri[5 * i + j];
+      h.fall.insert(h.fall.end(), f, f + 12);
+    } else if (ty == PYJAC_PLOG) {
+      if (h.plog_ptr.empty()) h.plog_ptr.push_back(0);
+      h.aux[r] = (int)h.plog_ptr.size() - 1;
+      for (int j = d->plog_ptr[i]; j < d->plog_ptr[i + 1]; ++j) {
+        h.plog_P.push_back(d->plog_P[j]); h.plog_lnP.push_back(std::log(d->plog_P[j]));
+        h.plog_lnA.push_back(std::log(d->plog_A[j])); h.plog_b.push_back(d->plog_beta[j]); h.plog_Ta.push_back(d->plog_Ta[j]);
+      }
+      h.plog_ptr.push_back((int)h.plog_P.size());
+    } else if (ty == PYJAC_CHEBYSHEV) {
+      h.aux[r] = (int)(h.cheb_meta.size() / 4);
+      const int nT = d->cheb_nT[i], nP = d->cheb_nP[i];
+      h.cheb_meta.insert(h.cheb_meta.end(), {nT, nP, (int)h.cheb_coef.size(), 0});
+      h.cheb_lim.insert(h.cheb_lim.end(), {1.0 / d->cheb_Tmin[i], 1.0 / d->cheb_Tmax[i], std::log10(d->cheb_Pmin[i]), std::log10(d->cheb_Pmax[i])});
+      for (int j = 0; j < nT * nP; ++j) h.cheb_coef.push_back(d->cheb_coef[d->cheb_ptr[i] + j]);
+    }
+  }
+  h.nslots = h.slot_base[nr];
+
+  // ---- gather maps and pattern (R5) ----------------------------------------
+  // Species-block entry (k, j), k, j < L:  J = sum_i nu_ki (Ghat^j_i - Ghat^L_i)  (R4-6):
+  // + every role of species j, - every role of the last species L (those hit ALL columns: dense rows).
+  std::vector<std::map<int, std::vector<int32_t>>> rowmap(L);   // row k -> col j -> entries
+  h.b_ptr.assign(1, 0); h.c_ptr.assign(1, 0);
+  std::vector<std::vector<int32_t>> bl(L), bql(L), cl(L);
+  auto push_n = [](std::vector<int32_t>& v, int32_t e, int n) { for (int c = 0; c < n; ++c) v.push_back(e); };
+  for (int r = 0; r < nr; ++r) {
+    for (auto& kv : net[r]) {
+      const int k = kv.first, nu = kv.second;
+      if (k == L) continue;
+      const uint32_t sgn = nu < 0 ? SIGN_BIT : 0u;
+      push_n(bl[k], (int32_t)((uint32_t)h.slot_base[r] | sgn), std::abs(nu));
+      push_n(bql[k], (int32_t)((uint32_t)r | sgn), std::abs(nu));
+      for (const Role& ro : roles[r]) {
+        if (ro.species != L) push_n(rowmap[k][ro.species], (int32_t)((uint32_t)ro.slot | sgn), std::abs(nu));
+        else for (int j = 0; j < L; ++j) push_n(rowmap[k][j], (int32_t)((uint32_t)ro.slot | (sgn ^ SIGN_BIT)), std::abs(nu));
+      }
+    }
+    if (!net[r].empty() && !(net[r].size() == 1 && net[r][0].first == L)) {
+      for (const Role& ro : roles[r]) {
+        if (ro.species != L) { cl[ro.species].push_back(ro.slot); cl[ro.species].push_back(r); }
+        else for (int j = 0; j < L; ++j) { cl[j].push_back((int32_t)((uint32_t)ro.slot | SIGN_BIT)); cl[j].push_back(r); }
+      }
+    }
+  }
+  // exact structural pattern by the rule of DESIGN.md R5: a pair (k, j) reached only through terms that
+  // cancel identically (alpha_ij == alpha_iL, both non-default) is NOT a structural nonzero.
+  {
+    std::vector<std::vector<char>> inpat(L, std::vector<char>(L, 0));
+    for (int r = 0; r < nr; ++r) {
+      const int i = h.perm[r];
+      const int ty = d->type[i];
+      const bool rev = d->reversible[i] != 0;
+      const bool tb = ty >= PYJAC_THIRD_BODY && ty <= PYJAC_FALLOFF_SRI;
+      auto dep = [&](int k) {
+        for (int j = d->reac_ptr[i]; j < d->reac_ptr[i + 1]; ++j) if (d->reac_species[j] == k) return true;
+        if (rev) for (int j = d->prod_ptr[i]; j < d->prod_ptr[i + 1]; ++j) if (d->prod_species[j] == k) return true;
+        return false;
+      };
+      auto alpha = [&](int k) {
+        if (d->collider[i] >= 0) return k == d->collider[i] ? 1.0 : 0.0;
+        for (int j = d->eff_ptr[i]; j < d->eff_ptr[i + 1]; ++j) if (d->eff_species[j] == k) return d->eff_value[j];
+        return 1.0;
+      };
+      const bool depL = dep(L);
+      const double aL = tb ? alpha(L) : 0.0;
+      for (auto& kv : net[r]) {
+        if (kv.first == L) continue;
+        for (int j = 0; j < L; ++j)
+          if (depL || dep(j) || (tb && alpha(j) != aL)) inpat[kv.first][j] = 1;
+      }
+    }
+    for (int k = 0; k < L; ++k) {
+      for (auto it = rowmap[k].begin(); it != rowmap[k].end();)
+        it = inpat[k][it->first] ? std::next(it) : rowmap[k].erase(it);
+      for (int j = 0; j < L; ++j)
+        if (inpat[k][j] && !rowmap[k].count(j)) MECH_FAIL("internal: pattern entry (" << k << "," << j << ") has no gather list");
+    }
+  }
+  for (int k = 0; k < L; ++k) {
+    h.b_ent.insert(h.b_ent.end(), bl[k].begin(), bl[k].end());
+    h.bq_ent.insert(h.bq_ent.end(), bql[k].begin(), bql[k].end());
+    h.b_ptr.push_back((int)h.b_ent.size());
+    h.c_ent.insert(h.c_ent.end(), cl[k].begin(), cl[k].end());
+    h.c_ptr.push_back((int)h.c_ent.size() / 2);
+  }
+  // pattern: rows T, E dense; columns T, E dense (R5 / S10); species block from rowmap
+  std::vector<std::vector<int>> rows(nvar);
+  for (int r = 0; r < 2; ++r) { rows[r].resize(nvar); std::iota(rows[r].begin(), rows[r].end(), 0); }
+  for (int k = 0; k < L; ++k) {
+    rows[2 + k] = {0, 1};
+    for (auto& kv : rowmap[k]) rows[2 + k].push_back(2 + kv.first);
+  }
+  h.csr_ptr.assign(1, 0);
+  for (int r = 0; r < nvar; ++r) { h.csr_idx.insert(h.csr_idx.end(), rows[r].begin(), rows[r].end()); h.csr_ptr.push_back((int)h.csr_idx.size()); }
+  h.nnz = (int64_t)h.csr_idx.size();
+  if ((int64_t)nvar * nvar > 2147483647LL) MECH_FAIL("n_var^2 exceeds int32");
+  // CSC = transpose; csr2csc[p] = position of CSR entry p in CSC value order
+  std::vector<int> colcount(nvar + 1, 0);
+  for (int c : h.csr_idx) colcount[c + 1]++;
+  h.csc_ptr.assign(nvar + 1, 0);
+  for (int c = 0; c < nvar; ++c) h.csc_ptr[c + 1] = h.csc_ptr[c] + colcount[c + 1];
+  h.csc_idx.resize(h.nnz);
+  std::vector<int> fill(h.csc_ptr.begin(), h.csc_ptr.end() - 1), csr2csc(h.nnz);
+  for (int r = 0; r < nvar; ++r)
+    for (int p = h.csr_ptr[r]; p < h.csr_ptr[r + 1]; ++p) { const int c = h.csr_idx[p]; csr2csc[p] = fill[c]; h.csc_idx[fill[c]++] = r; }
+  auto csr_pos = [&](int r, int c) {
+    auto b = h.csr_idx.begin() + h.csr_ptr[r], e = h.csr_idx.begin() + h.csr_ptr[r + 1];
+    return (int)(std::lower_bound(b, e, c) - h.csr_idx.begin());
+  };
+  auto pos_of = [&](int fmt, int r, int c) -> int32_t {
+    switch (fmt) {
+      case OUT_CSR: return csr_pos(r, c);
+      case OUT_CSC: return csr2csc[csr_pos(r, c)];
+      case OUT_DENSE_C: return r * nvar + c;
+      default: return c * nvar + r;
+    }
+  };
+  // class A items in row-major (plan 0) and column-major (plan 1) order
+  struct Item { int k, j; };
+  std::vector<Item> items[2];
+  for (int k = 0; k < L; ++k) for (auto& kv : rowmap[k]) items[0].push_back({k, kv.first});
+  items[1] = items[0];
+  std::stable_sort(items[1].begin(), items[1].end(), [](const Item& a, const Item& b) { return a.j < b.j; });
+  h.nA = (int)items[0].size();
+  for (int p = 0; p < 2; ++p) {
+    h.a_ptr[p].assign(1, 0);
+    for (const Item& it : items[p]) {
+      const auto& e = rowmap[it.k][it.j];
+      h.a_ent[p].insert(h.a_ent[p].end(), e.begin(), e.end());
+      h.a_ptr[p].push_back((int)h.a_ent[p].size());
+    }
+  }
+  for (int fmt = 0; fmt < 4; ++fmt) {
+    const int p = fmt & 1;
+    h.a_pos[fmt].resize(h.nA);
+    for (int e = 0; e < h.nA; ++e) h.a_pos[fmt][e] = pos_of(fmt, 2 + items[p][e].k, 2 + items[p][e].j);
+    h.b_pos[fmt].resize(2 * L); h.c_pos[fmt].resize(2 * L);
+    for (int k = 0; k < L; ++k) {
+      h.b_pos[fmt][k] = pos_of(fmt, 2 + k, 0); h.b_pos[fmt][L + k] = pos_of(fmt, 2 + k, 1);
+      h.c_pos[fmt][k] = pos_of(fmt, 0, 2 + k); h.c_pos[fmt][L + k] = pos_of(fmt, 1, 2 + k);
+    }
+    h.d_pos[fmt][0] = pos_of(fmt, 0, 0); h.d_pos[fmt][1] = pos_of(fmt, 0, 1);
+    h.d_pos[fmt][2] = pos_of(fmt, 1, 0); h.d_pos[fmt][3] = pos_of(fmt, 1, 1);
+  }
+  for (int p = 0; p < 2; ++p) {
+    h.nzmask[p].assign(((size_t)nvar * nvar + 31) / 32, 0u);
+    for (int r = 0; r < nvar; ++r)
+      for (int q = h.csr_ptr[r]; q < h.csr_ptr[r + 1]; ++q) {
+        const size_t e = p == 0 ? (size_t)r * nvar + h.csr_idx[q] : (size_t)h.csr_idx[q] * nvar + r;
+        h.nzmask[p][e >> 5] |= 1u << (e & 31);
+      }
+  }
+  return PYJAC_OK;
+}
+
+}  // namespace pyjac

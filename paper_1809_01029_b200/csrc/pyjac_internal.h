@@ -1,0 +1,104 @@
+// Internal definitions shared by the host preprocessing (pyjac_host.cpp), the kernels
+// (pyjac_kernels.cu) and the C ABI (pyjac_capi.cu).  Not part of the public boundary.
+#pragma once
+#include <cstdint>
+#include <string>
+#include <vector>
+
+#include "pyjac.h"
+
+namespace pyjac {
+
+constexpr double R_GAS = 8314.46261815324;  // J/(kmol K)   DESIGN.md R1
+constexpr double P_ATM = 101325.0;          // Pa
+
+// bit fields of RxTables::info
+constexpr int INFO_TYPE_MASK = 7;    // bits 0-2  reaction type
+constexpr int INFO_REV = 1 << 3;     // reversible
+constexpr int INFO_T2 = 1 << 4;      // Troe has T2
+constexpr int INFO_ADEF = 1 << 5;    // default third-body efficiency is 1 (mixture); 0: single collider
+constexpr int INFO_SNU_SHIFT = 8;    // bits 8-11: sum(nu) + 8
+constexpr int INFO_NREAC_SHIFT = 12; // bits 12-13: number of reactant entries
+constexpr int INFO_NPROD_SHIFT = 14; // bits 14-15: number of product entries
+constexpr uint32_t SIGN_BIT = 0x80000000u;
+
+enum OutFmt { OUT_CSR = 0, OUT_CSC = 1, OUT_DENSE_C = 2, OUT_DENSE_F = 3 };
+
+// ---- host-side tables (reactions in SORTED order: by type, then reversibility) ------------------
+struct HostTables {
+  int ns = 0, nr = 0, nvar = 0;
+  std::vector<int32_t> perm;                 // sorted index -> original reaction index
+  // species
+  std::vector<double> nasa;                  // [ns*16]: tmid, lo[7], hi[7], pad
+  std::vector<double> wr;                    // [ns] W_k / W_Ns
+  // reactions
+  std::vector<double> lnA, beta, Ta, dn;     // [nr]; dn = sum_k<Ns nu_ki (1 - W_k/W_Ns)
+  std::vector<int32_t> info, aux;            // [nr]; aux = index into fall / plog / cheb tables
+  std::vector<uint32_t> sp;                  // [nr*8]: 0-2 reactants, 3-5 products: species | nu << 16
+  std::vector<int32_t> eff_ptr, eff_sp;      // [nr+1], entries with alpha != default only
+  std::vector<double> eff_d;                 // alpha - default
+  std::vector<int32_t> slot_base;            // [nr+1] Jacobian slots: {T, E, reactant roles, product roles (rev), eff roles}
+  std::vector<double> fall;                  // [nf*12]: lnA0, beta0, Ta0, pad, then 5 blend parameters
+  std::vector<int32_t> plog_ptr;             // [npl+1]
+  std::vector<double> plog_P, plog_lnP, plog_lnA, plog_b, plog_Ta;
+  std::vector<int32_t> cheb_meta;            // [nc*4]: nT, nP, coef offset, 0
+  std::vector<double> cheb_lim, cheb_coef;   // [nc*4]: 1/Tmin, 1/Tmax, log10 Pmin, log10 Pmax
+  // pattern
+  int64_t nnz = 0;
+  std::vector<int32_t> csr_ptr, csr_idx, csc_ptr, csc_idx;
+  // gather maps.  Entries: slot offset | SIGN_BIT (a stoichiometric coefficient of magnitude m is m copies)
+  std::vector<int32_t> b_ptr, b_ent, bq_ent; // per species k < Ns-1: reactions with nu_ki != 0 (slot base / reaction index)
+  std::vector<int32_t> c_ptr, c_ent;         // per column j < Ns-1: pairs (slot | sign, reaction): T and E rows
+  // class A items (species-block nonzeros) in row-major [0] and column-major [1] order
+  int nA = 0;
+  std::vector<int32_t> a_ptr[2], a_ent[2];
+  std::vector<int32_t> a_pos[4];             // [OutFmt][nA] output element index (order of plan fmt&1)
+  std::vector<int32_t> b_pos[4], c_pos[4];   // [OutFmt][2*(ns-1)]: (k,T),(k,E) / (T,j),(E,j)
+  int32_t d_pos[4][4];                       // (T,T) (T,E) (E,T) (E,E)
+  std::vector<uint32_t> nzmask[2];           // dense bitmaps, bit e set iff dense element e ('C' / 'F' order) is in the pattern
+  int nslots = 0;                            // total Jacobian slots
+  int max_eff = 0;
+};
+
+// returns PYJAC_OK or an error code with a message in err
+int build_host_tables(const pyjac_mech_desc* d, HostTables& h, std::string& err);
+
+// ---- device views ------------------------------------------------------------------------------
+struct DevMech {
+  int ns, nr, nvar, nslots;
+  const double *nasa, *wr;
+  const double *lnA, *beta, *Ta, *dn;
+  const int32_t *info, *aux;
+  const uint32_t* sp;
+  const int32_t *eff_ptr, *eff_sp;
+  const double* eff_d;
+  const int32_t* slot_base;
+  const double* fall;
+  const int32_t* plog_ptr;
+  const double *plog_P, *plog_lnP, *plog_lnA, *plog_b, *plog_Ta;
+  const int32_t* cheb_meta;
+  const double *cheb_lim, *cheb_coef;
+  const int32_t *b_ptr, *b_ent, *bq_ent, *c_ptr, *c_ent;
+};
+
+struct DevPlan {
+  int nA;
+  int64_t n_e;               // elements per state in the output (nnz or nvar^2)
+  const int32_t *a_ptr, *a_ent, *a_pos, *b_pos, *c_pos;
+  int32_t d_pos[4];
+  const uint32_t* nzmask;    // dense only (else nullptr)
+};
+
+struct LaunchCfg { int S, threads; size_t smem; };
+
+// what: 0 source, 1 jacobian.  Chooses states-per-CTA from the shared-memory footprint and `tile`.
+LaunchCfg choose_cfg(const HostTables& h, bool jac, int64_t tile, int64_t n_states);
+
+// kernel launchers (pyjac_kernels.cu); return cudaError_t as int
+int launch_source(const DevMech& m, const LaunchCfg& cfg, int mode, int64_t n_states, int64_t ld, int64_t tile,
+                  const double* phi, const double* param, double* out, void* stream);
+int launch_jacobian(const DevMech& m, const DevPlan& p, const LaunchCfg& cfg, int mode, int64_t n_states, int64_t ld,
+                    int64_t tile, const double* phi, const double* param, double* out, void* stream);
+int set_kernel_attributes();
+
+}  // namespace pyjac

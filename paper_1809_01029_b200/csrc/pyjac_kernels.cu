@@ -1,0 +1,587 @@
+// fp64 kernels of the hot path for sm_100a (steps a1-a11 of SURVEY.md section 8a / DESIGN.md).
+//
+// Design: a CTA owns a TILE OF S STATES and keeps every per-state intermediate
+// on chip.  All work loops run over (item, state) pairs with the state index fastest inside the warp,
+// so every global access of a warp is a run of S consecutive states.
+//   phase 0  items = species    : concentrations (Eq. 6-7), NASA-7 thermo, D = sum C_k c_k
+//   phase 1  items = reactions  : k_f, K_c, k_r, third-body / falloff c_i, rates of progress and the
+//                                 per-reaction partials ("slots") dq_i/dT, dq_i/dE, dQ_i/dC_j -> shared
+//                                 memory; reaction-sum reductions for the T and E source terms
+//   phase 2  items = nonzeros   : every Jacobian nonzero gathers its static list of slots from shared
+//                                 memory, is finished in a register and stored ONCE (no zero-fill +
+//                                 "J[idx] += ..." read-modify-write as in PAPER.md L343, no index
+//                                 search as in PAPER.md L345)
+// No tensor cores: nothing here is a dense contraction.  No fast-math.
+#include <cuda_runtime.h>
+
+#include "pyjac_internal.h"
+
+namespace pyjac {
+
+namespace {
+
+constexpr int NT = 512;           // threads per CTA
+constexpr int NW = NT / 32;
+constexpr int NRED = 8;           // reduction slots
+// per-state scalars kept in shared memory
+enum { SC_T = 0, SC_V, SC_P, SC_CTOT, SC_SUMC, SC_SUMCC, SC_SUMCDC, SC_D, SC_DDDT, SC_CNS,
+       SC_R0, SC_R1, SC_R2, SC_R3, SC_R4, SC_R5, SC_R6, SC_R7, NSC };
+
+__host__ __device__ inline size_t smem_doubles(int ns, int nr, int nslots, int S, bool jac) {
+  size_t per_state = NSC + 6 * (size_t)ns + (jac ? (size_t)nslots + nr : (size_t)nr);
+  return per_state * S + (size_t)NW * NRED * S;
+}
+
+template <int S> __device__ __forceinline__ double group_sum(double v) {
+#pragma unroll
+  for (int o = 16; o >= S; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+
+__device__ __forceinline__ double apply_sign(double v, uint32_t ent) {
+  return __hiloint2double(__double2hiint(v) ^ (int)(ent & SIGN_BIT), __double2loint(v));
+}
+
+// block-wide sum of NV per-thread partials per state; result in sc[(first+j)*S + s]
+template <int S, int NV>
+__device__ __forceinline__ void block_reduce(double (&v)[NV], double* red, double* sc, int first) {
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+  for (int j = 0; j < NV; ++j) {
+    double t = group_sum<S>(v[j]);
+    if (lane < S) red[(warp * NRED + j) * S + lane] = t;
+  }
+  __syncthreads();
+  if (threadIdx.x < NV * S) {
+    const int j = threadIdx.x / S, s = threadIdx.x % S;
+    double t = 0.0;
+#pragma unroll
+    for (int w = 0; w < NW; ++w) t += red[(w * NRED + j) * S + s];
+    sc[(first + j) * S + s] = t;
+  }
+  __syncthreads();
+}
+
+__device__ __forceinline__ double ipow(double x, int n) {   // n in 0..3
+  double r = 1.0;
+  if (n >= 1) r = x;
+  if (n >= 2) r *= x;
+  if (n >= 3) r *= x;
+  return r;
+}
+// nu * x^(nu-1), nu in 0..3
+__device__ __forceinline__ double dpow(double x, int n) {
+  return n == 0 ? 0.0 : (n == 1 ? 1.0 : (n == 2 ? 2.0 * x : 3.0 * x * x));
+}
+
+struct Blend { double F, dF_dPr, dF_dT; };
+
+// Troe / SRI blending function and its partial derivatives (R2, R4-5)
+__device__ __forceinline__ Blend blend(int type, bool hasT2, const double* __restrict__ fp, double T, double invT, double lnT, double Pr_in) {
+  Blend b; b.F = 1.0; b.dF_dPr = 0.0; b.dF_dT = 0.0;
+  const double LN10 = 2.302585092994045684, ILN10 = 0.434294481903251828;
+  const double Pr = fmax(Pr_in, 1e-300);
+  if (type == PYJAC_FALLOFF_TROE) {
+    const double a = fp[4], iT3 = 1.0 / fp[5], iT1 = 1.0 / fp[6], T2 = fp[7];
+    const double e3 = exp(-T * iT3), e1 = exp(-T * iT1);
+    double Fc = (1.0 - a) * e3 + a * e1;
+    double dFc = -(1.0 - a) * iT3 * e3 - a * iT1 * e1;
+    if (hasT2) { const double e2 = exp(-T2 * invT); Fc += e2; dFc += T2 * invT * invT * e2; }
+    const double L = log(Pr) * ILN10, Lc = log(Fc) * ILN10;
+    const double n = 0.75 - 1.27 * Lc;
+    const double A = L - 0.4 - 0.67 * Lc;
+    const double B = n - 0.14 * A;
+    const double iB = 1.0 / B;
+    const double f = A * iB;
+    const double g = 1.0 / (1.0 + f * f);
+    b.F = exp(LN10 * Lc * g);
+    const double dlogF_df = -2.0 * Lc * f * g * g;
+    const double df_dL = n * iB * iB;
+    const double df_dLc = (-0.67 * B + 1.1762 * A) * iB * iB;
+    b.dF_dPr = b.F * dlogF_df * df_dL / Pr;
+    b.dF_dT = b.F * (g + dlogF_df * df_dLc) * dFc / Fc;
+  } else if (type == PYJAC_FALLOFF_SRI) {
+    const double a = fp[4], bb = fp[5], ic = 1.0 / fp[6], d = fp[7], e = fp[8];
+    const double L = log(Pr) * ILN10;
+    const double X = 1.0 / (1.0 + L * L);
+    const double eb = exp(-bb * invT), ec = exp(-T * ic);
+    const double base = a * eb + ec;
+    const double dbase = a * bb * invT * invT * eb - ec * ic;
+    const double lb = log(base);
+    b.F = d * exp(X * lb + e * lnT);
+    b.dF_dPr = b.F * lb * (-2.0 * L * X * X) * ILN10 / Pr;
+    b.dF_dT = b.F * (X * dbase / base + e * invT);
+  }
+  return b;
+}
+
+// ---------------------------------------------------------------------------------------------------
+// phases 0 and 1, shared by the source-term and the Jacobian kernels
+// ---------------------------------------------------------------------------------------------------
+template <int S, bool JAC>
+struct Tile {
+  double *sc, *C, *gRT, *hRT, *Et, *ct, *ck, *dE, *P, *red;
+  __device__ __forceinline__ Tile(double* smem, int ns, int nr, int nslots) {
+    sc = smem; C = sc + NSC * S; gRT = C + ns * S; hRT = gRT + ns * S; Et = hRT + ns * S; ct = Et + ns * S;
+    ck = ct + ns * S; dE = ck + ns * S; P = JAC ? dE + nr * S : dE; red = P + (JAC ? nslots : nr) * S;
+    // source kernel: dE unused, P[r] = q_r
+  }
+};
+
+// element offset of (element e, state s) in the library layout; base_s precomputed per thread
+__device__ __forceinline__ int64_t state_base(int64_t s, int64_t tile, int64_t n_e) { return (s / tile) * (n_e * tile) + (s % tile); }
+
+template <int S, bool JAC>
+__device__ __forceinline__ void phases01(const DevMech& m, Tile<S, JAC>& t, int mode, int64_t s0, int64_t n_states,
+                                         int64_t tile, const double* __restrict__ phi, const double* __restrict__ param) {
+  const int tid = threadIdx.x;
+  const int ns = m.ns, nr = m.nr, L = ns - 1;
+  const int s = tid % S;                        // NT % S == 0: a thread keeps its state in every loop
+  const int64_t sg = min(s0 + s, n_states - 1);  // ragged tail: recompute the last valid state, never store
+  const int64_t pbase = state_base(sg, tile, ns + 1);
+  // ---- phase 0a: scalars -------------------------------------------------------------------------
+  if (tid < S) {
+    const double T = phi[pbase], E = phi[pbase + tile], par = param[sg];
+    const double V = mode == PYJAC_CONP ? E : par, Pp = mode == PYJAC_CONP ? par : E;
+    t.sc[SC_T * S + s] = T; t.sc[SC_V * S + s] = V; t.sc[SC_P * S + s] = Pp;
+    t.sc[SC_CTOT * S + s] = Pp / (R_GAS * T);
+  }
+  __syncthreads();
+  const double T = t.sc[SC_T * S + s], V = t.sc[SC_V * S + s], Pp = t.sc[SC_P * S + s], Ctot = t.sc[SC_CTOT * S + s];
+  const double invT = 1.0 / T, lnT = log(T), RT = R_GAS * T;
+  // ---- phase 0b: species: C_k = n_k / V (Eq. 6), NASA-7 thermo (R2) --------------------------
+  {
+    double acc[3] = {0.0, 0.0, 0.0};
+    const double invV = 1.0 / V;
+    const double T2 = T * T, T3 = T2 * T, T4 = T3 * T;
+    for (int idx = tid; idx < ns * S; idx += NT) {
+      const int k = idx / S;
+      const double* __restrict__ a = m.nasa + 16 * k;
+      a += (T <= a[0]) ? 1 : 8;                      // low range iff T <= T_mid (R3); per-lane select
+      const double a0 = a[0], a1 = a[1], a2 = a[2], a3 = a[3], a4 = a[4], a5 = a[5], a6 = a[6];
+      const double cpR = a0 + a1 * T + a2 * T2 + a3 * T3 + a4 * T4;
+      const double dcpR = a1 + 2.0 * a2 * T + 3.0 * a3 * T2 + 4.0 * a4 * T3;
+      const double hRT = a0 + a1 * T * 0.5 + a2 * T2 * (1.0 / 3.0) + a3 * T3 * 0.25 + a4 * T4 * 0.2 + a5 * invT;
+      const double sR = a0 * lnT + a1 * T + a2 * T2 * 0.5 + a3 * T3 * (1.0 / 3.0) + a4 * T4 * 0.25 + a6;
+      const double c = R_GAS * (mode == PYJAC_CONP ? cpR : cpR - 1.0);   // c_p or c_v = c_p - R
+      t.gRT[idx] = hRT - sR;
+      t.hRT[idx] = hRT;
+      t.ck[idx] = c;
+      if (k < L) {
+        const double Ck = phi[pbase + (int64_t)(2 + k) * tile] * invV;
+        t.C[idx] = Ck;
+        acc[0] += Ck; acc[1] += Ck * c; acc[2] += Ck * (R_GAS * dcpR);
+      } else {
+        t.sc[SC_CNS * S + s] = R_GAS * dcpR;          // c'_Ns, consumed right below
+      }
+    }
+    block_reduce<S, 3>(acc, t.red, t.sc, SC_SUMC);
+    if (tid < S) {      // last species from the ideal-gas law, D and dD/dT sums over all species
+      const double CL = Ctot - t.sc[SC_SUMC * S + s];
+      t.C[L * S + s] = CL;
+      t.sc[SC_D * S + s] = t.sc[SC_SUMCC * S + s] + CL * t.ck[L * S + s];
+      t.sc[SC_DDDT * S + s] = t.sc[SC_SUMCDC * S + s] + CL * t.sc[SC_CNS * S + s];
+    }
+    __syncthreads();
+    // E~_k = E_k - (W_k/W_Ns) E_Ns, c~_k likewise (mass conservation folds the last species in, R1/A1)
+    const double eL = t.hRT[L * S + s] - (mode == PYJAC_CONP ? 0.0 : 1.0), cL = t.ck[L * S + s];
+    for (int idx = tid; idx < ns * S; idx += NT) {
+      const int k = idx / S;
+      const double w = m.wr[k];
+      const double e = t.hRT[idx] - (mode == PYJAC_CONP ? 0.0 : 1.0);
+      t.Et[idx] = k == L ? 0.0 : RT * (e - w * eL);
+      t.ct[idx] = k == L ? 0.0 : t.ck[idx] - w * cL;
+    }
+    __syncthreads();
+  }
+  // ---- phase 1: reactions ----------------------------------------------------------------------------
+  const double lnP = log(Pp);
+  const double ln_patm_rt = log(P_ATM / RT);
+  const double ctot_T = Ctot * invT;
+  double acc[7] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+  for (int idx = tid; idx < nr * S; idx += NT) {
+    const int r = idx / S;
+    const int info = m.info[r];
+    const int type = info & INFO_TYPE_MASK;
+    const bool rev = info & INFO_REV;
+    // a3: forward rate constant
+    double lnkf, lam_f, dlnk_dP = 0.0;
+    if (type <= PYJAC_FALLOFF_SRI) {
+      const double beta = m.beta[r], Ta = m.Ta[r];
+      lnkf = m.lnA[r] + beta * lnT - Ta * invT;
+      lam_f = (beta + Ta * invT) * invT;
+    } else if (type == PYJAC_PLOG) {
+      const int a = m.aux[r], p0 = m.plog_ptr[a], np = m.plog_ptr[a + 1] - p0;
+      int j = 0;
+      bool interp = true;
+      if (Pp <= m.plog_P[p0]) { interp = false; }
+      else if (Pp >= m.plog_P[p0 + np - 1]) { interp = false; j = np - 1; }
+      else { while (j + 2 < np && m.plog_P[p0 + j + 1] <= Pp) ++j; }     // last j with P_j <= P (R-S4)
+      const double b0 = m.plog_b[p0 + j], Ta0 = m.plog_Ta[p0 + j];
+      const double l0 = m.plog_lnA[p0 + j] + b0 * lnT - Ta0 * invT;
+      const double lam0 = (b0 + Ta0 * invT) * invT;
+      lnkf = l0; lam_f = lam0;
+      if (interp) {
+        const double b1 = m.plog_b[p0 + j + 1], Ta1 = m.plog_Ta[p0 + j + 1];
+        const double l1 = m.plog_lnA[p0 + j + 1] + b1 * lnT - Ta1 * invT;
+        const double lam1 = (b1 + Ta1 * invT) * invT;
+        const double idl = 1.0 / (m.plog_lnP[p0 + j + 1] - m.plog_lnP[p0 + j]);
+        const double w = (lnP - m.plog_lnP[p0 + j]) * idl;
+        lnkf = l0 + (l1 - l0) * w;
+        lam_f = (1.0 - w) * lam0 + w * lam1;
+        dlnk_dP = (l1 - l0) * idl / Pp;
+      }
+    } else {
+      const double LN10 = 2.302585092994045684, ILN10 = 0.434294481903251828;
+      const int a = m.aux[r];
+      const int nT = m.cheb_meta[4 * a], nP = m.cheb_meta[4 * a + 1];
+      const double* __restrict__ eta = m.cheb_coef + m.cheb_meta[4 * a + 2];
+      const double iTmin = m.cheb_lim[4 * a], iTmax = m.cheb_lim[4 * a + 1], lPmin = m.cheb_lim[4 * a + 2], lPmax = m.cheb_lim[4 * a + 3];
+      const double Tr = (2.0 * invT - iTmin - iTmax) / (iTmax - iTmin);
+      const double Pr_ = (2.0 * lnP * ILN10 - lPmin - lPmax) / (lPmax - lPmin);
+      double lg = 0.0, dlg_dT = 0.0, dlg_dP = 0.0;
+      double cT = 1.0, cTm = 0.0, dT = 0.0, dTm = 0.0;       // T_a(Tr), T_{a-1}, derivatives
+      for (int ia = 0; ia < nT; ++ia) {
+        if (ia == 1) { cTm = 1.0; cT = Tr; dTm = 0.0; dT = 1.0; }
+        else if (ia > 1) {
+          const double n1 = 2.0 * Tr * cT - cTm, d1 = 2.0 * cT + 2.0 * Tr * dT - dTm;
+          cTm = cT; cT = n1; dTm = dT; dT = d1;
+        }
+        double cP = 1.0, cPm = 0.0, dP = 0.0, dPm = 0.0;
+        double sv = 0.0, sd = 0.0;
+        for (int ib = 0; ib < nP; ++ib) {
+          if (ib == 1) { cPm = 1.0; cP = Pr_; dPm = 0.0; dP = 1.0; }
+          else if (ib > 1) {
+            const double n1 = 2.0 * Pr_ * cP - cPm, d1 = 2.0 * cP + 2.0 * Pr_ * dP - dPm;
+            cPm = cP; cP = n1; dPm = dP; dP = d1;
+          }
+          const double e = eta[ia * nP + ib];
+          sv += e * cP; sd += e * dP;
+        }
+        lg += cT * sv; dlg_dT += dT * sv; dlg_dP += cT * sd;
+      }
+      lnkf = LN10 * lg;
+      lam_f = LN10 * dlg_dT * (-2.0 * invT * invT / (iTmax - iTmin));
+      dlnk_dP = dlg_dP * 2.0 / (Pp * (lPmax - lPmin));
+    }
+    const double kf = exp(lnkf);
+    // stoichiometry: concentrations, products and one-factor-removed products (no division by C_k: R-S7)
+    const uint4 w0 = *reinterpret_cast<const uint4*>(m.sp + 8 * r);
+    const uint2 w1 = *reinterpret_cast<const uint2*>(m.sp + 8 * r + 4);
+    const uint32_t spw[6] = {w0.x, w0.y, w0.z, w0.w, w1.x, w1.y};
+    double pw[6], pm[6];
+    double dg = 0.0, dh = 0.0, dEt = 0.0, dct = 0.0;
+#pragma unroll
+    for (int a = 0; a < 6; ++a) {
+      const int nu = spw[a] >> 16, k = spw[a] & 0xffff;
+      const double Ck = nu ? t.C[k * S + s] : 1.0;
+      pw[a] = ipow(Ck, nu); pm[a] = dpow(Ck, nu);
+      const double snu = a < 3 ? -(double)nu : (double)nu;
+      if (nu) {
+        if (rev) { dg += snu * t.gRT[k * S + s]; dh += snu * t.hRT[k * S + s]; }
+        dEt += snu * t.Et[k * S + s];
+        if (JAC) dct += snu * t.ct[k * S + s];
+      }
+    }
+    const double Pif = pw[0] * pw[1] * pw[2], Pir = pw[3] * pw[4] * pw[5];
+    double kr = 0.0, lam_r = 0.0;
+    if (rev) {      // a4: K_c from Gibbs polynomials; k_r = k_f / K_c = exp(ln k_f - ln K_c)
+      const double snu = (double)(((info >> INFO_SNU_SHIFT) & 15) - 8);
+      kr = exp(lnkf + dg - snu * ln_patm_rt);
+      lam_r = lam_f - (dh - snu) * invT;
+    }
+    const double Rf = kf * Pif, Rr = kr * Pir, Rn = Rf - Rr;
+    const double dRdT = lam_f * Rf - lam_r * Rr;
+    // a5: third body / falloff
+    double c = 1.0, X = 0.0, GT = dRdT, MdcdM_R = 0.0;
+    const int e0 = m.eff_ptr[r], e1 = m.eff_ptr[r + 1];
+    const double adef = (info & INFO_ADEF) ? 1.0 : 0.0;
+    if (type >= PYJAC_THIRD_BODY && type <= PYJAC_FALLOFF_SRI) {
+      double M = adef * Ctot;                       // sum_k C_k == C_tot by construction of C_Ns
+      for (int e = e0; e < e1; ++e) M += m.eff_d[e] * t.C[m.eff_sp[e] * S + s];
+      if (type == PYJAC_THIRD_BODY) {
+        c = M; X = Rn; GT = M * dRdT; MdcdM_R = M * Rn;
+      } else {
+        const double* __restrict__ fp = m.fall + 12 * m.aux[r];
+        const double b0 = fp[1], Ta0 = fp[2];
+        const double k0_kinf = exp(fp[0] + b0 * lnT - Ta0 * invT - lnkf);
+        const double Pr = k0_kinf * M;
+        const Blend bl = blend(type, info & INFO_T2, fp, T, invT, lnT, Pr);
+        const double i1p = 1.0 / (1.0 + Pr);
+        c = bl.F * Pr * i1p;
+        const double dc_dPr = bl.F * i1p * i1p + Pr * i1p * bl.dF_dPr;
+        const double dPr_dT = Pr * (b0 - m.beta[r] + (Ta0 - m.Ta[r]) * invT) * invT;
+        X = dc_dPr * k0_kinf * Rn;
+        GT = (dc_dPr * dPr_dT + Pr * i1p * bl.dF_dT) * Rn + c * dRdT;
+        MdcdM_R = Pr * dc_dPr * Rn;
+      }
+    }
+    const double q = c * Rn;
+    // reaction-sum reductions (R4-7/8): N = sum dE~_i q_i, S = sum dn~_i q_i
+    const double dn = m.dn[r];
+    acc[0] += dEt * q; acc[1] += dn * q;
+    if (!JAC) {
+      t.P[idx] = q;
+    } else {
+      // a8: per-reaction partials -> slots
+      const int base = m.slot_base[r];
+      const int nre = (info >> INFO_NREAC_SHIFT) & 3, npr = (info >> INFO_NPROD_SHIFT) & 3;
+      const double a_ = c * kf, b_ = c * kr;
+      double GL = adef * X;                          // full dQ_i/dC_Ns
+      const double df[3] = {a_ * pm[0] * pw[1] * pw[2], a_ * pw[0] * pm[1] * pw[2], a_ * pw[0] * pw[1] * pm[2]};
+      const double dr[3] = {-b_ * pm[3] * pw[4] * pw[5], -b_ * pw[3] * pm[4] * pw[5], -b_ * pw[3] * pw[4] * pm[5]};
+      int slot = base + 2;
+#pragma unroll
+      for (int a = 0; a < 3; ++a)
+        if (a < nre) { t.P[(slot++) * S + s] = df[a]; if ((int)(spw[a] & 0xffff) == L) GL += df[a]; }
+      if (rev) {
+#pragma unroll
+        for (int a = 0; a < 3; ++a)
+          if (a < npr) { t.P[(slot++) * S + s] = dr[a]; if ((int)(spw[3 + a] & 0xffff) == L) GL += dr[a]; }
+      }
+      for (int e = e0; e < e1; ++e) {
+        const double v = m.eff_d[e] * X;
+        t.P[(slot++) * S + s] = v;
+        if (m.eff_sp[e] == L) GL += v;
+      }
+      // chain rule to the state variables (R4-2); E column in Euler-homogeneity form (R4-6)
+      const double slotT = V * (GT - ctot_T * GL);
+      double slotE;
+      if (mode == PYJAC_CONP) {
+        const int of = (int)(spw[0] >> 16) + (int)(spw[1] >> 16) + (int)(spw[2] >> 16);
+        const int orv = (int)(spw[3] >> 16) + (int)(spw[4] >> 16) + (int)(spw[5] >> 16);
+        slotE = q - c * ((double)of * Rf - (double)orv * Rr) - MdcdM_R + Ctot * GL;
+      } else {
+        slotE = V * (c * dlnk_dP * Rn + GL / RT);
+      }
+      t.P[base * S + s] = slotT;
+      t.P[(base + 1) * S + s] = slotE;
+      t.dE[idx] = dEt;
+      acc[2] += dEt * slotT; acc[3] += dn * slotT; acc[4] += dEt * slotE; acc[5] += dn * slotE; acc[6] += dct * q;
+    }
+  }
+  if (JAC) block_reduce<S, 7>(acc, t.red, t.sc, SC_R0);
+  else { double a2[2] = {acc[0], acc[1]}; block_reduce<S, 2>(a2, t.red, t.sc, SC_R0); }
+}
+
+}  // namespace
+
+namespace {
+
+// ---------------------------------------------------------------------------------------------------
+// source terms: Eqs. 3-8
+// ---------------------------------------------------------------------------------------------------
+template <int S>
+__global__ void __launch_bounds__(NT, 1)
+source_kernel(const DevMech m, int mode, int64_t n_states, int64_t tile, const double* __restrict__ phi,
+              const double* __restrict__ param, double* __restrict__ out) {
+  extern __shared__ __align__(16) double smem[];
+  Tile<S, false> t(smem, m.ns, m.nr, m.nslots);
+  const int64_t s0 = (int64_t)blockIdx.x * S;
+  phases01<S, false>(m, t, mode, s0, n_states, tile, phi, param);
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, s = lane % S, sub = lane / S;
+  const int L = m.ns - 1;
+  const bool valid = s0 + s < n_states;
+  const int64_t obase = state_base(min(s0 + s, n_states - 1), tile, m.nvar);
+  const double V = t.sc[SC_V * S + s];
+  // a7: omega_k = sum_i nu_ki q_i (Eq. 4), dn_k/dt = V omega_k (Eq. 3); a warp gathers one species
+  for (int k = warp; k < L; k += NW) {
+    const int p1 = m.b_ptr[k + 1];
+    double w = 0.0;
+    for (int p = m.b_ptr[k] + sub; p < p1; p += 32 / S) {
+      const uint32_t ent = (uint32_t)m.bq_ent[p];
+      w += apply_sign(t.P[(ent & ~SIGN_BIT) * S + s], ent);
+    }
+    w = group_sum<S>(w);
+    if (lane < S && valid) out[obase + (int64_t)(2 + k) * tile] = V * w;
+  }
+  if (threadIdx.x < S && valid) {
+    const double T = t.sc[SC_T * S + s], Pp = t.sc[SC_P * S + s];
+    const double fT = -t.sc[SC_R0 * S + s] / t.sc[SC_D * S + s];          // Eq. 5
+    const double Ssum = t.sc[SC_R1 * S + s];
+    const double fE = mode == PYJAC_CONP ? V * (T * R_GAS / Pp * Ssum + fT / T)   // Eq. 8a
+                                         : T * R_GAS * Ssum + Pp / T * fT;        // Eq. 8b
+    out[obase] = fT;
+    out[obase + tile] = fE;
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------
+// Jacobian (sparse CSR / CSC value order or dense 'C' / 'F'), Eq. 9
+// ---------------------------------------------------------------------------------------------------
+template <int S>
+__global__ void __launch_bounds__(NT, 1)
+jacobian_kernel(const DevMech m, const DevPlan pl, int mode, int64_t n_states, int64_t tile, const double* __restrict__ phi,
+                const double* __restrict__ param, double* __restrict__ out) {
+  extern __shared__ __align__(16) double smem[];
+  Tile<S, true> t(smem, m.ns, m.nr, m.nslots);
+  const int64_t s0 = (int64_t)blockIdx.x * S;
+  phases01<S, true>(m, t, mode, s0, n_states, tile, phi, param);
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, s = lane % S, sub = lane / S;
+  const int L = m.ns - 1;
+  const bool valid = s0 + s < n_states;
+  const int64_t obase = state_base(min(s0 + s, n_states - 1), tile, pl.n_e);
+  const double T = t.sc[SC_T * S + s], V = t.sc[SC_V * S + s], Pp = t.sc[SC_P * S + s], D = t.sc[SC_D * S + s];
+  const double N = t.sc[SC_R0 * S + s], Ssum = t.sc[SC_R1 * S + s];
+  const double fT = -N / D;
+  // dense output: structural zeros, each stored once (no memset pass)
+  if (pl.nzmask != nullptr) {
+    const int n2 = m.nvar * m.nvar;
+    for (int idx = tid; idx < n2 * S; idx += NT) {
+      const int e = idx / S;
+      if (!((pl.nzmask[e >> 5] >> (e & 31)) & 1u) && valid) out[obase + (int64_t)e * tile] = 0.0;
+    }
+  }
+  // a9: species block, J[k][j] = sum_i nu_ki (Ghat^j_i - Ghat^Ns_i): gather the static list, store once
+  for (int idx = tid; idx < pl.nA * S; idx += NT) {
+    const int e = idx / S;
+    const int p1 = pl.a_ptr[e + 1];
+    double v = 0.0;
+    for (int p = pl.a_ptr[e]; p < p1; ++p) {
+      const uint32_t ent = (uint32_t)pl.a_ent[p];
+      v += apply_sign(t.P[(ent & ~SIGN_BIT) * S + s], ent);
+    }
+    if (valid) out[obase + (int64_t)pl.a_pos[e] * tile] = v;
+  }
+  // a9: T and E columns of the species rows: J[k][T] = sum_i nu_ki slotT_i, J[k][E] = sum_i nu_ki slotE_i
+  for (int k = warp; k < L; k += NW) {
+    const int p1 = m.b_ptr[k + 1];
+    double vT = 0.0, vE = 0.0;
+    for (int p = m.b_ptr[k] + sub; p < p1; p += 32 / S) {
+      const uint32_t ent = (uint32_t)m.b_ent[p];
+      const int off = (ent & ~SIGN_BIT) * S + s;
+      vT += apply_sign(t.P[off], ent);
+      vE += apply_sign(t.P[off + S], ent);
+    }
+    vT = group_sum<S>(vT); vE = group_sum<S>(vE);
+    if (lane < S && valid) {
+      out[obase + (int64_t)pl.b_pos[k] * tile] = vT;
+      out[obase + (int64_t)pl.b_pos[L + k] * tile] = vE;
+    }
+  }
+  // a10: T and E rows, species columns: gather over reactions with the per-state weights dE~_i, dn~_i
+  const double cL = t.ck[L * S + s];
+  const double iDV = 1.0 / (D * V);
+  for (int j = warp; j < L; j += NW) {
+    const int p1 = m.c_ptr[j + 1];
+    double vT = 0.0, vS = 0.0;
+    for (int p = m.c_ptr[j] + sub; p < p1; p += 32 / S) {
+      const int2 pr = reinterpret_cast<const int2*>(m.c_ent)[p];
+      const uint32_t ent = (uint32_t)pr.x;
+      const double x = apply_sign(t.P[(ent & ~SIGN_BIT) * S + s], ent);
+      vT += t.dE[pr.y * S + s] * x;
+      vS += m.dn[pr.y] * x;
+    }
+    vT = group_sum<S>(vT); vS = group_sum<S>(vS);
+    if (lane < S && valid) {
+      const double JT = -(vT + fT * (t.ck[j * S + s] - cL)) * iDV;
+      const double JE = mode == PYJAC_CONP ? T * R_GAS * vS / Pp + V * JT / T : T * R_GAS * vS / V + Pp / T * JT;
+      out[obase + (int64_t)pl.c_pos[j] * tile] = JT;
+      out[obase + (int64_t)pl.c_pos[L + j] * tile] = JE;
+    }
+  }
+  // a10: the four corner entries from the phase-1 reductions (R4-7)
+  if (tid < S && valid) {
+    const double Ctot = t.sc[SC_CTOT * S + s];
+    const double AT = t.sc[SC_R2 * S + s], BT = t.sc[SC_R3 * S + s], AE = t.sc[SC_R4 * S + s], BE = t.sc[SC_R5 * S + s];
+    const double sumcw = t.sc[SC_R6 * S + s];
+    const double iV = 1.0 / V;
+    const double dN_dT = AT * iV + sumcw;
+    const double dD_dT = t.sc[SC_DDDT * S + s] - cL * Ctot / T;
+    const double JTT = -(dN_dT + fT * dD_dT) / D;
+    const double dS_dT = BT * iV;
+    double dN_dE, dD_dE, dS_dE, JET, JEE, JTE;
+    if (mode == PYJAC_CONP) {
+      const double fE = V * (T * R_GAS / Pp * Ssum + fT / T);
+      dN_dE = (AE - N) * iV; dD_dE = -(D - Ctot * cL) * iV; dS_dE = (BE - Ssum) * iV;
+      JTE = -(dN_dE + fT * dD_dE) / D;
+      JET = V * (T * R_GAS / Pp * dS_dT + JTT / T) + V * (R_GAS * Ssum / Pp - fT / (T * T));
+      JEE = V * (T * R_GAS / Pp * dS_dE + JTE / T) + fE * iV;
+    } else {
+      dN_dE = AE * iV; dD_dE = cL / (R_GAS * T); dS_dE = BE * iV;
+      JTE = -(dN_dE + fT * dD_dE) / D;
+      JET = T * R_GAS * dS_dT + Pp / T * JTT + R_GAS * Ssum - Pp * fT / (T * T);
+      JEE = T * R_GAS * dS_dE + Pp / T * JTE + fT / T;
+    }
+    out[obase + (int64_t)pl.d_pos[0] * tile] = JTT;
+    out[obase + (int64_t)pl.d_pos[1] * tile] = JTE;
+    out[obase + (int64_t)pl.d_pos[2] * tile] = JET;
+    out[obase + (int64_t)pl.d_pos[3] * tile] = JEE;
+  }
+}
+
+template <int S> int launch_source_S(const DevMech& m, const LaunchCfg& cfg, int mode, int64_t n, int64_t tile,
+                                     const double* phi, const double* param, double* out, cudaStream_t st) {
+  const int64_t blocks = (n + S - 1) / S;
+  source_kernel<S><<<(unsigned)blocks, NT, cfg.smem, st>>>(m, mode, n, tile, phi, param, out);
+  return (int)cudaGetLastError();
+}
+template <int S> int launch_jac_S(const DevMech& m, const DevPlan& p, const LaunchCfg& cfg, int mode, int64_t n, int64_t tile,
+                                  const double* phi, const double* param, double* out, cudaStream_t st) {
+  const int64_t blocks = (n + S - 1) / S;
+  jacobian_kernel<S><<<(unsigned)blocks, NT, cfg.smem, st>>>(m, p, mode, n, tile, phi, param, out);
+  return (int)cudaGetLastError();
+}
+
+constexpr size_t SMEM_LIMIT = 227 * 1024;
+
+}  // namespace
+
+LaunchCfg choose_cfg(const HostTables& h, bool jac, int64_t tile, int64_t n_states) {
+  LaunchCfg cfg{1, NT, 0};
+  for (int S = 32; S >= 1; S >>= 1) {
+    const size_t bytes = smem_doubles(h.ns, h.nr, h.nslots, S, jac) * sizeof(double);
+    cfg.S = S; cfg.smem = bytes;
+    if (bytes > SMEM_LIMIT) continue;
+    if ((int64_t)S > tile) continue;                       // lanes of one item must stay inside one tile
+    if (S > 1 && (n_states + S - 1) / S < 2 * 148) continue;  // small batches: spread over the 148 SMs first
+    break;
+  }
+  return cfg;
+}
+
+int launch_source(const DevMech& m, const LaunchCfg& cfg, int mode, int64_t n_states, int64_t ld, int64_t tile,
+                  const double* phi, const double* param, double* out, void* stream) {
+  (void)ld;
+  cudaStream_t st = (cudaStream_t)stream;
+  switch (cfg.S) {
+    case 1: return launch_source_S<1>(m, cfg, mode, n_states, tile, phi, param, out, st);
+    case 2: return launch_source_S<2>(m, cfg, mode, n_states, tile, phi, param, out, st);
+    case 4: return launch_source_S<4>(m, cfg, mode, n_states, tile, phi, param, out, st);
+    case 8: return launch_source_S<8>(m, cfg, mode, n_states, tile, phi, param, out, st);
+    case 16: return launch_source_S<16>(m, cfg, mode, n_states, tile, phi, param, out, st);
+    default: return launch_source_S<32>(m, cfg, mode, n_states, tile, phi, param, out, st);
+  }
+}
+
+int launch_jacobian(const DevMech& m, const DevPlan& p, const LaunchCfg& cfg, int mode, int64_t n_states, int64_t ld,
+                    int64_t tile, const double* phi, const double* param, double* out, void* stream) {
+  (void)ld;
+  cudaStream_t st = (cudaStream_t)stream;
+  switch (cfg.S) {
+    case 1: return launch_jac_S<1>(m, p, cfg, mode, n_states, tile, phi, param, out, st);
+    case 2: return launch_jac_S<2>(m, p, cfg, mode, n_states, tile, phi, param, out, st);
+    case 4: return launch_jac_S<4>(m, p, cfg, mode, n_states, tile, phi, param, out, st);
+    case 8: return launch_jac_S<8>(m, p, cfg, mode, n_states, tile, phi, param, out, st);
+    case 16: return launch_jac_S<16>(m, p, cfg, mode, n_states, tile, phi, param, out, st);
+    default: return launch_jac_S<32>(m, p, cfg, mode, n_states, tile, phi, param, out, st);
+  }
+}
+
+template <int S> static int set_attr_S() {
+  cudaError_t e = cudaFuncSetAttribute(source_kernel<S>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_LIMIT);
+  if (e != cudaSuccess) return (int)e;
+  return (int)cudaFuncSetAttribute(jacobian_kernel<S>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_LIMIT);
+}
+
+int set_kernel_attributes() {
+  int e;
+  if ((e = set_attr_S<1>())) return e;
+  if ((e = set_attr_S<2>())) return e;
+  if ((e = set_attr_S<4>())) return e;
+  if ((e = set_attr_S<8>())) return e;
+  if ((e = set_attr_S<16>())) return e;
+  return set_attr_S<32>();
+}
+
+}  // namespace pyjac
