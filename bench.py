@@ -1,0 +1,295 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the hot path on B200 (contract: see README / DESIGN.md "Measurement").
+
+Default workload = BASELINE.json configs[4] (C5): synthetic 360-species / 2172-reaction mechanism,
+2^18 fp64 states, CONP, sparse Jacobian in CSR value order.  One "step" = one pass of the whole hot
+path (steps a1-a11: concentrations, thermo, rate constants, falloff, rates of progress, per-reaction
+partials, species rows, T/E rows, store) over the batch = one pyjac_jacobian_sparse call.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 5] [--impl reference]
+
+Prints ONE JSON line.  `--impl reference` times the CPU oracle (oracle/) on the host cores instead.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import mechgen as mg  # noqa: E402
+from mechgen.mechanism import CONFIGS, pack_phi  # noqa: E402
+
+METRIC = "sparse Jacobian evals/s (states/s) and achieved HBM GB/s vs roofline"
+UNIT = "states/s"
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, copy read+write)"
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def ncu_traffic(config):
+    """dram bytes per launch of the Jacobian kernel from the committed ncu summary, if present."""
+    p = os.path.join(ROOT, "profiles", "r01_traffic.json")
+    if os.path.exists(p):
+        try:
+            return json.load(open(p)).get("c%d" % config)
+        except Exception:
+            return None
+    return None
+
+
+class ClockSampler:
+    """Samples nvidia-smi SM clocks and throttle reasons during the timed region."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+         "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index):
+        self.idx = gpu_index
+        self.samples = []
+        self.stop = False
+        self.th = threading.Thread(target=self._run, daemon=True)
+
+    def _run(self):
+        while not self.stop:
+            try:
+                out = subprocess.run(["nvidia-smi", "-i", str(self.idx), "--query-gpu=" + self.Q,
+                                      "--format=csv,noheader,nounits"], capture_output=True, text=True, timeout=5).stdout
+                f = [x.strip() for x in out.strip().split(",")]
+                if len(f) >= 9:
+                    self.samples.append(f)
+            except Exception:
+                pass
+            time.sleep(0.1)
+
+    def __enter__(self):
+        self.th.start()
+        return self
+
+    def __exit__(self, *a):
+        self.stop = True
+        self.th.join(timeout=6)
+
+    def summary(self):
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["unsampled"]}
+        sm = sorted(float(s[1]) for s in self.samples)
+        reasons = set()
+        for s in self.samples:
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), s[5:9]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": float(self.samples[0][2]), "reasons": sorted(reasons),
+                "samples": len(sm), "power_w_max": max(float(s[3]) for s in self.samples)}
+
+
+def oracle_rate(c, mode, what, target_s=12.0):
+    """Times the oracle as it stands on a bounded sample; returns (states/s, threads, n_sample)."""
+    from oracle import Oracle
+    o = Oracle(mg.config_mechanism(c))
+    n = 2 * o.threads
+    while True:
+        st = mg.config_states(c, n)
+        phi, par = o.pack(st, mode)
+        t0 = time.perf_counter()
+        if what == "sparse":
+            o.jacobian_sparse(mode, mg.CSR, phi, par)
+        elif what == "dense":
+            o.jacobian_dense(mode, phi, par)
+        else:
+            o.source(mode, phi, par)
+        dt = time.perf_counter() - t0
+        if dt >= 0.25 * target_s or n >= (1 << 16):
+            return n / dt, o.threads, n, dt
+        n = int(min(1 << 16, max(2 * n, n * 0.6 * target_s / max(dt, 1e-3))))
+
+
+def run_reference(args, rank, world):
+    if rank != 0:
+        return
+    c = args.config
+    cfg = CONFIGS[c]
+    what = "dense" if c in (1, 4) else "sparse"
+    vals, info = [], None
+    for i in range(args.warmup + args.steps):
+        r, threads, n, dt = oracle_rate(c, cfg["mode"], what, target_s=max(2.0, 40.0 / (args.warmup + args.steps)))
+        if i >= args.warmup:
+            vals.append((n, dt))
+        info = (threads, n)
+    tot_n = sum(v[0] for v in vals); tot_t = sum(v[1] for v in vals)
+    value = tot_n / tot_t
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * tot_t / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": workload_config(c, what, None, None),
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": info[0], "kind": "oracle",
+                             "sample": "%d states of the workload per step (oracle/, OpenMP over states)" % info[1]},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+def workload_config(c, what, tile, S):
+    cfg = CONFIGS[c]
+    return {"workload": "C%d: synthetic %d-species / %d-reaction mechanism, %d fp64 states, %s, %s Jacobian%s" % (
+        c, cfg["ns"], cfg["nr"], cfg["n_states"], "CONP" if cfg["mode"] == mg.CONP else "CONV", what,
+        " (CSR value order)" if what == "sparse" else " (row-major)"),
+        "n_states_per_gpu": cfg["n_states"], "layout_tile": tile, "states_per_cta": S,
+        "l2": "inputs+outputs larger than L2 (no flush needed)" if cfg["n_states"] * 8 * 1000 > 126e6 else "l2_flush_between_steps"}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=5)
+    ap.add_argument("--impl", default="b200")
+    ap.add_argument("--states", type=int, default=None, help="override states per GPU (sweeps)")
+    ap.add_argument("--tile", type=int, default=None, help="override layout tile (default: states per CTA)")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true")
+    args = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        return run_reference(args, rank, world)
+
+    import torch
+    import torch.distributed as dist
+    import paper_1809_01029_b200 as pj
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    c = args.config
+    cfg = CONFIGS[c]
+    mode = cfg["mode"]
+    what = "dense" if c in (1, 4) else "sparse"
+    N = args.states or cfg["n_states"]
+    mech = mg.config_mechanism(c)
+    M = pj.Mechanism(mech, local)
+    S, threads, smem = pj.pyjac_launch_info(M.h, pj.WHAT_SPARSE)
+    tile = args.tile or S
+    ld = (N + tile - 1) // tile * tile
+    n_e = M.nnz if what == "sparse" else M.nvar * M.nvar
+    # weak scaling: every rank owns its own N states (independent problems, no collective on the data path)
+    states = mg.config_states(c, N, start=rank * N)
+    phi_h, par_h = pack_phi(states, mode, ld, tile)
+    d_phi = torch.from_numpy(phi_h).cuda(); d_par = torch.from_numpy(par_h).cuda()
+    d_out = torch.empty(n_e * ld, dtype=torch.float64, device="cuda")
+    d_src = torch.empty(M.nvar * ld, dtype=torch.float64, device="cuda")
+    stream = torch.cuda.current_stream()
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda") if N * n_e * 8 < 512e6 else None
+
+    def step():
+        if what == "sparse":
+            pj.pyjac_jacobian_sparse(M.h, mode, pj.PYJAC_CSR, N, ld, tile, d_phi.data_ptr(), d_par.data_ptr(), d_out.data_ptr(), stream.cuda_stream)
+        else:
+            pj.pyjac_jacobian_dense(M.h, mode, "C", N, ld, tile, d_phi.data_ptr(), d_par.data_ptr(), d_out.data_ptr(), stream.cuda_stream)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(3, args.warmup)):
+        step()
+    barrier()
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    with ClockSampler(local) as clk:
+        barrier()
+        t0 = torch.cuda.Event(enable_timing=True); t1 = torch.cuda.Event(enable_timing=True)
+        t0.record(stream)
+        for a, b in evs:
+            if flush is not None:
+                flush.zero_()
+            a.record(stream); step(); b.record(stream)
+        t1.record(stream)
+        barrier()
+    kern_ms = [a.elapsed_time(b) for a, b in evs]
+    total_ms = sum(kern_ms) if flush is not None else t0.elapsed_time(t1)
+    tt = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+    total_ms = float(tt.item())
+    value = world * N * args.steps / (total_ms * 1e-3)
+    kavg_ms = float(np.mean(kern_ms))
+    alg_bytes = (8 * n_e + 8 * (M.ns + 2)) * N            # read phi+param once, write each output once
+    peak, peak_src = measured_peaks()
+    achieved = alg_bytes / (kavg_ms * 1e-3) / 1e9
+
+    # source terms, timed separately (BASELINE.json configs[4])
+    for _ in range(3):
+        pj.pyjac_source_terms(M.h, mode, N, ld, tile, d_phi.data_ptr(), d_par.data_ptr(), d_src.data_ptr(), stream.cuda_stream)
+    torch.cuda.synchronize()
+    a = torch.cuda.Event(enable_timing=True); b = torch.cuda.Event(enable_timing=True)
+    a.record(stream)
+    for _ in range(5):
+        pj.pyjac_source_terms(M.h, mode, N, ld, tile, d_phi.data_ptr(), d_par.data_ptr(), d_src.data_ptr(), stream.cuda_stream)
+    b.record(stream); torch.cuda.synchronize()
+    src_ms = a.elapsed_time(b) / 5
+
+    # e2e: the C-ABI call on HOST buffers, H2D + kernel + D2H inside the timed region (pinned memory)
+    e2e = None
+    if not args.no_e2e:
+        n2 = N
+        try:
+            h_out = torch.empty(n_e * ld, dtype=torch.float64).pin_memory()
+        except Exception:
+            n2 = min(N, 1 << 15); h_out = torch.empty(n_e * ld, dtype=torch.float64)
+        h_phi = torch.from_numpy(phi_h).pin_memory(); h_par = torch.from_numpy(par_h).pin_memory()
+        w = pj.WHAT_SPARSE if what == "sparse" else pj.WHAT_DENSE
+        f = pj.PYJAC_CSR if what == "sparse" else "C"
+        e_steps = max(1, min(args.steps, 3))
+        pj.pyjac_eval_host(M.h, w, mode, f, n2, ld, tile, h_phi.numpy(), h_par.numpy(), h_out.numpy())
+        barrier()
+        t_0 = time.perf_counter()
+        for _ in range(e_steps):
+            pj.pyjac_eval_host(M.h, w, mode, f, n2, ld, tile, h_phi.numpy(), h_par.numpy(), h_out.numpy())
+        torch.cuda.synchronize()
+        dt = time.perf_counter() - t_0
+        tt = torch.tensor([dt], dtype=torch.float64, device="cuda")
+        if world > 1:
+            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        e2e = {"value": world * n2 * e_steps / float(tt.item()), "unit": UNIT,
+               "h2d_bytes_per_step": int(8 * (M.nvar + 1) * n2), "d2h_bytes_per_step": int(8 * n_e * n2),
+               "steps": e_steps, "api": "pyjac_eval_host (chunked, double-buffered, pinned host buffers)"}
+        del h_out
+
+    if rank == 0:
+        cpu = None
+        if not args.no_cpu:
+            r, threads_cpu, n_s, dt = oracle_rate(c, mode, what)
+            cpu = {"value": r, "unit": UNIT, "cores": threads_cpu, "kind": "oracle",
+                   "sample": "%d states of the same workload in %.1f s (oracle/, OpenMP over states)" % (n_s, dt)}
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(3, args.warmup),
+                "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                "dtype": "f64", "data": "synthetic", "config": workload_config(c, what, tile, S),
+                "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                             "traffic": ncu_traffic(c), "peak_source": peak_src, "kernel": "jacobian_kernel<S=%d>" % S,
+                             "algorithmic_bytes_per_state": 8 * n_e + 8 * (M.ns + 2), "kernel_ms": kavg_ms,
+                             "ns_per_state": 1e6 * kavg_ms / N},
+                "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": args.steps, "clocks": clk.summary(),
+                "extra": {"source_terms_states_per_s": N / (src_ms * 1e-3), "source_terms_ms": src_ms,
+                          "nnz": M.nnz, "smem_bytes_per_cta": smem, "threads_per_cta": threads}}
+        print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -189,35 +189,85 @@ int pyjac_launch_info(const pyjac_mech* mech, int what, int32_t* states_per_cta,
   return PYJAC_OK;
 }
 
+// copies `rows` rows of `n_c` states between a host array in the library layout (ld, tile) starting at state c0
+// (c0 % tile == 0) and a device chunk buffer laid out with (ld = chunk, tile = tile_dev)
+static cudaError_t copy_chunk(bool to_device, double* dev, const double* host_c, double* host, int64_t rows, int64_t c0,
+                              int64_t n_c, int64_t ld, int64_t tile, int64_t chunk, int64_t tile_dev, cudaStream_t st) {
+  const cudaMemcpyKind kind = to_device ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToHost;
+  if (tile == ld) {      // pure SoA: rows x n_c block of a rows x ld matrix; device chunk is rows x chunk
+    if (to_device) return cudaMemcpy2DAsync(dev, chunk * 8, host_c + c0, ld * 8, n_c * 8, rows, kind, st);
+    return cudaMemcpy2DAsync(host + c0, ld * 8, dev, chunk * 8, n_c * 8, rows, kind, st);
+  }
+  (void)tile_dev;        // == tile: whole tiles are contiguous runs of rows * tile doubles
+  const int64_t full = n_c / tile, tail = n_c % tile;
+  const int64_t hoff = (c0 / tile) * rows * tile;
+  cudaError_t e = cudaSuccess;
+  if (full) {
+    if (to_device) e = cudaMemcpyAsync(dev, host_c + hoff, full * rows * tile * 8, kind, st);
+    else e = cudaMemcpyAsync(host + hoff, dev, full * rows * tile * 8, kind, st);
+    if (e != cudaSuccess) return e;
+  }
+  if (tail) {            // last partial tile: only the valid state slots (never touch s >= n_states)
+    const int64_t o = full * rows * tile;
+    if (to_device) e = cudaMemcpy2DAsync(dev + o, tile * 8, host_c + hoff + o, tile * 8, tail * 8, rows, kind, st);
+    else e = cudaMemcpy2DAsync(host + hoff + o, tile * 8, dev + o, tile * 8, tail * 8, rows, kind, st);
+  }
+  return e;
+}
+
 int pyjac_eval_host(const pyjac_mech* mech, int what, int mode, int fmt, int64_t n_states, int64_t ld, int64_t tile,
                     const double* h_phi, const double* h_param, double* h_out) {
   if (!mech) return fail(PYJAC_EINVAL, "pyjac_eval_host: null handle");
   if (what < 0 || what > 2) return fail(PYJAC_EINVAL, "pyjac_eval_host: what must be 0, 1 or 2");
   if (n_states < 0 || ld < n_states) return fail(PYJAC_EINVAL, "pyjac_eval_host: bad n_states / ld");
+  if (tile < 1 || (tile != ld && (tile & (tile - 1)) != 0) || (n_states > 0 && ld % tile != 0))
+    return fail(PYJAC_EINVAL, "pyjac_eval_host: tile must be a power of two dividing ld, or equal to ld");
   if (mech->device < 0) return fail(PYJAC_ECUDA, "pyjac_eval_host: host-only handle cannot compute");
   if (n_states == 0) return PYJAC_OK;
   if (!h_phi || !h_param || !h_out) return fail(PYJAC_EINVAL, "pyjac_eval_host: null buffer");
-  const int64_t n_e = what == 0 ? mech->h.nvar : (what == 1 ? mech->h.nnz : (int64_t)mech->h.nvar * mech->h.nvar);
+  const int64_t nvar = mech->h.nvar;
+  const int64_t n_e = what == 0 ? nvar : (what == 1 ? mech->h.nnz : nvar * nvar);
+  // chunked, double-buffered pipeline: H2D(c+1) and D2H(c-1) overlap the kernel of chunk c when the host
+  // buffers are pinned; with pageable memory the copies serialise but the result is the same
+  int64_t chunk = 8192;
+  while (chunk > 256 && chunk * n_e * 8 > (int64_t)1 << 30) chunk >>= 1;     // <= 1 GiB of output per buffer
+  if (tile != ld && tile > chunk) chunk = tile;
+  if (chunk > ld) chunk = ld;
+  if (tile != ld) chunk -= chunk % tile;
+  const int64_t tile_dev = tile == ld ? chunk : tile;
   int prev = 0;
   cudaGetDevice(&prev);
-  double *d_phi = nullptr, *d_param = nullptr, *d_out = nullptr;
+  double *d_phi[2] = {nullptr, nullptr}, *d_param[2] = {nullptr, nullptr}, *d_out[2] = {nullptr, nullptr};
+  cudaStream_t st[2] = {nullptr, nullptr};
   auto body = [&]() -> int {
     CK(cudaSetDevice(mech->device));
-    CK(cudaMalloc(&d_phi, sizeof(double) * mech->h.nvar * ld));
-    CK(cudaMalloc(&d_param, sizeof(double) * ld));
-    CK(cudaMalloc(&d_out, sizeof(double) * n_e * ld));
-    CK(cudaMemcpy(d_phi, h_phi, sizeof(double) * mech->h.nvar * ld, cudaMemcpyHostToDevice));
-    CK(cudaMemcpy(d_param, h_param, sizeof(double) * ld, cudaMemcpyHostToDevice));
-    int rc;
-    if (what == 0) rc = pyjac_source_terms(mech, mode, n_states, ld, tile, d_phi, d_param, d_out, nullptr);
-    else if (what == 1) rc = pyjac_jacobian_sparse(mech, mode, fmt, n_states, ld, tile, d_phi, d_param, d_out, nullptr);
-    else rc = pyjac_jacobian_dense(mech, mode, (char)fmt, n_states, ld, tile, d_phi, d_param, d_out, nullptr);
-    if (rc) return rc;
-    CK(cudaMemcpy(h_out, d_out, sizeof(double) * n_e * ld, cudaMemcpyDeviceToHost));
+    for (int b = 0; b < 2; ++b) {
+      CK(cudaStreamCreateWithFlags(&st[b], cudaStreamNonBlocking));
+      CK(cudaMalloc(&d_phi[b], sizeof(double) * nvar * chunk));
+      CK(cudaMalloc(&d_param[b], sizeof(double) * chunk));
+      CK(cudaMalloc(&d_out[b], sizeof(double) * n_e * chunk));
+    }
+    int b = 0;
+    for (int64_t c0 = 0; c0 < n_states; c0 += chunk, b ^= 1) {
+      const int64_t n_c = n_states - c0 < chunk ? n_states - c0 : chunk;
+      CK(copy_chunk(true, d_phi[b], h_phi, nullptr, nvar, c0, n_c, ld, tile, chunk, tile_dev, st[b]));
+      CK(cudaMemcpyAsync(d_param[b], h_param + c0, n_c * 8, cudaMemcpyHostToDevice, st[b]));
+      int rc;
+      if (what == 0) rc = pyjac_source_terms(mech, mode, n_c, chunk, tile_dev, d_phi[b], d_param[b], d_out[b], st[b]);
+      else if (what == 1) rc = pyjac_jacobian_sparse(mech, mode, fmt, n_c, chunk, tile_dev, d_phi[b], d_param[b], d_out[b], st[b]);
+      else rc = pyjac_jacobian_dense(mech, mode, (char)fmt, n_c, chunk, tile_dev, d_phi[b], d_param[b], d_out[b], st[b]);
+      if (rc) return rc;
+      CK(copy_chunk(false, d_out[b], nullptr, h_out, n_e, c0, n_c, ld, tile, chunk, tile_dev, st[b]));
+    }
+    CK(cudaStreamSynchronize(st[0]));
+    CK(cudaStreamSynchronize(st[1]));
     return PYJAC_OK;
   };
   int rc = body();
-  cudaFree(d_phi); cudaFree(d_param); cudaFree(d_out);
+  for (int b = 0; b < 2; ++b) {
+    if (st[b]) { cudaStreamSynchronize(st[b]); cudaStreamDestroy(st[b]); }
+    cudaFree(d_phi[b]); cudaFree(d_param[b]); cudaFree(d_out[b]);
+  }
   cudaSetDevice(prev);
   return rc;
 }
