@@ -75,8 +75,9 @@ int pyjac_mech_create(const pyjac_mech_desc* desc, int cuda_device, pyjac_mech**
 #define UP(field) if (int r_ = m->upload(h.field, &d.field)) return r_;
     UP(nasa) UP(wr) UP(lnA) UP(beta) UP(Ta) UP(dn) UP(info) UP(aux) UP(sp) UP(eff_ptr) UP(eff_sp) UP(eff_d)
     UP(slot_base) UP(fall) UP(plog_ptr) UP(plog_P) UP(plog_lnP) UP(plog_lnA) UP(plog_b) UP(plog_Ta)
-    UP(cheb_meta) UP(cheb_lim) UP(cheb_coef) UP(b_ptr) UP(b_ent) UP(bq_ent) UP(c_ptr) UP(c_ent)
+    UP(cheb_meta) UP(cheb_lim) UP(cheb_coef) UP(b_ptr) UP(b_ent) UP(bq_ent) UP(c_ptr) UP(c_ent) UP(b_item) UP(c_item)
 #undef UP
+    d.nb_long = h.nb_long; d.nc_long = h.nc_long;
     const int32_t *a_ptr[2], *a_ent[2];
     const uint32_t* mask[2];
     for (int p = 0; p < 2; ++p) {
@@ -86,7 +87,7 @@ int pyjac_mech_create(const pyjac_mech_desc* desc, int cuda_device, pyjac_mech**
     }
     for (int f = 0; f < 4; ++f) {
       DevPlan& pl = m->plan[f];
-      pl.nA = h.nA;
+      pl.nA = h.nA; pl.nA_long = h.nA_long[f & 1];
       pl.n_e = f < 2 ? h.nnz : (int64_t)h.nvar * h.nvar;
       pl.a_ptr = a_ptr[f & 1]; pl.a_ent = a_ent[f & 1];
       if (int r_ = m->upload(h.a_pos[f], &pl.a_pos)) return r_;

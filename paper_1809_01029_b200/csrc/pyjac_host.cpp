@@ -235,11 +235,24 @@ int build_host_tables(const pyjac_mech_desc* d, HostTables& h, std::string& err)
         if (inpat[k][j] && !rowmap[k].count(j)) MECH_FAIL("internal: pattern entry (" << k << "," << j << ") has no gather list");
     }
   }
-  for (int k = 0; k < L; ++k) {
+  // Load balance: items are processed in order of DESCENDING list length, so the
+  // 32 lists of a warp have (nearly) equal length; the few lists longer than LONG_LIST are gathered by a whole
+  // warp with a shuffle reduction instead.
+  auto order_by_len = [](int n, auto len_of, std::vector<int32_t>& order, int& n_long) {
+    order.resize(n);
+    std::iota(order.begin(), order.end(), 0);
+    std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return len_of(a) > len_of(b); });
+    n_long = 0;
+    while (n_long < n && len_of(order[n_long]) > LONG_LIST) ++n_long;
+  };
+  order_by_len(L, [&](int k) { return (int)bl[k].size(); }, h.b_item, h.nb_long);
+  order_by_len(L, [&](int k) { return (int)cl[k].size() / 2; }, h.c_item, h.nc_long);
+  for (int q = 0; q < L; ++q) {
+    const int k = h.b_item[q], j = h.c_item[q];
     h.b_ent.insert(h.b_ent.end(), bl[k].begin(), bl[k].end());
     h.bq_ent.insert(h.bq_ent.end(), bql[k].begin(), bql[k].end());
     h.b_ptr.push_back((int)h.b_ent.size());
-    h.c_ent.insert(h.c_ent.end(), cl[k].begin(), cl[k].end());
+    h.c_ent.insert(h.c_ent.end(), cl[j].begin(), cl[j].end());
     h.c_ptr.push_back((int)h.c_ent.size() / 2);
   }
   // pattern: rows T, E dense; columns T, E dense (R5 / S10); species block from rowmap
@@ -282,6 +295,10 @@ int build_host_tables(const pyjac_mech_desc* d, HostTables& h, std::string& err)
   std::stable_sort(items[1].begin(), items[1].end(), [](const Item& a, const Item& b) { return a.j < b.j; });
   h.nA = (int)items[0].size();
   for (int p = 0; p < 2; ++p) {
+    std::vector<int32_t> ord;
+    const std::vector<Item> base = items[p];
+    order_by_len(h.nA, [&](int e) { return (int)rowmap[base[e].k][base[e].j].size(); }, ord, h.nA_long[p]);
+    for (int e = 0; e < h.nA; ++e) items[p][e] = base[ord[e]];     // stable: equal lengths keep output order
     h.a_ptr[p].assign(1, 0);
     for (const Item& it : items[p]) {
       const auto& e = rowmap[it.k][it.j];

@@ -21,6 +21,7 @@ constexpr int INFO_SNU_SHIFT = 8;    // bits 8-11: sum(nu) + 8
 constexpr int INFO_NREAC_SHIFT = 12; // bits 12-13: number of reactant entries
 constexpr int INFO_NPROD_SHIFT = 14; // bits 14-15: number of product entries
 constexpr uint32_t SIGN_BIT = 0x80000000u;
+constexpr int LONG_LIST = 32;        // gather lists longer than this are processed by a whole warp
 
 enum OutFmt { OUT_CSR = 0, OUT_CSC = 1, OUT_DENSE_C = 2, OUT_DENSE_F = 3 };
 
@@ -47,7 +48,9 @@ struct HostTables {
   int64_t nnz = 0;
   std::vector<int32_t> csr_ptr, csr_idx, csc_ptr, csc_idx;
   // gather maps.  Entries: slot offset | SIGN_BIT (a stoichiometric coefficient of magnitude m is m copies)
-  std::vector<int32_t> b_ptr, b_ent, bq_ent; // per species k < Ns-1: reactions with nu_ki != 0 (slot base / reaction index)
+  std::vector<int32_t> b_ptr, b_ent, bq_ent; // per species k < Ns-1 (order b_item): reactions with nu_ki != 0 (slot base / reaction index)
+  std::vector<int32_t> b_item, c_item;       // processing order (descending list length) -> species / column
+  int nb_long = 0, nc_long = 0, nA_long[2] = {0, 0};   // leading items whose list is longer than LONG_LIST
   std::vector<int32_t> c_ptr, c_ent;         // per column j < Ns-1: pairs (slot | sign, reaction): T and E rows
   // class A items (species-block nonzeros) in row-major [0] and column-major [1] order
   int nA = 0;
@@ -78,11 +81,12 @@ struct DevMech {
   const double *plog_P, *plog_lnP, *plog_lnA, *plog_b, *plog_Ta;
   const int32_t* cheb_meta;
   const double *cheb_lim, *cheb_coef;
-  const int32_t *b_ptr, *b_ent, *bq_ent, *c_ptr, *c_ent;
+  const int32_t *b_ptr, *b_ent, *bq_ent, *c_ptr, *c_ent, *b_item, *c_item;
+  int nb_long, nc_long;
 };
 
 struct DevPlan {
-  int nA;
+  int nA, nA_long;
   int64_t n_e;               // elements per state in the output (nnz or nvar^2)
   const int32_t *a_ptr, *a_ent, *a_pos, *b_pos, *c_pos;
   int32_t d_pos[4];

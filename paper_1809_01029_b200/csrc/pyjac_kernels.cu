@@ -384,16 +384,27 @@ source_kernel(const DevMech m, int mode, int64_t n_states, int64_t tile, const d
   const bool valid = s0 + s < n_states;
   const int64_t obase = state_base(min(s0 + s, n_states - 1), tile, m.nvar);
   const double V = t.sc[SC_V * S + s];
-  // a7: omega_k = sum_i nu_ki q_i (Eq. 4), dn_k/dt = V omega_k (Eq. 3); a warp gathers one species
-  for (int k = warp; k < L; k += NW) {
-    const int p1 = m.b_ptr[k + 1];
+  // a7: omega_k = sum_i nu_ki q_i (Eq. 4), dn_k/dt = V omega_k (Eq. 3).  Species in order of descending list
+  // length: a warp gathers each long list cooperatively, then one thread per (species, state)
+  for (int q = warp; q < m.nb_long; q += NW) {
+    const int p1 = m.b_ptr[q + 1];
     double w = 0.0;
-    for (int p = m.b_ptr[k] + sub; p < p1; p += 32 / S) {
+    for (int p = m.b_ptr[q] + sub; p < p1; p += 32 / S) {
       const uint32_t ent = (uint32_t)m.bq_ent[p];
       w += apply_sign(t.P[(ent & ~SIGN_BIT) * S + s], ent);
     }
     w = group_sum<S>(w);
-    if (lane < S && valid) out[obase + (int64_t)(2 + k) * tile] = V * w;
+    if (lane < S && valid) out[obase + (int64_t)(2 + m.b_item[q]) * tile] = V * w;
+  }
+  for (int idx = m.nb_long * S + threadIdx.x; idx < L * S; idx += NT) {
+    const int q = idx / S;
+    const int p1 = m.b_ptr[q + 1];
+    double w = 0.0;
+    for (int p = m.b_ptr[q]; p < p1; ++p) {
+      const uint32_t ent = (uint32_t)m.bq_ent[p];
+      w += apply_sign(t.P[(ent & ~SIGN_BIT) * S + s], ent);
+    }
+    if (valid) out[obase + (int64_t)(2 + m.b_item[q]) * tile] = V * w;
   }
   if (threadIdx.x < S && valid) {
     const double T = t.sc[SC_T * S + s], Pp = t.sc[SC_P * S + s];
@@ -432,8 +443,21 @@ jacobian_kernel(const DevMech m, const DevPlan pl, int mode, int64_t n_states, i
       if (!((pl.nzmask[e >> 5] >> (e & 31)) & 1u) && valid) out[obase + (int64_t)e * tile] = 0.0;
     }
   }
-  // a9: species block, J[k][j] = sum_i nu_ki (Ghat^j_i - Ghat^Ns_i): gather the static list, store once
-  for (int idx = tid; idx < pl.nA * S; idx += NT) {
+  // Gather engine: items come in order of descending list length.  The first n_long items (list
+  // longer than LONG_LIST) are gathered by a whole warp (lanes stride the list, shuffle reduction); the others by
+  // one thread per (item, state) -- the 32 lists of a warp then have nearly the same length (no divergence tail).
+  // a9: species block, J[k][j] = sum_i nu_ki (Ghat^j_i - Ghat^Ns_i); every nonzero is stored once
+  for (int e = warp; e < pl.nA_long; e += NW) {
+    const int p1 = pl.a_ptr[e + 1];
+    double v = 0.0;
+    for (int p = pl.a_ptr[e] + sub; p < p1; p += 32 / S) {
+      const uint32_t ent = (uint32_t)pl.a_ent[p];
+      v += apply_sign(t.P[(ent & ~SIGN_BIT) * S + s], ent);
+    }
+    v = group_sum<S>(v);
+    if (lane < S && valid) out[obase + (int64_t)pl.a_pos[e] * tile] = v;
+  }
+  for (int idx = pl.nA_long * S + tid; idx < pl.nA * S; idx += NT) {
     const int e = idx / S;
     const int p1 = pl.a_ptr[e + 1];
     double v = 0.0;
@@ -444,10 +468,10 @@ jacobian_kernel(const DevMech m, const DevPlan pl, int mode, int64_t n_states, i
     if (valid) out[obase + (int64_t)pl.a_pos[e] * tile] = v;
   }
   // a9: T and E columns of the species rows: J[k][T] = sum_i nu_ki slotT_i, J[k][E] = sum_i nu_ki slotE_i
-  for (int k = warp; k < L; k += NW) {
-    const int p1 = m.b_ptr[k + 1];
+  for (int q = warp; q < m.nb_long; q += NW) {
+    const int p1 = m.b_ptr[q + 1];
     double vT = 0.0, vE = 0.0;
-    for (int p = m.b_ptr[k] + sub; p < p1; p += 32 / S) {
+    for (int p = m.b_ptr[q] + sub; p < p1; p += 32 / S) {
       const uint32_t ent = (uint32_t)m.b_ent[p];
       const int off = (ent & ~SIGN_BIT) * S + s;
       vT += apply_sign(t.P[off], ent);
@@ -455,18 +479,39 @@ jacobian_kernel(const DevMech m, const DevPlan pl, int mode, int64_t n_states, i
     }
     vT = group_sum<S>(vT); vE = group_sum<S>(vE);
     if (lane < S && valid) {
+      const int k = m.b_item[q];
+      out[obase + (int64_t)pl.b_pos[k] * tile] = vT;
+      out[obase + (int64_t)pl.b_pos[L + k] * tile] = vE;
+    }
+  }
+  for (int idx = m.nb_long * S + tid; idx < L * S; idx += NT) {
+    const int q = idx / S;
+    const int p1 = m.b_ptr[q + 1];
+    double vT = 0.0, vE = 0.0;
+    for (int p = m.b_ptr[q]; p < p1; ++p) {
+      const uint32_t ent = (uint32_t)m.b_ent[p];
+      const int off = (ent & ~SIGN_BIT) * S + s;
+      vT += apply_sign(t.P[off], ent);
+      vE += apply_sign(t.P[off + S], ent);
+    }
+    if (valid) {
+      const int k = m.b_item[q];
       out[obase + (int64_t)pl.b_pos[k] * tile] = vT;
       out[obase + (int64_t)pl.b_pos[L + k] * tile] = vE;
     }
   }
   // a10: T and E rows, species columns: gather over reactions with the per-state weights dE~_i, dn~_i
+  //   J[T][j] = -(sum_i dE~_i g_ij + f_T (c_j - c_Ns)) / (D V);  J[E][j] = cS sum_i dn~_i g_ij + cT J[T][j]
   const double cL = t.ck[L * S + s];
   const double iDV = 1.0 / (D * V);
-  for (int j = warp; j < L; j += NW) {
-    const int p1 = m.c_ptr[j + 1];
+  const double cS = mode == PYJAC_CONP ? T * R_GAS / Pp : T * R_GAS / V;
+  const double cT = mode == PYJAC_CONP ? V / T : Pp / T;
+  const int2* __restrict__ c_ent2 = reinterpret_cast<const int2*>(m.c_ent);
+  for (int q = warp; q < m.nc_long; q += NW) {
+    const int p1 = m.c_ptr[q + 1];
     double vT = 0.0, vS = 0.0;
-    for (int p = m.c_ptr[j] + sub; p < p1; p += 32 / S) {
-      const int2 pr = reinterpret_cast<const int2*>(m.c_ent)[p];
+    for (int p = m.c_ptr[q] + sub; p < p1; p += 32 / S) {
+      const int2 pr = c_ent2[p];
       const uint32_t ent = (uint32_t)pr.x;
       const double x = apply_sign(t.P[(ent & ~SIGN_BIT) * S + s], ent);
       vT += t.dE[pr.y * S + s] * x;
@@ -474,10 +519,28 @@ jacobian_kernel(const DevMech m, const DevPlan pl, int mode, int64_t n_states, i
     }
     vT = group_sum<S>(vT); vS = group_sum<S>(vS);
     if (lane < S && valid) {
+      const int j = m.c_item[q];
       const double JT = -(vT + fT * (t.ck[j * S + s] - cL)) * iDV;
-      const double JE = mode == PYJAC_CONP ? T * R_GAS * vS / Pp + V * JT / T : T * R_GAS * vS / V + Pp / T * JT;
       out[obase + (int64_t)pl.c_pos[j] * tile] = JT;
-      out[obase + (int64_t)pl.c_pos[L + j] * tile] = JE;
+      out[obase + (int64_t)pl.c_pos[L + j] * tile] = cS * vS + cT * JT;
+    }
+  }
+  for (int idx = m.nc_long * S + tid; idx < L * S; idx += NT) {
+    const int q = idx / S;
+    const int p1 = m.c_ptr[q + 1];
+    double vT = 0.0, vS = 0.0;
+    for (int p = m.c_ptr[q]; p < p1; ++p) {
+      const int2 pr = c_ent2[p];
+      const uint32_t ent = (uint32_t)pr.x;
+      const double x = apply_sign(t.P[(ent & ~SIGN_BIT) * S + s], ent);
+      vT += t.dE[pr.y * S + s] * x;
+      vS += m.dn[pr.y] * x;
+    }
+    if (valid) {
+      const int j = m.c_item[q];
+      const double JT = -(vT + fT * (t.ck[j * S + s] - cL)) * iDV;
+      out[obase + (int64_t)pl.c_pos[j] * tile] = JT;
+      out[obase + (int64_t)pl.c_pos[L + j] * tile] = cS * vS + cT * JT;
     }
   }
   // a10: the four corner entries from the phase-1 reductions (R4-7)
