@@ -43,7 +43,7 @@ class PyjacError(RuntimeError):
         self.code = code
 
 
-LIB_PATH = os.path.join(os.path.dirname(os.path.abspath(__file__)), "libpyjac_b200.so")
+LIB_PATH = os.environ.get("PYJAC_LIB") or os.path.join(os.path.dirname(os.path.abspath(__file__)), "libpyjac_b200.so")
 _lib = None
 
 

@@ -31,6 +31,13 @@ struct pyjac_mech {
   ~pyjac_mech() {
     for (void* p : allocs) cudaFree(p);
   }
+  int upload_plan(const GatherPlan& g, DevGather* out) {
+    out->n_long = g.n_long; out->n_sg = g.n_sg;
+    if (int r = upload(g.long_ptr, &out->long_ptr)) return r;
+    if (int r = upload(g.long_ent, &out->long_ent)) return r;
+    if (int r = upload(g.sg_meta, &out->sg_meta)) return r;
+    return upload(g.ell_ent, &out->ell_ent);
+  }
   template <class T> int upload(const std::vector<T>& v, const T** out) {
     void* p = nullptr;
     const size_t bytes = (v.size() ? v.size() : 1) * sizeof(T) + 32;   // +32: vector loads may touch padding
@@ -75,23 +82,22 @@ int pyjac_mech_create(const pyjac_mech_desc* desc, int cuda_device, pyjac_mech**
 #define UP(field) if (int r_ = m->upload(h.field, &d.field)) return r_;
     UP(nasa) UP(wr) UP(lnA) UP(beta) UP(Ta) UP(dn) UP(info) UP(aux) UP(sp) UP(eff_ptr) UP(eff_sp) UP(eff_d)
     UP(slot_base) UP(fall) UP(plog_ptr) UP(plog_P) UP(plog_lnP) UP(plog_lnA) UP(plog_b) UP(plog_Ta)
-    UP(cheb_meta) UP(cheb_lim) UP(cheb_coef) UP(b_ptr) UP(b_ent) UP(bq_ent) UP(c_ptr) UP(c_ent) UP(b_item) UP(c_item)
+    UP(cheb_meta) UP(cheb_lim) UP(cheb_coef)
 #undef UP
-    d.nb_long = h.nb_long; d.nc_long = h.nc_long;
-    const int32_t *a_ptr[2], *a_ent[2];
+    if (int r_ = m->upload_plan(h.cplan, &d.cplan)) return r_;
+    if (int r_ = m->upload_plan(h.qplan, &d.qplan)) return r_;
+    if (int r_ = m->upload(h.qplan.item, &d.q_item)) return r_;
+    if (int r_ = m->upload(h.cplan.item, &d.c_item)) return r_;
+    DevGather jplan;
+    if (int r_ = m->upload_plan(h.jplan, &jplan)) return r_;
     const uint32_t* mask[2];
-    for (int p = 0; p < 2; ++p) {
-      if (int r_ = m->upload(h.a_ptr[p], &a_ptr[p])) return r_;
-      if (int r_ = m->upload(h.a_ent[p], &a_ent[p])) return r_;
+    for (int p = 0; p < 2; ++p)
       if (int r_ = m->upload(h.nzmask[p], &mask[p])) return r_;
-    }
     for (int f = 0; f < 4; ++f) {
       DevPlan& pl = m->plan[f];
-      pl.nA = h.nA; pl.nA_long = h.nA_long[f & 1];
       pl.n_e = f < 2 ? h.nnz : (int64_t)h.nvar * h.nvar;
-      pl.a_ptr = a_ptr[f & 1]; pl.a_ent = a_ent[f & 1];
-      if (int r_ = m->upload(h.a_pos[f], &pl.a_pos)) return r_;
-      if (int r_ = m->upload(h.b_pos[f], &pl.b_pos)) return r_;
+      pl.jplan = jplan;
+      if (int r_ = m->upload(h.j_pos[f], &pl.j_pos)) return r_;
       if (int r_ = m->upload(h.c_pos[f], &pl.c_pos)) return r_;
       for (int j = 0; j < 4; ++j) pl.d_pos[j] = h.d_pos[f][j];
       pl.nzmask = f < 2 ? nullptr : mask[f & 1];

@@ -5,6 +5,8 @@
 // maps, as the paper itself proposes.
 #include <algorithm>
 #include <cmath>
+#include <cstdlib>
+#include <cstring>
 #include <map>
 #include <numeric>
 #include <sstream>
@@ -69,6 +71,56 @@ int validate(const pyjac_mech_desc* d, std::string& err) {
   return PYJAC_OK;
 }
 
+
+// Gather plan: items in order of DESCENDING list length.  Lists longer than LONG_LIST are kept in CSR form and
+// gathered by a whole warp; the others are packed in ELL "super-groups" of ELL_W items whose lists are padded
+// (with entries pointing at an always-zero slot) to the longest list of the group and stored entry-major, so
+// that the 32 lanes of a warp read 32 consecutive entries and a thread can keep several loads in flight.
+// stride = ints per entry (1: slot | sign; 2: slot | sign, reaction).
+int long_list_threshold() {
+  const char* e = std::getenv("PYJAC_LONG_LIST");
+  const int v = e ? std::atoi(e) : LONG_LIST_DEFAULT;
+  return v > 0 ? v : LONG_LIST_DEFAULT;
+}
+
+void build_gather(const std::vector<std::vector<int32_t>>& lists, int stride, int zero_slot, GatherPlan& g) {
+  const int LONG_LIST = long_list_threshold();
+  const int n = (int)lists.size();
+  std::vector<int> order(n);
+  std::iota(order.begin(), order.end(), 0);
+  auto len = [&](int i) { return (int)lists[i].size() / stride; };
+  std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return len(a) > len(b); });
+  g = GatherPlan();
+  g.stride = stride;
+  g.long_ptr.assign(1, 0);
+  while (g.n_long < n && len(order[g.n_long]) > LONG_LIST) {
+    const auto& l = lists[order[g.n_long]];
+    g.long_ent.insert(g.long_ent.end(), l.begin(), l.end());
+    g.long_ptr.push_back((int)g.long_ent.size() / stride);
+    g.item.push_back(order[g.n_long]);
+    ++g.n_long;
+  }
+  const int n_short = n - g.n_long;
+  g.n_sg = (n_short + ELL_W - 1) / ELL_W;
+  int off = 0;
+  for (int sg = 0; sg < g.n_sg; ++sg) {
+    const int i0 = g.n_long + sg * ELL_W;
+    const int width = len(order[i0]);                 // sorted: the first list of the group is the longest
+    g.sg_meta.push_back(off); g.sg_meta.push_back(width);
+    for (int p = 0; p < width; ++p)
+      for (int w = 0; w < ELL_W; ++w) {
+        const int i = i0 + w;
+        const bool real = i < n && p < len(order[i]);
+        for (int c = 0; c < stride; ++c) g.ell_ent.push_back(real ? lists[order[i]][p * stride + c] : (c == 0 ? zero_slot : 0));
+      }
+    off += width * ELL_W;
+    for (int w = 0; w < ELL_W; ++w) g.item.push_back(i0 + w < n ? order[i0 + w] : -1);
+  }
+  g.n_entries = 0;
+  for (int i = 0; i < n; ++i) g.n_entries += len(i);
+  g.n_padded = (int64_t)g.long_ent.size() / stride + off;
+}
+
 }  // namespace
 
 int build_host_tables(const pyjac_mech_desc* d, HostTables& h, std::string& err) {
@@ -85,16 +137,26 @@ int build_host_tables(const pyjac_mech_desc* d, HostTables& h, std::string& err)
     h.wr[k] = d->mol_weight[k] / d->mol_weight[L];
   }
 
-  // ---- sort reactions by (type, reversible): warps become type-uniform ------------
+  // ---- sort reactions by DESCENDING cost class (type, reversible, non-unit coefficients): warps become
+  // type-uniform (the paper's reaction-sorting idea) and the expensive falloff / P-Log / Chebyshev
+  // reactions are started first (the kernel hands out 32-reaction chunks dynamically) ---------------------------
   h.perm.resize(nr);
   std::iota(h.perm.begin(), h.perm.end(), 0);
   std::stable_sort(h.perm.begin(), h.perm.end(), [&](int a, int b) {
-    const int ka = d->type[a] * 2 + (d->reversible[a] ? 1 : 0), kb = d->type[b] * 2 + (d->reversible[b] ? 1 : 0);
-    return ka < kb;
+    auto simple = [&](int i) {
+      for (int j = d->reac_ptr[i]; j < d->reac_ptr[i + 1]; ++j) if (d->reac_nu[j] != 1) return 0;
+      for (int j = d->prod_ptr[i]; j < d->prod_ptr[i + 1]; ++j) if (d->prod_nu[j] != 1) return 0;
+      return 1;
+    };
+    auto cost = [&](int i) {
+      static const int rank[7] = {0, 1, 2, 5, 4, 3, 6};   // elementary < third body < Lindemann < P-Log < SRI < Troe < Chebyshev
+      return rank[d->type[i]] * 4 + (d->reversible[i] ? 2 : 0) + (simple(i) ? 0 : 1);
+    };
+    return cost(a) > cost(b);
   });
 
   h.lnA.resize(nr); h.beta.resize(nr); h.Ta.resize(nr); h.dn.resize(nr);
-  h.info.resize(nr); h.aux.assign(nr, -1); h.sp.assign((size_t)nr * 8, 0u);
+  h.info.resize(nr); h.aux.assign(nr, -1); h.sp.assign((size_t)nr * 8, (uint32_t)ns);
   h.eff_ptr.assign(1, 0); h.slot_base.assign(1, 0);
   std::vector<std::vector<Role>> roles(nr);
   std::vector<std::vector<std::pair<int, int>>> net(nr);   // (species k < Ns-1... incl. last, net nu != 0)
@@ -108,17 +170,20 @@ int build_host_tables(const pyjac_mech_desc* d, HostTables& h, std::string& err)
     h.lnA[r] = (ty <= PYJAC_FALLOFF_SRI) ? std::log(d->A[i]) : 0.0;
     h.beta[r] = d->beta[i]; h.Ta[r] = d->Ta[i];
     const int nre = d->reac_ptr[i + 1] - d->reac_ptr[i], npr = d->prod_ptr[i + 1] - d->prod_ptr[i];
-    int snu = 0;
+    int snu = 0, order_f = 0, order_r = 0;
+    bool simple = true;
     std::map<int, int> netnu;
     for (int a = 0; a < nre; ++a) {
       const int j = d->reac_ptr[i] + a;
       h.sp[8 * r + a] = (uint32_t)d->reac_species[j] | ((uint32_t)d->reac_nu[j] << 16);
       snu -= d->reac_nu[j]; netnu[d->reac_species[j]] -= d->reac_nu[j];
+      order_f += d->reac_nu[j]; simple &= d->reac_nu[j] == 1;
     }
     for (int b = 0; b < npr; ++b) {
       const int j = d->prod_ptr[i] + b;
       h.sp[8 * r + 3 + b] = (uint32_t)d->prod_species[j] | ((uint32_t)d->prod_nu[j] << 16);
       snu += d->prod_nu[j]; netnu[d->prod_species[j]] += d->prod_nu[j];
+      order_r += d->prod_nu[j]; simple &= d->prod_nu[j] == 1;
     }
     double dn = 0.0;
     for (auto& kv : netnu)
@@ -126,7 +191,8 @@ int build_host_tables(const pyjac_mech_desc* d, HostTables& h, std::string& err)
     h.dn[r] = dn;
     const bool adef = tb && d->collider[i] < 0;
     int info = ty | (rev ? INFO_REV : 0) | (adef ? INFO_ADEF : 0) | ((snu + 8) << INFO_SNU_SHIFT) |
-               (nre << INFO_NREAC_SHIFT) | (npr << INFO_NPROD_SHIFT);
+               (nre << INFO_NREAC_SHIFT) | (npr << INFO_NPROD_SHIFT) | (simple ? INFO_SIMPLE : 0) |
+               (order_f << INFO_OF_SHIFT) | (order_r << INFO_OR_SHIFT);
     if (ty == PYJAC_FALLOFF_TROE && d->troe_has_T2[i]) info |= INFO_T2;
     h.info[r] = info;
     // slots: 0 = T column, 1 = E column, then one per role
@@ -179,7 +245,6 @@ int build_host_tables(const pyjac_mech_desc* d, HostTables& h, std::string& err)
   // Species-block entry (k, j), k, j < L:  J = sum_i nu_ki (Ghat^j_i - Ghat^L_i)  (R4-6):
   // + every role of species j, - every role of the last species L (those hit ALL columns: dense rows).
   std::vector<std::map<int, std::vector<int32_t>>> rowmap(L);   // row k -> col j -> entries
-  h.b_ptr.assign(1, 0); h.c_ptr.assign(1, 0);
   std::vector<std::vector<int32_t>> bl(L), bql(L), cl(L);
   auto push_n = [](std::vector<int32_t>& v, int32_t e, int n) { for (int c = 0; c < n; ++c) v.push_back(e); };
   for (int r = 0; r < nr; ++r) {
@@ -235,26 +300,6 @@ int build_host_tables(const pyjac_mech_desc* d, HostTables& h, std::string& err)
         if (inpat[k][j] && !rowmap[k].count(j)) MECH_FAIL("internal: pattern entry (" << k << "," << j << ") has no gather list");
     }
   }
-  // Load balance: items are processed in order of DESCENDING list length, so the
-  // 32 lists of a warp have (nearly) equal length; the few lists longer than LONG_LIST are gathered by a whole
-  // warp with a shuffle reduction instead.
-  auto order_by_len = [](int n, auto len_of, std::vector<int32_t>& order, int& n_long) {
-    order.resize(n);
-    std::iota(order.begin(), order.end(), 0);
-    std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return len_of(a) > len_of(b); });
-    n_long = 0;
-    while (n_long < n && len_of(order[n_long]) > LONG_LIST) ++n_long;
-  };
-  order_by_len(L, [&](int k) { return (int)bl[k].size(); }, h.b_item, h.nb_long);
-  order_by_len(L, [&](int k) { return (int)cl[k].size() / 2; }, h.c_item, h.nc_long);
-  for (int q = 0; q < L; ++q) {
-    const int k = h.b_item[q], j = h.c_item[q];
-    h.b_ent.insert(h.b_ent.end(), bl[k].begin(), bl[k].end());
-    h.bq_ent.insert(h.bq_ent.end(), bql[k].begin(), bql[k].end());
-    h.b_ptr.push_back((int)h.b_ent.size());
-    h.c_ent.insert(h.c_ent.end(), cl[j].begin(), cl[j].end());
-    h.c_ptr.push_back((int)h.c_ent.size() / 2);
-  }
   // pattern: rows T, E dense; columns T, E dense (R5 / S10); species block from rowmap
   std::vector<std::vector<int>> rows(nvar);
   for (int r = 0; r < 2; ++r) { rows[r].resize(nvar); std::iota(rows[r].begin(), rows[r].end(), 0); }
@@ -287,34 +332,42 @@ int build_host_tables(const pyjac_mech_desc* d, HostTables& h, std::string& err)
       default: return c * nvar + r;
     }
   };
-  // class A items in row-major (plan 0) and column-major (plan 1) order
-  struct Item { int k, j; };
-  std::vector<Item> items[2];
-  for (int k = 0; k < L; ++k) for (auto& kv : rowmap[k]) items[0].push_back({k, kv.first});
-  items[1] = items[0];
-  std::stable_sort(items[1].begin(), items[1].end(), [](const Item& a, const Item& b) { return a.j < b.j; });
-  h.nA = (int)items[0].size();
-  for (int p = 0; p < 2; ++p) {
-    std::vector<int32_t> ord;
-    const std::vector<Item> base = items[p];
-    order_by_len(h.nA, [&](int e) { return (int)rowmap[base[e].k][base[e].j].size(); }, ord, h.nA_long[p]);
-    for (int e = 0; e < h.nA; ++e) items[p][e] = base[ord[e]];     // stable: equal lengths keep output order
-    h.a_ptr[p].assign(1, 0);
-    for (const Item& it : items[p]) {
-      const auto& e = rowmap[it.k][it.j];
-      h.a_ent[p].insert(h.a_ent[p].end(), e.begin(), e.end());
-      h.a_ptr[p].push_back((int)h.a_ent[p].size());
+  // ---- gather plans ------------------------------------------------------------
+  // J-plan items: species-block nonzeros (k, j) in row-major order, then the T and E columns of the species rows.
+  struct Item { int r, c; };
+  std::vector<Item> jitems;
+  std::vector<std::vector<int32_t>> jlists;
+  for (int k = 0; k < L; ++k)
+    for (auto& kv : rowmap[k]) { jitems.push_back({2 + k, 2 + kv.first}); jlists.push_back(kv.second); }
+  h.nA = (int)jitems.size();
+  for (int col = 0; col < 2; ++col)
+    for (int k = 0; k < L; ++k) {
+      std::vector<int32_t> l = bl[k];
+      for (auto& e : l) e += col;                      // slot base + 0: T column, + 1: E column (sign bit untouched)
+      jitems.push_back({2 + k, col}); jlists.push_back(std::move(l));
+    }
+  build_gather(jlists, 1, h.nslots, h.jplan);
+  std::vector<std::vector<int32_t>> clists(L), qlists(L);
+  for (int k = 0; k < L; ++k) {
+    qlists[k] = bql[k];
+    for (size_t e = 0; e + 1 < cl[k].size(); e += 2) {   // entry = (slot | sign, reaction, dn~ of the reaction as 2 ints)
+      int32_t w[2];
+      std::memcpy(w, &h.dn[cl[k][e + 1]], 8);
+      clists[k].insert(clists[k].end(), {cl[k][e], cl[k][e + 1], w[0], w[1]});
     }
   }
+  build_gather(clists, 4, h.nslots, h.cplan);            // T and E rows: (slot | sign, reaction, dn~)
+  build_gather(qlists, 1, nr, h.qplan);                  // source terms: omega_k = sum nu_ki q_i
   for (int fmt = 0; fmt < 4; ++fmt) {
-    const int p = fmt & 1;
-    h.a_pos[fmt].resize(h.nA);
-    for (int e = 0; e < h.nA; ++e) h.a_pos[fmt][e] = pos_of(fmt, 2 + items[p][e].k, 2 + items[p][e].j);
-    h.b_pos[fmt].resize(2 * L); h.c_pos[fmt].resize(2 * L);
-    for (int k = 0; k < L; ++k) {
-      h.b_pos[fmt][k] = pos_of(fmt, 2 + k, 0); h.b_pos[fmt][L + k] = pos_of(fmt, 2 + k, 1);
-      h.c_pos[fmt][k] = pos_of(fmt, 0, 2 + k); h.c_pos[fmt][L + k] = pos_of(fmt, 1, 2 + k);
-    }
+    h.j_pos[fmt].assign(h.jplan.item.size(), -1);
+    for (size_t e = 0; e < h.jplan.item.size(); ++e)
+      if (h.jplan.item[e] >= 0) h.j_pos[fmt][e] = pos_of(fmt, jitems[h.jplan.item[e]].r, jitems[h.jplan.item[e]].c);
+    h.c_pos[fmt].assign(2 * h.cplan.item.size(), -1);
+    for (size_t e = 0; e < h.cplan.item.size(); ++e)
+      if (h.cplan.item[e] >= 0) {
+        h.c_pos[fmt][2 * e] = pos_of(fmt, 0, 2 + h.cplan.item[e]);
+        h.c_pos[fmt][2 * e + 1] = pos_of(fmt, 1, 2 + h.cplan.item[e]);
+      }
     h.d_pos[fmt][0] = pos_of(fmt, 0, 0); h.d_pos[fmt][1] = pos_of(fmt, 0, 1);
     h.d_pos[fmt][2] = pos_of(fmt, 1, 0); h.d_pos[fmt][3] = pos_of(fmt, 1, 1);
   }

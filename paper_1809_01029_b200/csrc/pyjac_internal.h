@@ -17,13 +17,29 @@ constexpr int INFO_TYPE_MASK = 7;    // bits 0-2  reaction type
 constexpr int INFO_REV = 1 << 3;     // reversible
 constexpr int INFO_T2 = 1 << 4;      // Troe has T2
 constexpr int INFO_ADEF = 1 << 5;    // default third-body efficiency is 1 (mixture); 0: single collider
+constexpr int INFO_SIMPLE = 1 << 6;  // every stoichiometric coefficient is 1 (fast path, no powers)
 constexpr int INFO_SNU_SHIFT = 8;    // bits 8-11: sum(nu) + 8
 constexpr int INFO_NREAC_SHIFT = 12; // bits 12-13: number of reactant entries
 constexpr int INFO_NPROD_SHIFT = 14; // bits 14-15: number of product entries
+constexpr int INFO_OF_SHIFT = 16;    // bits 16-19: forward order  sum nu'
+constexpr int INFO_OR_SHIFT = 20;    // bits 20-23: reverse order  sum nu''
 constexpr uint32_t SIGN_BIT = 0x80000000u;
-constexpr int LONG_LIST = 32;        // gather lists longer than this are processed by a whole warp
+constexpr int LONG_LIST_DEFAULT = 64; // gather lists longer than this are processed by a whole warp (env PYJAC_LONG_LIST)
 
 enum OutFmt { OUT_CSR = 0, OUT_CSC = 1, OUT_DENSE_C = 2, OUT_DENSE_F = 3 };
+
+constexpr int ELL_W = 128;           // items per ELL super-group (4 items per lane at one state per CTA)
+
+struct GatherPlan {
+  int stride = 1;                            // ints per entry
+  int n_long = 0;                            // leading items gathered by a whole warp (CSR form)
+  std::vector<int32_t> long_ptr, long_ent;
+  int n_sg = 0;                              // ELL super-groups of ELL_W items
+  std::vector<int32_t> sg_meta;              // [n_sg*2]: entry offset, padded list length
+  std::vector<int32_t> ell_ent;              // entry (p, w) of group sg at (off + p*ELL_W + w) * stride
+  std::vector<int32_t> item;                 // [n_long + n_sg*ELL_W] processing slot -> item id, -1 = padding
+  int64_t n_entries = 0, n_padded = 0;       // real / stored entries (padding overhead report)
+};
 
 // ---- host-side tables (reactions in SORTED order: by type, then reversibility) ------------------
 struct HostTables {
@@ -35,7 +51,7 @@ struct HostTables {
   // reactions
   std::vector<double> lnA, beta, Ta, dn;     // [nr]; dn = sum_k<Ns nu_ki (1 - W_k/W_Ns)
   std::vector<int32_t> info, aux;            // [nr]; aux = index into fall / plog / cheb tables
-  std::vector<uint32_t> sp;                  // [nr*8]: 0-2 reactants, 3-5 products: species | nu << 16
+  std::vector<uint32_t> sp;                  // [nr*8]: 0-2 reactants, 3-5 products: species | nu << 16; unused: species = ns (dummy), nu = 0
   std::vector<int32_t> eff_ptr, eff_sp;      // [nr+1], entries with alpha != default only
   std::vector<double> eff_d;                 // alpha - default
   std::vector<int32_t> slot_base;            // [nr+1] Jacobian slots: {T, E, reactant roles, product roles (rev), eff roles}
@@ -47,16 +63,13 @@ struct HostTables {
   // pattern
   int64_t nnz = 0;
   std::vector<int32_t> csr_ptr, csr_idx, csc_ptr, csc_idx;
-  // gather maps.  Entries: slot offset | SIGN_BIT (a stoichiometric coefficient of magnitude m is m copies)
-  std::vector<int32_t> b_ptr, b_ent, bq_ent; // per species k < Ns-1 (order b_item): reactions with nu_ki != 0 (slot base / reaction index)
-  std::vector<int32_t> b_item, c_item;       // processing order (descending list length) -> species / column
-  int nb_long = 0, nc_long = 0, nA_long[2] = {0, 0};   // leading items whose list is longer than LONG_LIST
-  std::vector<int32_t> c_ptr, c_ent;         // per column j < Ns-1: pairs (slot | sign, reaction): T and E rows
-  // class A items (species-block nonzeros) in row-major [0] and column-major [1] order
-  int nA = 0;
-  std::vector<int32_t> a_ptr[2], a_ent[2];
-  std::vector<int32_t> a_pos[4];             // [OutFmt][nA] output element index (order of plan fmt&1)
-  std::vector<int32_t> b_pos[4], c_pos[4];   // [OutFmt][2*(ns-1)]: (k,T),(k,E) / (T,j),(E,j)
+  // gather plans.  Entries: slot offset | SIGN_BIT (a stoichiometric coefficient of magnitude m is m copies)
+  int nA = 0;                                // number of species-block nonzeros
+  GatherPlan jplan;                          // species rows: block nonzeros + their T and E columns
+  GatherPlan cplan;                          // T and E rows, species columns: pairs (slot | sign, reaction)
+  GatherPlan qplan;                          // source terms: omega_k gathers q_i
+  std::vector<int32_t> j_pos[4];             // [OutFmt][jplan.item.size()] output element (-1: padding)
+  std::vector<int32_t> c_pos[4];             // [OutFmt][2 * cplan.item.size()]: (T, j), (E, j)
   int32_t d_pos[4][4];                       // (T,T) (T,E) (E,T) (E,E)
   std::vector<uint32_t> nzmask[2];           // dense bitmaps, bit e set iff dense element e ('C' / 'F' order) is in the pattern
   int nslots = 0;                            // total Jacobian slots
@@ -67,6 +80,11 @@ struct HostTables {
 int build_host_tables(const pyjac_mech_desc* d, HostTables& h, std::string& err);
 
 // ---- device views ------------------------------------------------------------------------------
+struct DevGather {
+  int n_long, n_sg;
+  const int32_t *long_ptr, *long_ent, *sg_meta, *ell_ent;
+};
+
 struct DevMech {
   int ns, nr, nvar, nslots;
   const double *nasa, *wr;
@@ -81,14 +99,14 @@ struct DevMech {
   const double *plog_P, *plog_lnP, *plog_lnA, *plog_b, *plog_Ta;
   const int32_t* cheb_meta;
   const double *cheb_lim, *cheb_coef;
-  const int32_t *b_ptr, *b_ent, *bq_ent, *c_ptr, *c_ent, *b_item, *c_item;
-  int nb_long, nc_long;
+  DevGather cplan, qplan;
+  const int32_t *q_item, *c_item;   // processing slot -> species / column (-1: padding)
 };
 
 struct DevPlan {
-  int nA, nA_long;
   int64_t n_e;               // elements per state in the output (nnz or nvar^2)
-  const int32_t *a_ptr, *a_ent, *a_pos, *b_pos, *c_pos;
+  DevGather jplan;
+  const int32_t *j_pos, *c_pos;
   int32_t d_pos[4];
   const uint32_t* nzmask;    // dense only (else nullptr)
 };

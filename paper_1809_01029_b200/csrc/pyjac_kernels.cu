@@ -18,18 +18,55 @@
 
 namespace pyjac {
 
+#ifdef PYJAC_TIMING   // debug build only (tuning): per-phase clock64() sums over all CTAs, see _work/
+__device__ unsigned long long g_timing[16];
+#define TICK(i) do { __syncthreads(); if (threadIdx.x == 0) { const long long c_ = clock64(); atomicAdd(&g_timing[i], (unsigned long long)(c_ - tick_)); tick_ = c_; } } while (0)
+#define TICK_INIT long long tick_ = clock64()
+extern "C" int pyjac_debug_timing(unsigned long long* out, int reset) {
+  if (out) cudaMemcpyFromSymbol(out, g_timing, sizeof(g_timing));
+  if (reset) { unsigned long long z[16] = {0}; cudaMemcpyToSymbol(g_timing, z, sizeof(z)); }
+  return 0;
+}
+#else
+#define TICK(i) do { } while (0)
+#define TICK_INIT do { } while (0)
+#endif
+
 namespace {
 
-constexpr int NT = 512;           // threads per CTA
+#ifndef PYJAC_NT
+#define PYJAC_NT 512
+#endif
+#ifndef PYJAC_UJ
+#define PYJAC_UJ 4
+#endif
+#ifndef PYJAC_UC
+#define PYJAC_UC 1
+#endif
+#ifndef PYJAC_UQ
+#define PYJAC_UQ 1
+#endif
+constexpr int NT = PYJAC_NT;      // threads per CTA
 constexpr int NW = NT / 32;
 constexpr int NRED = 8;           // reduction slots
 // per-state scalars kept in shared memory
 enum { SC_T = 0, SC_V, SC_P, SC_CTOT, SC_SUMC, SC_SUMCC, SC_SUMCDC, SC_D, SC_DDDT, SC_CNS,
-       SC_R0, SC_R1, SC_R2, SC_R3, SC_R4, SC_R5, SC_R6, SC_R7, NSC };
+       SC_R0, SC_R1, SC_R2, SC_R3, SC_R4, SC_R5, SC_R6, SC_R7, SC_INVT, SC_LNT, SC_LNP, SC_LNPRT, NSC };
 
 __host__ __device__ inline size_t smem_doubles(int ns, int nr, int nslots, int S, bool jac) {
-  size_t per_state = NSC + 6 * (size_t)ns + (jac ? (size_t)nslots + nr : (size_t)nr);
+  // C[ns+1] (C[ns] = 1: dummy species of unused stoichiometric entries), th4[4(ns+1)], ck[ns], slots (+1 zero slot)
+  size_t per_state = NSC + 6 * (size_t)ns + 5 + (jac ? (size_t)nslots + nr : (size_t)nr) + 1;
   return per_state * S + (size_t)NW * NRED * S;
+}
+
+// Dynamic work distribution inside a CTA: items are sorted by descending cost at create time and warps take the
+// next chunk from a shared-memory counter (longest-processing-time-first scheduling); removes the tail in which a
+// few warps work on the heaviest reactions / longest gather lists while the others idle.
+enum { CNT_RX = 0, CNT_J, CNT_C, CNT_Q, N_CNT };
+__device__ __forceinline__ int next_chunk(int* counter) {
+  int c = 0;
+  if ((threadIdx.x & 31) == 0) c = atomicAdd(counter, 1);
+  return __shfl_sync(0xffffffffu, c, 0);
 }
 
 template <int S> __device__ __forceinline__ double group_sum(double v) {
@@ -120,11 +157,11 @@ __device__ __forceinline__ Blend blend(int type, bool hasT2, const double* __res
 // ---------------------------------------------------------------------------------------------------
 template <int S, bool JAC>
 struct Tile {
-  double *sc, *C, *gRT, *hRT, *Et, *ct, *ck, *dE, *P, *red;
+  // th4[(k*S + s)*4 + c]: c = 0 g_k/RT, 1 h_k/RT, 2 E~_k, 3 c~_k  (one 32-byte record per species and state)
+  double *sc, *C, *th4, *ck, *dE, *P, *red;
   __device__ __forceinline__ Tile(double* smem, int ns, int nr, int nslots) {
-    sc = smem; C = sc + NSC * S; gRT = C + ns * S; hRT = gRT + ns * S; Et = hRT + ns * S; ct = Et + ns * S;
-    ck = ct + ns * S; dE = ck + ns * S; P = JAC ? dE + nr * S : dE; red = P + (JAC ? nslots : nr) * S;
-    // source kernel: dE unused, P[r] = q_r
+    sc = smem; th4 = sc + NSC * S; C = th4 + 4 * (ns + 1) * S; ck = C + (ns + 1) * S; dE = ck + ns * S; P = JAC ? dE + nr * S : dE; red = P + ((JAC ? nslots : nr) + 1) * S;
+    // source kernel: dE unused, P[r] = q_r.  P[nslots] (JAC) / P[nr] is an always-zero slot (ELL padding)
   }
 };
 
@@ -133,22 +170,31 @@ __device__ __forceinline__ int64_t state_base(int64_t s, int64_t tile, int64_t n
 
 template <int S, bool JAC>
 __device__ __forceinline__ void phases01(const DevMech& m, Tile<S, JAC>& t, int mode, int64_t s0, int64_t n_states,
-                                         int64_t tile, const double* __restrict__ phi, const double* __restrict__ param) {
+                                         int64_t tile, const double* __restrict__ phi, const double* __restrict__ param,
+                                         int* cnt, long long& tick_) {
+  (void)tick_;
   const int tid = threadIdx.x;
   const int ns = m.ns, nr = m.nr, L = ns - 1;
   const int s = tid % S;                        // NT % S == 0: a thread keeps its state in every loop
   const int64_t sg = min(s0 + s, n_states - 1);  // ragged tail: recompute the last valid state, never store
   const int64_t pbase = state_base(sg, tile, ns + 1);
   // ---- phase 0a: scalars -------------------------------------------------------------------------
+  if (tid < N_CNT) cnt[tid] = 0;
   if (tid < S) {
     const double T = phi[pbase], E = phi[pbase + tile], par = param[sg];
     const double V = mode == PYJAC_CONP ? E : par, Pp = mode == PYJAC_CONP ? par : E;
     t.sc[SC_T * S + s] = T; t.sc[SC_V * S + s] = V; t.sc[SC_P * S + s] = Pp;
     t.sc[SC_CTOT * S + s] = Pp / (R_GAS * T);
+    t.sc[SC_INVT * S + s] = 1.0 / T; t.sc[SC_LNT * S + s] = log(T); t.sc[SC_LNP * S + s] = log(Pp);
+    t.sc[SC_LNPRT * S + s] = log(P_ATM / (R_GAS * T));
+    t.P[(JAC ? m.nslots : nr) * S + s] = 0.0;            // always-zero slot (ELL padding)
+    t.C[ns * S + s] = 1.0;                               // dummy species: unused stoichiometric entries
+#pragma unroll
+    for (int c = 0; c < 4; ++c) t.th4[(ns * S + s) * 4 + c] = 0.0;
   }
   __syncthreads();
   const double T = t.sc[SC_T * S + s], V = t.sc[SC_V * S + s], Pp = t.sc[SC_P * S + s], Ctot = t.sc[SC_CTOT * S + s];
-  const double invT = 1.0 / T, lnT = log(T), RT = R_GAS * T;
+  const double invT = t.sc[SC_INVT * S + s], lnT = t.sc[SC_LNT * S + s], RT = R_GAS * T;
   // ---- phase 0b: species: C_k = n_k / V (Eq. 6), NASA-7 thermo (R2) --------------------------
   {
     double acc[3] = {0.0, 0.0, 0.0};
@@ -157,15 +203,15 @@ __device__ __forceinline__ void phases01(const DevMech& m, Tile<S, JAC>& t, int 
     for (int idx = tid; idx < ns * S; idx += NT) {
       const int k = idx / S;
       const double* __restrict__ a = m.nasa + 16 * k;
-      a += (T <= a[0]) ? 1 : 8;                      // low range iff T <= T_mid (R3); per-lane select
-      const double a0 = a[0], a1 = a[1], a2 = a[2], a3 = a[3], a4 = a[4], a5 = a[5], a6 = a[6];
+      a += (T <= __ldg(a)) ? 1 : 8;                      // low range iff T <= T_mid (R3); per-lane select
+      const double a0 = __ldg(a), a1 = __ldg(a + 1), a2 = __ldg(a + 2), a3 = __ldg(a + 3), a4 = __ldg(a + 4), a5 = __ldg(a + 5), a6 = __ldg(a + 6);
       const double cpR = a0 + a1 * T + a2 * T2 + a3 * T3 + a4 * T4;
       const double dcpR = a1 + 2.0 * a2 * T + 3.0 * a3 * T2 + 4.0 * a4 * T3;
       const double hRT = a0 + a1 * T * 0.5 + a2 * T2 * (1.0 / 3.0) + a3 * T3 * 0.25 + a4 * T4 * 0.2 + a5 * invT;
       const double sR = a0 * lnT + a1 * T + a2 * T2 * 0.5 + a3 * T3 * (1.0 / 3.0) + a4 * T4 * 0.25 + a6;
       const double c = R_GAS * (mode == PYJAC_CONP ? cpR : cpR - 1.0);   // c_p or c_v = c_p - R
-      t.gRT[idx] = hRT - sR;
-      t.hRT[idx] = hRT;
+      t.th4[idx * 4] = hRT - sR;
+      t.th4[idx * 4 + 1] = hRT;
       t.ck[idx] = c;
       if (k < L) {
         const double Ck = phi[pbase + (int64_t)(2 + k) * tile] * invV;
@@ -184,31 +230,35 @@ __device__ __forceinline__ void phases01(const DevMech& m, Tile<S, JAC>& t, int 
     }
     __syncthreads();
     // E~_k = E_k - (W_k/W_Ns) E_Ns, c~_k likewise (mass conservation folds the last species in, R1/A1)
-    const double eL = t.hRT[L * S + s] - (mode == PYJAC_CONP ? 0.0 : 1.0), cL = t.ck[L * S + s];
+    const double eL = t.th4[(L * S + s) * 4 + 1] - (mode == PYJAC_CONP ? 0.0 : 1.0), cL = t.ck[L * S + s];
     for (int idx = tid; idx < ns * S; idx += NT) {
       const int k = idx / S;
-      const double w = m.wr[k];
-      const double e = t.hRT[idx] - (mode == PYJAC_CONP ? 0.0 : 1.0);
-      t.Et[idx] = k == L ? 0.0 : RT * (e - w * eL);
-      t.ct[idx] = k == L ? 0.0 : t.ck[idx] - w * cL;
+      const double w = __ldg(m.wr + k);
+      const double e = t.th4[idx * 4 + 1] - (mode == PYJAC_CONP ? 0.0 : 1.0);
+      t.th4[idx * 4 + 2] = k == L ? 0.0 : RT * (e - w * eL);
+      t.th4[idx * 4 + 3] = k == L ? 0.0 : t.ck[idx] - w * cL;
     }
     __syncthreads();
   }
+  TICK(0);
   // ---- phase 1: reactions ----------------------------------------------------------------------------
-  const double lnP = log(Pp);
-  const double ln_patm_rt = log(P_ATM / RT);
+  const double lnP = t.sc[SC_LNP * S + s];
+  const double ln_patm_rt = t.sc[SC_LNPRT * S + s];
   const double ctot_T = Ctot * invT;
   double acc[7] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
-  for (int idx = tid; idx < nr * S; idx += NT) {
+  const int n_rx_chunks = (nr * S + 31) / 32;
+  for (int chunk = next_chunk(cnt + CNT_RX); chunk < n_rx_chunks; chunk = next_chunk(cnt + CNT_RX)) {
+    const int idx = chunk * 32 + (tid & 31);
+    if (idx >= nr * S) continue;
     const int r = idx / S;
-    const int info = m.info[r];
+    const int info = __ldg(m.info + r);
     const int type = info & INFO_TYPE_MASK;
     const bool rev = info & INFO_REV;
     // a3: forward rate constant
     double lnkf, lam_f, dlnk_dP = 0.0;
     if (type <= PYJAC_FALLOFF_SRI) {
-      const double beta = m.beta[r], Ta = m.Ta[r];
-      lnkf = m.lnA[r] + beta * lnT - Ta * invT;
+      const double beta = __ldg(m.beta + r), Ta = __ldg(m.Ta + r);
+      lnkf = __ldg(m.lnA + r) + beta * lnT - Ta * invT;
       lam_f = (beta + Ta * invT) * invT;
     } else if (type == PYJAC_PLOG) {
       const int a = m.aux[r], p0 = m.plog_ptr[a], np = m.plog_ptr[a + 1] - p0;
@@ -265,22 +315,35 @@ __device__ __forceinline__ void phases01(const DevMech& m, Tile<S, JAC>& t, int 
       dlnk_dP = dlg_dP * 2.0 / (Pp * (lPmax - lPmin));
     }
     const double kf = exp(lnkf);
-    // stoichiometry: concentrations, products and one-factor-removed products (no division by C_k: R-S7)
-    const uint4 w0 = *reinterpret_cast<const uint4*>(m.sp + 8 * r);
-    const uint2 w1 = *reinterpret_cast<const uint2*>(m.sp + 8 * r + 4);
+    // stoichiometry: concentrations, products and one-factor-removed products (no division by C_k: R-S7).
+    // Unused entries point at the dummy species ns (C = 1, thermo = 0), so no predicates are needed.
+    const uint4 w0 = __ldg(reinterpret_cast<const uint4*>(m.sp + 8 * r));
+    const uint2 w1 = __ldg(reinterpret_cast<const uint2*>(m.sp + 8 * r + 4));
     const uint32_t spw[6] = {w0.x, w0.y, w0.z, w0.w, w1.x, w1.y};
     double pw[6], pm[6];
     double dg = 0.0, dh = 0.0, dEt = 0.0, dct = 0.0;
+    // Reactions are sorted so that a warp is (almost always) uniform in "all coefficients are 1": take the vote
+    // and branch once, so that the power / multiplicity arithmetic is not executed (if-converted) for the common case.
+    if (__all_sync(__activemask(), (info & INFO_SIMPLE) != 0)) {
 #pragma unroll
-    for (int a = 0; a < 6; ++a) {
-      const int nu = spw[a] >> 16, k = spw[a] & 0xffff;
-      const double Ck = nu ? t.C[k * S + s] : 1.0;
-      pw[a] = ipow(Ck, nu); pm[a] = dpow(Ck, nu);
-      const double snu = a < 3 ? -(double)nu : (double)nu;
-      if (nu) {
-        if (rev) { dg += snu * t.gRT[k * S + s]; dh += snu * t.hRT[k * S + s]; }
-        dEt += snu * t.Et[k * S + s];
-        if (JAC) dct += snu * t.ct[k * S + s];
+      for (int a = 0; a < 6; ++a) {
+        const int k = spw[a] & 0xffff;
+        pw[a] = t.C[k * S + s]; pm[a] = 1.0;
+        const double2 gh = *reinterpret_cast<const double2*>(t.th4 + (k * S + s) * 4);
+        const double2 ec = *reinterpret_cast<const double2*>(t.th4 + (k * S + s) * 4 + 2);
+        if (a < 3) { dg -= gh.x; dh -= gh.y; dEt -= ec.x; dct -= ec.y; }
+        else { dg += gh.x; dh += gh.y; dEt += ec.x; dct += ec.y; }
+      }
+    } else {
+#pragma unroll
+      for (int a = 0; a < 6; ++a) {
+        const int k = spw[a] & 0xffff, nu = spw[a] >> 16;
+        const double Ck = t.C[k * S + s];
+        pw[a] = ipow(Ck, nu); pm[a] = dpow(Ck, nu);
+        const double2 gh = *reinterpret_cast<const double2*>(t.th4 + (k * S + s) * 4);
+        const double2 ec = *reinterpret_cast<const double2*>(t.th4 + (k * S + s) * 4 + 2);
+        const double snu = a < 3 ? -(double)nu : (double)nu;
+        dg += snu * gh.x; dh += snu * gh.y; dEt += snu * ec.x; dct += snu * ec.y;
       }
     }
     const double Pif = pw[0] * pw[1] * pw[2], Pir = pw[3] * pw[4] * pw[5];
@@ -294,11 +357,11 @@ __device__ __forceinline__ void phases01(const DevMech& m, Tile<S, JAC>& t, int 
     const double dRdT = lam_f * Rf - lam_r * Rr;
     // a5: third body / falloff
     double c = 1.0, X = 0.0, GT = dRdT, MdcdM_R = 0.0;
-    const int e0 = m.eff_ptr[r], e1 = m.eff_ptr[r + 1];
+    const int e0 = __ldg(m.eff_ptr + r), e1 = __ldg(m.eff_ptr + r + 1);
     const double adef = (info & INFO_ADEF) ? 1.0 : 0.0;
     if (type >= PYJAC_THIRD_BODY && type <= PYJAC_FALLOFF_SRI) {
       double M = adef * Ctot;                       // sum_k C_k == C_tot by construction of C_Ns
-      for (int e = e0; e < e1; ++e) M += m.eff_d[e] * t.C[m.eff_sp[e] * S + s];
+      for (int e = e0; e < e1; ++e) M += __ldg(m.eff_d + e) * t.C[__ldg(m.eff_sp + e) * S + s];
       if (type == PYJAC_THIRD_BODY) {
         c = M; X = Rn; GT = M * dRdT; MdcdM_R = M * Rn;
       } else {
@@ -310,7 +373,7 @@ __device__ __forceinline__ void phases01(const DevMech& m, Tile<S, JAC>& t, int 
         const double i1p = 1.0 / (1.0 + Pr);
         c = bl.F * Pr * i1p;
         const double dc_dPr = bl.F * i1p * i1p + Pr * i1p * bl.dF_dPr;
-        const double dPr_dT = Pr * (b0 - m.beta[r] + (Ta0 - m.Ta[r]) * invT) * invT;
+        const double dPr_dT = Pr * (b0 - __ldg(m.beta + r) + (Ta0 - __ldg(m.Ta + r)) * invT) * invT;
         X = dc_dPr * k0_kinf * Rn;
         GT = (dc_dPr * dPr_dT + Pr * i1p * bl.dF_dT) * Rn + c * dRdT;
         MdcdM_R = Pr * dc_dPr * Rn;
@@ -318,13 +381,13 @@ __device__ __forceinline__ void phases01(const DevMech& m, Tile<S, JAC>& t, int 
     }
     const double q = c * Rn;
     // reaction-sum reductions (R4-7/8): N = sum dE~_i q_i, S = sum dn~_i q_i
-    const double dn = m.dn[r];
+    const double dn = __ldg(m.dn + r);
     acc[0] += dEt * q; acc[1] += dn * q;
     if (!JAC) {
       t.P[idx] = q;
     } else {
       // a8: per-reaction partials -> slots
-      const int base = m.slot_base[r];
+      const int base = __ldg(m.slot_base + r);
       const int nre = (info >> INFO_NREAC_SHIFT) & 3, npr = (info >> INFO_NPROD_SHIFT) & 3;
       const double a_ = c * kf, b_ = c * kr;
       double GL = adef * X;                          // full dQ_i/dC_Ns
@@ -340,16 +403,15 @@ __device__ __forceinline__ void phases01(const DevMech& m, Tile<S, JAC>& t, int 
           if (a < npr) { t.P[(slot++) * S + s] = dr[a]; if ((int)(spw[3 + a] & 0xffff) == L) GL += dr[a]; }
       }
       for (int e = e0; e < e1; ++e) {
-        const double v = m.eff_d[e] * X;
+        const double v = __ldg(m.eff_d + e) * X;
         t.P[(slot++) * S + s] = v;
-        if (m.eff_sp[e] == L) GL += v;
+        if (__ldg(m.eff_sp + e) == L) GL += v;
       }
       // chain rule to the state variables (R4-2); E column in Euler-homogeneity form (R4-6)
       const double slotT = V * (GT - ctot_T * GL);
       double slotE;
       if (mode == PYJAC_CONP) {
-        const int of = (int)(spw[0] >> 16) + (int)(spw[1] >> 16) + (int)(spw[2] >> 16);
-        const int orv = (int)(spw[3] >> 16) + (int)(spw[4] >> 16) + (int)(spw[5] >> 16);
+        const int of = (info >> INFO_OF_SHIFT) & 15, orv = (info >> INFO_OR_SHIFT) & 15;
         slotE = q - c * ((double)of * Rf - (double)orv * Rr) - MdcdM_R + Ctot * GL;
       } else {
         slotE = V * (c * dlnk_dP * Rn + GL / RT);
@@ -360,6 +422,7 @@ __device__ __forceinline__ void phases01(const DevMech& m, Tile<S, JAC>& t, int 
       acc[2] += dEt * slotT; acc[3] += dn * slotT; acc[4] += dEt * slotE; acc[5] += dn * slotE; acc[6] += dct * q;
     }
   }
+  TICK(1);
   if (JAC) block_reduce<S, 7>(acc, t.red, t.sc, SC_R0);
   else { double a2[2] = {acc[0], acc[1]}; block_reduce<S, 2>(a2, t.red, t.sc, SC_R0); }
 }
@@ -367,6 +430,56 @@ __device__ __forceinline__ void phases01(const DevMech& m, Tile<S, JAC>& t, int 
 }  // namespace
 
 namespace {
+
+// ---------------------------------------------------------------------------------------------------
+// Gather engine: every output gathers a static list of shared-memory slots.  Items come in order of
+// descending list length.  The first n_long items (lists longer than LONG_LIST) are gathered by a whole warp
+// (lanes stride the list, shuffle reduction).  The others sit in ELL super-groups of ELL_W = 128 items, lists padded
+// to the group's longest and stored entry-major: a thread owns 4 items of a group, so its 4 entry loads per step are
+// independent (latency hiding) and the 32 lanes read 32 consecutive entries (coalesced).
+//   acc(const int32_t* entry, double (&v)[NACC])      accumulate one entry
+//   store(int slot, const double (&v)[NACC])          slot = processing slot (index into the position arrays)
+// ---------------------------------------------------------------------------------------------------
+template <int S, int STRIDE, int NACC, int U, class AccF, class StoreF>
+__device__ __forceinline__ void gather(const DevGather& g, int* counter, AccF acc, StoreF store) {
+  const int lane = threadIdx.x & 31, sub = lane / S;
+  constexpr int IPW = 32 / S;                 // items of one warp per "u"
+  // a unit = U * IPW items of one super-group; a thread owns U items (U independent loads per step)
+  constexpr int UPG = ELL_W / (U * IPW);      // units per super-group
+  const int n_work = g.n_long + g.n_sg * UPG;
+  for (int w = next_chunk(counter); w < n_work; w = next_chunk(counter)) {
+    if (w < g.n_long) {                        // a long list: the whole warp strides it
+      const int p1 = __ldg(g.long_ptr + w + 1);
+      double v[NACC];
+#pragma unroll
+      for (int a = 0; a < NACC; ++a) v[a] = 0.0;
+#pragma unroll 2
+      for (int p = __ldg(g.long_ptr + w) + sub; p < p1; p += IPW) acc(g.long_ent + p * STRIDE, v);
+#pragma unroll
+      for (int a = 0; a < NACC; ++a) v[a] = group_sum<S>(v[a]);
+      if (lane < S) store(w, v);
+    } else {
+      const int unit = w - g.n_long;
+      const int sg = unit / UPG;
+      const int il0 = (unit % UPG) * (U * IPW) + sub;
+      const int2 meta = __ldg(reinterpret_cast<const int2*>(g.sg_meta) + sg);      // entry offset, padded length
+      const int32_t* __restrict__ e = g.ell_ent + (meta.x + il0) * STRIDE;
+      double v[U][NACC];
+#pragma unroll
+      for (int u = 0; u < U; ++u)
+#pragma unroll
+        for (int a = 0; a < NACC; ++a) v[u][a] = 0.0;
+#pragma unroll 4
+      for (int p = 0; p < meta.y; ++p) {
+#pragma unroll
+        for (int u = 0; u < U; ++u) acc(e + (p * ELL_W + u * IPW) * STRIDE, v[u]);
+      }
+      const int slot0 = g.n_long + sg * ELL_W + il0;
+#pragma unroll
+      for (int u = 0; u < U; ++u) store(slot0 + u * IPW, v[u]);
+    }
+  }
+}
 
 // ---------------------------------------------------------------------------------------------------
 // source terms: Eqs. 3-8
@@ -378,34 +491,24 @@ source_kernel(const DevMech m, int mode, int64_t n_states, int64_t tile, const d
   extern __shared__ __align__(16) double smem[];
   Tile<S, false> t(smem, m.ns, m.nr, m.nslots);
   const int64_t s0 = (int64_t)blockIdx.x * S;
-  phases01<S, false>(m, t, mode, s0, n_states, tile, phi, param);
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, s = lane % S, sub = lane / S;
-  const int L = m.ns - 1;
+  __shared__ int cnt[N_CNT];
+  long long tick_ = 0;
+  phases01<S, false>(m, t, mode, s0, n_states, tile, phi, param, cnt, tick_);
+  const int s = threadIdx.x % S;
   const bool valid = s0 + s < n_states;
   const int64_t obase = state_base(min(s0 + s, n_states - 1), tile, m.nvar);
   const double V = t.sc[SC_V * S + s];
-  // a7: omega_k = sum_i nu_ki q_i (Eq. 4), dn_k/dt = V omega_k (Eq. 3).  Species in order of descending list
-  // length: a warp gathers each long list cooperatively, then one thread per (species, state)
-  for (int q = warp; q < m.nb_long; q += NW) {
-    const int p1 = m.b_ptr[q + 1];
-    double w = 0.0;
-    for (int p = m.b_ptr[q] + sub; p < p1; p += 32 / S) {
-      const uint32_t ent = (uint32_t)m.bq_ent[p];
-      w += apply_sign(t.P[(ent & ~SIGN_BIT) * S + s], ent);
-    }
-    w = group_sum<S>(w);
-    if (lane < S && valid) out[obase + (int64_t)(2 + m.b_item[q]) * tile] = V * w;
-  }
-  for (int idx = m.nb_long * S + threadIdx.x; idx < L * S; idx += NT) {
-    const int q = idx / S;
-    const int p1 = m.b_ptr[q + 1];
-    double w = 0.0;
-    for (int p = m.b_ptr[q]; p < p1; ++p) {
-      const uint32_t ent = (uint32_t)m.bq_ent[p];
-      w += apply_sign(t.P[(ent & ~SIGN_BIT) * S + s], ent);
-    }
-    if (valid) out[obase + (int64_t)(2 + m.b_item[q]) * tile] = V * w;
-  }
+  // a7: omega_k = sum_i nu_ki q_i (Eq. 4), dn_k/dt = V omega_k (Eq. 3)
+  const double* __restrict__ P = t.P;
+  gather<S, 1, 1, PYJAC_UQ>(m.qplan, cnt + CNT_Q,
+      [&](const int32_t* e, double (&v)[1]) {
+        const uint32_t ent = (uint32_t)__ldg(e);
+        v[0] += apply_sign(P[(ent & ~SIGN_BIT) * S + s], ent);
+      },
+      [&](int slot, const double (&v)[1]) {
+        const int k = __ldg(m.q_item + slot);
+        if (k >= 0 && valid) out[obase + (int64_t)(2 + k) * tile] = V * v[0];
+      });
   if (threadIdx.x < S && valid) {
     const double T = t.sc[SC_T * S + s], Pp = t.sc[SC_P * S + s];
     const double fT = -t.sc[SC_R0 * S + s] / t.sc[SC_D * S + s];          // Eq. 5
@@ -427,8 +530,15 @@ jacobian_kernel(const DevMech m, const DevPlan pl, int mode, int64_t n_states, i
   extern __shared__ __align__(16) double smem[];
   Tile<S, true> t(smem, m.ns, m.nr, m.nslots);
   const int64_t s0 = (int64_t)blockIdx.x * S;
-  phases01<S, true>(m, t, mode, s0, n_states, tile, phi, param);
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, s = lane % S, sub = lane / S;
+  __shared__ int cnt[N_CNT];
+#ifdef PYJAC_TIMING
+  long long tick_ = clock64();
+#else
+  long long tick_ = 0;
+#endif
+  phases01<S, true>(m, t, mode, s0, n_states, tile, phi, param, cnt, tick_);
+  TICK(2);
+  const int tid = threadIdx.x, s = tid % S;
   const int L = m.ns - 1;
   const bool valid = s0 + s < n_states;
   const int64_t obase = state_base(min(s0 + s, n_states - 1), tile, pl.n_e);
@@ -443,106 +553,46 @@ jacobian_kernel(const DevMech m, const DevPlan pl, int mode, int64_t n_states, i
       if (!((pl.nzmask[e >> 5] >> (e & 31)) & 1u) && valid) out[obase + (int64_t)e * tile] = 0.0;
     }
   }
-  // Gather engine: items come in order of descending list length.  The first n_long items (list
-  // longer than LONG_LIST) are gathered by a whole warp (lanes stride the list, shuffle reduction); the others by
-  // one thread per (item, state) -- the 32 lists of a warp then have nearly the same length (no divergence tail).
-  // a9: species block, J[k][j] = sum_i nu_ki (Ghat^j_i - Ghat^Ns_i); every nonzero is stored once
-  for (int e = warp; e < pl.nA_long; e += NW) {
-    const int p1 = pl.a_ptr[e + 1];
-    double v = 0.0;
-    for (int p = pl.a_ptr[e] + sub; p < p1; p += 32 / S) {
-      const uint32_t ent = (uint32_t)pl.a_ent[p];
-      v += apply_sign(t.P[(ent & ~SIGN_BIT) * S + s], ent);
-    }
-    v = group_sum<S>(v);
-    if (lane < S && valid) out[obase + (int64_t)pl.a_pos[e] * tile] = v;
-  }
-  for (int idx = pl.nA_long * S + tid; idx < pl.nA * S; idx += NT) {
-    const int e = idx / S;
-    const int p1 = pl.a_ptr[e + 1];
-    double v = 0.0;
-    for (int p = pl.a_ptr[e]; p < p1; ++p) {
-      const uint32_t ent = (uint32_t)pl.a_ent[p];
-      v += apply_sign(t.P[(ent & ~SIGN_BIT) * S + s], ent);
-    }
-    if (valid) out[obase + (int64_t)pl.a_pos[e] * tile] = v;
-  }
-  // a9: T and E columns of the species rows: J[k][T] = sum_i nu_ki slotT_i, J[k][E] = sum_i nu_ki slotE_i
-  for (int q = warp; q < m.nb_long; q += NW) {
-    const int p1 = m.b_ptr[q + 1];
-    double vT = 0.0, vE = 0.0;
-    for (int p = m.b_ptr[q] + sub; p < p1; p += 32 / S) {
-      const uint32_t ent = (uint32_t)m.b_ent[p];
-      const int off = (ent & ~SIGN_BIT) * S + s;
-      vT += apply_sign(t.P[off], ent);
-      vE += apply_sign(t.P[off + S], ent);
-    }
-    vT = group_sum<S>(vT); vE = group_sum<S>(vE);
-    if (lane < S && valid) {
-      const int k = m.b_item[q];
-      out[obase + (int64_t)pl.b_pos[k] * tile] = vT;
-      out[obase + (int64_t)pl.b_pos[L + k] * tile] = vE;
-    }
-  }
-  for (int idx = m.nb_long * S + tid; idx < L * S; idx += NT) {
-    const int q = idx / S;
-    const int p1 = m.b_ptr[q + 1];
-    double vT = 0.0, vE = 0.0;
-    for (int p = m.b_ptr[q]; p < p1; ++p) {
-      const uint32_t ent = (uint32_t)m.b_ent[p];
-      const int off = (ent & ~SIGN_BIT) * S + s;
-      vT += apply_sign(t.P[off], ent);
-      vE += apply_sign(t.P[off + S], ent);
-    }
-    if (valid) {
-      const int k = m.b_item[q];
-      out[obase + (int64_t)pl.b_pos[k] * tile] = vT;
-      out[obase + (int64_t)pl.b_pos[L + k] * tile] = vE;
-    }
-  }
+  TICK(3);
+  // a9: species rows.  Block entries J[k][j] = sum_i nu_ki (Ghat^j_i - Ghat^Ns_i); T and E columns
+  // J[k][T] = sum_i nu_ki slotT_i, J[k][E] = sum_i nu_ki slotE_i.  Every nonzero is finished in a register and
+  // stored once.
+  const double* __restrict__ P = t.P;
+  gather<S, 1, 1, PYJAC_UJ>(pl.jplan, cnt + CNT_J,
+      [&](const int32_t* e, double (&v)[1]) {
+        const uint32_t ent = (uint32_t)__ldg(e);
+        v[0] += apply_sign(P[(ent & ~SIGN_BIT) * S + s], ent);
+      },
+      [&](int slot, const double (&v)[1]) {
+        const int pos = __ldg(pl.j_pos + slot);
+        if (pos >= 0 && valid) out[obase + (int64_t)pos * tile] = v[0];
+      });
+  TICK(4);
   // a10: T and E rows, species columns: gather over reactions with the per-state weights dE~_i, dn~_i
   //   J[T][j] = -(sum_i dE~_i g_ij + f_T (c_j - c_Ns)) / (D V);  J[E][j] = cS sum_i dn~_i g_ij + cT J[T][j]
   const double cL = t.ck[L * S + s];
   const double iDV = 1.0 / (D * V);
   const double cS = mode == PYJAC_CONP ? T * R_GAS / Pp : T * R_GAS / V;
   const double cT = mode == PYJAC_CONP ? V / T : Pp / T;
-  const int2* __restrict__ c_ent2 = reinterpret_cast<const int2*>(m.c_ent);
-  for (int q = warp; q < m.nc_long; q += NW) {
-    const int p1 = m.c_ptr[q + 1];
-    double vT = 0.0, vS = 0.0;
-    for (int p = m.c_ptr[q] + sub; p < p1; p += 32 / S) {
-      const int2 pr = c_ent2[p];
-      const uint32_t ent = (uint32_t)pr.x;
-      const double x = apply_sign(t.P[(ent & ~SIGN_BIT) * S + s], ent);
-      vT += t.dE[pr.y * S + s] * x;
-      vS += m.dn[pr.y] * x;
-    }
-    vT = group_sum<S>(vT); vS = group_sum<S>(vS);
-    if (lane < S && valid) {
-      const int j = m.c_item[q];
-      const double JT = -(vT + fT * (t.ck[j * S + s] - cL)) * iDV;
-      out[obase + (int64_t)pl.c_pos[j] * tile] = JT;
-      out[obase + (int64_t)pl.c_pos[L + j] * tile] = cS * vS + cT * JT;
-    }
-  }
-  for (int idx = m.nc_long * S + tid; idx < L * S; idx += NT) {
-    const int q = idx / S;
-    const int p1 = m.c_ptr[q + 1];
-    double vT = 0.0, vS = 0.0;
-    for (int p = m.c_ptr[q]; p < p1; ++p) {
-      const int2 pr = c_ent2[p];
-      const uint32_t ent = (uint32_t)pr.x;
-      const double x = apply_sign(t.P[(ent & ~SIGN_BIT) * S + s], ent);
-      vT += t.dE[pr.y * S + s] * x;
-      vS += m.dn[pr.y] * x;
-    }
-    if (valid) {
-      const int j = m.c_item[q];
-      const double JT = -(vT + fT * (t.ck[j * S + s] - cL)) * iDV;
-      out[obase + (int64_t)pl.c_pos[j] * tile] = JT;
-      out[obase + (int64_t)pl.c_pos[L + j] * tile] = cS * vS + cT * JT;
-    }
-  }
+  const double* __restrict__ dE = t.dE;
+  gather<S, 4, 2, PYJAC_UC>(m.cplan, cnt + CNT_C,
+      [&](const int32_t* e, double (&v)[2]) {
+        const int4 pr = __ldg(reinterpret_cast<const int4*>(e));      // slot | sign, reaction, dn~ (2 words)
+        const uint32_t ent = (uint32_t)pr.x;
+        const double x = apply_sign(P[(ent & ~SIGN_BIT) * S + s], ent);
+        v[0] += dE[pr.y * S + s] * x;
+        v[1] += __hiloint2double(pr.w, pr.z) * x;
+      },
+      [&](int slot, const double (&v)[2]) {
+        const int posT = __ldg(pl.c_pos + 2 * slot);
+        if (posT >= 0 && valid) {
+          const int j = m.c_item[slot];
+          const double JT = -(v[0] + fT * (t.ck[j * S + s] - cL)) * iDV;
+          out[obase + (int64_t)posT * tile] = JT;
+          out[obase + (int64_t)pl.c_pos[2 * slot + 1] * tile] = cS * v[1] + cT * JT;
+        }
+      });
+  TICK(5);
   // a10: the four corner entries from the phase-1 reductions (R4-7)
   if (tid < S && valid) {
     const double Ctot = t.sc[SC_CTOT * S + s];
@@ -586,7 +636,7 @@ template <int S> int launch_jac_S(const DevMech& m, const DevPlan& p, const Laun
   return (int)cudaGetLastError();
 }
 
-constexpr size_t SMEM_LIMIT = 227 * 1024;
+constexpr size_t SMEM_LIMIT = 227 * 1024 - 64;   // dynamic part; 64 B left for the static work counters
 
 }  // namespace
 

@@ -152,4 +152,5 @@ def test_eval_host_matches_device_path(pj):
     out = np.empty(M.nnz * 256)
     pj.pyjac_eval_host(M.h, pj.WHAT_SPARSE, mg.CONP, mg.CSR, 256, 256, 256, phi, par, out)
     got = run_gpu(pj, M, pj.WHAT_SPARSE, mg.CONP, mg.CSR, states)
-    assert np.array_equal(unpack(out, M.nnz, 256, 256, 256), got)
+    # not bitwise: warps take reaction chunks dynamically, so the order of the reaction sums varies run to run
+    np.testing.assert_allclose(unpack(out, M.nnz, 256, 256, 256), got, rtol=1e-11, atol=0)
