@@ -31,11 +31,11 @@ struct pyjac_mech {
   ~pyjac_mech() {
     for (void* p : allocs) cudaFree(p);
   }
-  int upload_plan(const GatherPlan& g, DevGather* out) {
-    out->n_long = g.n_long; out->n_sg = g.n_sg;
-    if (int r = upload(g.long_ptr, &out->long_ptr)) return r;
-    if (int r = upload(g.long_ent, &out->long_ent)) return r;
+  int upload_plan(const GatherPlan& g, int part_base, DevGather* out) {
+    out->n_sg = g.n_sg; out->n_comb = (int)g.comb_item.size(); out->part_base = part_base;
     if (int r = upload(g.sg_meta, &out->sg_meta)) return r;
+    if (int r = upload(g.comb_first, &out->comb_first)) return r;
+    if (int r = upload(g.comb_nseg, &out->comb_nseg)) return r;
     return upload(g.ell_ent, &out->ell_ent);
   }
   template <class T> int upload(const std::vector<T>& v, const T** out) {
@@ -79,17 +79,20 @@ int pyjac_mech_create(const pyjac_mech_desc* desc, int cuda_device, pyjac_mech**
     HostTables& h = m->h;
     DevMech& d = m->dm;
     d.ns = h.ns; d.nr = h.nr; d.nvar = h.nvar; d.nslots = h.nslots;
+    d.n_part_jac = h.n_part_jac; d.n_part_src = h.n_part_src;
 #define UP(field) if (int r_ = m->upload(h.field, &d.field)) return r_;
     UP(nasa) UP(wr) UP(lnA) UP(beta) UP(Ta) UP(dn) UP(info) UP(aux) UP(sp) UP(eff_ptr) UP(eff_sp) UP(eff_d)
     UP(slot_base) UP(fall) UP(plog_ptr) UP(plog_P) UP(plog_lnP) UP(plog_lnA) UP(plog_b) UP(plog_Ta)
     UP(cheb_meta) UP(cheb_lim) UP(cheb_coef)
 #undef UP
-    if (int r_ = m->upload_plan(h.cplan, &d.cplan)) return r_;
-    if (int r_ = m->upload_plan(h.qplan, &d.qplan)) return r_;
-    if (int r_ = m->upload(h.qplan.item, &d.q_item)) return r_;
-    if (int r_ = m->upload(h.cplan.item, &d.c_item)) return r_;
+    if (int r_ = m->upload_plan(h.cplan, h.jplan.n_part, &d.cplan)) return r_;      // C partials follow the J partials
+    if (int r_ = m->upload_plan(h.qplan, 0, &d.qplan)) return r_;
+    if (int r_ = m->upload(h.q_target, &d.q_target)) return r_;
+    if (int r_ = m->upload(h.cplan.target, &d.c_item)) return r_;
+    if (int r_ = m->upload(h.qplan.comb_item, &d.qc_item)) return r_;
+    if (int r_ = m->upload(h.cplan.comb_item, &d.cc_item)) return r_;
     DevGather jplan;
-    if (int r_ = m->upload_plan(h.jplan, &jplan)) return r_;
+    if (int r_ = m->upload_plan(h.jplan, 0, &jplan)) return r_;
     const uint32_t* mask[2];
     for (int p = 0; p < 2; ++p)
       if (int r_ = m->upload(h.nzmask[p], &mask[p])) return r_;
@@ -99,6 +102,8 @@ int pyjac_mech_create(const pyjac_mech_desc* desc, int cuda_device, pyjac_mech**
       pl.jplan = jplan;
       if (int r_ = m->upload(h.j_pos[f], &pl.j_pos)) return r_;
       if (int r_ = m->upload(h.c_pos[f], &pl.c_pos)) return r_;
+      if (int r_ = m->upload(h.jc_pos[f], &pl.jc_pos)) return r_;
+      if (int r_ = m->upload(h.cc_pos[f], &pl.cc_pos)) return r_;
       for (int j = 0; j < 4; ++j) pl.d_pos[j] = h.d_pos[f][j];
       pl.nzmask = f < 2 ? nullptr : mask[f & 1];
     }

@@ -72,53 +72,54 @@ int validate(const pyjac_mech_desc* d, std::string& err) {
 }
 
 
-// Gather plan: items in order of DESCENDING list length.  Lists longer than LONG_LIST are kept in CSR form and
-// gathered by a whole warp; the others are packed in ELL "super-groups" of ELL_W items whose lists are padded
-// (with entries pointing at an always-zero slot) to the longest list of the group and stored entry-major, so
-// that the 32 lanes of a warp read 32 consecutive entries and a thread can keep several loads in flight.
-// stride = ints per entry (1: slot | sign; 2: slot | sign, reaction).
-int long_list_threshold() {
-  const char* e = std::getenv("PYJAC_LONG_LIST");
-  const int v = e ? std::atoi(e) : LONG_LIST_DEFAULT;
-  return v > 0 ? v : LONG_LIST_DEFAULT;
+// Gather plan.  Every list is cut into segments of at most SEG entries; the segments,
+// sorted by DESCENDING length, are packed in ELL "super-groups" of ELL_W segments, padded (with entries pointing at
+// an always-zero slot) to the longest segment of the group and stored entry-major: the 32 lanes of a warp read 32
+// consecutive entries and a thread keeps several independent loads in flight.  A list that fits one segment is
+// stored straight to the output; the segments of a split list leave partial sums in shared memory which a short
+// second pass combines.  stride = ints per entry.
+int seg_len() {
+  const char* e = std::getenv("PYJAC_SEG_LEN");
+  const int v = e ? std::atoi(e) : SEG_LEN_DEFAULT;
+  return v > 0 ? v : SEG_LEN_DEFAULT;
 }
 
 void build_gather(const std::vector<std::vector<int32_t>>& lists, int stride, int zero_slot, GatherPlan& g) {
-  const int LONG_LIST = long_list_threshold();
+  const int SEG = seg_len();
   const int n = (int)lists.size();
-  std::vector<int> order(n);
-  std::iota(order.begin(), order.end(), 0);
-  auto len = [&](int i) { return (int)lists[i].size() / stride; };
-  std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return len(a) > len(b); });
   g = GatherPlan();
   g.stride = stride;
-  g.long_ptr.assign(1, 0);
-  while (g.n_long < n && len(order[g.n_long]) > LONG_LIST) {
-    const auto& l = lists[order[g.n_long]];
-    g.long_ent.insert(g.long_ent.end(), l.begin(), l.end());
-    g.long_ptr.push_back((int)g.long_ent.size() / stride);
-    g.item.push_back(order[g.n_long]);
-    ++g.n_long;
+  struct Seg { int item, p0, len, target; };
+  std::vector<Seg> segs;
+  for (int i = 0; i < n; ++i) {
+    const int len = (int)lists[i].size() / stride;
+    g.n_entries += len;
+    if (len <= SEG) { segs.push_back({i, 0, len, i}); continue; }
+    const int nseg = (len + SEG - 1) / SEG;
+    g.comb_item.push_back(i); g.comb_first.push_back(g.n_part); g.comb_nseg.push_back(nseg);
+    for (int q = 0; q < nseg; ++q) {               // nearly equal pieces
+      const int a = (int)((int64_t)len * q / nseg), b = (int)((int64_t)len * (q + 1) / nseg);
+      segs.push_back({i, a, b - a, -2 - g.n_part++});
+    }
   }
-  const int n_short = n - g.n_long;
-  g.n_sg = (n_short + ELL_W - 1) / ELL_W;
+  std::stable_sort(segs.begin(), segs.end(), [](const Seg& a, const Seg& b) { return a.len > b.len; });
+  const int ns_ = (int)segs.size();
+  g.n_sg = (ns_ + ELL_W - 1) / ELL_W;
   int off = 0;
   for (int sg = 0; sg < g.n_sg; ++sg) {
-    const int i0 = g.n_long + sg * ELL_W;
-    const int width = len(order[i0]);                 // sorted: the first list of the group is the longest
+    const int i0 = sg * ELL_W;
+    const int width = segs[i0].len;                   // sorted: the first segment of the group is the longest
     g.sg_meta.push_back(off); g.sg_meta.push_back(width);
     for (int p = 0; p < width; ++p)
       for (int w = 0; w < ELL_W; ++w) {
-        const int i = i0 + w;
-        const bool real = i < n && p < len(order[i]);
-        for (int c = 0; c < stride; ++c) g.ell_ent.push_back(real ? lists[order[i]][p * stride + c] : (c == 0 ? zero_slot : 0));
+        const bool real = i0 + w < ns_ && p < segs[i0 + w].len;
+        for (int c = 0; c < stride; ++c)
+          g.ell_ent.push_back(real ? lists[segs[i0 + w].item][(segs[i0 + w].p0 + p) * stride + c] : (c == 0 ? zero_slot : 0));
       }
     off += width * ELL_W;
-    for (int w = 0; w < ELL_W; ++w) g.item.push_back(i0 + w < n ? order[i0 + w] : -1);
+    for (int w = 0; w < ELL_W; ++w) g.target.push_back(i0 + w < ns_ ? segs[i0 + w].target : -1);
   }
-  g.n_entries = 0;
-  for (int i = 0; i < n; ++i) g.n_entries += len(i);
-  g.n_padded = (int64_t)g.long_ent.size() / stride + off;
+  g.n_padded = off;
 }
 
 }  // namespace
@@ -358,16 +359,23 @@ int build_host_tables(const pyjac_mech_desc* d, HostTables& h, std::string& err)
   }
   build_gather(clists, 4, h.nslots, h.cplan);            // T and E rows: (slot | sign, reaction, dn~)
   build_gather(qlists, 1, nr, h.qplan);                  // source terms: omega_k = sum nu_ki q_i
+  h.q_target = h.qplan.target;
+  h.n_part_jac = h.jplan.n_part + 2 * h.cplan.n_part;
+  h.n_part_src = h.qplan.n_part;
   for (int fmt = 0; fmt < 4; ++fmt) {
-    h.j_pos[fmt].assign(h.jplan.item.size(), -1);
-    for (size_t e = 0; e < h.jplan.item.size(); ++e)
-      if (h.jplan.item[e] >= 0) h.j_pos[fmt][e] = pos_of(fmt, jitems[h.jplan.item[e]].r, jitems[h.jplan.item[e]].c);
-    h.c_pos[fmt].assign(2 * h.cplan.item.size(), -1);
-    for (size_t e = 0; e < h.cplan.item.size(); ++e)
-      if (h.cplan.item[e] >= 0) {
-        h.c_pos[fmt][2 * e] = pos_of(fmt, 0, 2 + h.cplan.item[e]);
-        h.c_pos[fmt][2 * e + 1] = pos_of(fmt, 1, 2 + h.cplan.item[e]);
-      }
+    h.j_pos[fmt] = h.jplan.target;                     // padding and partial codes stay as they are
+    for (size_t e = 0; e < h.jplan.target.size(); ++e)
+      if (h.jplan.target[e] >= 0) h.j_pos[fmt][e] = pos_of(fmt, jitems[h.jplan.target[e]].r, jitems[h.jplan.target[e]].c);
+    h.jc_pos[fmt].clear();
+    for (int it : h.jplan.comb_item) h.jc_pos[fmt].push_back(pos_of(fmt, jitems[it].r, jitems[it].c));
+    h.c_pos[fmt].assign(2 * h.cplan.target.size(), -1);
+    for (size_t e = 0; e < h.cplan.target.size(); ++e) {
+      const int tg = h.cplan.target[e];
+      h.c_pos[fmt][2 * e] = tg;
+      if (tg >= 0) { h.c_pos[fmt][2 * e] = pos_of(fmt, 0, 2 + tg); h.c_pos[fmt][2 * e + 1] = pos_of(fmt, 1, 2 + tg); }
+    }
+    h.cc_pos[fmt].clear();
+    for (int it : h.cplan.comb_item) { h.cc_pos[fmt].push_back(pos_of(fmt, 0, 2 + it)); h.cc_pos[fmt].push_back(pos_of(fmt, 1, 2 + it)); }
     h.d_pos[fmt][0] = pos_of(fmt, 0, 0); h.d_pos[fmt][1] = pos_of(fmt, 0, 1);
     h.d_pos[fmt][2] = pos_of(fmt, 1, 0); h.d_pos[fmt][3] = pos_of(fmt, 1, 1);
   }

@@ -24,7 +24,7 @@ constexpr int INFO_NPROD_SHIFT = 14; // bits 14-15: number of product entries
 constexpr int INFO_OF_SHIFT = 16;    // bits 16-19: forward order  sum nu'
 constexpr int INFO_OR_SHIFT = 20;    // bits 20-23: reverse order  sum nu''
 constexpr uint32_t SIGN_BIT = 0x80000000u;
-constexpr int LONG_LIST_DEFAULT = 64; // gather lists longer than this are processed by a whole warp (env PYJAC_LONG_LIST)
+constexpr int SEG_LEN_DEFAULT = 32;   // gather lists longer than this are split into segments (env PYJAC_SEG_LEN)
 
 enum OutFmt { OUT_CSR = 0, OUT_CSC = 1, OUT_DENSE_C = 2, OUT_DENSE_F = 3 };
 
@@ -32,12 +32,14 @@ constexpr int ELL_W = 128;           // items per ELL super-group (4 items per l
 
 struct GatherPlan {
   int stride = 1;                            // ints per entry
-  int n_long = 0;                            // leading items gathered by a whole warp (CSR form)
-  std::vector<int32_t> long_ptr, long_ent;
-  int n_sg = 0;                              // ELL super-groups of ELL_W items
-  std::vector<int32_t> sg_meta;              // [n_sg*2]: entry offset, padded list length
+  int n_sg = 0;                              // ELL super-groups of ELL_W segments
+  std::vector<int32_t> sg_meta;              // [n_sg*2]: entry offset, padded segment length
   std::vector<int32_t> ell_ent;              // entry (p, w) of group sg at (off + p*ELL_W + w) * stride
-  std::vector<int32_t> item;                 // [n_long + n_sg*ELL_W] processing slot -> item id, -1 = padding
+  // processing slot (n_sg*ELL_W) -> what the segment's sum is: item id >= 0 (the whole list of that item: store
+  // the result), -1 padding, <= -2: partial sum number -2 - target of a list that was split into segments
+  std::vector<int32_t> target;
+  int n_part = 0;                            // partial sums (shared-memory scratch)
+  std::vector<int32_t> comb_item, comb_first, comb_nseg;   // split lists: item id, first partial, number of partials
   int64_t n_entries = 0, n_padded = 0;       // real / stored entries (padding overhead report)
 };
 
@@ -68,8 +70,11 @@ struct HostTables {
   GatherPlan jplan;                          // species rows: block nonzeros + their T and E columns
   GatherPlan cplan;                          // T and E rows, species columns: pairs (slot | sign, reaction)
   GatherPlan qplan;                          // source terms: omega_k gathers q_i
-  std::vector<int32_t> j_pos[4];             // [OutFmt][jplan.item.size()] output element (-1: padding)
-  std::vector<int32_t> c_pos[4];             // [OutFmt][2 * cplan.item.size()]: (T, j), (E, j)
+  std::vector<int32_t> j_pos[4];             // [OutFmt][jplan slots] output element; -1 padding; <= -2: partial -2 - x
+  std::vector<int32_t> c_pos[4];             // [OutFmt][2 * cplan slots]: (T, j), (E, j); same encoding in [2*slot]
+  std::vector<int32_t> jc_pos[4], cc_pos[4]; // [OutFmt] output elements of the split (combined) lists: [n_comb], [2*n_comb]
+  std::vector<int32_t> q_target;             // qplan: slot -> species (>= 0), -1, or partial code
+  int n_part_jac = 0, n_part_src = 0;        // doubles of partial-sum scratch per state
   int32_t d_pos[4][4];                       // (T,T) (T,E) (E,T) (E,E)
   std::vector<uint32_t> nzmask[2];           // dense bitmaps, bit e set iff dense element e ('C' / 'F' order) is in the pattern
   int nslots = 0;                            // total Jacobian slots
@@ -81,12 +86,12 @@ int build_host_tables(const pyjac_mech_desc* d, HostTables& h, std::string& err)
 
 // ---- device views ------------------------------------------------------------------------------
 struct DevGather {
-  int n_long, n_sg;
-  const int32_t *long_ptr, *long_ent, *sg_meta, *ell_ent;
+  int n_sg, n_comb, part_base;        // part_base: offset of this plan's partial sums in the scratch
+  const int32_t *sg_meta, *ell_ent, *comb_first, *comb_nseg;
 };
 
 struct DevMech {
-  int ns, nr, nvar, nslots;
+  int ns, nr, nvar, nslots, n_part_jac, n_part_src;
   const double *nasa, *wr;
   const double *lnA, *beta, *Ta, *dn;
   const int32_t *info, *aux;
@@ -100,13 +105,13 @@ struct DevMech {
   const int32_t* cheb_meta;
   const double *cheb_lim, *cheb_coef;
   DevGather cplan, qplan;
-  const int32_t *q_item, *c_item;   // processing slot -> species / column (-1: padding)
+  const int32_t *q_target, *c_item, *qc_item, *cc_item;   // slot -> species / column; combined lists -> species / column
 };
 
 struct DevPlan {
   int64_t n_e;               // elements per state in the output (nnz or nvar^2)
   DevGather jplan;
-  const int32_t *j_pos, *c_pos;
+  const int32_t *j_pos, *c_pos, *jc_pos, *cc_pos;
   int32_t d_pos[4];
   const uint32_t* nzmask;    // dense only (else nullptr)
 };

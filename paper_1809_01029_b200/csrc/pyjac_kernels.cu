@@ -53,10 +53,10 @@ constexpr int NRED = 8;           // reduction slots
 enum { SC_T = 0, SC_V, SC_P, SC_CTOT, SC_SUMC, SC_SUMCC, SC_SUMCDC, SC_D, SC_DDDT, SC_CNS,
        SC_R0, SC_R1, SC_R2, SC_R3, SC_R4, SC_R5, SC_R6, SC_R7, SC_INVT, SC_LNT, SC_LNP, SC_LNPRT, NSC };
 
-__host__ __device__ inline size_t smem_doubles(int ns, int nr, int nslots, int S, bool jac) {
+__host__ __device__ inline size_t smem_doubles(int ns, int nr, int nslots, int n_part, int S, bool jac) {
   // C[ns+1] (C[ns] = 1: dummy species of unused stoichiometric entries), th4[4(ns+1)], ck[ns], slots (+1 zero slot)
   size_t per_state = NSC + 6 * (size_t)ns + 5 + (jac ? (size_t)nslots + nr : (size_t)nr) + 1;
-  return per_state * S + (size_t)NW * NRED * S;
+  return (per_state + n_part) * S + (size_t)NW * NRED * S;      // n_part: partial sums of split gather lists
 }
 
 // Dynamic work distribution inside a CTA: items are sorted by descending cost at create time and warps take the
@@ -158,9 +158,9 @@ __device__ __forceinline__ Blend blend(int type, bool hasT2, const double* __res
 template <int S, bool JAC>
 struct Tile {
   // th4[(k*S + s)*4 + c]: c = 0 g_k/RT, 1 h_k/RT, 2 E~_k, 3 c~_k  (one 32-byte record per species and state)
-  double *sc, *C, *th4, *ck, *dE, *P, *red;
+  double *sc, *C, *th4, *ck, *dE, *P, *red, *part;
   __device__ __forceinline__ Tile(double* smem, int ns, int nr, int nslots) {
-    sc = smem; th4 = sc + NSC * S; C = th4 + 4 * (ns + 1) * S; ck = C + (ns + 1) * S; dE = ck + ns * S; P = JAC ? dE + nr * S : dE; red = P + ((JAC ? nslots : nr) + 1) * S;
+    sc = smem; th4 = sc + NSC * S; C = th4 + 4 * (ns + 1) * S; ck = C + (ns + 1) * S; dE = ck + ns * S; P = JAC ? dE + nr * S : dE; red = P + ((JAC ? nslots : nr) + 1) * S; part = red + NW * NRED * S;
     // source kernel: dE unused, P[r] = q_r.  P[nslots] (JAC) / P[nr] is an always-zero slot (ELL padding)
   }
 };
@@ -440,44 +440,60 @@ namespace {
 //   acc(const int32_t* entry, double (&v)[NACC])      accumulate one entry
 //   store(int slot, const double (&v)[NACC])          slot = processing slot (index into the position arrays)
 // ---------------------------------------------------------------------------------------------------
-template <int S, int STRIDE, int NACC, int U, class AccF, class StoreF>
-__device__ __forceinline__ void gather(const DevGather& g, int* counter, AccF acc, StoreF store) {
+template <int S, int STRIDE, int NACC, int U, class AccF, class PosF, class StoreF>
+__device__ __forceinline__ void gather(const DevGather& g, int* counter, AccF acc, PosF pos_of, StoreF store) {
   const int lane = threadIdx.x & 31, sub = lane / S;
-  constexpr int IPW = 32 / S;                 // items of one warp per "u"
-  // a unit = U * IPW items of one super-group; a thread owns U items (U independent loads per step)
+  constexpr int IPW = 32 / S;                 // segments of one warp per "u"
+  // a unit = U * IPW segments of one super-group; a thread owns U segments (U independent loads per step)
   constexpr int UPG = ELL_W / (U * IPW);      // units per super-group
-  const int n_work = g.n_long + g.n_sg * UPG;
-  for (int w = next_chunk(counter); w < n_work; w = next_chunk(counter)) {
-    if (w < g.n_long) {                        // a long list: the whole warp strides it
-      const int p1 = __ldg(g.long_ptr + w + 1);
-      double v[NACC];
+  const int n_work = g.n_sg * UPG;
+  const int2* __restrict__ metas = reinterpret_cast<const int2*>(g.sg_meta);      // entry offset, padded length
+  // software pipeline: the next unit's number and metadata are fetched while the current unit is processed, and
+  // the output positions are requested before the entry loop, so a unit costs one exposed L2 round trip, not three
+  int unit = next_chunk(counter);
+  int2 meta = make_int2(0, 0);
+  if (unit < n_work) meta = __ldg(metas + unit / UPG);
+  while (unit < n_work) {
+    const int next = next_chunk(counter);
+    int2 nmeta = make_int2(0, 0);
+    if (next < n_work) nmeta = __ldg(metas + next / UPG);
+    const int sg = unit / UPG;
+    const int il0 = (unit % UPG) * (U * IPW) + sub;
+    const int slot0 = sg * ELL_W + il0;
+    int pos[U];
 #pragma unroll
-      for (int a = 0; a < NACC; ++a) v[a] = 0.0;
-#pragma unroll 2
-      for (int p = __ldg(g.long_ptr + w) + sub; p < p1; p += IPW) acc(g.long_ent + p * STRIDE, v);
+    for (int u = 0; u < U; ++u) pos[u] = pos_of(slot0 + u * IPW);
+    const int32_t* __restrict__ e = g.ell_ent + (meta.x + il0) * STRIDE;
+    double v[U][NACC];
 #pragma unroll
-      for (int a = 0; a < NACC; ++a) v[a] = group_sum<S>(v[a]);
-      if (lane < S) store(w, v);
-    } else {
-      const int unit = w - g.n_long;
-      const int sg = unit / UPG;
-      const int il0 = (unit % UPG) * (U * IPW) + sub;
-      const int2 meta = __ldg(reinterpret_cast<const int2*>(g.sg_meta) + sg);      // entry offset, padded length
-      const int32_t* __restrict__ e = g.ell_ent + (meta.x + il0) * STRIDE;
-      double v[U][NACC];
+    for (int u = 0; u < U; ++u)
 #pragma unroll
-      for (int u = 0; u < U; ++u)
-#pragma unroll
-        for (int a = 0; a < NACC; ++a) v[u][a] = 0.0;
+      for (int a = 0; a < NACC; ++a) v[u][a] = 0.0;
 #pragma unroll 4
-      for (int p = 0; p < meta.y; ++p) {
+    for (int p = 0; p < meta.y; ++p) {
 #pragma unroll
-        for (int u = 0; u < U; ++u) acc(e + (p * ELL_W + u * IPW) * STRIDE, v[u]);
-      }
-      const int slot0 = g.n_long + sg * ELL_W + il0;
-#pragma unroll
-      for (int u = 0; u < U; ++u) store(slot0 + u * IPW, v[u]);
+      for (int u = 0; u < U; ++u) acc(e + (p * ELL_W + u * IPW) * STRIDE, v[u]);
     }
+#pragma unroll
+    for (int u = 0; u < U; ++u) store(slot0 + u * IPW, pos[u], v[u]);
+    unit = next; meta = nmeta;
+  }
+}
+
+// second pass over the lists that were split into segments: sum the partial sums, then finish(list, sums)
+template <int S, int NACC, class FinishF>
+__device__ __forceinline__ void combine(const DevGather& g, const double* __restrict__ part, FinishF finish) {
+  const int s = threadIdx.x % S;
+  for (int idx = threadIdx.x; idx < g.n_comb * S; idx += NT) {
+    const int c = idx / S;
+    const int first = g.part_base + NACC * __ldg(g.comb_first + c), n = __ldg(g.comb_nseg + c);
+    double v[NACC];
+#pragma unroll
+    for (int a = 0; a < NACC; ++a) v[a] = 0.0;
+    for (int q = 0; q < n; ++q)
+#pragma unroll
+      for (int a = 0; a < NACC; ++a) v[a] += part[(first + NACC * q + a) * S + s];
+    finish(c, v);
   }
 }
 
@@ -505,10 +521,17 @@ source_kernel(const DevMech m, int mode, int64_t n_states, int64_t tile, const d
         const uint32_t ent = (uint32_t)__ldg(e);
         v[0] += apply_sign(P[(ent & ~SIGN_BIT) * S + s], ent);
       },
-      [&](int slot, const double (&v)[1]) {
-        const int k = __ldg(m.q_item + slot);
-        if (k >= 0 && valid) out[obase + (int64_t)(2 + k) * tile] = V * v[0];
+      [&](int slot) { return __ldg(m.q_target + slot); },
+      [&](int, int k, const double (&v)[1]) {
+        if (k >= 0) { if (valid) out[obase + (int64_t)(2 + k) * tile] = V * v[0]; }
+        else if (k <= -2) t.part[(-2 - k) * S + s] = v[0];
       });
+  if (m.qplan.n_comb) {
+    __syncthreads();
+    combine<S, 1>(m.qplan, t.part, [&](int c, const double (&v)[1]) {
+      if (valid) out[obase + (int64_t)(2 + __ldg(m.qc_item + c)) * tile] = V * v[0];
+    });
+  }
   if (threadIdx.x < S && valid) {
     const double T = t.sc[SC_T * S + s], Pp = t.sc[SC_P * S + s];
     const double fT = -t.sc[SC_R0 * S + s] / t.sc[SC_D * S + s];          // Eq. 5
@@ -563,9 +586,10 @@ jacobian_kernel(const DevMech m, const DevPlan pl, int mode, int64_t n_states, i
         const uint32_t ent = (uint32_t)__ldg(e);
         v[0] += apply_sign(P[(ent & ~SIGN_BIT) * S + s], ent);
       },
-      [&](int slot, const double (&v)[1]) {
-        const int pos = __ldg(pl.j_pos + slot);
-        if (pos >= 0 && valid) out[obase + (int64_t)pos * tile] = v[0];
+      [&](int slot) { return __ldg(pl.j_pos + slot); },
+      [&](int, int pos, const double (&v)[1]) {
+        if (pos >= 0) { if (valid) out[obase + (int64_t)pos * tile] = v[0]; }
+        else if (pos <= -2) t.part[(-2 - pos) * S + s] = v[0];
       });
   TICK(4);
   // a10: T and E rows, species columns: gather over reactions with the per-state weights dE~_i, dn~_i
@@ -583,15 +607,34 @@ jacobian_kernel(const DevMech m, const DevPlan pl, int mode, int64_t n_states, i
         v[0] += dE[pr.y * S + s] * x;
         v[1] += __hiloint2double(pr.w, pr.z) * x;
       },
-      [&](int slot, const double (&v)[2]) {
-        const int posT = __ldg(pl.c_pos + 2 * slot);
-        if (posT >= 0 && valid) {
-          const int j = m.c_item[slot];
-          const double JT = -(v[0] + fT * (t.ck[j * S + s] - cL)) * iDV;
-          out[obase + (int64_t)posT * tile] = JT;
-          out[obase + (int64_t)pl.c_pos[2 * slot + 1] * tile] = cS * v[1] + cT * JT;
+      [&](int slot) { return __ldg(pl.c_pos + 2 * slot); },
+      [&](int slot, int posT, const double (&v)[2]) {
+        if (posT >= 0) {
+          if (valid) {
+            const int j = __ldg(m.c_item + slot);
+            const double JT = -(v[0] + fT * (t.ck[j * S + s] - cL)) * iDV;
+            out[obase + (int64_t)posT * tile] = JT;
+            out[obase + (int64_t)__ldg(pl.c_pos + 2 * slot + 1) * tile] = cS * v[1] + cT * JT;
+          }
+        } else if (posT <= -2) {
+          const int pi = m.cplan.part_base + 2 * (-2 - posT);
+          t.part[pi * S + s] = v[0]; t.part[(pi + 1) * S + s] = v[1];
         }
       });
+  if (pl.jplan.n_comb + m.cplan.n_comb) {
+    __syncthreads();
+    combine<S, 1>(pl.jplan, t.part, [&](int c, const double (&v)[1]) {
+      if (valid) out[obase + (int64_t)__ldg(pl.jc_pos + c) * tile] = v[0];
+    });
+    combine<S, 2>(m.cplan, t.part, [&](int c, const double (&v)[2]) {
+      if (valid) {
+        const int j = __ldg(m.cc_item + c);
+        const double JT = -(v[0] + fT * (t.ck[j * S + s] - cL)) * iDV;
+        out[obase + (int64_t)__ldg(pl.cc_pos + 2 * c) * tile] = JT;
+        out[obase + (int64_t)__ldg(pl.cc_pos + 2 * c + 1) * tile] = cS * v[1] + cT * JT;
+      }
+    });
+  }
   TICK(5);
   // a10: the four corner entries from the phase-1 reductions (R4-7)
   if (tid < S && valid) {
@@ -643,7 +686,7 @@ constexpr size_t SMEM_LIMIT = 227 * 1024 - 64;   // dynamic part; 64 B left for 
 LaunchCfg choose_cfg(const HostTables& h, bool jac, int64_t tile, int64_t n_states) {
   LaunchCfg cfg{1, NT, 0};
   for (int S = 32; S >= 1; S >>= 1) {
-    const size_t bytes = smem_doubles(h.ns, h.nr, h.nslots, S, jac) * sizeof(double);
+    const size_t bytes = smem_doubles(h.ns, h.nr, h.nslots, jac ? h.n_part_jac : h.n_part_src, S, jac) * sizeof(double);
     cfg.S = S; cfg.smem = bytes;
     if (bytes > SMEM_LIMIT) continue;
     if ((int64_t)S > tile) continue;                       // lanes of one item must stay inside one tile
