@@ -178,65 +178,79 @@ __device__ __forceinline__ void phases01(const DevMech& m, Tile<S, JAC>& t, int 
   const int s = tid % S;                        // NT % S == 0: a thread keeps its state in every loop
   const int64_t sg = min(s0 + s, n_states - 1);  // ragged tail: recompute the last valid state, never store
   const int64_t pbase = state_base(sg, tile, ns + 1);
-  // ---- phase 0a: scalars -------------------------------------------------------------------------
+  // ---- phase 0: scalars, species (C_k = n_k / V, Eq. 6; NASA-7 thermo, R2) ------------------------
+  // Every thread reads T, E and the parameter itself (same address for the lanes of a state: one broadcast
+  // request) so that no barrier separates the state load from the species loop.
   if (tid < N_CNT) cnt[tid] = 0;
+  const double T = phi[pbase], E_ = phi[pbase + tile], par_ = param[sg];
+  const double V = mode == PYJAC_CONP ? E_ : par_, Pp = mode == PYJAC_CONP ? par_ : E_;
+  const double invT = 1.0 / T, lnT = log(T), RT = R_GAS * T, Ctot = Pp / RT;
   if (tid < S) {
-    const double T = phi[pbase], E = phi[pbase + tile], par = param[sg];
-    const double V = mode == PYJAC_CONP ? E : par, Pp = mode == PYJAC_CONP ? par : E;
-    t.sc[SC_T * S + s] = T; t.sc[SC_V * S + s] = V; t.sc[SC_P * S + s] = Pp;
-    t.sc[SC_CTOT * S + s] = Pp / (R_GAS * T);
-    t.sc[SC_INVT * S + s] = 1.0 / T; t.sc[SC_LNT * S + s] = log(T); t.sc[SC_LNP * S + s] = log(Pp);
-    t.sc[SC_LNPRT * S + s] = log(P_ATM / (R_GAS * T));
+    t.sc[SC_T * S + s] = T; t.sc[SC_V * S + s] = V; t.sc[SC_P * S + s] = Pp; t.sc[SC_CTOT * S + s] = Ctot;
+    t.sc[SC_LNP * S + s] = log(Pp);
+    t.sc[SC_LNPRT * S + s] = log(P_ATM / RT);
     t.P[(JAC ? m.nslots : nr) * S + s] = 0.0;            // always-zero slot (ELL padding)
     t.C[ns * S + s] = 1.0;                               // dummy species: unused stoichiometric entries
 #pragma unroll
     for (int c = 0; c < 4; ++c) t.th4[(ns * S + s) * 4 + c] = 0.0;
   }
-  __syncthreads();
-  const double T = t.sc[SC_T * S + s], V = t.sc[SC_V * S + s], Pp = t.sc[SC_P * S + s], Ctot = t.sc[SC_CTOT * S + s];
-  const double invT = t.sc[SC_INVT * S + s], lnT = t.sc[SC_LNT * S + s], RT = R_GAS * T;
-  // ---- phase 0b: species: C_k = n_k / V (Eq. 6), NASA-7 thermo (R2) --------------------------
   {
+    const double T2 = T * T, T3 = T2 * T, T4 = T3 * T;
+    // thermo of the LAST species, evaluated by every thread (cheap, warp-uniform loads): E~_k and c~_k fold the
+    // last species in through mass conservation (R1/A1) and need it; saves a second pass and two barriers
+    double cL, dcL, eL;
+    {
+      const double* __restrict__ a = m.nasa + 16 * L;
+      a += (T <= __ldg(a)) ? 1 : 8;
+      const double a0 = __ldg(a), a1 = __ldg(a + 1), a2 = __ldg(a + 2), a3 = __ldg(a + 3), a4 = __ldg(a + 4), a5 = __ldg(a + 5);
+      const double cpR = a0 + a1 * T + a2 * T2 + a3 * T3 + a4 * T4;
+      const double hRT = a0 + a1 * T * 0.5 + a2 * T2 * (1.0 / 3.0) + a3 * T3 * 0.25 + a4 * T4 * 0.2 + a5 * invT;
+      cL = R_GAS * (mode == PYJAC_CONP ? cpR : cpR - 1.0);
+      dcL = R_GAS * (a1 + 2.0 * a2 * T + 3.0 * a3 * T2 + 4.0 * a4 * T3);
+      eL = hRT - (mode == PYJAC_CONP ? 0.0 : 1.0);
+    }
     double acc[3] = {0.0, 0.0, 0.0};
     const double invV = 1.0 / V;
-    const double T2 = T * T, T3 = T2 * T, T4 = T3 * T;
     for (int idx = tid; idx < ns * S; idx += NT) {
       const int k = idx / S;
       const double* __restrict__ a = m.nasa + 16 * k;
       a += (T <= __ldg(a)) ? 1 : 8;                      // low range iff T <= T_mid (R3); per-lane select
       const double a0 = __ldg(a), a1 = __ldg(a + 1), a2 = __ldg(a + 2), a3 = __ldg(a + 3), a4 = __ldg(a + 4), a5 = __ldg(a + 5), a6 = __ldg(a + 6);
+      const double w = __ldg(m.wr + k);
       const double cpR = a0 + a1 * T + a2 * T2 + a3 * T3 + a4 * T4;
       const double dcpR = a1 + 2.0 * a2 * T + 3.0 * a3 * T2 + 4.0 * a4 * T3;
       const double hRT = a0 + a1 * T * 0.5 + a2 * T2 * (1.0 / 3.0) + a3 * T3 * 0.25 + a4 * T4 * 0.2 + a5 * invT;
       const double sR = a0 * lnT + a1 * T + a2 * T2 * 0.5 + a3 * T3 * (1.0 / 3.0) + a4 * T4 * 0.25 + a6;
       const double c = R_GAS * (mode == PYJAC_CONP ? cpR : cpR - 1.0);   // c_p or c_v = c_p - R
+      const double e = hRT - (mode == PYJAC_CONP ? 0.0 : 1.0);           // h/RT or u/RT
       t.th4[idx * 4] = hRT - sR;
       t.th4[idx * 4 + 1] = hRT;
+      t.th4[idx * 4 + 2] = k == L ? 0.0 : RT * (e - w * eL);            // E~_k = E_k - (W_k/W_Ns) E_Ns
+      t.th4[idx * 4 + 3] = k == L ? 0.0 : c - w * cL;                   // c~_k
       t.ck[idx] = c;
       if (k < L) {
         const double Ck = phi[pbase + (int64_t)(2 + k) * tile] * invV;
         t.C[idx] = Ck;
         acc[0] += Ck; acc[1] += Ck * c; acc[2] += Ck * (R_GAS * dcpR);
-      } else {
-        t.sc[SC_CNS * S + s] = R_GAS * dcpR;          // c'_Ns, consumed right below
       }
     }
-    block_reduce<S, 3>(acc, t.red, t.sc, SC_SUMC);
-    if (tid < S) {      // last species from the ideal-gas law, D and dD/dT sums over all species
-      const double CL = Ctot - t.sc[SC_SUMC * S + s];
-      t.C[L * S + s] = CL;
-      t.sc[SC_D * S + s] = t.sc[SC_SUMCC * S + s] + CL * t.ck[L * S + s];
-      t.sc[SC_DDDT * S + s] = t.sc[SC_SUMCDC * S + s] + CL * t.sc[SC_CNS * S + s];
+    // block sums; the S finishing threads add the last species: C_Ns from the ideal-gas law
+    const int lane = tid & 31, warp = tid >> 5;
+#pragma unroll
+    for (int j = 0; j < 3; ++j) {
+      const double v = group_sum<S>(acc[j]);
+      if (lane < S) t.red[(warp * NRED + j) * S + lane] = v;
     }
     __syncthreads();
-    // E~_k = E_k - (W_k/W_Ns) E_Ns, c~_k likewise (mass conservation folds the last species in, R1/A1)
-    const double eL = t.th4[(L * S + s) * 4 + 1] - (mode == PYJAC_CONP ? 0.0 : 1.0), cL = t.ck[L * S + s];
-    for (int idx = tid; idx < ns * S; idx += NT) {
-      const int k = idx / S;
-      const double w = __ldg(m.wr + k);
-      const double e = t.th4[idx * 4 + 1] - (mode == PYJAC_CONP ? 0.0 : 1.0);
-      t.th4[idx * 4 + 2] = k == L ? 0.0 : RT * (e - w * eL);
-      t.th4[idx * 4 + 3] = k == L ? 0.0 : t.ck[idx] - w * cL;
+    if (tid < S) {
+      double sum[3] = {0.0, 0.0, 0.0};
+      for (int w = 0; w < NW; ++w)
+#pragma unroll
+        for (int j = 0; j < 3; ++j) sum[j] += t.red[(w * NRED + j) * S + s];
+      const double CL = Ctot - sum[0];
+      t.C[L * S + s] = CL;
+      t.sc[SC_D * S + s] = sum[1] + CL * cL;
+      t.sc[SC_DDDT * S + s] = sum[2] + CL * dcL;
     }
     __syncthreads();
   }
@@ -568,12 +582,27 @@ jacobian_kernel(const DevMech m, const DevPlan pl, int mode, int64_t n_states, i
   const double T = t.sc[SC_T * S + s], V = t.sc[SC_V * S + s], Pp = t.sc[SC_P * S + s], D = t.sc[SC_D * S + s];
   const double N = t.sc[SC_R0 * S + s], Ssum = t.sc[SC_R1 * S + s];
   const double fT = -N / D;
-  // dense output: structural zeros, each stored once (no memset pass)
+  // dense output: structural zeros, each stored once (no memset pass).  A warp takes 32 bitmap words (1024
+  // elements) at a time: one coalesced mask load, then 32 fully coalesced predicated store instructions.
   if (pl.nzmask != nullptr) {
     const int n2 = m.nvar * m.nvar;
-    for (int idx = tid; idx < n2 * S; idx += NT) {
-      const int e = idx / S;
-      if (!((pl.nzmask[e >> 5] >> (e & 31)) & 1u) && valid) out[obase + (int64_t)e * tile] = 0.0;
+    if (S == 1) {
+      const int lane = tid & 31, warp = tid >> 5;
+      const int n_words = (n2 + 31) / 32;
+      for (int w0 = warp * 32; w0 < n_words; w0 += NW * 32) {
+        const uint32_t mine = w0 + lane < n_words ? __ldg(pl.nzmask + w0 + lane) : 0xffffffffu;
+#pragma unroll 8
+        for (int j = 0; j < 32; ++j) {
+          const uint32_t wj = __shfl_sync(0xffffffffu, mine, j);
+          const int e = (w0 + j) * 32 + lane;
+          if (!((wj >> lane) & 1u) && e < n2 && valid) out[obase + (int64_t)e * tile] = 0.0;
+        }
+      }
+    } else {
+      for (int idx = tid; idx < n2 * S; idx += NT) {
+        const int e = idx / S;
+        if (!((__ldg(pl.nzmask + (e >> 5)) >> (e & 31)) & 1u) && valid) out[obase + (int64_t)e * tile] = 0.0;
+      }
     }
   }
   TICK(3);
