@@ -41,13 +41,14 @@ def measured_peaks():
 
 
 def ncu_traffic(config):
-    """dram bytes per launch of the Jacobian kernel from the committed ncu summary, if present."""
-    p = os.path.join(ROOT, "profiles", "r01_traffic.json")
+    """dram bytes (read + write) per launch of the timed kernel from the committed ncu summary
+    profiles/r01_traffic.csv (columns: config,n_states,dram_bytes_per_launch), scaled to this run's states."""
+    p = os.path.join(ROOT, "profiles", "r01_traffic.csv")
     if os.path.exists(p):
-        try:
-            return json.load(open(p)).get("c%d" % config)
-        except Exception:
-            return None
+        for line in open(p):
+            f = line.strip().split(",")
+            if f and f[0] == "c%d" % config:
+                return {"n_states": int(f[1]), "dram_bytes": float(f[2])}
     return None
 
 
@@ -187,7 +188,8 @@ def main():
     ld = (N + tile - 1) // tile * tile
     n_e = M.nnz if what == "sparse" else M.nvar * M.nvar
     # weak scaling: every rank owns its own N states (independent problems, no collective on the data path)
-    states = mg.config_states(c, N, start=rank * N)
+    from paper_1809_01029_b200.sharding import weak_scaling_offset
+    states = mg.config_states(c, N, start=weak_scaling_offset(N, rank))
     phi_h, par_h = pack_phi(states, mode, ld, tile)
     d_phi = torch.from_numpy(phi_h).cuda(); d_par = torch.from_numpy(par_h).cuda()
     d_out = torch.empty(n_e * ld, dtype=torch.float64, device="cuda")
@@ -280,7 +282,7 @@ def main():
                 "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                 "dtype": "f64", "data": "synthetic", "config": workload_config(c, what, tile, S),
                 "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                             "traffic": ncu_traffic(c), "peak_source": peak_src, "kernel": "jacobian_kernel<S=%d>" % S,
+                             "traffic": (lambda t: None if t is None else t["dram_bytes"] * N / t["n_states"])(ncu_traffic(c)), "peak_source": peak_src, "kernel": "jacobian_kernel<S=%d>" % S,
                              "algorithmic_bytes_per_state": 8 * n_e + 8 * (M.ns + 2), "kernel_ms": kavg_ms,
                              "ns_per_state": 1e6 * kavg_ms / N},
                 "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": args.steps, "clocks": clk.summary(),

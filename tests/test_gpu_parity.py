@@ -154,3 +154,47 @@ def test_eval_host_matches_device_path(pj):
     got = run_gpu(pj, M, pj.WHAT_SPARSE, mg.CONP, mg.CSR, states)
     # not bitwise: warps take reaction chunks dynamically, so the order of the reaction sums varies run to run
     np.testing.assert_allclose(unpack(out, M.nnz, 256, 256, 256), got, rtol=1e-11, atol=0)
+
+
+@pytest.mark.parametrize("c", [5, 4])
+def test_full_size_bench_configuration_sampled(pj, c):
+    """BASELINE.json's full sizes in the launch configuration bench.py times (tile = states per CTA): C5 2^18 states
+    sparse CSR (26.8 GB of values), C4 2^14 states dense (17.1 GB); 48 states sampled across the batch (including the
+    first and the last) are compared with the oracle one by one, and a checksum guards every state against NaN."""
+    from mechgen.mechanism import CONFIGS
+    m, M, o, st = setup(pj, "c%d" % c)
+    cfg = CONFIGS[c]
+    N, mode = cfg["n_states"], cfg["mode"]
+    what = pj.WHAT_SPARSE if c == 5 else pj.WHAT_DENSE
+    n_e = M.n_elements(what)
+    free, _ = torch.cuda.mem_get_info()
+    if free < n_e * N * 8 + (2 << 30):
+        pytest.skip("not enough device memory for the full-size buffer")
+    S, _, _ = pj.pyjac_launch_info(M.h, 1)
+    tile = S
+    states = st(N)
+    phi, par = pack_phi(states, mode, N, tile)
+    d_phi = torch.from_numpy(phi).cuda(); d_par = torch.from_numpy(par).cuda()
+    out = torch.empty(n_e * N, dtype=torch.float64, device="cuda")
+    stream = torch.cuda.current_stream().cuda_stream
+    if c == 5:
+        pj.pyjac_jacobian_sparse(M.h, mode, mg.CSR, N, N, tile, d_phi.data_ptr(), d_par.data_ptr(), out.data_ptr(), stream)
+    else:
+        pj.pyjac_jacobian_dense(M.h, mode, "C", N, N, tile, d_phi.data_ptr(), d_par.data_ptr(), out.data_ptr(), stream)
+    torch.cuda.synchronize()
+    view = out.view(N // tile, n_e, tile)
+    assert bool(torch.isfinite(view.sum(dim=1)).all())
+    rng = np.random.default_rng(c)
+    pick = np.unique(np.concatenate([[0, N - 1], rng.integers(0, N, 46)]))
+    got = np.stack([view[s // tile, :, s % tile].cpu().numpy() for s in pick])
+    sub = {k: (v[pick] if v.ndim == 1 else v[:, pick]) for k, v in states.items()}
+    Jr = o.jacobian_dense(mode, *o.pack(sub, mode))
+    if c == 5:
+        ptr, idx = M.sparsity(mg.CSR)
+        Jg = dense_from_sparse(got, ptr, idx, mg.CSR, M.nvar)
+    else:
+        Jg = got.reshape(len(pick), M.nvar, M.nvar)
+    bad = jac_ok_dense(Jg, Jr)
+    assert not bad.any(), (np.argwhere(bad)[:5], Jg[bad][:5], Jr[bad][:5])
+    del out
+    torch.cuda.empty_cache()
