@@ -43,6 +43,12 @@ namespace {
 #ifndef PYJAC_UC
 #define PYJAC_UC 1
 #endif
+#ifndef PYJAC_UNJ
+#define PYJAC_UNJ 4
+#endif
+#ifndef PYJAC_UNC
+#define PYJAC_UNC 4
+#endif
 #ifndef PYJAC_UQ
 #define PYJAC_UQ 1
 #endif
@@ -454,7 +460,7 @@ namespace {
 //   acc(const int32_t* entry, double (&v)[NACC])      accumulate one entry
 //   store(int slot, const double (&v)[NACC])          slot = processing slot (index into the position arrays)
 // ---------------------------------------------------------------------------------------------------
-template <int S, int STRIDE, int NACC, int U, class AccF, class PosF, class StoreF>
+template <int S, int STRIDE, int NACC, int U, int UNROLL, class AccF, class PosF, class StoreF>
 __device__ __forceinline__ void gather(const DevGather& g, int* counter, AccF acc, PosF pos_of, StoreF store) {
   const int lane = threadIdx.x & 31, sub = lane / S;
   constexpr int IPW = 32 / S;                 // segments of one warp per "u"
@@ -483,7 +489,7 @@ __device__ __forceinline__ void gather(const DevGather& g, int* counter, AccF ac
     for (int u = 0; u < U; ++u)
 #pragma unroll
       for (int a = 0; a < NACC; ++a) v[u][a] = 0.0;
-#pragma unroll 4
+#pragma unroll UNROLL
     for (int p = 0; p < meta.y; ++p) {
 #pragma unroll
       for (int u = 0; u < U; ++u) acc(e + (p * ELL_W + u * IPW) * STRIDE, v[u]);
@@ -530,7 +536,7 @@ source_kernel(const DevMech m, int mode, int64_t n_states, int64_t tile, const d
   const double V = t.sc[SC_V * S + s];
   // a7: omega_k = sum_i nu_ki q_i (Eq. 4), dn_k/dt = V omega_k (Eq. 3)
   const double* __restrict__ P = t.P;
-  gather<S, 1, 1, PYJAC_UQ>(m.qplan, cnt + CNT_Q,
+  gather<S, 1, 1, PYJAC_UQ, 4>(m.qplan, cnt + CNT_Q,
       [&](const int32_t* e, double (&v)[1]) {
         const uint32_t ent = (uint32_t)__ldg(e);
         v[0] += apply_sign(P[(ent & ~SIGN_BIT) * S + s], ent);
@@ -610,7 +616,7 @@ jacobian_kernel(const DevMech m, const DevPlan pl, int mode, int64_t n_states, i
   // J[k][T] = sum_i nu_ki slotT_i, J[k][E] = sum_i nu_ki slotE_i.  Every nonzero is finished in a register and
   // stored once.
   const double* __restrict__ P = t.P;
-  gather<S, 1, 1, PYJAC_UJ>(pl.jplan, cnt + CNT_J,
+  gather<S, 1, 1, PYJAC_UJ, PYJAC_UNJ>(pl.jplan, cnt + CNT_J,
       [&](const int32_t* e, double (&v)[1]) {
         const uint32_t ent = (uint32_t)__ldg(e);
         v[0] += apply_sign(P[(ent & ~SIGN_BIT) * S + s], ent);
@@ -628,7 +634,7 @@ jacobian_kernel(const DevMech m, const DevPlan pl, int mode, int64_t n_states, i
   const double cS = mode == PYJAC_CONP ? T * R_GAS / Pp : T * R_GAS / V;
   const double cT = mode == PYJAC_CONP ? V / T : Pp / T;
   const double* __restrict__ dE = t.dE;
-  gather<S, 4, 2, PYJAC_UC>(m.cplan, cnt + CNT_C,
+  gather<S, 4, 2, PYJAC_UC, PYJAC_UNC>(m.cplan, cnt + CNT_C,
       [&](const int32_t* e, double (&v)[2]) {
         const int4 pr = __ldg(reinterpret_cast<const int4*>(e));      // slot | sign, reaction, dn~ (2 words)
         const uint32_t ent = (uint32_t)pr.x;
