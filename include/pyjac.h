@@ -87,6 +87,16 @@ typedef struct {
  * call fails with PYJAC_ECUDA) -- there is no CPU compute path.  The compute calls launch on the
  * caller's current device, which must be the handle's device. */
 int pyjac_mech_create(const pyjac_mech_desc *desc, int cuda_device, pyjac_mech **out);
+
+/* Same with flags.  PYJAC_APPROX_JACOBIAN selects the paper's "approximate" Jacobian: with the
+ * third-body concentration written as [M] = C_tot + sum_k (alpha_k - 1) C_k, the derivatives of the rates of
+ * progress and pressure-modification terms THROUGH THE LAST SPECIES' CONCENTRATION with respect to the other
+ * species' moles are ignored (R6).  The dense rows caused by a reacting last species or by a non-default
+ * efficiency of the last species disappear; pyjac_sparsity returns the sparser pattern; the T and E columns, the
+ * source terms and everything else are unchanged.  For mechanisms whose last species is inert with default
+ * efficiencies the two Jacobians are identical. */
+enum { PYJAC_APPROX_JACOBIAN = 1 };
+int pyjac_mech_create_ex(const pyjac_mech_desc *desc, int cuda_device, uint32_t flags, pyjac_mech **out);
 void pyjac_mech_destroy(pyjac_mech *mech);
 
 int pyjac_mech_dims(const pyjac_mech *mech, int32_t *ns, int32_t *nr, int32_t *nvar, int64_t *nnz);

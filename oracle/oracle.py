@@ -41,6 +41,8 @@ def _load():
         lib = C.CDLL(_build.build())
         lib.orc_create.restype = C.c_void_p
         lib.orc_create.argtypes = [C.POINTER(_Desc)]
+        lib.orc_create2.restype = C.c_void_p
+        lib.orc_create2.argtypes = [C.POINTER(_Desc), C.c_int]
         lib.orc_destroy.argtypes = [C.c_void_p]
         lib.orc_nnz.restype = C.c_int64
         lib.orc_nnz.argtypes = [C.c_void_p]
@@ -61,7 +63,8 @@ def _p(a, t=_D):
 
 
 class Oracle:
-    def __init__(self, mech):
+    def __init__(self, mech, approx=False):
+        """approx=True: the paper's "approximate" Jacobian and its sparser pattern."""
         lib = _load()
         self._keep = []
         d = _Desc()
@@ -73,7 +76,7 @@ class Oracle:
             self._keep.append(a)
             setattr(d, name, _p(a, ct))
         self.ns = d.n_species; self.nr = d.n_reactions; self.nvar = self.ns + 1
-        self._h = C.c_void_p(lib.orc_create(C.byref(d)))
+        self._h = C.c_void_p(lib.orc_create2(C.byref(d), 1 if approx else 0))
         self.nnz = int(lib.orc_nnz(self._h))
         self.threads = int(lib.orc_max_threads())
 

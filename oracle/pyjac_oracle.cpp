@@ -132,7 +132,10 @@ template <class T> Blend<T> blend(const Mech& m, int i, const T& Tt, const T& Pr
 
 // ---- source terms, Eqs. 3-8, with every intermediate -------------------------------------------
 template <class T>
-void eval_source(const Mech& m, int mode, const T* phi, const T& param, T* f, Inter<T>& w) {
+// CL_rates (test hook for the "approximate" Jacobian pin): when non-null the rate expressions see
+// this value as the last species' concentration (held fixed instead of C_tot - sum C_k) and the third-body
+// concentration of a mixture is written [M] = C_tot + sum_k (alpha_k - 1) C_k; D and everything else are unchanged.
+void eval_source(const Mech& m, int mode, const T* phi, const T& param, T* f, Inter<T>& w, const T* CL_rates = nullptr) {
     const int ns = m.ns, nr = m.nr;
     const double ln10 = std::log(10.0);
     const T Tt = phi[0];
@@ -144,6 +147,8 @@ void eval_source(const Mech& m, int mode, const T* phi, const T& param, T* f, In
     T sumC = T(0.0);
     for (int k = 0; k < ns - 1; ++k) { w.C[k] = phi[2 + k] / V; sumC = sumC + w.C[k]; }
     w.C[ns - 1] = w.Ctot - sumC;
+    const T CL_true = w.C[ns - 1];
+    if (CL_rates) w.C[ns - 1] = *CL_rates;
     // a2: NASA-7 thermo (c-2), low range iff T <= T_mid (reading S3)
     const T lnT = log(Tt);
     for (int k = 0; k < ns; ++k) {
@@ -239,7 +244,8 @@ void eval_source(const Mech& m, int mode, const T* phi, const T& param, T* f, In
         // a5: pressure modification c_i
         T c = T(1.0), M = T(0.0), Pr = T(0.0), F = T(1.0);
         if (m.has_third_body(i)) {
-            for (int k = 0; k < ns; ++k) M = M + m.alpha(i, k) * w.C[k];
+            if (CL_rates && m.collider[i] < 0) { M = w.Ctot; for (int k = 0; k < ns; ++k) M = M + (m.alpha(i, k) - 1.0) * w.C[k]; }
+            else for (int k = 0; k < ns; ++k) M = M + m.alpha(i, k) * w.C[k];
             if (ty == T_THIRD) c = M;
             else {
                 T k0 = exp(std::log(m.lowA[i]) + m.lowb[i] * lnT - m.lowTa[i] / Tt);
@@ -251,6 +257,7 @@ void eval_source(const Mech& m, int mode, const T* phi, const T& param, T* f, In
         w.M[i] = M; w.Pr[i] = Pr; w.F[i] = F; w.c[i] = c;
         w.q[i] = c * (Rf - Rr);                                   // Eq. 4
     }
+    w.C[ns - 1] = CL_true;
     // a7: production rates (Eq. 4), last species by mass conservation (L122, reading A1)
     for (int k = 0; k < ns - 1; ++k) {
         T s = T(0.0);
@@ -282,7 +289,9 @@ void eval_source(const Mech& m, int mode, const T* phi, const T& param, T* f, In
 }
 
 // ---- analytical Jacobian, dense, row-major nvar x nvar ------------------
-void eval_jacobian(const Mech& m, int mode, const double* phi, double param, double* J, Inter<double>& w) {
+// approx: the paper's "approximate" Jacobian (R6): in the species columns the
+// derivatives of q_i through the last species' concentration are ignored, with [M] = C_tot + sum (alpha_k - 1) C_k.
+void eval_jacobian(const Mech& m, int mode, bool approx, const double* phi, double param, double* J, Inter<double>& w) {
     const int ns = m.ns, nr = m.nr, nvar = ns + 1, L = ns - 1;
     std::vector<double> f(nvar);
     eval_source(m, mode, phi, param, f.data(), w);
@@ -317,7 +326,9 @@ void eval_jacobian(const Mech& m, int mode, const double* phi, double param, dou
         const double dRdT = lam_f * w.Rf[i] - lam_r * w.Rr[i];
         // item 4: partials of q_i = Q_i(T, P, C_1..C_Ns) by type
         double GT, GP = w.c[i] * w.dlnkf_dP[i] * R;
+        double Xdef = 0.0;      // dQ_i/d[M] for a mixture third body: the part of G^k common to all default-efficiency species
         if (ty == T_THIRD) {
+            if (m.collider[i] < 0) Xdef = R;
             for (int k = 0; k < ns; ++k) G[k] = m.alpha(i, k) * R + w.M[i] * dRdC[k];
             GT = w.M[i] * dRdT;
         } else if (ty == T_LIND || ty == T_TROE || ty == T_SRI) {
@@ -327,6 +338,7 @@ void eval_jacobian(const Mech& m, int mode, const double* phi, double param, dou
             const double lnT = std::log(Tt);
             const double k0 = std::exp(std::log(m.lowA[i]) + m.lowb[i] * lnT - m.lowTa[i] / Tt);
             const double dPr_dT = Pr * (m.lowb[i] - m.beta[i] + (m.lowTa[i] - m.Ta[i]) / Tt) / Tt;
+            if (m.collider[i] < 0) Xdef = dc_dPr * (k0 / w.kf[i]) * R;
             for (int k = 0; k < ns; ++k) G[k] = m.alpha(i, k) * dc_dPr * (k0 / w.kf[i]) * R + w.c[i] * dRdC[k];
             GT = (dc_dPr * dPr_dT + (Pr / (1.0 + Pr)) * b.dF_dT) * R + w.c[i] * dRdT;
         } else {
@@ -342,7 +354,7 @@ void eval_jacobian(const Mech& m, int mode, const double* phi, double param, dou
         } else {
             dq[1] = GP + G[L] / (R_GAS * Tt);
         }
-        for (int j = 0; j < L; ++j) dq[2 + j] = (G[j] - G[L]) / V;
+        for (int j = 0; j < L; ++j) dq[2 + j] = approx ? (G[j] - Xdef) / V : (G[j] - G[L]) / V;
         for (int k = 0; k < L; ++k) {
             int nu = m.nu_p(i, k) - m.nu_r(i, k);
             if (nu == 0) continue;
@@ -396,7 +408,7 @@ void eval_jacobian(const Mech& m, int mode, const double* phi, double param, dou
 }
 
 // ---- sparsity pattern, SURVEY.md 8c-5 ---------------------------------------
-void pattern_dense_mask(const Mech& m, std::vector<uint8_t>& mask) {
+void pattern_dense_mask(const Mech& m, bool approx, std::vector<uint8_t>& mask) {
     const int ns = m.ns, nvar = ns + 1, L = ns - 1;
     mask.assign((size_t)nvar * nvar, 0);
     for (int c = 0; c < nvar; ++c) { mask[c] = 1; mask[(size_t)nvar + c] = 1; }           // rows T, E dense
@@ -407,7 +419,8 @@ void pattern_dense_mask(const Mech& m, std::vector<uint8_t>& mask) {
         for (int k = 0; k < L; ++k) {
             if (m.nu_p(i, k) - m.nu_r(i, k) == 0) continue;
             for (int j = 0; j < L; ++j) {
-                bool in = dep(j) || depL || (m.has_third_body(i) && m.alpha(i, j) != m.alpha(i, L));
+                bool in = approx ? (dep(j) || (m.has_third_body(i) && m.alpha(i, j) != (m.collider[i] >= 0 ? 0.0 : 1.0)))
+                                 : (dep(j) || depL || (m.has_third_body(i) && m.alpha(i, j) != m.alpha(i, L)));
                 if (in) mask[(size_t)(2 + k) * nvar + 2 + j] = 1;
             }
         }
@@ -416,6 +429,7 @@ void pattern_dense_mask(const Mech& m, std::vector<uint8_t>& mask) {
 
 struct Handle {
     Mech m;
+    bool approx = false;
     std::vector<uint8_t> mask;
     std::vector<int> csr_ptr, csr_idx, csc_ptr, csc_idx;
 };
@@ -440,8 +454,9 @@ struct orc_desc {
     const double *cheb_Tmin, *cheb_Tmax, *cheb_Pmin, *cheb_Pmax, *cheb_coef;
 };
 
-void* orc_create(const orc_desc* d) {
+void* orc_create2(const orc_desc* d, int approx) {
     Handle* h = new Handle();
+    h->approx = approx != 0;
     Mech& m = h->m;
     const int ns = d->n_species, nr = d->n_reactions;
     m.ns = ns; m.nr = nr;
@@ -464,7 +479,7 @@ void* orc_create(const orc_desc* d) {
     copy_in(m.chebTmin, d->cheb_Tmin, nr); copy_in(m.chebTmax, d->cheb_Tmax, nr);
     copy_in(m.chebPmin, d->cheb_Pmin, nr); copy_in(m.chebPmax, d->cheb_Pmax, nr);
     copy_in(m.cheb_coef, d->cheb_coef, d->cheb_ptr[nr]);
-    pattern_dense_mask(m, h->mask);
+    pattern_dense_mask(m, h->approx, h->mask);
     const int nvar = ns + 1;
     h->csr_ptr.assign(1, 0); h->csc_ptr.assign(1, 0);
     for (int r = 0; r < nvar; ++r) {
@@ -477,6 +492,8 @@ void* orc_create(const orc_desc* d) {
     }
     return h;
 }
+
+void* orc_create(const orc_desc* d) { return orc_create2(d, 0); }
 
 void orc_destroy(void* hv) { delete (Handle*)hv; }
 
@@ -516,7 +533,7 @@ void orc_jacobian_dense(void* hv, int mode, int64_t n, const double* phi, const 
     {
         Inter<double> w; w.resize(m.ns, m.nr);
 #pragma omp for schedule(static)
-        for (int64_t s = 0; s < n; ++s) eval_jacobian(m, mode, phi + s * nvar, param[s], J + (size_t)s * nvar * nvar, w);
+        for (int64_t s = 0; s < n; ++s) eval_jacobian(m, mode, h->approx, phi + s * nvar, param[s], J + (size_t)s * nvar * nvar, w);
     }
 }
 
@@ -530,7 +547,7 @@ void orc_jacobian_sparse(void* hv, int mode, int fmt, int64_t n, const double* p
         std::vector<double> J((size_t)nvar * nvar);
 #pragma omp for schedule(static)
         for (int64_t s = 0; s < n; ++s) {
-            eval_jacobian(m, mode, phi + s * nvar, param[s], J.data(), w);
+            eval_jacobian(m, mode, h->approx, phi + s * nvar, param[s], J.data(), w);
             double* o = vals + (size_t)s * nnz;
             size_t e = 0;
             if (fmt == 0) { for (int r = 0; r < nvar; ++r) for (int p = h->csr_ptr[r]; p < h->csr_ptr[r + 1]; ++p) o[e++] = J[(size_t)r * nvar + h->csr_idx[p]]; }
@@ -580,6 +597,13 @@ void orc_cs_jacobian(void* hv, int mode, const double* phi, double param, double
         double hc = rel * std::max(std::fabs(phi[c]), floor_[c]);
         for (int k = 0; k < nvar; ++k) x[k] = cplx(phi[k], 0.0);
         x[c] = cplx(phi[c], hc);
+        if (h->approx && c >= 2) {          // approximate Jacobian: C_Ns held fixed inside the rates for the species columns
+            double sum = 0.0;
+            const double Vr = mode == CONP ? phi[1] : param, Pr = mode == CONP ? param : phi[1];
+            for (int k = 0; k < m.ns - 1; ++k) sum += phi[2 + k] / Vr;
+            const cplx CL(Pr / (R_GAS * phi[0]) - sum, 0.0);
+            eval_source<cplx>(m, mode, x.data(), cplx(param, 0.0), f.data(), w, &CL);
+        } else
         eval_source<cplx>(m, mode, x.data(), cplx(param, 0.0), f.data(), w);
         for (int r = 0; r < nvar; ++r) J[(size_t)r * nvar + c] = f[r].imag() / hc;
     }

@@ -15,6 +15,7 @@ import numpy as np
 PYJAC_OK, PYJAC_EINVAL, PYJAC_EMECH, PYJAC_ECUDA, PYJAC_ENOMEM = range(5)
 PYJAC_CONP, PYJAC_CONV = 0, 1
 PYJAC_CSR, PYJAC_CSC = 0, 1
+PYJAC_APPROX_JACOBIAN = 1
 WHAT_SOURCE, WHAT_SPARSE, WHAT_DENSE = 0, 1, 2
 
 _D = C.POINTER(C.c_double)
@@ -58,6 +59,7 @@ def lib():
         vp, i32, i64 = C.c_void_p, C.c_int, C.c_int64
         L.pyjac_last_error.restype = C.c_char_p
         L.pyjac_mech_create.argtypes = [C.POINTER(pyjac_mech_desc), i32, C.POINTER(vp)]
+        L.pyjac_mech_create_ex.argtypes = [C.POINTER(pyjac_mech_desc), i32, C.c_uint32, C.POINTER(vp)]
         L.pyjac_mech_destroy.argtypes = [vp]
         L.pyjac_mech_destroy.restype = None
         L.pyjac_mech_dims.argtypes = [vp, _I, _I, _I, C.POINTER(i64)]
@@ -94,6 +96,13 @@ def pyjac_mech_create(mech, cuda_device=0):
     d, keep = make_desc(mech)
     h = C.c_void_p()
     _check(lib().pyjac_mech_create(C.byref(d), int(cuda_device), C.byref(h)))
+    return h
+
+
+def pyjac_mech_create_ex(mech, cuda_device=0, flags=0):
+    d, keep = make_desc(mech)
+    h = C.c_void_p()
+    _check(lib().pyjac_mech_create_ex(C.byref(d), int(cuda_device), int(flags), C.byref(h)))
     return h
 
 
@@ -146,8 +155,8 @@ def pyjac_launch_info(h, what):
 class Mechanism:
     """RAII convenience around the handle; methods forward to the C ABI."""
 
-    def __init__(self, mech, cuda_device=0):
-        self.h = pyjac_mech_create(mech, cuda_device)
+    def __init__(self, mech, cuda_device=0, flags=0):
+        self.h = pyjac_mech_create_ex(mech, cuda_device, flags) if flags else pyjac_mech_create(mech, cuda_device)
         self.ns, self.nr, self.nvar, self.nnz = pyjac_mech_dims(self.h)
 
     def close(self):

@@ -55,12 +55,17 @@ extern "C" {
 const char* pyjac_last_error(void) { return g_err.c_str(); }
 
 int pyjac_mech_create(const pyjac_mech_desc* desc, int cuda_device, pyjac_mech** out) {
+  return pyjac_mech_create_ex(desc, cuda_device, 0u, out);
+}
+
+int pyjac_mech_create_ex(const pyjac_mech_desc* desc, int cuda_device, uint32_t flags, pyjac_mech** out) {
   if (!desc || !out) return fail(PYJAC_EINVAL, "pyjac_mech_create: null argument");
+  if (flags & ~(uint32_t)PYJAC_APPROX_JACOBIAN) return fail(PYJAC_EINVAL, "pyjac_mech_create_ex: unknown flag");
   *out = nullptr;
   pyjac_mech* m = new (std::nothrow) pyjac_mech();
   if (!m) return fail(PYJAC_ENOMEM, "out of host memory");
   std::string err;
-  int rc = build_host_tables(desc, m->h, err);
+  int rc = build_host_tables(desc, (flags & PYJAC_APPROX_JACOBIAN) != 0, m->h, err);
   if (rc != PYJAC_OK) { delete m; return fail(rc, err); }
   if (cuda_device == -1) { m->device = -1; *out = m; return PYJAC_OK; }   // host-only handle: pattern and dims only
   int ndev = 0;

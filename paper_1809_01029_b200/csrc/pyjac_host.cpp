@@ -124,7 +124,7 @@ void build_gather(const std::vector<std::vector<int32_t>>& lists, int stride, in
 
 }  // namespace
 
-int build_host_tables(const pyjac_mech_desc* d, HostTables& h, std::string& err) {
+int build_host_tables(const pyjac_mech_desc* d, bool approx, HostTables& h, std::string& err) {
   if (int rc = validate(d, err)) return rc;
   const int ns = d->n_species, nr = d->n_reactions, nvar = ns + 1, L = ns - 1;
   h.ns = ns; h.nr = nr; h.nvar = nvar;
@@ -257,13 +257,15 @@ int build_host_tables(const pyjac_mech_desc* d, HostTables& h, std::string& err)
       push_n(bql[k], (int32_t)((uint32_t)r | sgn), std::abs(nu));
       for (const Role& ro : roles[r]) {
         if (ro.species != L) push_n(rowmap[k][ro.species], (int32_t)((uint32_t)ro.slot | sgn), std::abs(nu));
-        else for (int j = 0; j < L; ++j) push_n(rowmap[k][j], (int32_t)((uint32_t)ro.slot | (sgn ^ SIGN_BIT)), std::abs(nu));
+        else if (!approx)      // exact Jacobian: C_Ns depends on every n_j -> dense row; dropped by the
+                               // "approximate" switch of PAPER.md L313-317
+          for (int j = 0; j < L; ++j) push_n(rowmap[k][j], (int32_t)((uint32_t)ro.slot | (sgn ^ SIGN_BIT)), std::abs(nu));
       }
     }
     if (!net[r].empty() && !(net[r].size() == 1 && net[r][0].first == L)) {
       for (const Role& ro : roles[r]) {
         if (ro.species != L) { cl[ro.species].push_back(ro.slot); cl[ro.species].push_back(r); }
-        else for (int j = 0; j < L; ++j) { cl[j].push_back((int32_t)((uint32_t)ro.slot | SIGN_BIT)); cl[j].push_back(r); }
+        else if (!approx) for (int j = 0; j < L; ++j) { cl[j].push_back((int32_t)((uint32_t)ro.slot | SIGN_BIT)); cl[j].push_back(r); }
       }
     }
   }
@@ -291,7 +293,8 @@ int build_host_tables(const pyjac_mech_desc* d, HostTables& h, std::string& err)
       for (auto& kv : net[r]) {
         if (kv.first == L) continue;
         for (int j = 0; j < L; ++j)
-          if (depL || dep(j) || (tb && alpha(j) != aL)) inpat[kv.first][j] = 1;
+          if (approx ? (dep(j) || (tb && alpha(j) != (d->collider[i] >= 0 ? 0.0 : 1.0)))
+                     : (depL || dep(j) || (tb && alpha(j) != aL))) inpat[kv.first][j] = 1;
       }
     }
     for (int k = 0; k < L; ++k) {

@@ -82,7 +82,9 @@ struct HostTables {
 };
 
 // returns PYJAC_OK or an error code with a message in err
-int build_host_tables(const pyjac_mech_desc* d, HostTables& h, std::string& err);
+// approx: the "approximate" Jacobian of PAPER.md L313-317 (derivatives through the last species' concentration with
+// respect to the other species' moles are ignored: sparser pattern, inexact values)
+int build_host_tables(const pyjac_mech_desc* d, bool approx, HostTables& h, std::string& err);
 
 // ---- device views ------------------------------------------------------------------------------
 struct DevGather {
