@@ -612,21 +612,9 @@ jacobian_kernel(const DevMech m, const DevPlan pl, int mode, int64_t n_states, i
     }
   }
   TICK(3);
-  // a9: species rows.  Block entries J[k][j] = sum_i nu_ki (Ghat^j_i - Ghat^Ns_i); T and E columns
-  // J[k][T] = sum_i nu_ki slotT_i, J[k][E] = sum_i nu_ki slotE_i.  Every nonzero is finished in a register and
-  // stored once.
   const double* __restrict__ P = t.P;
-  gather<S, 1, 1, PYJAC_UJ, PYJAC_UNJ>(pl.jplan, cnt + CNT_J,
-      [&](const int32_t* e, double (&v)[1]) {
-        const uint32_t ent = (uint32_t)__ldg(e);
-        v[0] += apply_sign(P[(ent & ~SIGN_BIT) * S + s], ent);
-      },
-      [&](int slot) { return __ldg(pl.j_pos + slot); },
-      [&](int, int pos, const double (&v)[1]) {
-        if (pos >= 0) { if (valid) out[obase + (int64_t)pos * tile] = v[0]; }
-        else if (pos <= -2) t.part[(-2 - pos) * S + s] = v[0];
-      });
-  TICK(4);
+  // The T/E-row gather goes FIRST: it has few, long units; warps that finish it early move on to the many short
+  // units of the species rows (no barrier in between), so its latency tail is hidden behind them.
   // a10: T and E rows, species columns: gather over reactions with the per-state weights dE~_i, dn~_i
   //   J[T][j] = -(sum_i dE~_i g_ij + f_T (c_j - c_Ns)) / (D V);  J[E][j] = cS sum_i dn~_i g_ij + cT J[T][j]
   const double cL = t.ck[L * S + s];
@@ -655,6 +643,20 @@ jacobian_kernel(const DevMech m, const DevPlan pl, int mode, int64_t n_states, i
           const int pi = m.cplan.part_base + 2 * (-2 - posT);
           t.part[pi * S + s] = v[0]; t.part[(pi + 1) * S + s] = v[1];
         }
+      });
+  TICK(4);
+  // a9: species rows.  Block entries J[k][j] = sum_i nu_ki (Ghat^j_i - Ghat^Ns_i); T and E columns
+  // J[k][T] = sum_i nu_ki slotT_i, J[k][E] = sum_i nu_ki slotE_i.  Every nonzero is finished in a register and
+  // stored once.
+  gather<S, 1, 1, PYJAC_UJ, PYJAC_UNJ>(pl.jplan, cnt + CNT_J,
+      [&](const int32_t* e, double (&v)[1]) {
+        const uint32_t ent = (uint32_t)__ldg(e);
+        v[0] += apply_sign(P[(ent & ~SIGN_BIT) * S + s], ent);
+      },
+      [&](int slot) { return __ldg(pl.j_pos + slot); },
+      [&](int, int pos, const double (&v)[1]) {
+        if (pos >= 0) { if (valid) out[obase + (int64_t)pos * tile] = v[0]; }
+        else if (pos <= -2) t.part[(-2 - pos) * S + s] = v[0];
       });
   if (pl.jplan.n_comb + m.cplan.n_comb) {
     __syncthreads();
