@@ -75,10 +75,20 @@ __device__ __forceinline__ int next_chunk(int* counter) {
   return __shfl_sync(0xffffffffu, c, 0);
 }
 
+template <int S> __device__ __forceinline__ double red_sum(const double* red, int j, int s);
+
 template <int S> __device__ __forceinline__ double group_sum(double v) {
 #pragma unroll
   for (int o = 16; o >= S; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
   return v;
+}
+
+// sum over the warps of reduction slot j of state s (partials written by phases01)
+template <int S> __device__ __forceinline__ double red_sum(const double* red, int j, int s) {
+  double t = 0.0;
+#pragma unroll
+  for (int w = 0; w < NW; ++w) t += red[(w * NRED + j) * S + s];
+  return t;
 }
 
 __device__ __forceinline__ double apply_sign(double v, uint32_t ent) {
@@ -443,8 +453,17 @@ __device__ __forceinline__ void phases01(const DevMech& m, Tile<S, JAC>& t, int 
     }
   }
   TICK(1);
-  if (JAC) block_reduce<S, 7>(acc, t.red, t.sc, SC_R0);
-  else { double a2[2] = {acc[0], acc[1]}; block_reduce<S, 2>(a2, t.red, t.sc, SC_R0); }
+  // reaction sums: only the per-warp partials are written here; the single barrier below also publishes the slots.
+  // Consumers add the NW partials themselves (red_sum), which saves the second reduction stage and its barrier.
+  {
+    const int lane = tid & 31, warp = tid >> 5;
+#pragma unroll
+    for (int j = 0; j < (JAC ? 7 : 2); ++j) {
+      const double v = group_sum<S>(acc[j]);
+      if (lane < S) t.red[(warp * NRED + j) * S + lane] = v;
+    }
+  }
+  __syncthreads();
 }
 
 }  // namespace
@@ -554,8 +573,8 @@ source_kernel(const DevMech m, int mode, int64_t n_states, int64_t tile, const d
   }
   if (threadIdx.x < S && valid) {
     const double T = t.sc[SC_T * S + s], Pp = t.sc[SC_P * S + s];
-    const double fT = -t.sc[SC_R0 * S + s] / t.sc[SC_D * S + s];          // Eq. 5
-    const double Ssum = t.sc[SC_R1 * S + s];
+    const double fT = -red_sum<S>(t.red, 0, s) / t.sc[SC_D * S + s];          // Eq. 5
+    const double Ssum = red_sum<S>(t.red, 1, s);
     const double fE = mode == PYJAC_CONP ? V * (T * R_GAS / Pp * Ssum + fT / T)   // Eq. 8a
                                          : T * R_GAS * Ssum + Pp / T * fT;        // Eq. 8b
     out[obase] = fT;
@@ -586,7 +605,7 @@ jacobian_kernel(const DevMech m, const DevPlan pl, int mode, int64_t n_states, i
   const bool valid = s0 + s < n_states;
   const int64_t obase = state_base(min(s0 + s, n_states - 1), tile, pl.n_e);
   const double T = t.sc[SC_T * S + s], V = t.sc[SC_V * S + s], Pp = t.sc[SC_P * S + s], D = t.sc[SC_D * S + s];
-  const double N = t.sc[SC_R0 * S + s], Ssum = t.sc[SC_R1 * S + s];
+  const double N = red_sum<S>(t.red, 0, s);
   const double fT = -N / D;
   // dense output: structural zeros, each stored once (no memset pass).  A warp takes 32 bitmap words (1024
   // elements) at a time: one coalesced mask load, then 32 fully coalesced predicated store instructions.
@@ -676,8 +695,9 @@ jacobian_kernel(const DevMech m, const DevPlan pl, int mode, int64_t n_states, i
   // a10: the four corner entries from the phase-1 reductions (R4-7)
   if (tid < S && valid) {
     const double Ctot = t.sc[SC_CTOT * S + s];
-    const double AT = t.sc[SC_R2 * S + s], BT = t.sc[SC_R3 * S + s], AE = t.sc[SC_R4 * S + s], BE = t.sc[SC_R5 * S + s];
-    const double sumcw = t.sc[SC_R6 * S + s];
+    const double Ssum = red_sum<S>(t.red, 1, s);
+    const double AT = red_sum<S>(t.red, 2, s), BT = red_sum<S>(t.red, 3, s), AE = red_sum<S>(t.red, 4, s), BE = red_sum<S>(t.red, 5, s);
+    const double sumcw = red_sum<S>(t.red, 6, s);
     const double iV = 1.0 / V;
     const double dN_dT = AT * iV + sumcw;
     const double dD_dT = t.sc[SC_DDDT * S + s] - cL * Ctot / T;
