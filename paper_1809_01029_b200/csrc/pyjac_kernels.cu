@@ -479,7 +479,7 @@ namespace {
 //   acc(const int32_t* entry, double (&v)[NACC])      accumulate one entry
 //   store(int slot, const double (&v)[NACC])          slot = processing slot (index into the position arrays)
 // ---------------------------------------------------------------------------------------------------
-template <int S, int STRIDE, int NACC, int U, int UNROLL, class AccF, class PosF, class StoreF>
+template <int S, int STRIDE, int NACC, int U, int UNROLL, class P, class AccF, class PosF, class StoreF>
 __device__ __forceinline__ void gather(const DevGather& g, int* counter, AccF acc, PosF pos_of, StoreF store) {
   const int lane = threadIdx.x & 31, sub = lane / S;
   constexpr int IPW = 32 / S;                 // segments of one warp per "u"
@@ -499,7 +499,7 @@ __device__ __forceinline__ void gather(const DevGather& g, int* counter, AccF ac
     const int sg = unit / UPG;
     const int il0 = (unit % UPG) * (U * IPW) + sub;
     const int slot0 = sg * ELL_W + il0;
-    int pos[U];
+    P pos[U];
 #pragma unroll
     for (int u = 0; u < U; ++u) pos[u] = pos_of(slot0 + u * IPW);
     const int32_t* __restrict__ e = g.ell_ent + (meta.x + il0) * STRIDE;
@@ -555,7 +555,7 @@ source_kernel(const DevMech m, int mode, int64_t n_states, int64_t tile, const d
   const double V = t.sc[SC_V * S + s];
   // a7: omega_k = sum_i nu_ki q_i (Eq. 4), dn_k/dt = V omega_k (Eq. 3)
   const double* __restrict__ P = t.P;
-  gather<S, 1, 1, PYJAC_UQ, 4>(m.qplan, cnt + CNT_Q,
+  gather<S, 1, 1, PYJAC_UQ, 4, int>(m.qplan, cnt + CNT_Q,
       [&](const int32_t* e, double (&v)[1]) {
         const uint32_t ent = (uint32_t)__ldg(e);
         v[0] += apply_sign(P[(ent & ~SIGN_BIT) * S + s], ent);
@@ -641,7 +641,7 @@ jacobian_kernel(const DevMech m, const DevPlan pl, int mode, int64_t n_states, i
   const double cS = mode == PYJAC_CONP ? T * R_GAS / Pp : T * R_GAS / V;
   const double cT = mode == PYJAC_CONP ? V / T : Pp / T;
   const double* __restrict__ dE = t.dE;
-  gather<S, 4, 2, PYJAC_UC, PYJAC_UNC>(m.cplan, cnt + CNT_C,
+  gather<S, 4, 2, PYJAC_UC, PYJAC_UNC, int4>(m.cplan, cnt + CNT_C,
       [&](const int32_t* e, double (&v)[2]) {
         const int4 pr = __ldg(reinterpret_cast<const int4*>(e));      // slot | sign, reaction, dn~ (2 words)
         const uint32_t ent = (uint32_t)pr.x;
@@ -649,17 +649,19 @@ jacobian_kernel(const DevMech m, const DevPlan pl, int mode, int64_t n_states, i
         v[0] += dE[pr.y * S + s] * x;
         v[1] += __hiloint2double(pr.w, pr.z) * x;
       },
-      [&](int slot) { return __ldg(pl.c_pos + 2 * slot); },
-      [&](int slot, int posT, const double (&v)[2]) {
-        if (posT >= 0) {
+      [&](int slot) {                                     // (T, j) position or partial code, (E, j) position, column j:
+        const int2 pp = __ldg(reinterpret_cast<const int2*>(pl.c_pos) + slot);   // all requested before the entry loop
+        return make_int4(pp.x, pp.y, __ldg(m.c_item + slot), 0);
+      },
+      [&](int, int4 pp, const double (&v)[2]) {
+        if (pp.x >= 0) {
           if (valid) {
-            const int j = __ldg(m.c_item + slot);
-            const double JT = -(v[0] + fT * (t.ck[j * S + s] - cL)) * iDV;
-            out[obase + (int64_t)posT * tile] = JT;
-            out[obase + (int64_t)__ldg(pl.c_pos + 2 * slot + 1) * tile] = cS * v[1] + cT * JT;
+            const double JT = -(v[0] + fT * (t.ck[pp.z * S + s] - cL)) * iDV;
+            out[obase + (int64_t)pp.x * tile] = JT;
+            out[obase + (int64_t)pp.y * tile] = cS * v[1] + cT * JT;
           }
-        } else if (posT <= -2) {
-          const int pi = m.cplan.part_base + 2 * (-2 - posT);
+        } else if (pp.x <= -2) {
+          const int pi = m.cplan.part_base + 2 * (-2 - pp.x);
           t.part[pi * S + s] = v[0]; t.part[(pi + 1) * S + s] = v[1];
         }
       });
@@ -667,7 +669,7 @@ jacobian_kernel(const DevMech m, const DevPlan pl, int mode, int64_t n_states, i
   // a9: species rows.  Block entries J[k][j] = sum_i nu_ki (Ghat^j_i - Ghat^Ns_i); T and E columns
   // J[k][T] = sum_i nu_ki slotT_i, J[k][E] = sum_i nu_ki slotE_i.  Every nonzero is finished in a register and
   // stored once.
-  gather<S, 1, 1, PYJAC_UJ, PYJAC_UNJ>(pl.jplan, cnt + CNT_J,
+  gather<S, 1, 1, PYJAC_UJ, PYJAC_UNJ, int>(pl.jplan, cnt + CNT_J,
       [&](const int32_t* e, double (&v)[1]) {
         const uint32_t ent = (uint32_t)__ldg(e);
         v[0] += apply_sign(P[(ent & ~SIGN_BIT) * S + s], ent);
