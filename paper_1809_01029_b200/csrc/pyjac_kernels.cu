@@ -281,64 +281,91 @@ __device__ __forceinline__ void phases01(const DevMech& m, Tile<S, JAC>& t, int 
     const int idx = chunk * 32 + (tid & 31);
     if (idx >= nr * S) continue;
     const int r = idx / S;
+    // All per-reaction table words are requested back to back at the top of the iteration and pinned (the empty asm
+    // makes every one of them live here), so the reaction costs ONE exposed L2 round trip instead of one per first
+    // use further down (the compiler otherwise sinks each load to its consumer: ~3 serialized round trips).
     const int info = __ldg(m.info + r);
+    const double rx_lnA = __ldg(m.lnA + r), rx_beta = __ldg(m.beta + r), rx_Ta = __ldg(m.Ta + r), rx_dn = __ldg(m.dn + r);
+    const uint4 w0 = __ldg(reinterpret_cast<const uint4*>(m.sp + 8 * r));
+    const uint2 w1 = __ldg(reinterpret_cast<const uint2*>(m.sp + 8 * r + 4));
+    const int rx_base = JAC ? __ldg(m.slot_base + r) : 0;
+    const int e0 = __ldg(m.eff_ptr + r), e1 = __ldg(m.eff_ptr + r + 1);
+    const int rx_aux = __ldg(m.aux + r);
+    asm volatile("" :: "r"(info), "d"(rx_lnA), "d"(rx_beta), "d"(rx_Ta), "d"(rx_dn), "r"(w0.x), "r"(w0.y), "r"(w0.z), "r"(w0.w),
+                 "r"(w1.x), "r"(w1.y), "r"(rx_base), "r"(e0), "r"(e1), "r"(rx_aux));
     const int type = info & INFO_TYPE_MASK;
     const bool rev = info & INFO_REV;
     // a3: forward rate constant
     double lnkf, lam_f, dlnk_dP = 0.0;
     if (type <= PYJAC_FALLOFF_SRI) {
-      const double beta = __ldg(m.beta + r), Ta = __ldg(m.Ta + r);
-      lnkf = __ldg(m.lnA + r) + beta * lnT - Ta * invT;
+      const double beta = rx_beta, Ta = rx_Ta;
+      lnkf = rx_lnA + beta * lnT - Ta * invT;
       lam_f = (beta + Ta * invT) * invT;
     } else if (type == PYJAC_PLOG) {
-      const int a = m.aux[r], p0 = m.plog_ptr[a], np = m.plog_ptr[a + 1] - p0;
-      int j = 0;
-      bool interp = true;
-      if (Pp <= m.plog_P[p0]) { interp = false; }
-      else if (Pp >= m.plog_P[p0 + np - 1]) { interp = false; j = np - 1; }
-      else { while (j + 2 < np && m.plog_P[p0 + j + 1] <= Pp) ++j; }     // last j with P_j <= P (R-S4)
-      const double b0 = m.plog_b[p0 + j], Ta0 = m.plog_Ta[p0 + j];
-      const double l0 = m.plog_lnA[p0 + j] + b0 * lnT - Ta0 * invT;
+      // table loads are batched (8 independent requests per round trip) instead of one per loop iteration
+      const int2 pp = make_int2(__ldg(m.plog_ptr + rx_aux), __ldg(m.plog_ptr + rx_aux + 1));
+      const int p0 = pp.x, np = pp.y - pp.x;
+      int cnt_le = 0;                                   // number of table pressures <= P
+      for (int b = 0; b < np; b += 8) {
+        double pq[8];
+#pragma unroll
+        for (int q = 0; q < 8; ++q) pq[q] = b + q < np ? __ldg(m.plog_P + p0 + b + q) : 1e300;
+#pragma unroll
+        for (int q = 0; q < 8; ++q) cnt_le += pq[q] <= Pp ? 1 : 0;
+      }
+      // P <= P_0: first point; P >= P_last: last point; else interval j = last j with P_j <= P (S4)
+      const bool interp = cnt_le >= 1 && cnt_le < np && !(cnt_le == 1 && Pp <= __ldg(m.plog_P + p0));
+      const int j = cnt_le >= np ? np - 1 : (cnt_le >= 1 ? cnt_le - 1 : 0);
+      const int j1 = interp ? j + 1 : j;
+      const double b0 = __ldg(m.plog_b + p0 + j), Ta0 = __ldg(m.plog_Ta + p0 + j), lA0 = __ldg(m.plog_lnA + p0 + j), lP0 = __ldg(m.plog_lnP + p0 + j);
+      const double b1 = __ldg(m.plog_b + p0 + j1), Ta1 = __ldg(m.plog_Ta + p0 + j1), lA1 = __ldg(m.plog_lnA + p0 + j1), lP1 = __ldg(m.plog_lnP + p0 + j1);
+      asm volatile("" :: "d"(b0), "d"(Ta0), "d"(lA0), "d"(lP0), "d"(b1), "d"(Ta1), "d"(lA1), "d"(lP1));
+      const double l0 = lA0 + b0 * lnT - Ta0 * invT;
       const double lam0 = (b0 + Ta0 * invT) * invT;
       lnkf = l0; lam_f = lam0;
       if (interp) {
-        const double b1 = m.plog_b[p0 + j + 1], Ta1 = m.plog_Ta[p0 + j + 1];
-        const double l1 = m.plog_lnA[p0 + j + 1] + b1 * lnT - Ta1 * invT;
+        const double l1 = lA1 + b1 * lnT - Ta1 * invT;
         const double lam1 = (b1 + Ta1 * invT) * invT;
-        const double idl = 1.0 / (m.plog_lnP[p0 + j + 1] - m.plog_lnP[p0 + j]);
-        const double w = (lnP - m.plog_lnP[p0 + j]) * idl;
+        const double idl = 1.0 / (lP1 - lP0);
+        const double w = (lnP - lP0) * idl;
         lnkf = l0 + (l1 - l0) * w;
         lam_f = (1.0 - w) * lam0 + w * lam1;
         dlnk_dP = (l1 - l0) * idl / Pp;
       }
     } else {
       const double LN10 = 2.302585092994045684, ILN10 = 0.434294481903251828;
-      const int a = m.aux[r];
-      const int nT = m.cheb_meta[4 * a], nP = m.cheb_meta[4 * a + 1];
-      const double* __restrict__ eta = m.cheb_coef + m.cheb_meta[4 * a + 2];
-      const double iTmin = m.cheb_lim[4 * a], iTmax = m.cheb_lim[4 * a + 1], lPmin = m.cheb_lim[4 * a + 2], lPmax = m.cheb_lim[4 * a + 3];
+      const int4 cm = __ldg(reinterpret_cast<const int4*>(m.cheb_meta) + rx_aux);          // nT, nP, coefficient offset
+      const double2 cl0 = __ldg(reinterpret_cast<const double2*>(m.cheb_lim) + 2 * rx_aux);
+      const double2 cl1 = __ldg(reinterpret_cast<const double2*>(m.cheb_lim) + 2 * rx_aux + 1);
+      const int nP = cm.y, n_coef = cm.x * cm.y;
+      const double* __restrict__ eta = m.cheb_coef + cm.z;
+      const double iTmin = cl0.x, iTmax = cl0.y, lPmin = cl1.x, lPmax = cl1.y;
       const double Tr = (2.0 * invT - iTmin - iTmax) / (iTmax - iTmin);
       const double Pr_ = (2.0 * lnP * ILN10 - lPmin - lPmax) / (lPmax - lPmin);
       double lg = 0.0, dlg_dT = 0.0, dlg_dP = 0.0;
+      // the row-major coefficients are consumed in order by a running pair of three-term recurrences
+      // (T_a(Tr), T_b(Pr) and their derivatives); they are fetched 8 at a time (one round trip per 8, not per 1)
       double cT = 1.0, cTm = 0.0, dT = 0.0, dTm = 0.0;       // T_a(Tr), T_{a-1}, derivatives
-      for (int ia = 0; ia < nT; ++ia) {
-        if (ia == 1) { cTm = 1.0; cT = Tr; dTm = 0.0; dT = 1.0; }
-        else if (ia > 1) {
-          const double n1 = 2.0 * Tr * cT - cTm, d1 = 2.0 * cT + 2.0 * Tr * dT - dTm;
-          cTm = cT; cT = n1; dTm = dT; dT = d1;
-        }
-        double cP = 1.0, cPm = 0.0, dP = 0.0, dPm = 0.0;
-        double sv = 0.0, sd = 0.0;
-        for (int ib = 0; ib < nP; ++ib) {
-          if (ib == 1) { cPm = 1.0; cP = Pr_; dPm = 0.0; dP = 1.0; }
-          else if (ib > 1) {
-            const double n1 = 2.0 * Pr_ * cP - cPm, d1 = 2.0 * cP + 2.0 * Pr_ * dP - dPm;
-            cPm = cP; cP = n1; dPm = dP; dP = d1;
+      double cP = 1.0, cPm = 0.0, dP = 0.0, dPm = 0.0;
+      int ia = 0, ib = 0;
+      for (int b = 0; b < n_coef; b += 8) {
+        double eq[8];
+#pragma unroll
+        for (int q = 0; q < 8; ++q) eq[q] = b + q < n_coef ? __ldg(eta + b + q) : 0.0;
+#pragma unroll
+        for (int q = 0; q < 8; ++q) {
+          if (b + q < n_coef) {
+            const double e = eq[q];
+            lg += e * cT * cP; dlg_dT += e * dT * cP; dlg_dP += e * cT * dP;
+            if (++ib == nP) {                    // next row: advance T_a, restart T_b
+              ib = 0; ++ia;
+              if (ia == 1) { cTm = 1.0; cT = Tr; dTm = 0.0; dT = 1.0; }
+              else { const double n1 = 2.0 * Tr * cT - cTm, d1 = 2.0 * cT + 2.0 * Tr * dT - dTm; cTm = cT; cT = n1; dTm = dT; dT = d1; }
+              cP = 1.0; cPm = 0.0; dP = 0.0; dPm = 0.0;
+            } else if (ib == 1) { cPm = 1.0; cP = Pr_; dPm = 0.0; dP = 1.0; }
+            else { const double n1 = 2.0 * Pr_ * cP - cPm, d1 = 2.0 * cP + 2.0 * Pr_ * dP - dPm; cPm = cP; cP = n1; dPm = dP; dP = d1; }
           }
-          const double e = eta[ia * nP + ib];
-          sv += e * cP; sd += e * dP;
         }
-        lg += cT * sv; dlg_dT += dT * sv; dlg_dP += cT * sd;
       }
       lnkf = LN10 * lg;
       lam_f = LN10 * dlg_dT * (-2.0 * invT * invT / (iTmax - iTmin));
@@ -347,8 +374,6 @@ __device__ __forceinline__ void phases01(const DevMech& m, Tile<S, JAC>& t, int 
     const double kf = exp(lnkf);
     // stoichiometry: concentrations, products and one-factor-removed products (no division by C_k: R-S7).
     // Unused entries point at the dummy species ns (C = 1, thermo = 0), so no predicates are needed.
-    const uint4 w0 = __ldg(reinterpret_cast<const uint4*>(m.sp + 8 * r));
-    const uint2 w1 = __ldg(reinterpret_cast<const uint2*>(m.sp + 8 * r + 4));
     const uint32_t spw[6] = {w0.x, w0.y, w0.z, w0.w, w1.x, w1.y};
     double pw[6], pm[6];
     double dg = 0.0, dh = 0.0, dEt = 0.0, dct = 0.0;
@@ -387,15 +412,27 @@ __device__ __forceinline__ void phases01(const DevMech& m, Tile<S, JAC>& t, int 
     const double dRdT = lam_f * Rf - lam_r * Rr;
     // a5: third body / falloff
     double c = 1.0, X = 0.0, GT = dRdT, MdcdM_R = 0.0;
-    const int e0 = __ldg(m.eff_ptr + r), e1 = __ldg(m.eff_ptr + r + 1);
     const double adef = (info & INFO_ADEF) ? 1.0 : 0.0;
     if (type >= PYJAC_THIRD_BODY && type <= PYJAC_FALLOFF_SRI) {
       double M = adef * Ctot;                       // sum_k C_k == C_tot by construction of C_Ns
-      for (int e = e0; e < e1; ++e) M += __ldg(m.eff_d + e) * t.C[__ldg(m.eff_sp + e) * S + s];
+      for (int eb = e0; eb < e1; eb += 4) {           // efficiency list, 4 entries per round trip
+        int esp[4]; double ed[4];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) { esp[q] = eb + q < e1 ? __ldg(m.eff_sp + eb + q) : ns; ed[q] = eb + q < e1 ? __ldg(m.eff_d + eb + q) : 0.0; }
+#pragma unroll
+        for (int q = 0; q < 4; ++q) M += ed[q] * t.C[esp[q] * S + s];
+      }
       if (type == PYJAC_THIRD_BODY) {
         c = M; X = Rn; GT = M * dRdT; MdcdM_R = M * Rn;
       } else {
-        const double* __restrict__ fp = m.fall + 12 * m.aux[r];
+        // the 10 falloff parameters of the reaction in one batch of 16-byte loads
+        double fp[10];
+        {
+          const double2* __restrict__ f2 = reinterpret_cast<const double2*>(m.fall + 12 * rx_aux);
+#pragma unroll
+          for (int q = 0; q < 5; ++q) { const double2 v2 = __ldg(f2 + q); fp[2 * q] = v2.x; fp[2 * q + 1] = v2.y; }
+          asm volatile("" :: "d"(fp[0]), "d"(fp[1]), "d"(fp[2]), "d"(fp[4]), "d"(fp[5]), "d"(fp[6]), "d"(fp[7]), "d"(fp[8]));
+        }
         const double b0 = fp[1], Ta0 = fp[2];
         const double k0_kinf = exp(fp[0] + b0 * lnT - Ta0 * invT - lnkf);
         const double Pr = k0_kinf * M;
@@ -403,7 +440,7 @@ __device__ __forceinline__ void phases01(const DevMech& m, Tile<S, JAC>& t, int 
         const double i1p = 1.0 / (1.0 + Pr);
         c = bl.F * Pr * i1p;
         const double dc_dPr = bl.F * i1p * i1p + Pr * i1p * bl.dF_dPr;
-        const double dPr_dT = Pr * (b0 - __ldg(m.beta + r) + (Ta0 - __ldg(m.Ta + r)) * invT) * invT;
+        const double dPr_dT = Pr * (b0 - rx_beta + (Ta0 - rx_Ta) * invT) * invT;
         X = dc_dPr * k0_kinf * Rn;
         GT = (dc_dPr * dPr_dT + Pr * i1p * bl.dF_dT) * Rn + c * dRdT;
         MdcdM_R = Pr * dc_dPr * Rn;
@@ -411,13 +448,13 @@ __device__ __forceinline__ void phases01(const DevMech& m, Tile<S, JAC>& t, int 
     }
     const double q = c * Rn;
     // reaction-sum reductions (R4-7/8): N = sum dE~_i q_i, S = sum dn~_i q_i
-    const double dn = __ldg(m.dn + r);
+    const double dn = rx_dn;
     acc[0] += dEt * q; acc[1] += dn * q;
     if (!JAC) {
       t.P[idx] = q;
     } else {
       // a8: per-reaction partials -> slots
-      const int base = __ldg(m.slot_base + r);
+      const int base = rx_base;
       const int nre = (info >> INFO_NREAC_SHIFT) & 3, npr = (info >> INFO_NPROD_SHIFT) & 3;
       const double a_ = c * kf, b_ = c * kr;
       double GL = adef * X;                          // full dQ_i/dC_Ns
@@ -432,10 +469,17 @@ __device__ __forceinline__ void phases01(const DevMech& m, Tile<S, JAC>& t, int 
         for (int a = 0; a < 3; ++a)
           if (a < npr) { t.P[(slot++) * S + s] = dr[a]; if ((int)(spw[3 + a] & 0xffff) == L) GL += dr[a]; }
       }
-      for (int e = e0; e < e1; ++e) {
-        const double v = __ldg(m.eff_d + e) * X;
-        t.P[(slot++) * S + s] = v;
-        if (__ldg(m.eff_sp + e) == L) GL += v;
+      for (int eb = e0; eb < e1; eb += 4) {
+        int esp[4]; double ed[4];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) { esp[q] = eb + q < e1 ? __ldg(m.eff_sp + eb + q) : ns; ed[q] = eb + q < e1 ? __ldg(m.eff_d + eb + q) : 0.0; }
+#pragma unroll
+        for (int q = 0; q < 4; ++q)
+          if (eb + q < e1) {
+            const double v = ed[q] * X;
+            t.P[(slot++) * S + s] = v;
+            if (esp[q] == L) GL += v;
+          }
       }
       // chain rule to the state variables (R4-2); E column in Euler-homogeneity form (R4-6)
       const double slotT = V * (GT - ctot_T * GL);
