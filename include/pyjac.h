@@ -124,6 +124,18 @@ int pyjac_jacobian_dense(const pyjac_mech *mech, int mode, char order, int64_t n
                          int64_t tile, const double *d_phi, const double *d_param, double *d_J,
                          void *stream);
 
+/* First-order forward finite-difference Jacobian: the paper's own comparison baseline (Fig. 12;
+ * "implemented for comparison purposes only").  The paper gives no step rule; R7:
+ *     xp_c = fl(phi_c + fma(rel_step, |phi_c|, abs_step)),  h_c = fl(xp_c - phi_c),
+ *     J(i, c) = fl(fl(f_i(phi with phi_c := xp_c) - f_i(phi)) / h_c),
+ * n_var + 1 source-term evaluations (steps a1-a7) per state, all inside one kernel.  fmt: PYJAC_CSR / PYJAC_CSC store
+ * the nnz entries of the handle's pattern in that value order (entries outside the pattern are not formed); 'C' /
+ * 'F' store all n_var^2 entries in that order.  rel_step, abs_step >= 0, not both 0 (PYJAC_EINVAL); a step that
+ * rounds to h_c = 0 gives inf/NaN in that column.  Truncation error O(h): this is NOT the analytical Jacobian and is
+ * only compared with an oracle doing the same arithmetic. */
+int pyjac_jacobian_fd(const pyjac_mech *mech, int mode, int fmt, double rel_step, double abs_step, int64_t n_states,
+                      int64_t ld, int64_t tile, const double *d_phi, const double *d_param, double *d_out, void *stream);
+
 /* End-to-end convenience calls on HOST buffers (same layouts): allocate device scratch, copy in,
  * run, copy out, synchronise.  what: 0 = source terms, 1 = sparse Jacobian (fmt), 2 = dense Jacobian
  * (fmt = 'C' or 'F').  h_out must hold n_e * ld doubles. */
@@ -131,7 +143,8 @@ int pyjac_eval_host(const pyjac_mech *mech, int what, int mode, int fmt, int64_t
                     int64_t tile, const double *h_phi, const double *h_param, double *h_out);
 
 /* Launch geometry chosen for a call (for DESIGN/bench reporting): states per CTA, threads per CTA,
- * dynamic shared memory bytes.  what as in pyjac_eval_host. */
+ * dynamic shared memory bytes.  what as in pyjac_eval_host; 3 = finite-difference Jacobian (states_per_cta is then
+ * the number of perturbed columns one CTA evaluates per pass over its single state). */
 int pyjac_launch_info(const pyjac_mech *mech, int what, int32_t *states_per_cta, int32_t *threads,
                       int64_t *smem_bytes);
 

@@ -54,6 +54,7 @@ def _load():
         lib.orc_intermediates.argtypes = [C.c_void_p, C.c_int, _D, C.c_double] + [_D] * 17
         lib.orc_fd_jacobian.argtypes = [C.c_void_p, C.c_int, _D, C.c_double, C.c_double, _D, _D]
         lib.orc_cs_jacobian.argtypes = [C.c_void_p, C.c_int, _D, C.c_double, C.c_double, _D, _D]
+        lib.orc_fd1_jacobian.argtypes = [C.c_void_p, C.c_int, C.c_int64, _D, _D, C.c_double, C.c_double, _D]
         _lib = lib
     return _lib
 
@@ -136,6 +137,14 @@ class Oracle:
             ntot = np.abs(phi[2:]).sum()
             floor = np.concatenate([[1.0, 1e-30], np.full(self.nvar - 2, 1e-3 * ntot)])
         return np.ascontiguousarray(floor, np.float64)
+
+    def fd1_jacobian(self, mode, phi, param, rel_step, abs_step):
+        """First-order forward finite-difference Jacobian (step rule DESIGN.md R7), dense [n, nvar, nvar]."""
+        phi = np.ascontiguousarray(phi, np.float64).reshape(-1, self.nvar)
+        param = np.ascontiguousarray(param, np.float64).reshape(-1)
+        J = np.empty((phi.shape[0], self.nvar, self.nvar))
+        _lib.orc_fd1_jacobian(self._h, mode, phi.shape[0], _p(phi), _p(param), float(rel_step), float(abs_step), _p(J))
+        return J
 
     def fd_jacobian(self, mode, phi, param, rel=1e-4, floor=None):
         phi = np.ascontiguousarray(phi, np.float64).reshape(self.nvar)

@@ -570,6 +570,33 @@ void orc_intermediates(void* hv, int mode, const double* phi, double param, doub
     scal[0] = w.Ctot; scal[1] = w.D; scal[2] = w.N; scal[3] = w.S;
 }
 
+// First-order forward finite-difference Jacobian, the paper's comparison baseline (Fig. 12), written
+// out column by column in double.  The paper gives no step rule; R7:
+//     xp_c = phi_c + fma(rel, |phi_c|, abs),  h_c = xp_c - phi_c,  J(i,c) = (f_i(phi; phi_c := xp_c) - f_i(phi)) / h_c.
+// J [n][nvar][nvar] row-major.  Pinned against the analytical Jacobian (first-order convergence, test P13).
+void orc_fd1_jacobian(void* hv, int mode, int64_t n, const double* phi, const double* param, double rel, double abs_, double* J) {
+    Handle* h = (Handle*)hv; const Mech& m = h->m; const int nvar = m.ns + 1;
+#pragma omp parallel
+    {
+        Inter<double> w; w.resize(m.ns, m.nr);
+        std::vector<double> x(nvar), f0(nvar), f1(nvar);
+#pragma omp for schedule(static)
+        for (int64_t s = 0; s < n; ++s) {
+            const double* ph = phi + s * nvar;
+            double* Js = J + (size_t)s * nvar * nvar;
+            eval_source<double>(m, mode, ph, param[s], f0.data(), w);
+            for (int c = 0; c < nvar; ++c) {
+                for (int k = 0; k < nvar; ++k) x[k] = ph[k];
+                const double xp = ph[c] + std::fma(rel, std::fabs(ph[c]), abs_);
+                const double hc = xp - ph[c];
+                x[c] = xp;
+                eval_source<double>(m, mode, x.data(), param[s], f1.data(), w);
+                for (int r = 0; r < nvar; ++r) Js[(size_t)r * nvar + c] = (f1[r] - f0[r]) / hc;
+            }
+        }
+    }
+}
+
 // pin P3: 4th-order central finite differences of the oracle's own f, evaluated in long double.
 // step h_c = rel * max(|phi_c|, floor_c); J row-major nvar x nvar (double)
 void orc_fd_jacobian(void* hv, int mode, const double* phi, double param, double rel, const double* floor_, double* J) {

@@ -67,6 +67,7 @@ def lib():
         L.pyjac_source_terms.argtypes = [vp, i32, i64, i64, i64, vp, vp, vp, vp]
         L.pyjac_jacobian_sparse.argtypes = [vp, i32, i32, i64, i64, i64, vp, vp, vp, vp]
         L.pyjac_jacobian_dense.argtypes = [vp, i32, C.c_char, i64, i64, i64, vp, vp, vp, vp]
+        L.pyjac_jacobian_fd.argtypes = [vp, i32, i32, C.c_double, C.c_double, i64, i64, i64, vp, vp, vp, vp]
         L.pyjac_eval_host.argtypes = [vp, i32, i32, i32, i64, i64, i64, vp, vp, vp]
         L.pyjac_launch_info.argtypes = [vp, i32, _I, _I, C.POINTER(i64)]
         _lib = L
@@ -134,6 +135,12 @@ def pyjac_jacobian_sparse(h, mode, fmt, n_states, ld, tile, d_phi, d_param, d_va
 def pyjac_jacobian_dense(h, mode, order, n_states, ld, tile, d_phi, d_param, d_J, stream=0):
     _check(lib().pyjac_jacobian_dense(h, mode, order.encode() if isinstance(order, str) else order, n_states, ld, tile,
                                       d_phi, d_param, d_J, stream))
+
+
+def pyjac_jacobian_fd(h, mode, fmt, rel_step, abs_step, n_states, ld, tile, d_phi, d_param, d_out, stream=0):
+    """fmt: CSR / CSC (the handle's pattern) or 'C' / 'F' (dense)."""
+    _check(lib().pyjac_jacobian_fd(h, mode, ord(fmt) if isinstance(fmt, str) else fmt, rel_step, abs_step, n_states, ld,
+                                   tile, d_phi, d_param, d_out, stream))
 
 
 def pyjac_eval_host(h, what, mode, fmt, n_states, ld, tile, h_phi, h_param, h_out):

@@ -96,6 +96,9 @@ int pyjac_mech_create_ex(const pyjac_mech_desc* desc, int cuda_device, uint32_t 
     if (int r_ = m->upload(h.cplan.target, &d.c_item)) return r_;
     if (int r_ = m->upload(h.qplan.comb_item, &d.qc_item)) return r_;
     if (int r_ = m->upload(h.cplan.comb_item, &d.cc_item)) return r_;
+    if (int r_ = m->upload(h.csc_ptr, &d.csc_ptr)) return r_;
+    if (int r_ = m->upload(h.csc_idx, &d.csc_idx)) return r_;
+    if (int r_ = m->upload(h.csc2csr, &d.csc2csr)) return r_;
     DevGather jplan;
     if (int r_ = m->upload_plan(h.jplan, 0, &jplan)) return r_;
     const uint32_t* mask[2];
@@ -197,9 +200,29 @@ int pyjac_jacobian_dense(const pyjac_mech* mech, int mode, char order, int64_t n
   return run_jac("pyjac_jacobian_dense", mech, mode, order == 'C' ? OUT_DENSE_C : OUT_DENSE_F, n_states, ld, tile, d_phi, d_param, d_J, stream);
 }
 
+int pyjac_jacobian_fd(const pyjac_mech* mech, int mode, int fmt, double rel_step, double abs_step, int64_t n_states,
+                      int64_t ld, int64_t tile, const double* d_phi, const double* d_param, double* d_out, void* stream) {
+  int ofmt;
+  if (fmt == PYJAC_CSR) ofmt = OUT_CSR;
+  else if (fmt == PYJAC_CSC) ofmt = OUT_CSC;
+  else if (fmt == 'C') ofmt = OUT_DENSE_C;
+  else if (fmt == 'F') ofmt = OUT_DENSE_F;
+  else return fail(PYJAC_EINVAL, "pyjac_jacobian_fd: fmt must be PYJAC_CSR, PYJAC_CSC, 'C' or 'F'");
+  if (!(rel_step >= 0.0) || !(abs_step >= 0.0) || !(rel_step + abs_step > 0.0))
+    return fail(PYJAC_EINVAL, "pyjac_jacobian_fd: steps must be >= 0 and not both zero");
+  if (int rc = check_common("pyjac_jacobian_fd", mech, mode, n_states, ld, tile, d_phi, d_param, d_out)) return rc;
+  if (n_states == 0) return PYJAC_OK;
+  const LaunchCfg cfg = choose_cfg_fd(mech->h);
+  if (cfg.smem > 227 * 1024) return fail(PYJAC_ENOMEM, "pyjac_jacobian_fd: mechanism too large for shared memory");
+  const int64_t n_e = ofmt < OUT_DENSE_C ? mech->h.nnz : (int64_t)mech->h.nvar * mech->h.nvar;
+  int e = launch_fd(mech->dm, cfg, mode, ofmt, n_e, rel_step, abs_step, n_states, ld, tile, d_phi, d_param, d_out, stream);
+  if (e) return cuda_fail((cudaError_t)e, "fd_kernel launch");
+  return PYJAC_OK;
+}
+
 int pyjac_launch_info(const pyjac_mech* mech, int what, int32_t* states_per_cta, int32_t* threads, int64_t* smem_bytes) {
   if (!mech) return fail(PYJAC_EINVAL, "pyjac_launch_info: null handle");
-  const LaunchCfg cfg = choose_cfg(mech->h, what != 0, (int64_t)1 << 40, (int64_t)1 << 40);
+  const LaunchCfg cfg = what == 3 ? choose_cfg_fd(mech->h) : choose_cfg(mech->h, what != 0, (int64_t)1 << 40, (int64_t)1 << 40);
   if (states_per_cta) *states_per_cta = cfg.S;
   if (threads) *threads = cfg.threads;
   if (smem_bytes) *smem_bytes = (int64_t)cfg.smem;

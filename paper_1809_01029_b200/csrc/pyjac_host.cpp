@@ -324,6 +324,10 @@ int build_host_tables(const pyjac_mech_desc* d, bool approx, HostTables& h, std:
   std::vector<int> fill(h.csc_ptr.begin(), h.csc_ptr.end() - 1), csr2csc(h.nnz);
   for (int r = 0; r < nvar; ++r)
     for (int p = h.csr_ptr[r]; p < h.csr_ptr[r + 1]; ++p) { const int c = h.csr_idx[p]; csr2csc[p] = fill[c]; h.csc_idx[fill[c]++] = r; }
+  // finite-difference kernel: it works column by column, so it walks the CSC pattern and needs the
+  // CSR value position of every CSC entry
+  h.csc2csr.resize(h.nnz);
+  for (int64_t p = 0; p < h.nnz; ++p) h.csc2csr[csr2csc[p]] = (int32_t)p;
   auto csr_pos = [&](int r, int c) {
     auto b = h.csr_idx.begin() + h.csr_ptr[r], e = h.csr_idx.begin() + h.csr_ptr[r + 1];
     return (int)(std::lower_bound(b, e, c) - h.csr_idx.begin());

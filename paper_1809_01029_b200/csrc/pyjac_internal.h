@@ -65,6 +65,7 @@ struct HostTables {
   // pattern
   int64_t nnz = 0;
   std::vector<int32_t> csr_ptr, csr_idx, csc_ptr, csc_idx;
+  std::vector<int32_t> csc2csr;              // [nnz] CSR value position of CSC entry p (finite-difference kernel)
   // gather plans.  Entries: slot offset | SIGN_BIT (a stoichiometric coefficient of magnitude m is m copies)
   int nA = 0;                                // number of species-block nonzeros
   GatherPlan jplan;                          // species rows: block nonzeros + their T and E columns
@@ -108,6 +109,7 @@ struct DevMech {
   const double *cheb_lim, *cheb_coef;
   DevGather cplan, qplan;
   const int32_t *q_target, *c_item, *qc_item, *cc_item;   // slot -> species / column; combined lists -> species / column
+  const int32_t *csc_ptr, *csc_idx, *csc2csr;             // pattern by columns (finite-difference kernel)
 };
 
 struct DevPlan {
@@ -128,6 +130,10 @@ int launch_source(const DevMech& m, const LaunchCfg& cfg, int mode, int64_t n_st
                   const double* phi, const double* param, double* out, void* stream);
 int launch_jacobian(const DevMech& m, const DevPlan& p, const LaunchCfg& cfg, int mode, int64_t n_states, int64_t ld,
                     int64_t tile, const double* phi, const double* param, double* out, void* stream);
+// first-order forward finite-difference Jacobian.  ofmt: OutFmt.  S = columns per pass.
+LaunchCfg choose_cfg_fd(const HostTables& h);
+int launch_fd(const DevMech& m, const LaunchCfg& cfg, int mode, int ofmt, int64_t n_e, double rel_step, double abs_step,
+              int64_t n_states, int64_t ld, int64_t tile, const double* phi, const double* param, double* out, void* stream);
 int set_kernel_attributes();
 
 }  // namespace pyjac

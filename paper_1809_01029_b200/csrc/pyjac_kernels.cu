@@ -184,21 +184,20 @@ struct Tile {
 // element offset of (element e, state s) in the library layout; base_s precomputed per thread
 __device__ __forceinline__ int64_t state_base(int64_t s, int64_t tile, int64_t n_e) { return (s / tile) * (n_e * tile) + (s % tile); }
 
-template <int S, bool JAC>
-__device__ __forceinline__ void phases01(const DevMech& m, Tile<S, JAC>& t, int mode, int64_t s0, int64_t n_states,
-                                         int64_t tile, const double* __restrict__ phi, const double* __restrict__ param,
+// phi_of(e): element e of the state vector of THIS thread's lane (tid % S); par_: that lane's parameter.  The
+// analytical kernels read the caller's arrays; the finite-difference kernel adds the perturbation of its column.
+template <int S, bool JAC, class PhiF>
+__device__ __forceinline__ void phases01(const DevMech& m, Tile<S, JAC>& t, int mode, PhiF phi_of, double par_,
                                          int* cnt, long long& tick_) {
   (void)tick_;
   const int tid = threadIdx.x;
   const int ns = m.ns, nr = m.nr, L = ns - 1;
   const int s = tid % S;                        // NT % S == 0: a thread keeps its state in every loop
-  const int64_t sg = min(s0 + s, n_states - 1);  // ragged tail: recompute the last valid state, never store
-  const int64_t pbase = state_base(sg, tile, ns + 1);
   // ---- phase 0: scalars, species (C_k = n_k / V, Eq. 6; NASA-7 thermo, R2) ------------------------
   // Every thread reads T, E and the parameter itself (same address for the lanes of a state: one broadcast
   // request) so that no barrier separates the state load from the species loop.
   if (tid < N_CNT) cnt[tid] = 0;
-  const double T = phi[pbase], E_ = phi[pbase + tile], par_ = param[sg];
+  const double T = phi_of(0), E_ = phi_of(1);
   const double V = mode == PYJAC_CONP ? E_ : par_, Pp = mode == PYJAC_CONP ? par_ : E_;
   const double invT = 1.0 / T, lnT = log(T), RT = R_GAS * T, Ctot = Pp / RT;
   if (tid < S) {
@@ -245,7 +244,7 @@ __device__ __forceinline__ void phases01(const DevMech& m, Tile<S, JAC>& t, int 
       t.th4[idx * 4 + 3] = k == L ? 0.0 : c - w * cL;                   // c~_k
       t.ck[idx] = c;
       if (k < L) {
-        const double Ck = phi[pbase + (int64_t)(2 + k) * tile] * invV;
+        const double Ck = phi_of(2 + k) * invV;
         t.C[idx] = Ck;
         acc[0] += Ck; acc[1] += Ck * c; acc[2] += Ck * (R_GAS * dcpR);
       }
@@ -592,10 +591,11 @@ source_kernel(const DevMech m, int mode, int64_t n_states, int64_t tile, const d
   const int64_t s0 = (int64_t)blockIdx.x * S;
   __shared__ int cnt[N_CNT];
   long long tick_ = 0;
-  phases01<S, false>(m, t, mode, s0, n_states, tile, phi, param, cnt, tick_);
   const int s = threadIdx.x % S;
   const bool valid = s0 + s < n_states;
-  const int64_t obase = state_base(min(s0 + s, n_states - 1), tile, m.nvar);
+  const int64_t sg = min(s0 + s, n_states - 1);   // ragged tail: recompute the last valid state, never store
+  const int64_t pbase = state_base(sg, tile, m.nvar), obase = pbase;
+  phases01<S, false>(m, t, mode, [&](int e) { return phi[pbase + (int64_t)e * tile]; }, param[sg], cnt, tick_);
   const double V = t.sc[SC_V * S + s];
   // a7: omega_k = sum_i nu_ki q_i (Eq. 4), dn_k/dt = V omega_k (Eq. 3)
   const double* __restrict__ P = t.P;
@@ -627,6 +627,84 @@ source_kernel(const DevMech m, int mode, int64_t n_states, int64_t tile, const d
 }
 
 // ---------------------------------------------------------------------------------------------------
+// First-order forward finite-difference Jacobian -- the paper's own comparison baseline (Fig. 12),
+// DESIGN.md R7:   J(i, c) ~ (f_i(phi + h_c e_c) - f_i(phi)) / h_c,   h_c = fl(phi_c + fma(rel, |phi_c|, abs)) - phi_c.
+// One CTA per state.  The S lanes of the tile are S perturbed copies of that state: lane s of pass p evaluates the
+// source terms at column c = p*S + s - 1; c = -1 (lane 0 of pass 0) is the unperturbed state.  n_var + 1 source
+// evaluations per state, against one analytical evaluation: that ratio is what Fig. 12 shows.
+// ---------------------------------------------------------------------------------------------------
+template <int S>
+__global__ void __launch_bounds__(NT, 1)
+fd_kernel(const DevMech m, int mode, int ofmt, double rel, double ab, int64_t tile, int64_t n_e,
+          const double* __restrict__ phi, const double* __restrict__ param, double* __restrict__ out) {
+  extern __shared__ __align__(16) double smem[];
+  Tile<S, false> t(smem, m.ns, m.nr, m.nslots);
+  double* __restrict__ f0 = t.part + m.n_part_src * S;        // f(phi)           [nvar]
+  double* __restrict__ fc = f0 + m.nvar;                      // f(phi + h_c e_c) [nvar][S]
+  __shared__ int cnt[N_CNT];
+  long long tick_ = 0;
+  const int tid = threadIdx.x, s = tid % S, nvar = m.nvar;
+  const int64_t sg = blockIdx.x;
+  const int64_t pbase = state_base(sg, tile, nvar), obase = state_base(sg, tile, n_e);
+  const double par = param[sg];
+  const int n_pass = (nvar + 1 + S - 1) / S;
+  for (int pass = 0; pass < n_pass; ++pass) {
+    const int c_raw = pass * S + s - 1;
+    const int c = c_raw < nvar ? c_raw : -1;                  // lanes past the last column repeat the base state
+    double x = 0.0, xp = 0.0;
+    if (c >= 0) { x = phi[pbase + (int64_t)c * tile]; xp = x + fma(rel, fabs(x), ab); }
+    phases01<S, false>(m, t, mode, [&](int e) { const double v = phi[pbase + (int64_t)e * tile]; return e == c ? xp : v; },
+                       par, cnt, tick_);
+    const double V = t.sc[SC_V * S + s];
+    const double* __restrict__ P = t.P;
+    gather<S, 1, 1, PYJAC_UQ, 4, int>(m.qplan, cnt + CNT_Q,
+        [&](const int32_t* e, double (&v)[1]) {
+          const uint32_t ent = (uint32_t)__ldg(e);
+          v[0] += apply_sign(P[(ent & ~SIGN_BIT) * S + s], ent);
+        },
+        [&](int slot) { return __ldg(m.q_target + slot); },
+        [&](int, int k, const double (&v)[1]) {
+          if (k >= 0) fc[(2 + k) * S + s] = V * v[0];
+          else if (k <= -2) t.part[(-2 - k) * S + s] = v[0];
+        });
+    if (m.qplan.n_comb) {
+      __syncthreads();
+      combine<S, 1>(m.qplan, t.part, [&](int q, const double (&v)[1]) { fc[(2 + __ldg(m.qc_item + q)) * S + s] = V * v[0]; });
+    }
+    if (tid < S) {
+      const double T = t.sc[SC_T * S + s], Pp = t.sc[SC_P * S + s];
+      const double fT = -red_sum<S>(t.red, 0, s) / t.sc[SC_D * S + s];          // Eq. 5
+      const double Ssum = red_sum<S>(t.red, 1, s);
+      fc[s] = fT;
+      fc[S + s] = mode == PYJAC_CONP ? V * (T * R_GAS / Pp * Ssum + fT / T)      // Eq. 8a
+                                     : T * R_GAS * Ssum + Pp / T * fT;           // Eq. 8b
+    }
+    __syncthreads();
+    if (pass == 0) {
+      for (int i = tid; i < nvar; i += NT) f0[i] = fc[i * S];
+      __syncthreads();
+    }
+    if (c >= 0) {
+      const double h = xp - x;                                // the step actually taken
+      if (ofmt >= OUT_DENSE_C) {
+        for (int i = tid / S; i < nvar; i += NT / S) {
+          const int64_t e = ofmt == OUT_DENSE_C ? (int64_t)i * nvar + c : (int64_t)c * nvar + i;
+          out[obase + e * tile] = (fc[i * S + s] - f0[i]) / h;
+        }
+      } else {                                                // the handle's pattern, walked by columns
+        const int p1 = __ldg(m.csc_ptr + c + 1);
+        for (int p = __ldg(m.csc_ptr + c) + tid / S; p < p1; p += NT / S) {
+          const int i = __ldg(m.csc_idx + p);
+          const int64_t e = ofmt == OUT_CSC ? p : __ldg(m.csc2csr + p);
+          out[obase + e * tile] = (fc[i * S + s] - f0[i]) / h;
+        }
+      }
+    }
+    __syncthreads();                                          // fc, the slots and the work counters are reused
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------
 // Jacobian (sparse CSR / CSC value order or dense 'C' / 'F'), Eq. 9
 // ---------------------------------------------------------------------------------------------------
 template <int S>
@@ -642,12 +720,13 @@ jacobian_kernel(const DevMech m, const DevPlan pl, int mode, int64_t n_states, i
 #else
   long long tick_ = 0;
 #endif
-  phases01<S, true>(m, t, mode, s0, n_states, tile, phi, param, cnt, tick_);
-  TICK(2);
   const int tid = threadIdx.x, s = tid % S;
   const int L = m.ns - 1;
   const bool valid = s0 + s < n_states;
-  const int64_t obase = state_base(min(s0 + s, n_states - 1), tile, pl.n_e);
+  const int64_t sg = min(s0 + s, n_states - 1);   // ragged tail: recompute the last valid state, never store
+  const int64_t pbase = state_base(sg, tile, m.nvar), obase = state_base(sg, tile, pl.n_e);
+  phases01<S, true>(m, t, mode, [&](int e) { return phi[pbase + (int64_t)e * tile]; }, param[sg], cnt, tick_);
+  TICK(2);
   const double T = t.sc[SC_T * S + s], V = t.sc[SC_V * S + s], Pp = t.sc[SC_P * S + s], D = t.sc[SC_D * S + s];
   const double N = red_sum<S>(t.red, 0, s);
   const double fT = -N / D;
@@ -782,6 +861,12 @@ template <int S> int launch_jac_S(const DevMech& m, const DevPlan& p, const Laun
   return (int)cudaGetLastError();
 }
 
+template <int S> int launch_fd_S(const DevMech& m, const LaunchCfg& cfg, int mode, int ofmt, double rel, double ab, int64_t n,
+                                 int64_t tile, int64_t n_e, const double* phi, const double* param, double* out, cudaStream_t st) {
+  fd_kernel<S><<<(unsigned)n, NT, cfg.smem, st>>>(m, mode, ofmt, rel, ab, tile, n_e, phi, param, out);
+  return (int)cudaGetLastError();
+}
+
 constexpr size_t SMEM_LIMIT = 227 * 1024 - 64;   // dynamic part; 64 B left for the static work counters
 
 }  // namespace
@@ -797,6 +882,31 @@ LaunchCfg choose_cfg(const HostTables& h, bool jac, int64_t tile, int64_t n_stat
     break;
   }
   return cfg;
+}
+
+// finite differences: S = columns per pass; the largest that fits, but no wider than the n_var + 1 evaluations
+LaunchCfg choose_cfg_fd(const HostTables& h) {
+  LaunchCfg cfg{1, NT, 0};
+  for (int S = 32; S >= 1; S >>= 1) {
+    const size_t bytes = (smem_doubles(h.ns, h.nr, h.nslots, h.n_part_src, S, false) + (size_t)h.nvar * (S + 1)) * sizeof(double);
+    cfg.S = S; cfg.smem = bytes;
+    if (bytes > SMEM_LIMIT) continue;
+    if (S > 1 && S / 2 >= h.nvar + 1) continue;
+    break;
+  }
+  return cfg;
+}
+
+int launch_fd(const DevMech& m, const LaunchCfg& cfg, int mode, int ofmt, int64_t n_e, double rel_step, double abs_step,
+              int64_t n_states, int64_t ld, int64_t tile, const double* phi, const double* param, double* out, void* stream) {
+  (void)ld;
+  cudaStream_t st = (cudaStream_t)stream;
+#define FD_CASE(S_) case S_: return launch_fd_S<S_>(m, cfg, mode, ofmt, rel_step, abs_step, n_states, tile, n_e, phi, param, out, st);
+  switch (cfg.S) {
+    FD_CASE(1) FD_CASE(2) FD_CASE(4) FD_CASE(8) FD_CASE(16)
+    default: return launch_fd_S<32>(m, cfg, mode, ofmt, rel_step, abs_step, n_states, tile, n_e, phi, param, out, st);
+  }
+#undef FD_CASE
 }
 
 int launch_source(const DevMech& m, const LaunchCfg& cfg, int mode, int64_t n_states, int64_t ld, int64_t tile,
@@ -829,6 +939,8 @@ int launch_jacobian(const DevMech& m, const DevPlan& p, const LaunchCfg& cfg, in
 
 template <int S> static int set_attr_S() {
   cudaError_t e = cudaFuncSetAttribute(source_kernel<S>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_LIMIT);
+  if (e != cudaSuccess) return (int)e;
+  e = cudaFuncSetAttribute(fd_kernel<S>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_LIMIT);
   if (e != cudaSuccess) return (int)e;
   return (int)cudaFuncSetAttribute(jacobian_kernel<S>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_LIMIT);
 }

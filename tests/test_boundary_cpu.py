@@ -18,7 +18,7 @@ def test_library_exports_every_declared_symbol():
     hdr = open(os.path.join(ROOT, "include", "pyjac.h")).read()
     names = set(re.findall(r"\b(pyjac_[a-z_]+)\s*\(", hdr))
     assert {"pyjac_mech_create", "pyjac_mech_destroy", "pyjac_mech_dims", "pyjac_sparsity", "pyjac_source_terms",
-            "pyjac_jacobian_sparse", "pyjac_jacobian_dense", "pyjac_eval_host", "pyjac_launch_info",
+            "pyjac_jacobian_sparse", "pyjac_jacobian_dense", "pyjac_jacobian_fd", "pyjac_eval_host", "pyjac_launch_info",
             "pyjac_last_error"} <= names
     lib = ctypes.CDLL(pj.LIB_PATH)
     for n in names:
