@@ -163,6 +163,7 @@ def main():
     ap.add_argument("--tile", type=int, default=None, help="override layout tile (default: states per CTA)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--no-fd", action="store_true", help="skip the finite-difference comparison")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
@@ -258,6 +259,28 @@ def main():
     b.record(stream); torch.cuda.synchronize()
     src_ms = a.elapsed_time(b) / 5
 
+    # the paper's comparison (Fig. 12): first-order finite-difference Jacobian in the same output
+    # format, same layout, on a bounded sample of the same states (it costs n_var + 1 source evaluations per state)
+    fd = None
+    if not args.no_fd:
+        n_fd = min(N, (2048 + tile - 1) // tile * tile)      # one CTA per state: ~14 waves over the 148 SMs
+        ffmt = pj.PYJAC_CSR if what == "sparse" else "C"
+
+        def fd_step():
+            pj.pyjac_jacobian_fd(M.h, mode, ffmt, 2.0 ** -26, 1e-14, n_fd, ld, tile, d_phi.data_ptr(), d_par.data_ptr(),
+                                 d_out.data_ptr(), stream.cuda_stream)
+
+        fd_step(); torch.cuda.synchronize()
+        a = torch.cuda.Event(enable_timing=True); b = torch.cuda.Event(enable_timing=True)
+        a.record(stream)
+        for _ in range(3):
+            fd_step()
+        b.record(stream); torch.cuda.synchronize()
+        fd_ms = a.elapsed_time(b) / 3
+        fd = {"states": n_fd, "ns_per_state": 1e6 * fd_ms / n_fd, "states_per_s": n_fd / (fd_ms * 1e-3),
+              "columns_per_pass": pj.pyjac_launch_info(M.h, 3)[0], "rel_step": 2.0 ** -26, "abs_step": 1e-14,
+              "analytical_speedup": (fd_ms / n_fd) / (kavg_ms / N)}
+
     # e2e: the C-ABI call on HOST buffers, H2D + kernel + D2H inside the timed region (pinned memory)
     e2e = None
     if not args.no_e2e:
@@ -300,7 +323,7 @@ def main():
                              "ns_per_state": 1e6 * kavg_ms / N},
                 "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": args.steps, "clocks": clk.summary(),
                 "extra": {"source_terms_states_per_s": N / (src_ms * 1e-3), "source_terms_ms": src_ms, "source_terms_tile": tile_s,
-                          "nnz": M.nnz, "smem_bytes_per_cta": smem, "threads_per_cta": threads}}
+                          "nnz": M.nnz, "smem_bytes_per_cta": smem, "threads_per_cta": threads, "fd_jacobian": fd}}
         print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
