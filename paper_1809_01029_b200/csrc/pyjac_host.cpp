@@ -4,6 +4,8 @@
 // kernels are mechanism-agnostic and read tables, and the run-time search is replaced by static
 // maps, as the paper itself proposes.
 #include <algorithm>
+#include <array>
+#include <functional>
 #include <cmath>
 #include <cstdlib>
 #include <cstring>
@@ -105,16 +107,66 @@ void build_gather(const std::vector<std::vector<int32_t>>& lists, int stride, in
   std::stable_sort(segs.begin(), segs.end(), [](const Seg& a, const Seg& b) { return a.len > b.len; });
   const int ns_ = (int)segs.size();
   g.n_sg = (ns_ + ELL_W - 1) / ELL_W;
+  // Shared-memory banks.  At step p the 16 lanes of a half-warp read the p-th entries of 16 consecutive segments,
+  // one 8-byte slot each (S = 1; with S states per item the half-warp covers 16/S segments and needs distinct slots
+  // mod 16/S, which distinct mod 16 implies).  The order of the entries inside a segment is free, so every block of
+  // 16 segments is scheduled step by step with a maximum bipartite matching lanes <-> banks (slot mod 16); padding
+  // entries take whichever of the N_ZERO_SLOTS always-zero slots falls in a free bank.
+  std::vector<std::vector<int>> order(ns_);           // per sorted segment: entry indices in issue order
+  for (int b0 = 0; b0 < ns_; b0 += 16) {
+    const int nb = std::min(16, ns_ - b0);
+    std::vector<std::vector<int>> rem(nb);
+    for (int l = 0; l < nb; ++l) for (int e = 0; e < segs[b0 + l].len; ++e) rem[l].push_back(segs[b0 + l].p0 + e);
+    auto bank_of = [&](int l, int e) { return (int)((uint32_t)lists[segs[b0 + l].item][(size_t)e * stride] & ~SIGN_BIT) & 15; };
+    for (;;) {
+      bool any = false;
+      for (int l = 0; l < nb; ++l) any |= !rem[l].empty();
+      if (!any) break;
+      int owner[16]; std::fill(owner, owner + 16, -1);            // bank -> lane
+      std::function<bool(int, uint32_t&)> augment = [&](int l, uint32_t& seen) -> bool {
+        for (int e : rem[l]) {
+          const int bk = bank_of(l, e);
+          if (seen >> bk & 1) continue;
+          seen |= 1u << bk;
+          if (owner[bk] < 0 || augment(owner[bk], seen)) { owner[bk] = l; return true; }
+        }
+        return false;
+      };
+      // longest remaining lists first: they have the fewest later chances to dodge a conflict
+      std::vector<int> lanes;
+      for (int l = 0; l < nb; ++l) if (!rem[l].empty()) lanes.push_back(l);
+      std::stable_sort(lanes.begin(), lanes.end(), [&](int a, int b) { return rem[a].size() > rem[b].size(); });
+      for (int l : lanes) { uint32_t seen = 0; augment(l, seen); }
+      int pick[16]; std::fill(pick, pick + 16, -1);
+      for (int bk = 0; bk < 16; ++bk) if (owner[bk] >= 0) pick[owner[bk]] = bk;
+      for (int l : lanes) {
+        size_t at = 0;
+        if (pick[l] >= 0) for (size_t q = 0; q < rem[l].size(); ++q) if (bank_of(l, rem[l][q]) == pick[l]) { at = q; break; }
+        order[b0 + l].push_back(rem[l][at]);
+        rem[l].erase(rem[l].begin() + at);
+      }
+    }
+  }
   int off = 0;
   for (int sg = 0; sg < g.n_sg; ++sg) {
     const int i0 = sg * ELL_W;
     const int width = segs[i0].len;                   // sorted: the first segment of the group is the longest
     g.sg_meta.push_back(off); g.sg_meta.push_back(width);
     for (int p = 0; p < width; ++p)
-      for (int w = 0; w < ELL_W; ++w) {
-        const bool real = i0 + w < ns_ && p < segs[i0 + w].len;
-        for (int c = 0; c < stride; ++c)
-          g.ell_ent.push_back(real ? lists[segs[i0 + w].item][(segs[i0 + w].p0 + p) * stride + c] : (c == 0 ? zero_slot : 0));
+      for (int w0 = 0; w0 < ELL_W; w0 += 16) {
+        uint32_t used = 0;                            // banks taken by the real entries of this half-warp step
+        for (int w = w0; w < w0 + 16; ++w)
+          if (i0 + w < ns_ && p < segs[i0 + w].len)
+            used |= 1u << (((uint32_t)lists[segs[i0 + w].item][(size_t)order[i0 + w][p] * stride] & ~SIGN_BIT) & 15);
+        for (int w = w0; w < w0 + 16; ++w) {
+          const bool real = i0 + w < ns_ && p < segs[i0 + w].len;
+          int zs = zero_slot;
+          if (!real) {                                // a zero slot in a free bank, if one is left
+            for (int z = 0; z < N_ZERO_SLOTS; ++z) if (!(used >> ((zero_slot + z) & 15) & 1)) { zs = zero_slot + z; used |= 1u << (zs & 15); break; }
+          }
+          for (int c = 0; c < stride; ++c)
+            g.ell_ent.push_back(real ? lists[segs[i0 + w].item][(size_t)order[i0 + w][p] * stride + c] : (c == 0 ? zs : 0));
+        }
       }
     off += width * ELL_W;
     for (int w = 0; w < ELL_W; ++w) g.target.push_back(i0 + w < ns_ ? segs[i0 + w].target : -1);
@@ -155,6 +207,64 @@ int build_host_tables(const pyjac_mech_desc* d, bool approx, HostTables& h, std:
     };
     return cost(a) > cost(b);
   });
+  // ---- shared-memory banks of phase 1.  Lane r % 32 of a warp reads the thermo records (16-byte loads: a
+  // quarter-warp = 8 consecutive reactions is conflict-free iff their species at stoichiometric position a differ
+  // mod 8) and the concentrations (8-byte loads: half-warp, species distinct mod 16) of its reaction's species.
+  // Inside a cost class the order of the reactions is free, and so is the order of the species on a side: both are
+  // chosen greedily to keep the species of neighbouring lanes in different banks.
+  std::vector<std::array<int, 6>> sp_order(nr);       // [sorted r][position a] -> index into the reactant (a < 3) / product list, -1 unused
+  {
+    auto cost_class = [&](int i) {
+      static const int rank[7] = {0, 1, 2, 5, 4, 3, 6};
+      bool simple = true;
+      for (int j = d->reac_ptr[i]; j < d->reac_ptr[i + 1]; ++j) simple &= d->reac_nu[j] == 1;
+      for (int j = d->prod_ptr[i]; j < d->prod_ptr[i + 1]; ++j) simple &= d->prod_nu[j] == 1;
+      return rank[d->type[i]] * 4 + (d->reversible[i] ? 2 : 0) + (simple ? 0 : 1);
+    };
+    std::vector<std::array<int, 6>> placed(nr);       // species at each position of the reactions placed so far (ns = dummy)
+    auto species_at = [&](int i, const std::array<int, 6>& o, int a) {
+      if (o[a] < 0) return ns;
+      return a < 3 ? d->reac_species[d->reac_ptr[i] + o[a]] : d->prod_species[d->prod_ptr[i] + o[a]];
+    };
+    auto conflicts = [&](int r, const std::array<int, 6>& spc) {      // against the lanes already placed
+      int c = 0;
+      for (int q = r - r % 16; q < r; ++q)
+        for (int a = 0; a < 6; ++a) {
+          if (placed[q][a] == spc[a]) continue;                      // same address: broadcast
+          if (q >= r - r % 8 && (placed[q][a] & 7) == (spc[a] & 7)) c += 4;   // two 16-byte loads per species
+          if ((placed[q][a] & 15) == (spc[a] & 15)) c += 1;
+        }
+      return c;
+    };
+    int r0 = 0;
+    while (r0 < nr) {
+      int r1 = r0;
+      while (r1 < nr && cost_class(h.perm[r1]) == cost_class(h.perm[r0])) ++r1;
+      std::vector<int> pool(h.perm.begin() + r0, h.perm.begin() + r1);
+      for (int r = r0; r < r1; ++r) {
+        int best = -1, best_c = 1 << 30; std::array<int, 6> best_o{}, best_s{};
+        for (size_t c = 0; c < pool.size(); ++c) {
+          const int i = pool[c];
+          const int nre = d->reac_ptr[i + 1] - d->reac_ptr[i], npr = d->prod_ptr[i + 1] - d->prod_ptr[i];
+          for (int sw = 0; sw < 4; ++sw) {                           // swap the first two reactants / products
+            if ((sw & 1) && nre < 2) continue;
+            if ((sw & 2) && npr < 2) continue;
+            std::array<int, 6> o = {nre > 0 ? 0 : -1, nre > 1 ? 1 : -1, nre > 2 ? 2 : -1, npr > 0 ? 0 : -1, npr > 1 ? 1 : -1, npr > 2 ? 2 : -1};
+            if (sw & 1) std::swap(o[0], o[1]);
+            if (sw & 2) std::swap(o[3], o[4]);
+            std::array<int, 6> spc;
+            for (int a = 0; a < 6; ++a) spc[a] = species_at(i, o, a);
+            const int cc = conflicts(r, spc);
+            if (cc < best_c) { best_c = cc; best = (int)c; best_o = o; best_s = spc; }
+          }
+          if (best_c == 0) break;
+        }
+        h.perm[r] = pool[best]; sp_order[r] = best_o; placed[r] = best_s;
+        pool.erase(pool.begin() + best);
+      }
+      r0 = r1;
+    }
+  }
 
   h.lnA.resize(nr); h.beta.resize(nr); h.Ta.resize(nr); h.dn.resize(nr);
   h.info.resize(nr); h.aux.assign(nr, -1); h.sp.assign((size_t)nr * 8, (uint32_t)ns);
@@ -175,13 +285,13 @@ int build_host_tables(const pyjac_mech_desc* d, bool approx, HostTables& h, std:
     bool simple = true;
     std::map<int, int> netnu;
     for (int a = 0; a < nre; ++a) {
-      const int j = d->reac_ptr[i] + a;
+      const int j = d->reac_ptr[i] + sp_order[r][a];
       h.sp[8 * r + a] = (uint32_t)d->reac_species[j] | ((uint32_t)d->reac_nu[j] << 16);
       snu -= d->reac_nu[j]; netnu[d->reac_species[j]] -= d->reac_nu[j];
       order_f += d->reac_nu[j]; simple &= d->reac_nu[j] == 1;
     }
     for (int b = 0; b < npr; ++b) {
-      const int j = d->prod_ptr[i] + b;
+      const int j = d->prod_ptr[i] + sp_order[r][3 + b];
       h.sp[8 * r + 3 + b] = (uint32_t)d->prod_species[j] | ((uint32_t)d->prod_nu[j] << 16);
       snu += d->prod_nu[j]; netnu[d->prod_species[j]] += d->prod_nu[j];
       order_r += d->prod_nu[j]; simple &= d->prod_nu[j] == 1;
@@ -198,8 +308,8 @@ int build_host_tables(const pyjac_mech_desc* d, bool approx, HostTables& h, std:
     h.info[r] = info;
     // slots: 0 = T column, 1 = E column, then one per role
     int slot = h.slot_base[r] + 2;
-    for (int a = 0; a < nre; ++a) roles[r].push_back({d->reac_species[d->reac_ptr[i] + a], slot++});
-    if (rev) for (int b = 0; b < npr; ++b) roles[r].push_back({d->prod_species[d->prod_ptr[i] + b], slot++});
+    for (int a = 0; a < nre; ++a) roles[r].push_back({d->reac_species[d->reac_ptr[i] + sp_order[r][a]], slot++});
+    if (rev) for (int b = 0; b < npr; ++b) roles[r].push_back({d->prod_species[d->prod_ptr[i] + sp_order[r][3 + b]], slot++});
     if (tb) {
       if (d->collider[i] >= 0) {           // [M] = C_collider: default 0, one efficiency of 1
         h.eff_sp.push_back(d->collider[i]); h.eff_d.push_back(1.0);

@@ -60,8 +60,8 @@ enum { SC_T = 0, SC_V, SC_P, SC_CTOT, SC_SUMC, SC_SUMCC, SC_SUMCDC, SC_D, SC_DDD
        SC_R0, SC_R1, SC_R2, SC_R3, SC_R4, SC_R5, SC_R6, SC_R7, SC_INVT, SC_LNT, SC_LNP, SC_LNPRT, NSC };
 
 __host__ __device__ inline size_t smem_doubles(int ns, int nr, int nslots, int n_part, int S, bool jac) {
-  // C[ns+1] (C[ns] = 1: dummy species of unused stoichiometric entries), th4[4(ns+1)], ck[ns], slots (+1 zero slot)
-  size_t per_state = NSC + 6 * (size_t)ns + 5 + (jac ? (size_t)nslots + nr : (size_t)nr) + 1;
+  // C[ns+1] (C[ns] = 1: dummy species of unused stoichiometric entries), gh, ec [2(ns+1)] each, ck[ns], slots (+ zero slots)
+  size_t per_state = NSC + 6 * (size_t)ns + 5 + (jac ? (size_t)nslots + nr : (size_t)nr) + N_ZERO_SLOTS;
   return (per_state + n_part) * S + (size_t)NW * NRED * S;      // n_part: partial sums of split gather lists
 }
 
@@ -173,11 +173,13 @@ __device__ __forceinline__ Blend blend(int type, bool hasT2, const double* __res
 // ---------------------------------------------------------------------------------------------------
 template <int S, bool JAC>
 struct Tile {
-  // th4[(k*S + s)*4 + c]: c = 0 g_k/RT, 1 h_k/RT, 2 E~_k, 3 c~_k  (one 32-byte record per species and state)
-  double *sc, *C, *th4, *ck, *dE, *P, *red, *part;
+  // gh[k*S + s] = (g_k/RT, h_k/RT), ec[k*S + s] = (E~_k, c~_k): two arrays of 16-byte records, so that the 8 lanes of a
+  // quarter-warp reading 8 different species can hit 8 different bank groups (one 32-byte record would allow only 4)
+  double *sc, *C, *ck, *dE, *P, *red, *part;
+  double2 *gh, *ec;
   __device__ __forceinline__ Tile(double* smem, int ns, int nr, int nslots) {
-    sc = smem; th4 = sc + NSC * S; C = th4 + 4 * (ns + 1) * S; ck = C + (ns + 1) * S; dE = ck + ns * S; P = JAC ? dE + nr * S : dE; red = P + ((JAC ? nslots : nr) + 1) * S; part = red + NW * NRED * S;
-    // source kernel: dE unused, P[r] = q_r.  P[nslots] (JAC) / P[nr] is an always-zero slot (ELL padding)
+    sc = smem; gh = reinterpret_cast<double2*>(sc + NSC * S); ec = gh + (ns + 1) * S; C = reinterpret_cast<double*>(ec + (ns + 1) * S); ck = C + (ns + 1) * S; dE = ck + ns * S; P = JAC ? dE + nr * S : dE; red = P + ((JAC ? nslots : nr) + N_ZERO_SLOTS) * S; part = red + NW * NRED * S;
+    // source kernel: dE unused, P[r] = q_r.  P[nslots ..] (JAC) / P[nr ..]: N_ZERO_SLOTS always-zero slots (ELL padding)
   }
 };
 
@@ -197,6 +199,7 @@ __device__ __forceinline__ void phases01(const DevMech& m, Tile<S, JAC>& t, int 
   // Every thread reads T, E and the parameter itself (same address for the lanes of a state: one broadcast
   // request) so that no barrier separates the state load from the species loop.
   if (tid < N_CNT) cnt[tid] = 0;
+  if (tid < N_ZERO_SLOTS * S) t.P[(JAC ? m.nslots : nr) * S + tid] = 0.0;   // always-zero slots (ELL padding)
   const double T = phi_of(0), E_ = phi_of(1);
   const double V = mode == PYJAC_CONP ? E_ : par_, Pp = mode == PYJAC_CONP ? par_ : E_;
   const double invT = 1.0 / T, lnT = log(T), RT = R_GAS * T, Ctot = Pp / RT;
@@ -204,10 +207,8 @@ __device__ __forceinline__ void phases01(const DevMech& m, Tile<S, JAC>& t, int 
     t.sc[SC_T * S + s] = T; t.sc[SC_V * S + s] = V; t.sc[SC_P * S + s] = Pp; t.sc[SC_CTOT * S + s] = Ctot;
     t.sc[SC_LNP * S + s] = log(Pp);
     t.sc[SC_LNPRT * S + s] = log(P_ATM / RT);
-    t.P[(JAC ? m.nslots : nr) * S + s] = 0.0;            // always-zero slot (ELL padding)
     t.C[ns * S + s] = 1.0;                               // dummy species: unused stoichiometric entries
-#pragma unroll
-    for (int c = 0; c < 4; ++c) t.th4[(ns * S + s) * 4 + c] = 0.0;
+    t.gh[ns * S + s] = make_double2(0.0, 0.0); t.ec[ns * S + s] = make_double2(0.0, 0.0);
   }
   {
     const double T2 = T * T, T3 = T2 * T, T4 = T3 * T;
@@ -238,10 +239,9 @@ __device__ __forceinline__ void phases01(const DevMech& m, Tile<S, JAC>& t, int 
       const double sR = a0 * lnT + a1 * T + a2 * T2 * 0.5 + a3 * T3 * (1.0 / 3.0) + a4 * T4 * 0.25 + a6;
       const double c = R_GAS * (mode == PYJAC_CONP ? cpR : cpR - 1.0);   // c_p or c_v = c_p - R
       const double e = hRT - (mode == PYJAC_CONP ? 0.0 : 1.0);           // h/RT or u/RT
-      t.th4[idx * 4] = hRT - sR;
-      t.th4[idx * 4 + 1] = hRT;
-      t.th4[idx * 4 + 2] = k == L ? 0.0 : RT * (e - w * eL);            // E~_k = E_k - (W_k/W_Ns) E_Ns
-      t.th4[idx * 4 + 3] = k == L ? 0.0 : c - w * cL;                   // c~_k
+      t.gh[idx] = make_double2(hRT - sR, hRT);
+      // E~_k = E_k - (W_k/W_Ns) E_Ns, c~_k likewise
+      t.ec[idx] = k == L ? make_double2(0.0, 0.0) : make_double2(RT * (e - w * eL), c - w * cL);
       t.ck[idx] = c;
       if (k < L) {
         const double Ck = phi_of(2 + k) * invV;
@@ -383,8 +383,7 @@ __device__ __forceinline__ void phases01(const DevMech& m, Tile<S, JAC>& t, int 
       for (int a = 0; a < 6; ++a) {
         const int k = spw[a] & 0xffff;
         pw[a] = t.C[k * S + s]; pm[a] = 1.0;
-        const double2 gh = *reinterpret_cast<const double2*>(t.th4 + (k * S + s) * 4);
-        const double2 ec = *reinterpret_cast<const double2*>(t.th4 + (k * S + s) * 4 + 2);
+        const double2 gh = t.gh[k * S + s], ec = t.ec[k * S + s];
         if (a < 3) { dg -= gh.x; dh -= gh.y; dEt -= ec.x; dct -= ec.y; }
         else { dg += gh.x; dh += gh.y; dEt += ec.x; dct += ec.y; }
       }
@@ -394,8 +393,7 @@ __device__ __forceinline__ void phases01(const DevMech& m, Tile<S, JAC>& t, int 
         const int k = spw[a] & 0xffff, nu = spw[a] >> 16;
         const double Ck = t.C[k * S + s];
         pw[a] = ipow(Ck, nu); pm[a] = dpow(Ck, nu);
-        const double2 gh = *reinterpret_cast<const double2*>(t.th4 + (k * S + s) * 4);
-        const double2 ec = *reinterpret_cast<const double2*>(t.th4 + (k * S + s) * 4 + 2);
+        const double2 gh = t.gh[k * S + s], ec = t.ec[k * S + s];
         const double snu = a < 3 ? -(double)nu : (double)nu;
         dg += snu * gh.x; dh += snu * gh.y; dEt += snu * ec.x; dct += snu * ec.y;
       }
