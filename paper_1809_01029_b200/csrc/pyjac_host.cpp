@@ -182,11 +182,11 @@ int build_host_tables(const pyjac_mech_desc* d, bool approx, HostTables& h, std:
   h.ns = ns; h.nr = nr; h.nvar = nvar;
 
   // ---- species tables ---------------------------------------------------------------------------
-  h.nasa.assign((size_t)ns * 16, 0.0);
+  h.nasa.assign((size_t)ns * 15, 0.0);                 // coefficient-major: [0] tmid, [1..7] low range, [8..14] high range
   h.wr.resize(ns);
   for (int k = 0; k < ns; ++k) {
-    h.nasa[16 * k] = d->nasa_tmid[k];
-    for (int j = 0; j < 7; ++j) { h.nasa[16 * k + 1 + j] = d->nasa_lo[7 * k + j]; h.nasa[16 * k + 8 + j] = d->nasa_hi[7 * k + j]; }
+    h.nasa[k] = d->nasa_tmid[k];
+    for (int j = 0; j < 7; ++j) { h.nasa[(size_t)(1 + j) * ns + k] = d->nasa_lo[7 * k + j]; h.nasa[(size_t)(8 + j) * ns + k] = d->nasa_hi[7 * k + j]; }
     h.wr[k] = d->mol_weight[k] / d->mol_weight[L];
   }
 

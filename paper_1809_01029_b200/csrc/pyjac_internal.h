@@ -49,7 +49,7 @@ struct HostTables {
   int ns = 0, nr = 0, nvar = 0;
   std::vector<int32_t> perm;                 // sorted index -> original reaction index
   // species
-  std::vector<double> nasa;                  // [ns*16]: tmid, lo[7], hi[7], pad
+  std::vector<double> nasa;                  // [15*ns] coefficient-major: tmid, lo[7], hi[7]
   std::vector<double> wr;                    // [ns] W_k / W_Ns
   // reactions
   std::vector<double> lnA, beta, Ta, dn;     // [nr]; dn = sum_k<Ns nu_ki (1 - W_k/W_Ns)

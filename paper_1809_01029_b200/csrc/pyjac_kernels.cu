@@ -216,9 +216,8 @@ __device__ __forceinline__ void phases01(const DevMech& m, Tile<S, JAC>& t, int 
     // last species in through mass conservation (R1/A1) and need it; saves a second pass and two barriers
     double cL, dcL, eL;
     {
-      const double* __restrict__ a = m.nasa + 16 * L;
-      a += (T <= __ldg(a)) ? 1 : 8;
-      const double a0 = __ldg(a), a1 = __ldg(a + 1), a2 = __ldg(a + 2), a3 = __ldg(a + 3), a4 = __ldg(a + 4), a5 = __ldg(a + 5);
+      const double* __restrict__ a = m.nasa + L + ((T <= __ldg(m.nasa + L)) ? 1 : 8) * ns;   // table is coefficient-major
+      const double a0 = __ldg(a), a1 = __ldg(a + ns), a2 = __ldg(a + 2 * ns), a3 = __ldg(a + 3 * ns), a4 = __ldg(a + 4 * ns), a5 = __ldg(a + 5 * ns);
       const double cpR = a0 + a1 * T + a2 * T2 + a3 * T3 + a4 * T4;
       const double hRT = a0 + a1 * T * 0.5 + a2 * T2 * (1.0 / 3.0) + a3 * T3 * 0.25 + a4 * T4 * 0.2 + a5 * invT;
       cL = R_GAS * (mode == PYJAC_CONP ? cpR : cpR - 1.0);
@@ -229,9 +228,16 @@ __device__ __forceinline__ void phases01(const DevMech& m, Tile<S, JAC>& t, int 
     const double invV = 1.0 / V;
     for (int idx = tid; idx < ns * S; idx += NT) {
       const int k = idx / S;
-      const double* __restrict__ a = m.nasa + 16 * k;
-      a += (T <= __ldg(a)) ? 1 : 8;                      // low range iff T <= T_mid (R3); per-lane select
-      const double a0 = __ldg(a), a1 = __ldg(a + 1), a2 = __ldg(a + 2), a3 = __ldg(a + 3), a4 = __ldg(a + 4), a5 = __ldg(a + 5), a6 = __ldg(a + 6);
+      // coefficient-major table (entry c of species k at nasa[c * ns + k]): consecutive lanes read consecutive
+      // addresses, and BOTH ranges are requested before T is known, so the loads do not wait for the state load
+      const double* __restrict__ a = m.nasa + k;
+      double lo[7], hi[7];
+      const double tmid = __ldg(a);
+#pragma unroll
+      for (int c = 0; c < 7; ++c) { lo[c] = __ldg(a + (1 + c) * ns); hi[c] = __ldg(a + (8 + c) * ns); }
+      const bool low = T <= tmid;                        // low range iff T <= T_mid (R3); per-lane select
+      const double a0 = low ? lo[0] : hi[0], a1 = low ? lo[1] : hi[1], a2 = low ? lo[2] : hi[2], a3 = low ? lo[3] : hi[3],
+                   a4 = low ? lo[4] : hi[4], a5 = low ? lo[5] : hi[5], a6 = low ? lo[6] : hi[6];
       const double w = __ldg(m.wr + k);
       const double cpR = a0 + a1 * T + a2 * T2 + a3 * T3 + a4 * T4;
       const double dcpR = a1 + 2.0 * a2 * T + 3.0 * a3 * T2 + 4.0 * a4 * T3;
@@ -378,9 +384,12 @@ __device__ __forceinline__ void phases01(const DevMech& m, Tile<S, JAC>& t, int 
     double dg = 0.0, dh = 0.0, dEt = 0.0, dct = 0.0;
     // Reactions are sorted so that a warp is (almost always) uniform in "all coefficients are 1": take the vote
     // and branch once, so that the power / multiplicity arithmetic is not executed (if-converted) for the common case.
+    // Likewise "no side has a third species" (nearly every reaction): the third positions are skipped warp-wide.
+    const bool two = __all_sync(__activemask(), ((info >> INFO_NREAC_SHIFT) & 3) < 3 && ((info >> INFO_NPROD_SHIFT) & 3) < 3);
     if (__all_sync(__activemask(), (info & INFO_SIMPLE) != 0)) {
 #pragma unroll
       for (int a = 0; a < 6; ++a) {
+        if ((a == 2 || a == 5) && two) { pw[a] = 1.0; pm[a] = 1.0; continue; }
         const int k = spw[a] & 0xffff;
         pw[a] = t.C[k * S + s]; pm[a] = 1.0;
         const double2 gh = t.gh[k * S + s], ec = t.ec[k * S + s];
@@ -390,6 +399,7 @@ __device__ __forceinline__ void phases01(const DevMech& m, Tile<S, JAC>& t, int 
     } else {
 #pragma unroll
       for (int a = 0; a < 6; ++a) {
+        if ((a == 2 || a == 5) && two) { pw[a] = 1.0; pm[a] = 0.0; continue; }
         const int k = spw[a] & 0xffff, nu = spw[a] >> 16;
         const double Ck = t.C[k * S + s];
         pw[a] = ipow(Ck, nu); pm[a] = dpow(Ck, nu);
