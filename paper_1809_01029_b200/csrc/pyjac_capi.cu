@@ -32,7 +32,7 @@ struct pyjac_mech {
     for (void* p : allocs) cudaFree(p);
   }
   int upload_plan(const GatherPlan& g, int part_base, DevGather* out) {
-    out->n_sg = g.n_sg; out->n_comb = (int)g.comb_item.size(); out->part_base = part_base;
+    out->n_sg = g.n_sg; out->n_wide = g.n_wide; out->n_comb = (int)g.comb_item.size(); out->part_base = part_base;
     if (int r = upload(g.sg_meta, &out->sg_meta)) return r;
     if (int r = upload(g.comb_first, &out->comb_first)) return r;
     if (int r = upload(g.comb_nseg, &out->comb_nseg)) return r;

@@ -86,7 +86,7 @@ int seg_len() {
   return v > 0 ? v : SEG_LEN_DEFAULT;
 }
 
-void build_gather(const std::vector<std::vector<int32_t>>& lists, int stride, int zero_slot, GatherPlan& g) {
+void build_gather(const std::vector<std::vector<int32_t>>& lists, int stride, int zero_slot, int narrow_len, GatherPlan& g) {
   const int SEG = seg_len();
   const int n = (int)lists.size();
   g = GatherPlan();
@@ -106,7 +106,16 @@ void build_gather(const std::vector<std::vector<int32_t>>& lists, int stride, in
   }
   std::stable_sort(segs.begin(), segs.end(), [](const Seg& a, const Seg& b) { return a.len > b.len; });
   const int ns_ = (int)segs.size();
-  g.n_sg = (ns_ + ELL_W - 1) / ELL_W;
+  // Wide super-groups of ELL_W segments first; the tail of short segments (<= narrow_len entries) goes into NARROW
+  // super-groups of ELL_W_NARROW segments: a thread then owns 4x as many segments of a unit, so the fixed cost of a
+  // unit (work counter, metadata, one exposed round trip for the first entries) is paid a quarter as often.
+  int i_n = ns_;
+  for (int i = 0; i < ns_; ++i) if (segs[i].len <= narrow_len) { i_n = i; break; }
+  g.n_wide = (i_n + ELL_W - 1) / ELL_W;
+  const int rest = std::max(0, ns_ - g.n_wide * ELL_W);
+  g.n_sg = g.n_wide + (rest + ELL_W_NARROW - 1) / ELL_W_NARROW;
+  auto group_first = [&](int sg) { return sg < g.n_wide ? sg * ELL_W : g.n_wide * ELL_W + (sg - g.n_wide) * ELL_W_NARROW; };
+  auto group_size = [&](int sg) { return sg < g.n_wide ? ELL_W : ELL_W_NARROW; };
   // Shared-memory banks.  At step p the 16 lanes of a half-warp read the p-th entries of 16 consecutive segments,
   // one 8-byte slot each (S = 1; with S states per item the half-warp covers 16/S segments and needs distinct slots
   // mod 16/S, which distinct mod 16 implies).  The order of the entries inside a segment is free, so every block of
@@ -149,11 +158,11 @@ void build_gather(const std::vector<std::vector<int32_t>>& lists, int stride, in
   }
   int off = 0;
   for (int sg = 0; sg < g.n_sg; ++sg) {
-    const int i0 = sg * ELL_W;
+    const int i0 = group_first(sg), EW = group_size(sg);
     const int width = segs[i0].len;                   // sorted: the first segment of the group is the longest
     g.sg_meta.push_back(off); g.sg_meta.push_back(width);
     for (int p = 0; p < width; ++p)
-      for (int w0 = 0; w0 < ELL_W; w0 += 16) {
+      for (int w0 = 0; w0 < EW; w0 += 16) {
         uint32_t used = 0;                            // banks taken by the real entries of this half-warp step
         for (int w = w0; w < w0 + 16; ++w)
           if (i0 + w < ns_ && p < segs[i0 + w].len)
@@ -168,8 +177,8 @@ void build_gather(const std::vector<std::vector<int32_t>>& lists, int stride, in
             g.ell_ent.push_back(real ? lists[segs[i0 + w].item][(size_t)order[i0 + w][p] * stride + c] : (c == 0 ? zs : 0));
         }
       }
-    off += width * ELL_W;
-    for (int w = 0; w < ELL_W; ++w) g.target.push_back(i0 + w < ns_ ? segs[i0 + w].target : -1);
+    off += width * EW;
+    for (int w = 0; w < EW; ++w) g.target.push_back(i0 + w < ns_ ? segs[i0 + w].target : -1);
   }
   g.n_padded = off;
 }
@@ -464,7 +473,7 @@ int build_host_tables(const pyjac_mech_desc* d, bool approx, HostTables& h, std:
       for (auto& e : l) e += col;                      // slot base + 0: T column, + 1: E column (sign bit untouched)
       jitems.push_back({2 + k, col}); jlists.push_back(std::move(l));
     }
-  build_gather(jlists, 1, h.nslots, h.jplan);
+  build_gather(jlists, 1, h.nslots, NARROW_LEN, h.jplan);
   std::vector<std::vector<int32_t>> clists(L), qlists(L);
   for (int k = 0; k < L; ++k) {
     qlists[k] = bql[k];
@@ -474,8 +483,8 @@ int build_host_tables(const pyjac_mech_desc* d, bool approx, HostTables& h, std:
       clists[k].insert(clists[k].end(), {cl[k][e], cl[k][e + 1], w[0], w[1]});
     }
   }
-  build_gather(clists, 4, h.nslots, h.cplan);            // T and E rows: (slot | sign, reaction, dn~)
-  build_gather(qlists, 1, nr, h.qplan);                  // source terms: omega_k = sum nu_ki q_i
+  build_gather(clists, 4, h.nslots, 0, h.cplan);            // T and E rows: (slot | sign, reaction, dn~)
+  build_gather(qlists, 1, nr, 0, h.qplan);                  // source terms: omega_k = sum nu_ki q_i
   h.q_target = h.qplan.target;
   h.n_part_jac = h.jplan.n_part + 2 * h.cplan.n_part;
   h.n_part_src = h.qplan.n_part;

@@ -30,10 +30,13 @@ constexpr int SEG_LEN_DEFAULT = 32;   // gather lists longer than this are split
 enum OutFmt { OUT_CSR = 0, OUT_CSC = 1, OUT_DENSE_C = 2, OUT_DENSE_F = 3 };
 
 constexpr int ELL_W = 128;           // items per ELL super-group (4 items per lane at one state per CTA)
+constexpr int ELL_W_NARROW = 512;    // items per NARROW super-group (segments of <= NARROW_LEN entries; species rows only)
+constexpr int NARROW_LEN = 2;
 
 struct GatherPlan {
   int stride = 1;                            // ints per entry
-  int n_sg = 0;                              // ELL super-groups of ELL_W segments
+  int n_sg = 0;                              // ELL super-groups: n_wide of ELL_W segments, then n_sg - n_wide of ELL_W_NARROW
+  int n_wide = 0;
   std::vector<int32_t> sg_meta;              // [n_sg*2]: entry offset, padded segment length
   std::vector<int32_t> ell_ent;              // entry (p, w) of group sg at (off + p*ELL_W + w) * stride
   // processing slot (n_sg*ELL_W) -> what the segment's sum is: item id >= 0 (the whole list of that item: store
@@ -90,7 +93,7 @@ int build_host_tables(const pyjac_mech_desc* d, bool approx, HostTables& h, std:
 
 // ---- device views ------------------------------------------------------------------------------
 struct DevGather {
-  int n_sg, n_comb, part_base;        // part_base: offset of this plan's partial sums in the scratch
+  int n_sg, n_wide, n_comb, part_base;   // part_base: offset of this plan's partial sums in the scratch
   const int32_t *sg_meta, *ell_ent, *comb_first, *comb_nseg;
 };
 

@@ -59,16 +59,17 @@ constexpr int NRED = 8;           // reduction slots
 enum { SC_T = 0, SC_V, SC_P, SC_CTOT, SC_SUMC, SC_SUMCC, SC_SUMCDC, SC_D, SC_DDDT, SC_CNS,
        SC_R0, SC_R1, SC_R2, SC_R3, SC_R4, SC_R5, SC_R6, SC_R7, SC_INVT, SC_LNT, SC_LNP, SC_LNPRT, NSC };
 
-__host__ __device__ inline size_t smem_doubles(int ns, int nr, int nslots, int n_part, int S, bool jac) {
+__host__ __device__ inline size_t smem_doubles(int ns, int nr, int nslots, int n_part, int n_meta, int S, bool jac) {
   // C[ns+1] (C[ns] = 1: dummy species of unused stoichiometric entries), gh, ec [2(ns+1)] each, ck[ns], slots (+ zero slots)
   size_t per_state = NSC + 6 * (size_t)ns + 5 + (jac ? (size_t)nslots + nr : (size_t)nr) + N_ZERO_SLOTS;
-  return (per_state + n_part) * S + (size_t)NW * NRED * S;      // n_part: partial sums of split gather lists
+  // n_part: partial sums of split gather lists; n_meta: (offset, width) of every ELL super-group (8 bytes each)
+  return (per_state + n_part) * S + (size_t)NW * NRED * S + n_meta;
 }
 
 // Dynamic work distribution inside a CTA: items are sorted by descending cost at create time and warps take the
 // next chunk from a shared-memory counter (longest-processing-time-first scheduling); removes the tail in which a
 // few warps work on the heaviest reactions / longest gather lists while the others idle.
-enum { CNT_RX = 0, CNT_J, CNT_C, CNT_Q, N_CNT };
+enum { CNT_RX = 0, CNT_J, CNT_J2, CNT_C, CNT_Q, N_CNT };
 __device__ __forceinline__ int next_chunk(int* counter) {
   int c = 0;
   if ((threadIdx.x & 31) == 0) c = atomicAdd(counter, 1);
@@ -177,8 +178,10 @@ struct Tile {
   // quarter-warp reading 8 different species can hit 8 different bank groups (one 32-byte record would allow only 4)
   double *sc, *C, *ck, *dE, *P, *red, *part;
   double2 *gh, *ec;
-  __device__ __forceinline__ Tile(double* smem, int ns, int nr, int nslots) {
+  int2* meta;     // (entry offset, width) of every ELL super-group of the plans this kernel gathers: read per unit
+  __device__ __forceinline__ Tile(double* smem, int ns, int nr, int nslots, int n_part) {
     sc = smem; gh = reinterpret_cast<double2*>(sc + NSC * S); ec = gh + (ns + 1) * S; C = reinterpret_cast<double*>(ec + (ns + 1) * S); ck = C + (ns + 1) * S; dE = ck + ns * S; P = JAC ? dE + nr * S : dE; red = P + ((JAC ? nslots : nr) + N_ZERO_SLOTS) * S; part = red + NW * NRED * S;
+    meta = reinterpret_cast<int2*>(part + n_part * S);
     // source kernel: dE unused, P[r] = q_r.  P[nslots ..] (JAC) / P[nr ..]: N_ZERO_SLOTS always-zero slots (ELL padding)
   }
 };
@@ -530,30 +533,31 @@ namespace {
 //   acc(const int32_t* entry, double (&v)[NACC])      accumulate one entry
 //   store(int slot, const double (&v)[NACC])          slot = processing slot (index into the position arrays)
 // ---------------------------------------------------------------------------------------------------
-template <int S, int STRIDE, int NACC, int U, int UNROLL, class P, class AccF, class PosF, class StoreF>
-__device__ __forceinline__ void gather(const DevGather& g, int* counter, AccF acc, PosF pos_of, StoreF store) {
+// EW = segments per super-group (ELL_W, or ELL_W_NARROW for the narrow tail of the species-row plan); metas points at
+// the first of n_groups super-groups, whose first segment has processing slot slot_base.
+template <int S, int STRIDE, int NACC, int U, int UNROLL, int EW, class P, class AccF, class PosF, class StoreF>
+__device__ __forceinline__ void gather(const int32_t* __restrict__ ell_ent, const int2* __restrict__ metas, int n_groups,
+                                       int slot_base, int* counter, AccF acc, PosF pos_of, StoreF store) {
   const int lane = threadIdx.x & 31, sub = lane / S;
   constexpr int IPW = 32 / S;                 // segments of one warp per "u"
   // a unit = U * IPW segments of one super-group; a thread owns U segments (U independent loads per step)
-  constexpr int UPG = ELL_W / (U * IPW);      // units per super-group
-  const int n_work = g.n_sg * UPG;
-  const int2* __restrict__ metas = reinterpret_cast<const int2*>(g.sg_meta);      // entry offset, padded length
-  // software pipeline: the next unit's number and metadata are fetched while the current unit is processed, and
-  // the output positions are requested before the entry loop, so a unit costs one exposed L2 round trip, not three
+  static_assert(EW % (U * IPW) == 0, "super-group must be a whole number of units");
+  constexpr int UPG = EW / (U * IPW);         // units per super-group
+  const int n_work = n_groups * UPG;
+  // metas: (entry offset, padded length) per super-group, in SHARED memory.  Software pipeline: the next unit's
+  // number is fetched while the current unit is processed and the output positions are requested before the entry
+  // loop, so a unit costs one exposed L2 round trip (its first entries), not three.
   int unit = next_chunk(counter);
-  int2 meta = make_int2(0, 0);
-  if (unit < n_work) meta = __ldg(metas + unit / UPG);
   while (unit < n_work) {
     const int next = next_chunk(counter);
-    int2 nmeta = make_int2(0, 0);
-    if (next < n_work) nmeta = __ldg(metas + next / UPG);
+    const int2 meta = metas[unit / UPG];
     const int sg = unit / UPG;
     const int il0 = (unit % UPG) * (U * IPW) + sub;
-    const int slot0 = sg * ELL_W + il0;
+    const int slot0 = slot_base + sg * EW + il0;
     P pos[U];
 #pragma unroll
     for (int u = 0; u < U; ++u) pos[u] = pos_of(slot0 + u * IPW);
-    const int32_t* __restrict__ e = g.ell_ent + (meta.x + il0) * STRIDE;
+    const int32_t* __restrict__ e = ell_ent + (meta.x + il0) * STRIDE;
     double v[U][NACC];
 #pragma unroll
     for (int u = 0; u < U; ++u)
@@ -562,12 +566,18 @@ __device__ __forceinline__ void gather(const DevGather& g, int* counter, AccF ac
 #pragma unroll UNROLL
     for (int p = 0; p < meta.y; ++p) {
 #pragma unroll
-      for (int u = 0; u < U; ++u) acc(e + (p * ELL_W + u * IPW) * STRIDE, v[u]);
+      for (int u = 0; u < U; ++u) acc(e + (p * EW + u * IPW) * STRIDE, v[u]);
     }
 #pragma unroll
     for (int u = 0; u < U; ++u) store(slot0 + u * IPW, pos[u], v[u]);
-    unit = next; meta = nmeta;
+    unit = next;
   }
+}
+
+// copies the super-group metadata of a plan to shared memory (visible after the next barrier)
+__device__ __forceinline__ void load_meta(const DevGather& g, int2* dst) {
+  const int2* __restrict__ src = reinterpret_cast<const int2*>(g.sg_meta);
+  for (int i = threadIdx.x; i < g.n_sg; i += NT) dst[i] = __ldg(src + i);
 }
 
 // second pass over the lists that were split into segments: sum the partial sums, then finish(list, sums)
@@ -595,7 +605,8 @@ __global__ void __launch_bounds__(NT, 1)
 source_kernel(const DevMech m, int mode, int64_t n_states, int64_t tile, const double* __restrict__ phi,
               const double* __restrict__ param, double* __restrict__ out) {
   extern __shared__ __align__(16) double smem[];
-  Tile<S, false> t(smem, m.ns, m.nr, m.nslots);
+  Tile<S, false> t(smem, m.ns, m.nr, m.nslots, m.n_part_src);
+  load_meta(m.qplan, t.meta);
   const int64_t s0 = (int64_t)blockIdx.x * S;
   __shared__ int cnt[N_CNT];
   long long tick_ = 0;
@@ -607,7 +618,7 @@ source_kernel(const DevMech m, int mode, int64_t n_states, int64_t tile, const d
   const double V = t.sc[SC_V * S + s];
   // a7: omega_k = sum_i nu_ki q_i (Eq. 4), dn_k/dt = V omega_k (Eq. 3)
   const double* __restrict__ P = t.P;
-  gather<S, 1, 1, PYJAC_UQ, 4, int>(m.qplan, cnt + CNT_Q,
+  gather<S, 1, 1, PYJAC_UQ, 4, ELL_W, int>(m.qplan.ell_ent, t.meta, m.qplan.n_sg, 0, cnt + CNT_Q,
       [&](const int32_t* e, double (&v)[1]) {
         const uint32_t ent = (uint32_t)__ldg(e);
         v[0] += apply_sign(P[(ent & ~SIGN_BIT) * S + s], ent);
@@ -646,8 +657,9 @@ __global__ void __launch_bounds__(NT, 1)
 fd_kernel(const DevMech m, int mode, int ofmt, double rel, double ab, int64_t tile, int64_t n_e,
           const double* __restrict__ phi, const double* __restrict__ param, double* __restrict__ out) {
   extern __shared__ __align__(16) double smem[];
-  Tile<S, false> t(smem, m.ns, m.nr, m.nslots);
-  double* __restrict__ f0 = t.part + m.n_part_src * S;        // f(phi)           [nvar]
+  Tile<S, false> t(smem, m.ns, m.nr, m.nslots, m.n_part_src);
+  load_meta(m.qplan, t.meta);
+  double* __restrict__ f0 = reinterpret_cast<double*>(t.meta + m.qplan.n_sg);   // f(phi)           [nvar]
   double* __restrict__ fc = f0 + m.nvar;                      // f(phi + h_c e_c) [nvar][S]
   __shared__ int cnt[N_CNT];
   long long tick_ = 0;
@@ -665,7 +677,7 @@ fd_kernel(const DevMech m, int mode, int ofmt, double rel, double ab, int64_t ti
                        par, cnt, tick_);
     const double V = t.sc[SC_V * S + s];
     const double* __restrict__ P = t.P;
-    gather<S, 1, 1, PYJAC_UQ, 4, int>(m.qplan, cnt + CNT_Q,
+    gather<S, 1, 1, PYJAC_UQ, 4, ELL_W, int>(m.qplan.ell_ent, t.meta, m.qplan.n_sg, 0, cnt + CNT_Q,
         [&](const int32_t* e, double (&v)[1]) {
           const uint32_t ent = (uint32_t)__ldg(e);
           v[0] += apply_sign(P[(ent & ~SIGN_BIT) * S + s], ent);
@@ -720,7 +732,9 @@ __global__ void __launch_bounds__(NT, 1)
 jacobian_kernel(const DevMech m, const DevPlan pl, int mode, int64_t n_states, int64_t tile, const double* __restrict__ phi,
                 const double* __restrict__ param, double* __restrict__ out) {
   extern __shared__ __align__(16) double smem[];
-  Tile<S, true> t(smem, m.ns, m.nr, m.nslots);
+  Tile<S, true> t(smem, m.ns, m.nr, m.nslots, m.n_part_jac);
+  load_meta(m.cplan, t.meta);
+  load_meta(pl.jplan, t.meta + m.cplan.n_sg);
   const int64_t s0 = (int64_t)blockIdx.x * S;
   __shared__ int cnt[N_CNT];
 #ifdef PYJAC_TIMING
@@ -772,7 +786,7 @@ jacobian_kernel(const DevMech m, const DevPlan pl, int mode, int64_t n_states, i
   const double cS = mode == PYJAC_CONP ? T * R_GAS / Pp : T * R_GAS / V;
   const double cT = mode == PYJAC_CONP ? V / T : Pp / T;
   const double* __restrict__ dE = t.dE;
-  gather<S, 4, 2, PYJAC_UC, PYJAC_UNC, int4>(m.cplan, cnt + CNT_C,
+  gather<S, 4, 2, PYJAC_UC, PYJAC_UNC, ELL_W, int4>(m.cplan.ell_ent, t.meta, m.cplan.n_sg, 0, cnt + CNT_C,
       [&](const int32_t* e, double (&v)[2]) {
         const int4 pr = __ldg(reinterpret_cast<const int4*>(e));      // slot | sign, reaction, dn~ (2 words)
         const uint32_t ent = (uint32_t)pr.x;
@@ -800,16 +814,24 @@ jacobian_kernel(const DevMech m, const DevPlan pl, int mode, int64_t n_states, i
   // a9: species rows.  Block entries J[k][j] = sum_i nu_ki (Ghat^j_i - Ghat^Ns_i); T and E columns
   // J[k][T] = sum_i nu_ki slotT_i, J[k][E] = sum_i nu_ki slotE_i.  Every nonzero is finished in a register and
   // stored once.
-  gather<S, 1, 1, PYJAC_UJ, PYJAC_UNJ, int>(pl.jplan, cnt + CNT_J,
-      [&](const int32_t* e, double (&v)[1]) {
-        const uint32_t ent = (uint32_t)__ldg(e);
-        v[0] += apply_sign(P[(ent & ~SIGN_BIT) * S + s], ent);
-      },
-      [&](int slot) { return __ldg(pl.j_pos + slot); },
-      [&](int, int pos, const double (&v)[1]) {
-        if (pos >= 0) { if (valid) out[obase + (int64_t)pos * tile] = v[0]; }
-        else if (pos <= -2) t.part[(-2 - pos) * S + s] = v[0];
-      });
+  {
+    auto accJ = [&](const int32_t* e, double (&v)[1]) {
+      const uint32_t ent = (uint32_t)__ldg(e);
+      v[0] += apply_sign(P[(ent & ~SIGN_BIT) * S + s], ent);
+    };
+    auto posJ = [&](int slot) { return __ldg(pl.j_pos + slot); };
+    auto storeJ = [&](int, int pos, const double (&v)[1]) {
+      if (pos >= 0) { if (valid) out[obase + (int64_t)pos * tile] = v[0]; }
+      else if (pos <= -2) t.part[(-2 - pos) * S + s] = v[0];
+    };
+    const int2* metaJ = t.meta + m.cplan.n_sg;
+    const int n_wide = pl.jplan.n_wide;
+    gather<S, 1, 1, PYJAC_UJ, PYJAC_UNJ, ELL_W, int>(pl.jplan.ell_ent, metaJ, n_wide, 0, cnt + CNT_J, accJ, posJ, storeJ);
+    // the narrow tail (lists of one or two entries: most nonzeros of a sparse mechanism): 16 segments per thread
+    gather<S, 1, 1, 16, 1, ELL_W_NARROW, int>(pl.jplan.ell_ent, metaJ + n_wide, pl.jplan.n_sg - n_wide, n_wide * ELL_W,
+                                              cnt + CNT_J2, accJ, posJ, storeJ);
+  }
+  TICK(6);
   if (pl.jplan.n_comb + m.cplan.n_comb) {
     __syncthreads();
     combine<S, 1>(pl.jplan, t.part, [&](int c, const double (&v)[1]) {
@@ -882,7 +904,7 @@ constexpr size_t SMEM_LIMIT = 227 * 1024 - 64;   // dynamic part; 64 B left for 
 LaunchCfg choose_cfg(const HostTables& h, bool jac, int64_t tile, int64_t n_states) {
   LaunchCfg cfg{1, NT, 0};
   for (int S = 32; S >= 1; S >>= 1) {
-    const size_t bytes = smem_doubles(h.ns, h.nr, h.nslots, jac ? h.n_part_jac : h.n_part_src, S, jac) * sizeof(double);
+    const size_t bytes = smem_doubles(h.ns, h.nr, h.nslots, jac ? h.n_part_jac : h.n_part_src, jac ? h.jplan.n_sg + h.cplan.n_sg : h.qplan.n_sg, S, jac) * sizeof(double);
     cfg.S = S; cfg.smem = bytes;
     if (bytes > SMEM_LIMIT) continue;
     if ((int64_t)S > tile) continue;                       // lanes of one item must stay inside one tile
@@ -896,7 +918,7 @@ LaunchCfg choose_cfg(const HostTables& h, bool jac, int64_t tile, int64_t n_stat
 LaunchCfg choose_cfg_fd(const HostTables& h) {
   LaunchCfg cfg{1, NT, 0};
   for (int S = 32; S >= 1; S >>= 1) {
-    const size_t bytes = (smem_doubles(h.ns, h.nr, h.nslots, h.n_part_src, S, false) + (size_t)h.nvar * (S + 1)) * sizeof(double);
+    const size_t bytes = (smem_doubles(h.ns, h.nr, h.nslots, h.n_part_src, h.qplan.n_sg, S, false) + (size_t)h.nvar * (S + 1)) * sizeof(double);
     cfg.S = S; cfg.smem = bytes;
     if (bytes > SMEM_LIMIT) continue;
     if (S > 1 && S / 2 >= h.nvar + 1) continue;
