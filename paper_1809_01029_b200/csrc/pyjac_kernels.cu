@@ -834,17 +834,32 @@ jacobian_kernel(const DevMech m, const DevPlan pl, int mode, int64_t n_states, i
   TICK(6);
   if (pl.jplan.n_comb + m.cplan.n_comb) {
     __syncthreads();
-    combine<S, 1>(pl.jplan, t.part, [&](int c, const double (&v)[1]) {
-      if (valid) out[obase + (int64_t)__ldg(pl.jc_pos + c) * tile] = v[0];
-    });
-    combine<S, 2>(m.cplan, t.part, [&](int c, const double (&v)[2]) {
-      if (valid) {
+    // second pass over the split lists of both plans in ONE index space, with every table word (first partial,
+    // count, output positions) requested before the partial sums are added: one L2 round trip for the whole pass
+    const int nJ = pl.jplan.n_comb * S, nC = m.cplan.n_comb * S;
+    const double* __restrict__ part = t.part;
+    for (int idx = tid; idx < nJ + nC; idx += NT) {
+      if (idx < nJ) {
+        const int c = idx / S;
+        const int first = pl.jplan.part_base + __ldg(pl.jplan.comb_first + c), n = __ldg(pl.jplan.comb_nseg + c);
+        const int pos = __ldg(pl.jc_pos + c);
+        double v = 0.0;
+        for (int q = 0; q < n; ++q) v += part[(first + q) * S + s];
+        if (valid) out[obase + (int64_t)pos * tile] = v;
+      } else {
+        const int c = (idx - nJ) / S;
+        const int first = m.cplan.part_base + 2 * __ldg(m.cplan.comb_first + c), n = __ldg(m.cplan.comb_nseg + c);
         const int j = __ldg(m.cc_item + c);
-        const double JT = -(v[0] + fT * (t.ck[j * S + s] - cL)) * iDV;
-        out[obase + (int64_t)__ldg(pl.cc_pos + 2 * c) * tile] = JT;
-        out[obase + (int64_t)__ldg(pl.cc_pos + 2 * c + 1) * tile] = cS * v[1] + cT * JT;
+        const int2 pos = __ldg(reinterpret_cast<const int2*>(pl.cc_pos) + c);
+        double v0 = 0.0, v1 = 0.0;
+        for (int q = 0; q < n; ++q) { v0 += part[(first + 2 * q) * S + s]; v1 += part[(first + 2 * q + 1) * S + s]; }
+        if (valid) {
+          const double JT = -(v0 + fT * (t.ck[j * S + s] - cL)) * iDV;
+          out[obase + (int64_t)pos.x * tile] = JT;
+          out[obase + (int64_t)pos.y * tile] = cS * v1 + cT * JT;
+        }
       }
-    });
+    }
   }
   TICK(5);
   // a10: the four corner entries from the phase-1 reductions (R4-7)
