@@ -69,7 +69,8 @@ __host__ __device__ inline size_t smem_doubles(int ns, int nr, int nslots, int n
 // Dynamic work distribution inside a CTA: items are sorted by descending cost at create time and warps take the
 // next chunk from a shared-memory counter (longest-processing-time-first scheduling); removes the tail in which a
 // few warps work on the heaviest reactions / longest gather lists while the others idle.
-enum { CNT_RX = 0, CNT_J, CNT_J2, CNT_C, CNT_Q, N_CNT };
+constexpr int ZERO_WARP_MIN_SLICES = 32;   // dense matrices of >= 32 K elements get a dedicated zero-fill warp
+enum { CNT_RX = 0, CNT_J, CNT_J2, CNT_C, CNT_Q, CNT_Z, N_CNT };
 __device__ __forceinline__ int next_chunk(int* counter) {
   int c = 0;
   if ((threadIdx.x & 31) == 0) c = atomicAdd(counter, 1);
@@ -191,9 +192,15 @@ __device__ __forceinline__ int64_t state_base(int64_t s, int64_t tile, int64_t n
 
 // phi_of(e): element e of the state vector of THIS thread's lane (tid % S); par_: that lane's parameter.  The
 // analytical kernels read the caller's arrays; the finite-difference kernel adds the perturbation of its column.
-template <int S, bool JAC, class PhiF>
+// Side job of the dense Jacobian: its DRAM-bound zero fill is done by ONE warp while the other warps work through the
+// reaction chunks / gather units (the store queue then blocks that warp only, and the store stream overlaps the
+// latency-bound arithmetic).  side(counter, n): true if this warp does the side job instead of taking work items; it
+// returns when the items are exhausted (*counter >= n) or the side job is finished.
+struct NoSide { __device__ __forceinline__ bool operator()(const int*, int) const { return false; } };
+
+template <int S, bool JAC, class PhiF, class SideF>
 __device__ __forceinline__ void phases01(const DevMech& m, Tile<S, JAC>& t, int mode, PhiF phi_of, double par_,
-                                         int* cnt, long long& tick_) {
+                                         int* cnt, long long& tick_, SideF side) {
   (void)tick_;
   const int tid = threadIdx.x;
   const int ns = m.ns, nr = m.nr, L = ns - 1;
@@ -285,6 +292,7 @@ __device__ __forceinline__ void phases01(const DevMech& m, Tile<S, JAC>& t, int 
   const double ctot_T = Ctot * invT;
   double acc[7] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
   const int n_rx_chunks = (nr * S + 31) / 32;
+  if (!side(cnt + CNT_RX, n_rx_chunks))
   for (int chunk = next_chunk(cnt + CNT_RX); chunk < n_rx_chunks; chunk = next_chunk(cnt + CNT_RX)) {
     const int idx = chunk * 32 + (tid & 31);
     if (idx >= nr * S) continue;
@@ -535,9 +543,9 @@ namespace {
 // ---------------------------------------------------------------------------------------------------
 // EW = segments per super-group (ELL_W, or ELL_W_NARROW for the narrow tail of the species-row plan); metas points at
 // the first of n_groups super-groups, whose first segment has processing slot slot_base.
-template <int S, int STRIDE, int NACC, int U, int UNROLL, int EW, class P, class AccF, class PosF, class StoreF>
+template <int S, int STRIDE, int NACC, int U, int UNROLL, int EW, class P, class AccF, class PosF, class StoreF, class SideF>
 __device__ __forceinline__ void gather(const int32_t* __restrict__ ell_ent, const int2* __restrict__ metas, int n_groups,
-                                       int slot_base, int* counter, AccF acc, PosF pos_of, StoreF store) {
+                                       int slot_base, int* counter, AccF acc, PosF pos_of, StoreF store, SideF side) {
   const int lane = threadIdx.x & 31, sub = lane / S;
   constexpr int IPW = 32 / S;                 // segments of one warp per "u"
   // a unit = U * IPW segments of one super-group; a thread owns U segments (U independent loads per step)
@@ -547,6 +555,7 @@ __device__ __forceinline__ void gather(const int32_t* __restrict__ ell_ent, cons
   // metas: (entry offset, padded length) per super-group, in SHARED memory.  Software pipeline: the next unit's
   // number is fetched while the current unit is processed and the output positions are requested before the entry
   // loop, so a unit costs one exposed L2 round trip (its first entries), not three.
+  if (side(counter, n_work)) return;
   int unit = next_chunk(counter);
   while (unit < n_work) {
     const int next = next_chunk(counter);
@@ -614,7 +623,7 @@ source_kernel(const DevMech m, int mode, int64_t n_states, int64_t tile, const d
   const bool valid = s0 + s < n_states;
   const int64_t sg = min(s0 + s, n_states - 1);   // ragged tail: recompute the last valid state, never store
   const int64_t pbase = state_base(sg, tile, m.nvar), obase = pbase;
-  phases01<S, false>(m, t, mode, [&](int e) { return phi[pbase + (int64_t)e * tile]; }, param[sg], cnt, tick_);
+  phases01<S, false>(m, t, mode, [&](int e) { return phi[pbase + (int64_t)e * tile]; }, param[sg], cnt, tick_, NoSide());
   const double V = t.sc[SC_V * S + s];
   // a7: omega_k = sum_i nu_ki q_i (Eq. 4), dn_k/dt = V omega_k (Eq. 3)
   const double* __restrict__ P = t.P;
@@ -627,7 +636,7 @@ source_kernel(const DevMech m, int mode, int64_t n_states, int64_t tile, const d
       [&](int, int k, const double (&v)[1]) {
         if (k >= 0) { if (valid) out[obase + (int64_t)(2 + k) * tile] = V * v[0]; }
         else if (k <= -2) t.part[(-2 - k) * S + s] = v[0];
-      });
+      }, NoSide());
   if (m.qplan.n_comb) {
     __syncthreads();
     combine<S, 1>(m.qplan, t.part, [&](int c, const double (&v)[1]) {
@@ -674,7 +683,7 @@ fd_kernel(const DevMech m, int mode, int ofmt, double rel, double ab, int64_t ti
     double x = 0.0, xp = 0.0;
     if (c >= 0) { x = phi[pbase + (int64_t)c * tile]; xp = x + fma(rel, fabs(x), ab); }
     phases01<S, false>(m, t, mode, [&](int e) { const double v = phi[pbase + (int64_t)e * tile]; return e == c ? xp : v; },
-                       par, cnt, tick_);
+                       par, cnt, tick_, NoSide());
     const double V = t.sc[SC_V * S + s];
     const double* __restrict__ P = t.P;
     gather<S, 1, 1, PYJAC_UQ, 4, ELL_W, int>(m.qplan.ell_ent, t.meta, m.qplan.n_sg, 0, cnt + CNT_Q,
@@ -686,7 +695,7 @@ fd_kernel(const DevMech m, int mode, int ofmt, double rel, double ab, int64_t ti
         [&](int, int k, const double (&v)[1]) {
           if (k >= 0) fc[(2 + k) * S + s] = V * v[0];
           else if (k <= -2) t.part[(-2 - k) * S + s] = v[0];
-        });
+        }, NoSide());
     if (m.qplan.n_comb) {
       __syncthreads();
       combine<S, 1>(m.qplan, t.part, [&](int q, const double (&v)[1]) { fc[(2 + __ldg(m.qc_item + q)) * S + s] = V * v[0]; });
@@ -727,7 +736,7 @@ fd_kernel(const DevMech m, int mode, int ofmt, double rel, double ab, int64_t ti
 // ---------------------------------------------------------------------------------------------------
 // Jacobian (sparse CSR / CSC value order or dense 'C' / 'F'), Eq. 9
 // ---------------------------------------------------------------------------------------------------
-template <int S>
+template <int S, bool DENSE>
 __global__ void __launch_bounds__(NT, 1)
 jacobian_kernel(const DevMech m, const DevPlan pl, int mode, int64_t n_states, int64_t tile, const double* __restrict__ phi,
                 const double* __restrict__ param, double* __restrict__ out) {
@@ -747,34 +756,43 @@ jacobian_kernel(const DevMech m, const DevPlan pl, int mode, int64_t n_states, i
   const bool valid = s0 + s < n_states;
   const int64_t sg = min(s0 + s, n_states - 1);   // ragged tail: recompute the last valid state, never store
   const int64_t pbase = state_base(sg, tile, m.nvar), obase = state_base(sg, tile, pl.n_e);
-  phases01<S, true>(m, t, mode, [&](int e) { return phi[pbase + (int64_t)e * tile]; }, param[sg], cnt, tick_);
+  // dense output: structural zeros, each stored once (no memset pass), in slices of 32 bitmap words (1024 elements:
+  // one coalesced mask load, then 32 coalesced predicated store instructions at S = 1).  For large matrices the
+  // last warp streams the slices while the others compute (see NoSide above); what is left is shared at the end.
+  const int n2 = m.nvar * m.nvar;
+  const int n_zslices = DENSE ? (n2 + 1023) / 1024 : 0;
+  auto zero_slice = [&](int slice) {
+    if (S == 1) {
+      const int lane = tid & 31, w0 = slice * 32, n_words = (n2 + 31) / 32;
+      const uint32_t mine = w0 + lane < n_words ? __ldg(pl.nzmask + w0 + lane) : 0xffffffffu;
+#pragma unroll 8
+      for (int j = 0; j < 32; ++j) {
+        const uint32_t wj = __shfl_sync(0xffffffffu, mine, j);
+        const int e = (w0 + j) * 32 + lane;
+        if (!((wj >> lane) & 1u) && e < n2 && valid) out[obase + (int64_t)e * tile] = 0.0;
+      }
+    } else {
+      for (int q = (tid & 31) / S; q < 1024; q += 32 / S) {
+        const int e = slice * 1024 + q;
+        if (e < n2 && !((__ldg(pl.nzmask + (e >> 5)) >> (e & 31)) & 1u) && valid) out[obase + (int64_t)e * tile] = 0.0;
+      }
+    }
+  };
+  const bool zero_warp = DENSE && n_zslices >= ZERO_WARP_MIN_SLICES && (tid >> 5) == NW - 1;
+  auto side = [&](const int* counter, int n) -> bool {
+    if (!DENSE || !zero_warp) return false;
+    while (*reinterpret_cast<const volatile int*>(counter) < n) {
+      const int z = next_chunk(cnt + CNT_Z);
+      if (z >= n_zslices) break;
+      zero_slice(z);
+    }
+    return true;
+  };
+  phases01<S, true>(m, t, mode, [&](int e) { return phi[pbase + (int64_t)e * tile]; }, param[sg], cnt, tick_, side);
   TICK(2);
   const double T = t.sc[SC_T * S + s], V = t.sc[SC_V * S + s], Pp = t.sc[SC_P * S + s], D = t.sc[SC_D * S + s];
   const double N = red_sum<S>(t.red, 0, s);
   const double fT = -N / D;
-  // dense output: structural zeros, each stored once (no memset pass).  A warp takes 32 bitmap words (1024
-  // elements) at a time: one coalesced mask load, then 32 fully coalesced predicated store instructions.
-  if (pl.nzmask != nullptr) {
-    const int n2 = m.nvar * m.nvar;
-    if (S == 1) {
-      const int lane = tid & 31, warp = tid >> 5;
-      const int n_words = (n2 + 31) / 32;
-      for (int w0 = warp * 32; w0 < n_words; w0 += NW * 32) {
-        const uint32_t mine = w0 + lane < n_words ? __ldg(pl.nzmask + w0 + lane) : 0xffffffffu;
-#pragma unroll 8
-        for (int j = 0; j < 32; ++j) {
-          const uint32_t wj = __shfl_sync(0xffffffffu, mine, j);
-          const int e = (w0 + j) * 32 + lane;
-          if (!((wj >> lane) & 1u) && e < n2 && valid) out[obase + (int64_t)e * tile] = 0.0;
-        }
-      }
-    } else {
-      for (int idx = tid; idx < n2 * S; idx += NT) {
-        const int e = idx / S;
-        if (!((__ldg(pl.nzmask + (e >> 5)) >> (e & 31)) & 1u) && valid) out[obase + (int64_t)e * tile] = 0.0;
-      }
-    }
-  }
   TICK(3);
   const double* __restrict__ P = t.P;
   // The T/E-row gather goes FIRST: it has few, long units; warps that finish it early move on to the many short
@@ -809,7 +827,7 @@ jacobian_kernel(const DevMech m, const DevPlan pl, int mode, int64_t n_states, i
           const int pi = m.cplan.part_base + 2 * (-2 - pp.x);
           t.part[pi * S + s] = v[0]; t.part[(pi + 1) * S + s] = v[1];
         }
-      });
+      }, side);
   TICK(4);
   // a9: species rows.  Block entries J[k][j] = sum_i nu_ki (Ghat^j_i - Ghat^Ns_i); T and E columns
   // J[k][T] = sum_i nu_ki slotT_i, J[k][E] = sum_i nu_ki slotE_i.  Every nonzero is finished in a register and
@@ -826,11 +844,13 @@ jacobian_kernel(const DevMech m, const DevPlan pl, int mode, int64_t n_states, i
     };
     const int2* metaJ = t.meta + m.cplan.n_sg;
     const int n_wide = pl.jplan.n_wide;
-    gather<S, 1, 1, PYJAC_UJ, PYJAC_UNJ, ELL_W, int>(pl.jplan.ell_ent, metaJ, n_wide, 0, cnt + CNT_J, accJ, posJ, storeJ);
+    gather<S, 1, 1, PYJAC_UJ, PYJAC_UNJ, ELL_W, int>(pl.jplan.ell_ent, metaJ, n_wide, 0, cnt + CNT_J, accJ, posJ, storeJ, side);
     // the narrow tail (lists of one or two entries: most nonzeros of a sparse mechanism): 16 segments per thread
     gather<S, 1, 1, 16, 1, ELL_W_NARROW, int>(pl.jplan.ell_ent, metaJ + n_wide, pl.jplan.n_sg - n_wide, n_wide * ELL_W,
-                                              cnt + CNT_J2, accJ, posJ, storeJ);
+                                              cnt + CNT_J2, accJ, posJ, storeJ, side);
   }
+  if (DENSE)                                      // whatever is left of the zero fill
+    for (int z = next_chunk(cnt + CNT_Z); z < n_zslices; z = next_chunk(cnt + CNT_Z)) zero_slice(z);
   TICK(6);
   if (pl.jplan.n_comb + m.cplan.n_comb) {
     __syncthreads();
@@ -902,7 +922,8 @@ template <int S> int launch_source_S(const DevMech& m, const LaunchCfg& cfg, int
 template <int S> int launch_jac_S(const DevMech& m, const DevPlan& p, const LaunchCfg& cfg, int mode, int64_t n, int64_t tile,
                                   const double* phi, const double* param, double* out, cudaStream_t st) {
   const int64_t blocks = (n + S - 1) / S;
-  jacobian_kernel<S><<<(unsigned)blocks, NT, cfg.smem, st>>>(m, p, mode, n, tile, phi, param, out);
+  if (p.nzmask != nullptr) jacobian_kernel<S, true><<<(unsigned)blocks, NT, cfg.smem, st>>>(m, p, mode, n, tile, phi, param, out);
+  else jacobian_kernel<S, false><<<(unsigned)blocks, NT, cfg.smem, st>>>(m, p, mode, n, tile, phi, param, out);
   return (int)cudaGetLastError();
 }
 
@@ -987,7 +1008,9 @@ template <int S> static int set_attr_S() {
   if (e != cudaSuccess) return (int)e;
   e = cudaFuncSetAttribute(fd_kernel<S>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_LIMIT);
   if (e != cudaSuccess) return (int)e;
-  return (int)cudaFuncSetAttribute(jacobian_kernel<S>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_LIMIT);
+  e = cudaFuncSetAttribute(jacobian_kernel<S, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_LIMIT);
+  if (e != cudaSuccess) return (int)e;
+  return (int)cudaFuncSetAttribute(jacobian_kernel<S, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_LIMIT);
 }
 
 int set_kernel_attributes() {
