@@ -49,6 +49,9 @@ namespace {
 #ifndef PYJAC_UNC
 #define PYJAC_UNC 4
 #endif
+#ifndef PYJAC_ZERO_WARPS
+#define PYJAC_ZERO_WARPS 1
+#endif
 #ifndef PYJAC_UQ
 #define PYJAC_UQ 1
 #endif
@@ -92,6 +95,10 @@ template <int S> __device__ __forceinline__ double red_sum(const double* red, in
   for (int w = 0; w < NW; ++w) t += red[(w * NRED + j) * S + s];
   return t;
 }
+
+// Outputs are written once and never read back by the kernel: streaming stores (evict-first in L2), so that the
+// write stream (up to 1 MB per state in flight per SM) does not push the mechanism tables and gather plans out of L2.
+__device__ __forceinline__ void st_out(double* p, double v) { __stcs(p, v); }
 
 __device__ __forceinline__ double apply_sign(double v, uint32_t ent) {
   return __hiloint2double(__double2hiint(v) ^ (int)(ent & SIGN_BIT), __double2loint(v));
@@ -634,13 +641,13 @@ source_kernel(const DevMech m, int mode, int64_t n_states, int64_t tile, const d
       },
       [&](int slot) { return __ldg(m.q_target + slot); },
       [&](int, int k, const double (&v)[1]) {
-        if (k >= 0) { if (valid) out[obase + (int64_t)(2 + k) * tile] = V * v[0]; }
+        if (k >= 0) { if (valid) st_out(out + obase + (int64_t)(2 + k) * tile, V * v[0]); }
         else if (k <= -2) t.part[(-2 - k) * S + s] = v[0];
       }, NoSide());
   if (m.qplan.n_comb) {
     __syncthreads();
     combine<S, 1>(m.qplan, t.part, [&](int c, const double (&v)[1]) {
-      if (valid) out[obase + (int64_t)(2 + __ldg(m.qc_item + c)) * tile] = V * v[0];
+      if (valid) st_out(out + obase + (int64_t)(2 + __ldg(m.qc_item + c)) * tile, V * v[0]);
     });
   }
   if (threadIdx.x < S && valid) {
@@ -649,8 +656,8 @@ source_kernel(const DevMech m, int mode, int64_t n_states, int64_t tile, const d
     const double Ssum = red_sum<S>(t.red, 1, s);
     const double fE = mode == PYJAC_CONP ? V * (T * R_GAS / Pp * Ssum + fT / T)   // Eq. 8a
                                          : T * R_GAS * Ssum + Pp / T * fT;        // Eq. 8b
-    out[obase] = fT;
-    out[obase + tile] = fE;
+    st_out(out + obase, fT);
+    st_out(out + obase + tile, fE);
   }
 }
 
@@ -718,14 +725,14 @@ fd_kernel(const DevMech m, int mode, int ofmt, double rel, double ab, int64_t ti
       if (ofmt >= OUT_DENSE_C) {
         for (int i = tid / S; i < nvar; i += NT / S) {
           const int64_t e = ofmt == OUT_DENSE_C ? (int64_t)i * nvar + c : (int64_t)c * nvar + i;
-          out[obase + e * tile] = (fc[i * S + s] - f0[i]) / h;
+          st_out(out + obase + e * tile, (fc[i * S + s] - f0[i]) / h);
         }
       } else {                                                // the handle's pattern, walked by columns
         const int p1 = __ldg(m.csc_ptr + c + 1);
         for (int p = __ldg(m.csc_ptr + c) + tid / S; p < p1; p += NT / S) {
           const int i = __ldg(m.csc_idx + p);
           const int64_t e = ofmt == OUT_CSC ? p : __ldg(m.csc2csr + p);
-          out[obase + e * tile] = (fc[i * S + s] - f0[i]) / h;
+          st_out(out + obase + e * tile, (fc[i * S + s] - f0[i]) / h);
         }
       }
     }
@@ -769,16 +776,16 @@ jacobian_kernel(const DevMech m, const DevPlan pl, int mode, int64_t n_states, i
       for (int j = 0; j < 32; ++j) {
         const uint32_t wj = __shfl_sync(0xffffffffu, mine, j);
         const int e = (w0 + j) * 32 + lane;
-        if (!((wj >> lane) & 1u) && e < n2 && valid) out[obase + (int64_t)e * tile] = 0.0;
+        if (!((wj >> lane) & 1u) && e < n2 && valid) st_out(out + obase + (int64_t)e * tile, 0.0);
       }
     } else {
       for (int q = (tid & 31) / S; q < 1024; q += 32 / S) {
         const int e = slice * 1024 + q;
-        if (e < n2 && !((__ldg(pl.nzmask + (e >> 5)) >> (e & 31)) & 1u) && valid) out[obase + (int64_t)e * tile] = 0.0;
+        if (e < n2 && !((__ldg(pl.nzmask + (e >> 5)) >> (e & 31)) & 1u) && valid) st_out(out + obase + (int64_t)e * tile, 0.0);
       }
     }
   };
-  const bool zero_warp = DENSE && n_zslices >= ZERO_WARP_MIN_SLICES && (tid >> 5) == NW - 1;
+  const bool zero_warp = DENSE && n_zslices >= ZERO_WARP_MIN_SLICES && (tid >> 5) >= NW - PYJAC_ZERO_WARPS;
   auto side = [&](const int* counter, int n) -> bool {
     if (!DENSE || !zero_warp) return false;
     while (*reinterpret_cast<const volatile int*>(counter) < n) {
@@ -820,8 +827,8 @@ jacobian_kernel(const DevMech m, const DevPlan pl, int mode, int64_t n_states, i
         if (pp.x >= 0) {
           if (valid) {
             const double JT = -(v[0] + fT * (t.ck[pp.z * S + s] - cL)) * iDV;
-            out[obase + (int64_t)pp.x * tile] = JT;
-            out[obase + (int64_t)pp.y * tile] = cS * v[1] + cT * JT;
+            st_out(out + obase + (int64_t)pp.x * tile, JT);
+            st_out(out + obase + (int64_t)pp.y * tile, cS * v[1] + cT * JT);
           }
         } else if (pp.x <= -2) {
           const int pi = m.cplan.part_base + 2 * (-2 - pp.x);
@@ -839,7 +846,7 @@ jacobian_kernel(const DevMech m, const DevPlan pl, int mode, int64_t n_states, i
     };
     auto posJ = [&](int slot) { return __ldg(pl.j_pos + slot); };
     auto storeJ = [&](int, int pos, const double (&v)[1]) {
-      if (pos >= 0) { if (valid) out[obase + (int64_t)pos * tile] = v[0]; }
+      if (pos >= 0) { if (valid) st_out(out + obase + (int64_t)pos * tile, v[0]); }
       else if (pos <= -2) t.part[(-2 - pos) * S + s] = v[0];
     };
     const int2* metaJ = t.meta + m.cplan.n_sg;
@@ -865,7 +872,7 @@ jacobian_kernel(const DevMech m, const DevPlan pl, int mode, int64_t n_states, i
         const int pos = __ldg(pl.jc_pos + c);
         double v = 0.0;
         for (int q = 0; q < n; ++q) v += part[(first + q) * S + s];
-        if (valid) out[obase + (int64_t)pos * tile] = v;
+        if (valid) st_out(out + obase + (int64_t)pos * tile, v);
       } else {
         const int c = (idx - nJ) / S;
         const int first = m.cplan.part_base + 2 * __ldg(m.cplan.comb_first + c), n = __ldg(m.cplan.comb_nseg + c);
@@ -875,8 +882,8 @@ jacobian_kernel(const DevMech m, const DevPlan pl, int mode, int64_t n_states, i
         for (int q = 0; q < n; ++q) { v0 += part[(first + 2 * q) * S + s]; v1 += part[(first + 2 * q + 1) * S + s]; }
         if (valid) {
           const double JT = -(v0 + fT * (t.ck[j * S + s] - cL)) * iDV;
-          out[obase + (int64_t)pos.x * tile] = JT;
-          out[obase + (int64_t)pos.y * tile] = cS * v1 + cT * JT;
+          st_out(out + obase + (int64_t)pos.x * tile, JT);
+          st_out(out + obase + (int64_t)pos.y * tile, cS * v1 + cT * JT);
         }
       }
     }
