@@ -143,13 +143,24 @@ def run_reference(args, rank, world):
     print(json.dumps(line))
 
 
-def workload_config(c, what, tile, S):
+def workload_config(c, what, tile, S, N=None, mode=None):
     cfg = CONFIGS[c]
+    N = cfg["n_states"] if N is None else N
+    mode = cfg["mode"] if mode is None else mode
     return {"workload": "C%d: synthetic %d-species / %d-reaction mechanism, %d fp64 states, %s, %s Jacobian%s" % (
-        c, cfg["ns"], cfg["nr"], cfg["n_states"], "CONP" if cfg["mode"] == mg.CONP else "CONV", what,
+        c, cfg["ns"], cfg["nr"], N, "CONP" if mode == mg.CONP else "CONV", what,
         " (CSR value order)" if what == "sparse" else " (row-major)"),
-        "n_states_per_gpu": cfg["n_states"], "layout_tile": tile, "states_per_cta": S,
-        "l2": "inputs+outputs larger than L2 (no flush needed)" if cfg["n_states"] * 8 * 1000 > 126e6 else "l2_flush_between_steps"}
+        "n_states_per_gpu": N, "layout_tile": tile, "states_per_cta": S,
+        "l2": "inputs+outputs larger than L2 (no flush needed)" if N * 8 * 1000 > 126e6 else "l2_flush_between_steps"}
+
+
+def states_per_cta(S_max, tile, N):
+    """Mirror of the library's launch choice (choose_cfg): largest power of two <= S_max that fits inside a layout
+    tile and still leaves two CTAs per SM."""
+    S = S_max
+    while S > 1 and (S > tile or (N + S - 1) // S < 2 * 148):
+        S //= 2
+    return S
 
 
 def main():
@@ -161,6 +172,7 @@ def main():
     ap.add_argument("--impl", default="b200")
     ap.add_argument("--states", type=int, default=None, help="override states per GPU (sweeps)")
     ap.add_argument("--tile", type=int, default=None, help="override layout tile (default: states per CTA)")
+    ap.add_argument("--mode", choices=["conp", "conv"], default=None, help="override the config's mode (sweeps)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-fd", action="store_true", help="skip the finite-difference comparison")
@@ -179,7 +191,7 @@ def main():
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     c = args.config
     cfg = CONFIGS[c]
-    mode = cfg["mode"]
+    mode = cfg["mode"] if args.mode is None else (mg.CONP if args.mode == "conp" else mg.CONV)
     what = "dense" if c in (1, 4) else "sparse"
     N = args.states or cfg["n_states"]
     mech = mg.config_mechanism(c)
@@ -316,9 +328,11 @@ def main():
                    "sample": "%d states of the same workload in %.1f s (oracle/, OpenMP over states)" % (n_s, dt)}
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(3, args.warmup),
                 "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-                "dtype": "f64", "data": "synthetic", "config": workload_config(c, what, tile, S),
+                "dtype": "f64", "data": "synthetic", "config": dict(workload_config(c, what, tile, states_per_cta(S, tile, N), N, mode),
+                                                                   l2="l2_flush_between_steps (256 MB written)" if flush is not None
+                                                                   else "inputs+outputs larger than L2 (no flush needed)"),
                 "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                             "traffic": (lambda t: None if t is None else t["dram_bytes"] * N / t["n_states"])(ncu_traffic(c)), "peak_source": peak_src, "kernel": "jacobian_kernel<S=%d>" % S,
+                             "traffic": (lambda t: None if t is None else t["dram_bytes"] * N / t["n_states"])(ncu_traffic(c)), "peak_source": peak_src, "kernel": "jacobian_kernel<S=%d>" % states_per_cta(S, tile, N),
                              "algorithmic_bytes_per_state": 8 * n_e + 8 * (M.ns + 2), "kernel_ms": kavg_ms,
                              "ns_per_state": 1e6 * kavg_ms / N},
                 "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": args.steps, "clocks": clk.summary(),
