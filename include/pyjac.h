@@ -75,6 +75,10 @@ typedef struct {
   const int32_t *cheb_ptr, *cheb_nT, *cheb_nP;       /* Chebyshev: coefficient offset, grid sizes      */
   const double *cheb_Tmin, *cheb_Tmax, *cheb_Pmin, *cheb_Pmax; /* [Nr]                                 */
   const double *cheb_coef;                           /* row-major nT x nP, log10 of k in SI            */
+  const uint8_t *chem_activated;                     /* [Nr] or NULL (= none).  1 on a falloff-type reaction:
+                                                        chemically-activated bimolecular reaction (PAPER.md L143,
+                                                        DESIGN.md R8): (A, beta, Ta) = k_inf and low_* = k_0 as for
+                                                        falloff, P_r = k_0 [M] / k_inf, but k = k_0 F / (1 + P_r)   */
 } pyjac_mech_desc;
 
 /* Step a0 (one-time, host): validate, sort reactions by type, pack device tables, build the exact
@@ -82,7 +86,8 @@ typedef struct {
  * paper's run-time index search.  Uploads the tables to `cuda_device`.
  * PYJAC_EMECH: Ns < 2, Nr < 1, index out of range, nu outside 1..3, more than 3 species per side,
  * A <= 0, W <= 0, tmid <= 0, negative efficiency, P-Log with < 2 points or non-ascending pressures,
- * empty Chebyshev grid or Tmin >= Tmax or Pmin >= Pmax, unknown type.  PYJAC_ECUDA: no such device.
+ * empty Chebyshev grid or Tmin >= Tmax or Pmin >= Pmax, unknown type, chem_activated on a reaction that is not of a
+ * falloff type.  PYJAC_ECUDA: no such device.
  * cuda_device = -1 builds a HOST-ONLY handle (pyjac_mech_dims / pyjac_sparsity work; every compute
  * call fails with PYJAC_ECUDA) -- there is no CPU compute path.  The compute calls launch on the
  * caller's current device, which must be the handle's device. */

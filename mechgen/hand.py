@@ -106,3 +106,28 @@ def hand_all_types(last_reacts=True, last_eff=True, seed=7):
                     cheb=dict(Tmin=300.0, Tmax=3000.0, Pmin=0.01 * P_ATM, Pmax=100.0 * P_ATM, coef=coef))
     mb.add_reaction({1: 1, 2: 1}, {0: 1, 3: 1}, A=1e10, beta=0.0, Ta=6000.0, rev=False)                      # irreversible 2-2
     return mb.build()
+
+
+def hand_chem_activated():
+    """Five species A, B, C, D and bath N (last): every falloff form once as a chemically-activated reaction
+    (k = k_0 F / (1 + P_r)) next to its plain falloff twin with the same parameters, plus one
+    elementary reaction so that all species take part.  A = X, B = X, C = X2, D = X2 (isomers), so A + B <=> C is
+    balanced."""
+    mb = MechBuilder()
+    W = [10.0, 10.0, 20.0, 20.0, 28.0]
+    th = [_const_cp(2.6, 1.5e4, 5.0), _const_cp(2.9, 1.1e4, 5.5), _const_cp(3.6, 2.0e3, 7.0), _const_cp(3.9, 1.0e3, 7.5),
+          _const_cp(3.5, -1.0e3, 6.5)]
+    for w, t in zip(W, th):
+        mb.add_species(w, t)
+    A, B, C, D = 0, 1, 2, 3
+    hi = dict(A=3.0e10, beta=0.4, Ta=2500.0)
+    low = (7.0e11, -0.6, 1200.0)
+    eff = {C: 2.5, D: 0.4}
+    for chem in (True, False):
+        mb.add_reaction({A: 1, B: 1}, {C: 1}, rev=True, type=FALLOFF_LINDEMANN, low=low, eff=eff, chem_activated=chem, **hi)
+        mb.add_reaction({A: 2}, {D: 1}, rev=True, type=FALLOFF_TROE, low=low, troe=(0.6, 200.0, 1800.0, 5000.0), eff=eff,
+                        chem_activated=chem, **hi)
+        mb.add_reaction({A: 1, B: 1}, {D: 1}, rev=False, type=FALLOFF_SRI, low=low, sri=(0.8, 300.0, 2000.0, 1.2, 0.1),
+                        chem_activated=chem, **hi)
+    mb.add_reaction({C: 1}, {D: 1}, A=4.0e7, beta=0.2, Ta=6000.0, rev=True)
+    return mb.build()

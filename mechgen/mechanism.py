@@ -43,10 +43,12 @@ class MechBuilder:
         return len(self.W) - 1
 
     def add_reaction(self, reac, prod, A=1.0, beta=0.0, Ta=0.0, rev=True, type=ELEMENTARY, eff=None,
-                     collider=-1, low=None, troe=None, sri=None, plog=None, cheb=None):
+                     collider=-1, low=None, troe=None, sri=None, plog=None, cheb=None, chem_activated=False):
+        """chem_activated (falloff types only): chemically-activated bimolecular reaction; (A, beta, Ta) stay the
+        high-pressure limit k_inf and `low` the low-pressure limit k_0, but k = k_0 F / (1 + P_r)."""
         self.reactions.append(dict(reac=dict(reac), prod=dict(prod), A=A, beta=beta, Ta=Ta, rev=rev,
                                    type=type, eff=dict(eff or {}), collider=collider, low=low,
-                                   troe=troe, sri=sri, plog=plog, cheb=cheb))
+                                   troe=troe, sri=sri, plog=plog, cheb=cheb, chem_activated=bool(chem_activated)))
         return len(self.reactions) - 1
 
     def build(self):
@@ -119,6 +121,7 @@ class MechBuilder:
         d["cheb_Tmin"] = np.ascontiguousarray(lim[:, 0]); d["cheb_Tmax"] = np.ascontiguousarray(lim[:, 1])
         d["cheb_Pmin"] = np.ascontiguousarray(lim[:, 2]); d["cheb_Pmax"] = np.ascontiguousarray(lim[:, 3])
         d["cheb_coef"] = np.array(coef, np.float64)
+        d["chem_activated"] = np.array([1 if r["chem_activated"] else 0 for r in self.reactions], np.uint8)
         return d
 
 

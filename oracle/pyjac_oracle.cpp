@@ -61,6 +61,7 @@ struct Mech {
     std::vector<int> collider;
     std::vector<double> lowA, lowb, lowTa, troe;
     std::vector<int> troe_t2;
+    std::vector<int> chem;                   // chemically-activated falloff (reading R8): k = k_0 F / (1 + P_r)
     std::vector<double> sri;
     std::vector<int> plog_ptr;
     std::vector<double> plogP, plogA, plogb, plogTa;
@@ -84,12 +85,13 @@ template <class T> struct Inter {
     std::vector<T> C, cp, h, s, g;            // [ns]  cp [J/kmol/K], h [J/kmol], s/R, g/(RT)
     std::vector<T> dcp;                       // [ns]  d cp / dT
     std::vector<T> kf, kr, Kc, M, Pr, F, c, Rf, Rr, q;   // [nr]
+    std::vector<T> k0_kinf;                               // [nr] falloff: k_0 / k_inf (= dP_r/d[M])
     std::vector<T> dlnkf_dT, dlnkf_dP, dlnKc_dT;         // [nr]
     std::vector<T> wdot;                      // [ns]; wdot[ns-1] from mass conservation (reading A1)
     T Ctot, D, N, S, Tt, P, V;
     void resize(int ns, int nr) {
         for (auto* v : {&C, &cp, &h, &s, &g, &dcp, &wdot}) v->assign(ns, T(0.0));
-        for (auto* v : {&kf, &kr, &Kc, &M, &Pr, &F, &c, &Rf, &Rr, &q, &dlnkf_dT, &dlnkf_dP, &dlnKc_dT}) v->assign(nr, T(0.0));
+        for (auto* v : {&kf, &kr, &Kc, &M, &Pr, &F, &c, &Rf, &Rr, &q, &dlnkf_dT, &dlnkf_dP, &dlnKc_dT, &k0_kinf}) v->assign(nr, T(0.0));
     }
 };
 
@@ -216,6 +218,15 @@ void eval_source(const Mech& m, int mode, const T* phi, const T& param, T* f, In
             kf = exp(std::log(m.A[i]) + m.beta[i] * lnT - m.Ta[i] / Tt);      // Arrhenius (c-2)
             lam_f = (m.beta[i] + m.Ta[i] / Tt) / Tt;
         }
+        // Chemically-activated bimolecular reaction (reading R8): (A, beta, Ta) is still the
+        // high-pressure limit k_inf and `low` the low-pressure limit k_0, P_r = k_0 [M] / k_inf as for falloff, but
+        // the rate constant of the rates of progress is k_0 and the pressure modification is c = F / (1 + P_r).
+        const bool chem = (ty == T_LIND || ty == T_TROE || ty == T_SRI) && m.chem[i];
+        const T kinf = kf;
+        if (chem) {
+            kf = exp(std::log(m.lowA[i]) + m.lowb[i] * lnT - m.lowTa[i] / Tt);
+            lam_f = (m.lowb[i] + m.lowTa[i] / Tt) / Tt;
+        }
         w.kf[i] = kf; w.dlnkf_dT[i] = lam_f; w.dlnkf_dP[i] = dlnk_dP;
         // a4: equilibrium constant from Gibbs polynomials, reverse rate constant
         T kr = T(0.0), Kc = T(0.0), dlnKc = T(0.0);
@@ -249,9 +260,10 @@ void eval_source(const Mech& m, int mode, const T* phi, const T& param, T* f, In
             if (ty == T_THIRD) c = M;
             else {
                 T k0 = exp(std::log(m.lowA[i]) + m.lowb[i] * lnT - m.lowTa[i] / Tt);
-                Pr = k0 * M / kf;
+                w.k0_kinf[i] = k0 / kinf;
+                Pr = k0 * M / kinf;
                 F = blend(m, i, Tt, Pr).F;
-                c = F * Pr / (1.0 + Pr);
+                c = chem ? F / (1.0 + Pr) : F * Pr / (1.0 + Pr);
             }
         }
         w.M[i] = M; w.Pr[i] = Pr; w.F[i] = F; w.c[i] = c;
@@ -334,13 +346,17 @@ void eval_jacobian(const Mech& m, int mode, bool approx, const double* phi, doub
         } else if (ty == T_LIND || ty == T_TROE || ty == T_SRI) {
             const double Pr = w.Pr[i], F = w.F[i];
             Blend<double> b = blend(m, i, Tt, Pr);
-            const double dc_dPr = F / ((1.0 + Pr) * (1.0 + Pr)) + (Pr / (1.0 + Pr)) * b.dF_dPr;
-            const double lnT = std::log(Tt);
-            const double k0 = std::exp(std::log(m.lowA[i]) + m.lowb[i] * lnT - m.lowTa[i] / Tt);
+            // c = F Pr / (1 + Pr) (falloff) or F / (1 + Pr) (chemically activated): dc/dPr at constant T, and the
+            // factor of dF/dT
+            const bool chem = m.chem[i] != 0;
+            const double dc_dPr = chem ? -F / ((1.0 + Pr) * (1.0 + Pr)) + b.dF_dPr / (1.0 + Pr)
+                                       : F / ((1.0 + Pr) * (1.0 + Pr)) + (Pr / (1.0 + Pr)) * b.dF_dPr;
+            const double cF = chem ? 1.0 / (1.0 + Pr) : Pr / (1.0 + Pr);
+            const double rat = w.k0_kinf[i];                              // dPr/d[M]
             const double dPr_dT = Pr * (m.lowb[i] - m.beta[i] + (m.lowTa[i] - m.Ta[i]) / Tt) / Tt;
-            if (m.collider[i] < 0) Xdef = dc_dPr * (k0 / w.kf[i]) * R;
-            for (int k = 0; k < ns; ++k) G[k] = m.alpha(i, k) * dc_dPr * (k0 / w.kf[i]) * R + w.c[i] * dRdC[k];
-            GT = (dc_dPr * dPr_dT + (Pr / (1.0 + Pr)) * b.dF_dT) * R + w.c[i] * dRdT;
+            if (m.collider[i] < 0) Xdef = dc_dPr * rat * R;
+            for (int k = 0; k < ns; ++k) G[k] = m.alpha(i, k) * dc_dPr * rat * R + w.c[i] * dRdC[k];
+            GT = (dc_dPr * dPr_dT + cF * b.dF_dT) * R + w.c[i] * dRdT;
         } else {
             for (int k = 0; k < ns; ++k) G[k] = dRdC[k];
             GT = dRdT;
@@ -452,6 +468,7 @@ struct orc_desc {
     const int32_t* plog_ptr; const double *plog_P, *plog_A, *plog_beta, *plog_Ta;
     const int32_t *cheb_ptr, *cheb_nT, *cheb_nP;
     const double *cheb_Tmin, *cheb_Tmax, *cheb_Pmin, *cheb_Pmax, *cheb_coef;
+    const uint8_t* chem_activated;            // [Nr] or NULL
 };
 
 void* orc_create2(const orc_desc* d, int approx) {
@@ -472,6 +489,7 @@ void* orc_create2(const orc_desc* d, int approx) {
     copy_in(m.lowA, d->low_A, nr); copy_in(m.lowb, d->low_beta, nr); copy_in(m.lowTa, d->low_Ta, nr);
     copy_in(m.troe, d->troe, 4 * nr); m.troe_t2.resize(nr); for (int i = 0; i < nr; ++i) m.troe_t2[i] = d->troe_has_T2[i];
     copy_in(m.sri, d->sri, 5 * nr);
+    m.chem.assign(nr, 0); if (d->chem_activated) for (int i = 0; i < nr; ++i) m.chem[i] = d->chem_activated[i];
     copy_in(m.plog_ptr, d->plog_ptr, nr + 1);
     copy_in(m.plogP, d->plog_P, d->plog_ptr[nr]); copy_in(m.plogA, d->plog_A, d->plog_ptr[nr]);
     copy_in(m.plogb, d->plog_beta, d->plog_ptr[nr]); copy_in(m.plogTa, d->plog_Ta, d->plog_ptr[nr]);

@@ -49,6 +49,8 @@ int validate(const pyjac_mech_desc* d, std::string& err) {
       }
     }
     if (ty <= PYJAC_FALLOFF_SRI && !(d->A[i] > 0.0)) MECH_FAIL("reaction " << i << ": A must be > 0 (ln A is tabulated)");
+    if (d->chem_activated && d->chem_activated[i] && !(ty >= PYJAC_FALLOFF_LINDEMANN && ty <= PYJAC_FALLOFF_SRI))
+      MECH_FAIL("reaction " << i << ": chem_activated needs a falloff type");
     if (ty >= PYJAC_FALLOFF_LINDEMANN && ty <= PYJAC_FALLOFF_SRI && !(d->low_A[i] > 0.0))
       MECH_FAIL("reaction " << i << ": low-pressure A must be > 0");
     if (d->collider[i] < -1 || d->collider[i] >= ns) MECH_FAIL("reaction " << i << ": collider index out of range");
@@ -287,8 +289,11 @@ int build_host_tables(const pyjac_mech_desc* d, bool approx, HostTables& h, std:
     const bool rev = d->reversible[i] != 0;
     const bool tb = ty >= PYJAC_THIRD_BODY && ty <= PYJAC_FALLOFF_SRI;
     const bool falloff = ty >= PYJAC_FALLOFF_LINDEMANN && ty <= PYJAC_FALLOFF_SRI;
-    h.lnA[r] = (ty <= PYJAC_FALLOFF_SRI) ? std::log(d->A[i]) : 0.0;
-    h.beta[r] = d->beta[i]; h.Ta[r] = d->Ta[i];
+    // chemically activated (R8): the rate constant of the rates of progress is k_0, so the Arrhenius
+    // columns take the LOW parameters and the falloff record the high-pressure ones (the kernel inverts the ratio)
+    const bool chem = falloff && d->chem_activated && d->chem_activated[i];
+    h.lnA[r] = (ty <= PYJAC_FALLOFF_SRI) ? std::log(chem ? d->low_A[i] : d->A[i]) : 0.0;
+    h.beta[r] = chem ? d->low_beta[i] : d->beta[i]; h.Ta[r] = chem ? d->low_Ta[i] : d->Ta[i];
     const int nre = d->reac_ptr[i + 1] - d->reac_ptr[i], npr = d->prod_ptr[i + 1] - d->prod_ptr[i];
     int snu = 0, order_f = 0, order_r = 0;
     bool simple = true;
@@ -314,6 +319,7 @@ int build_host_tables(const pyjac_mech_desc* d, bool approx, HostTables& h, std:
                (nre << INFO_NREAC_SHIFT) | (npr << INFO_NPROD_SHIFT) | (simple ? INFO_SIMPLE : 0) |
                (order_f << INFO_OF_SHIFT) | (order_r << INFO_OR_SHIFT);
     if (ty == PYJAC_FALLOFF_TROE && d->troe_has_T2[i]) info |= INFO_T2;
+    if (chem) info |= INFO_CHEM;
     h.info[r] = info;
     // slots: 0 = T column, 1 = E column, then one per role
     int slot = h.slot_base[r] + 2;
@@ -339,7 +345,8 @@ int build_host_tables(const pyjac_mech_desc* d, bool approx, HostTables& h, std:
     h.slot_base.push_back(slot);
     if (falloff) {
       h.aux[r] = (int)(h.fall.size() / 12);
-      double f[12] = {std::log(d->low_A[i]), d->low_beta[i], d->low_Ta[i], 0, 0, 0, 0, 0, 0, 0, 0, 0};
+      double f[12] = {std::log(chem ? d->A[i] : d->low_A[i]), chem ? d->beta[i] : d->low_beta[i], chem ? d->Ta[i] : d->low_Ta[i],
+                      0, 0, 0, 0, 0, 0, 0, 0, 0};
       if (ty == PYJAC_FALLOFF_TROE) for (int j = 0; j < 4; ++j) f[4 + j] = d->troe[4 * i + j];
       if (ty == PYJAC_FALLOFF_SRI) for (int j = 0; j < 5; ++j) f[4 + j] = d->sri[5 * i + j];
       h.fall.insert(h.fall.end(), f, f + 12);

@@ -18,6 +18,7 @@ constexpr int INFO_REV = 1 << 3;     // reversible
 constexpr int INFO_T2 = 1 << 4;      // Troe has T2
 constexpr int INFO_ADEF = 1 << 5;    // default third-body efficiency is 1 (mixture); 0: single collider
 constexpr int INFO_SIMPLE = 1 << 6;  // every stoichiometric coefficient is 1 (fast path, no powers)
+constexpr int INFO_CHEM = 1 << 7;    // chemically-activated falloff: Arrhenius columns hold k_0, the falloff record k_inf
 constexpr int INFO_SNU_SHIFT = 8;    // bits 8-11: sum(nu) + 8
 constexpr int INFO_NREAC_SHIFT = 12; // bits 12-13: number of reactant entries
 constexpr int INFO_NPROD_SHIFT = 14; // bits 14-15: number of product entries

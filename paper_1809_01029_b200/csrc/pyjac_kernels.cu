@@ -458,16 +458,23 @@ __device__ __forceinline__ void phases01(const DevMech& m, Tile<S, JAC>& t, int 
           for (int q = 0; q < 5; ++q) { const double2 v2 = __ldg(f2 + q); fp[2 * q] = v2.x; fp[2 * q + 1] = v2.y; }
           asm volatile("" :: "d"(fp[0]), "d"(fp[1]), "d"(fp[2]), "d"(fp[4]), "d"(fp[5]), "d"(fp[6]), "d"(fp[7]), "d"(fp[8]));
         }
+        // falloff: the record holds k_0 and lnkf = ln k_inf.  Chemically activated (R8): the record holds k_inf and
+        // lnkf = ln k_0, so the ratio k_0 / k_inf and its temperature derivative change sign in the exponent, and
+        // c = F / (1 + Pr) instead of F Pr / (1 + Pr).
+        const bool chem = (info & INFO_CHEM) != 0;
         const double b0 = fp[1], Ta0 = fp[2];
-        const double k0_kinf = exp(fp[0] + b0 * lnT - Ta0 * invT - lnkf);
+        const double lnrat = fp[0] + b0 * lnT - Ta0 * invT - lnkf;
+        const double k0_kinf = exp(chem ? -lnrat : lnrat);
         const double Pr = k0_kinf * M;
         const Blend bl = blend(type, info & INFO_T2, fp, T, invT, lnT, Pr);
         const double i1p = 1.0 / (1.0 + Pr);
-        c = bl.F * Pr * i1p;
-        const double dc_dPr = bl.F * i1p * i1p + Pr * i1p * bl.dF_dPr;
-        const double dPr_dT = Pr * (b0 - rx_beta + (Ta0 - rx_Ta) * invT) * invT;
+        const double cF = chem ? i1p : Pr * i1p;            // dc/dF
+        c = bl.F * cF;
+        const double dc_dPr = (chem ? -bl.F : bl.F) * i1p * i1p + cF * bl.dF_dPr;
+        const double dlnrat_dT = (b0 - rx_beta + (Ta0 - rx_Ta) * invT) * invT;
+        const double dPr_dT = Pr * (chem ? -dlnrat_dT : dlnrat_dT);
         X = dc_dPr * k0_kinf * Rn;
-        GT = (dc_dPr * dPr_dT + Pr * i1p * bl.dF_dT) * Rn + c * dRdT;
+        GT = (dc_dPr * dPr_dT + cF * bl.dF_dT) * Rn + c * dRdT;
         MdcdM_R = Pr * dc_dPr * Rn;
       }
     }

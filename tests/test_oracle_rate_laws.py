@@ -156,3 +156,43 @@ def test_zero_concentration_is_safe():
     assert np.isfinite(J).all()
     rowmax = np.abs(Jc).max(axis=1, keepdims=True)
     assert np.all(np.abs(J - Jc) <= np.maximum(1e-8 * np.abs(Jc), 1e-12 * rowmax))
+
+
+# ---- chemically-activated bimolecular reactions (R8) ---------------------------------------
+def _two(**rx):
+    """A + B <=> C test bed (the bimolecular form chemical activation applies to); bath N last."""
+    mb = MechBuilder()
+    mb.add_species(10.0, CP(2.6, 15000.0, 5.0)); mb.add_species(20.0, CP(3.0, 9000.0, 4.0))
+    mb.add_species(30.0, CP(3.8, 4000.0, 6.0)); mb.add_species(28.0, CP(3.5, -1000.0, 6.5))
+    mb.add_reaction({0: 1, 1: 1}, {2: 1}, **rx)
+    return mb.build()
+
+
+@pytest.mark.parametrize("form", [dict(type=mg.FALLOFF_LINDEMANN), dict(type=mg.FALLOFF_TROE, troe=(0.6, 200.0, 1800.0, 5000.0)),
+                                  dict(type=mg.FALLOFF_SRI, sri=(0.8, 300.0, 2000.0, 1.2, 0.1))])
+def test_chem_activated_is_falloff_over_third_body_concentration(form):
+    """k_chem = k_0 F / (1 + Pr) and k_falloff = k_inf F Pr / (1 + Pr) with Pr = k_0 [M] / k_inf: k_chem [M] = k_falloff.
+    Ties the new form to the falloff forms already pinned above (same F: it depends on T and Pr only)."""
+    eff = {0: 2.0, 2: 0.5}
+    fall = _run(_two(low=LOW, eff=eff, **form, **ARR))
+    chem = _run(_two(low=LOW, eff=eff, chem_activated=True, **form, **ARR))
+    M = fall[1]["M"][0]
+    assert chem[1]["M"][0] == M and chem[1]["Pr"][0] == pytest.approx(fall[1]["Pr"][0], rel=1e-15)
+    assert chem[1]["F"][0] == pytest.approx(fall[1]["F"][0], rel=1e-15)
+    np.testing.assert_allclose(chem[2] * M, fall[2], rtol=1e-13)
+    T = 1300.0
+    k0 = LOW[0] * T ** LOW[1] * math.exp(-LOW[2] / T)
+    assert chem[1]["kf"][0] == pytest.approx(k0, rel=1e-14)            # the rate constant of the rates of progress is k_0
+    assert chem[1]["c"][0] == pytest.approx(chem[1]["F"][0] / (1.0 + chem[1]["Pr"][0]), rel=1e-15)
+
+
+def test_chem_activated_limits():
+    """Pr -> 0: k -> k_0 (an elementary reaction with the low-pressure parameters); Pr -> inf: k [M] -> k_inf."""
+    lo = _run(_two(type=mg.FALLOFF_LINDEMANN, low=LOW, chem_activated=True, A=4e43, beta=0.3, Ta=22000.0))   # k_inf huge
+    elem = _run(_two(A=LOW[0], beta=LOW[1], Ta=LOW[2]))
+    np.testing.assert_allclose(lo[2], elem[2], rtol=1e-12)
+    np.testing.assert_allclose(lo[3], elem[3], rtol=1e-9, atol=1e-30 * np.abs(elem[3]).max())
+    hi = _run(_two(type=mg.FALLOFF_LINDEMANN, low=(6e45, -1.0, 20000.0), chem_activated=True, **ARR))        # k_0 huge
+    T = 1300.0
+    kinf = ARR["A"] * T ** ARR["beta"] * math.exp(-ARR["Ta"] / T)
+    assert hi[1]["c"][0] * hi[1]["kf"][0] * hi[1]["M"][0] == pytest.approx(kinf, rel=1e-12)
