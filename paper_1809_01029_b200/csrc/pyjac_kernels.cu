@@ -808,12 +808,46 @@ jacobian_kernel(const DevMech m, const DevPlan pl, int mode, int64_t n_states, i
   const double N = red_sum<S>(t.red, 0, s);
   const double fT = -N / D;
   TICK(3);
+  const double cL = t.ck[L * S + s];
+  // a10: the four corner entries from the phase-1 reductions (R4-7), by the last warp (it has no item of
+  // the second pass).  With several states per CTA they are done BEFORE the gathers (that warp joins the dynamically
+  // scheduled gather a little late instead of leaving a serial tail); at one state per CTA the tail measured shorter.
+  auto corners = [&]() {
+    if ((tid >> 5) == NW - 1 && (tid & 31) < S && valid) {      // the last warp: it has no item of the second pass
+      const double Ctot = t.sc[SC_CTOT * S + s];
+      const double Ssum = red_sum<S>(t.red, 1, s);
+      const double AT = red_sum<S>(t.red, 2, s), BT = red_sum<S>(t.red, 3, s), AE = red_sum<S>(t.red, 4, s), BE = red_sum<S>(t.red, 5, s);
+      const double sumcw = red_sum<S>(t.red, 6, s);
+      const double iV = 1.0 / V;
+      const double dN_dT = AT * iV + sumcw;
+      const double dD_dT = t.sc[SC_DDDT * S + s] - cL * Ctot / T;
+      const double JTT = -(dN_dT + fT * dD_dT) / D;
+      const double dS_dT = BT * iV;
+      double dN_dE, dD_dE, dS_dE, JET, JEE, JTE;
+      if (mode == PYJAC_CONP) {
+        const double fE = V * (T * R_GAS / Pp * Ssum + fT / T);
+        dN_dE = (AE - N) * iV; dD_dE = -(D - Ctot * cL) * iV; dS_dE = (BE - Ssum) * iV;
+        JTE = -(dN_dE + fT * dD_dE) / D;
+        JET = V * (T * R_GAS / Pp * dS_dT + JTT / T) + V * (R_GAS * Ssum / Pp - fT / (T * T));
+        JEE = V * (T * R_GAS / Pp * dS_dE + JTE / T) + fE * iV;
+      } else {
+        dN_dE = AE * iV; dD_dE = cL / (R_GAS * T); dS_dE = BE * iV;
+        JTE = -(dN_dE + fT * dD_dE) / D;
+        JET = T * R_GAS * dS_dT + Pp / T * JTT + R_GAS * Ssum - Pp * fT / (T * T);
+        JEE = T * R_GAS * dS_dE + Pp / T * JTE + fT / T;
+      }
+      out[obase + (int64_t)pl.d_pos[0] * tile] = JTT;
+      out[obase + (int64_t)pl.d_pos[1] * tile] = JTE;
+      out[obase + (int64_t)pl.d_pos[2] * tile] = JET;
+      out[obase + (int64_t)pl.d_pos[3] * tile] = JEE;
+    }
+  };
+  if (S > 1) corners();
   const double* __restrict__ P = t.P;
   // The T/E-row gather goes FIRST: it has few, long units; warps that finish it early move on to the many short
   // units of the species rows (no barrier in between), so its latency tail is hidden behind them.
   // a10: T and E rows, species columns: gather over reactions with the per-state weights dE~_i, dn~_i
   //   J[T][j] = -(sum_i dE~_i g_ij + f_T (c_j - c_Ns)) / (D V);  J[E][j] = cS sum_i dn~_i g_ij + cT J[T][j]
-  const double cL = t.ck[L * S + s];
   const double iDV = 1.0 / (D * V);
   const double cS = mode == PYJAC_CONP ? T * R_GAS / Pp : T * R_GAS / V;
   const double cT = mode == PYJAC_CONP ? V / T : Pp / T;
@@ -895,36 +929,8 @@ jacobian_kernel(const DevMech m, const DevPlan pl, int mode, int64_t n_states, i
       }
     }
   }
+  if (S == 1) corners();
   TICK(5);
-  // a10: the four corner entries from the phase-1 reductions (R4-7)
-  if (tid < S && valid) {
-    const double Ctot = t.sc[SC_CTOT * S + s];
-    const double Ssum = red_sum<S>(t.red, 1, s);
-    const double AT = red_sum<S>(t.red, 2, s), BT = red_sum<S>(t.red, 3, s), AE = red_sum<S>(t.red, 4, s), BE = red_sum<S>(t.red, 5, s);
-    const double sumcw = red_sum<S>(t.red, 6, s);
-    const double iV = 1.0 / V;
-    const double dN_dT = AT * iV + sumcw;
-    const double dD_dT = t.sc[SC_DDDT * S + s] - cL * Ctot / T;
-    const double JTT = -(dN_dT + fT * dD_dT) / D;
-    const double dS_dT = BT * iV;
-    double dN_dE, dD_dE, dS_dE, JET, JEE, JTE;
-    if (mode == PYJAC_CONP) {
-      const double fE = V * (T * R_GAS / Pp * Ssum + fT / T);
-      dN_dE = (AE - N) * iV; dD_dE = -(D - Ctot * cL) * iV; dS_dE = (BE - Ssum) * iV;
-      JTE = -(dN_dE + fT * dD_dE) / D;
-      JET = V * (T * R_GAS / Pp * dS_dT + JTT / T) + V * (R_GAS * Ssum / Pp - fT / (T * T));
-      JEE = V * (T * R_GAS / Pp * dS_dE + JTE / T) + fE * iV;
-    } else {
-      dN_dE = AE * iV; dD_dE = cL / (R_GAS * T); dS_dE = BE * iV;
-      JTE = -(dN_dE + fT * dD_dE) / D;
-      JET = T * R_GAS * dS_dT + Pp / T * JTT + R_GAS * Ssum - Pp * fT / (T * T);
-      JEE = T * R_GAS * dS_dE + Pp / T * JTE + fT / T;
-    }
-    out[obase + (int64_t)pl.d_pos[0] * tile] = JTT;
-    out[obase + (int64_t)pl.d_pos[1] * tile] = JTE;
-    out[obase + (int64_t)pl.d_pos[2] * tile] = JET;
-    out[obase + (int64_t)pl.d_pos[3] * tile] = JEE;
-  }
 }
 
 template <int S> int launch_source_S(const DevMech& m, const LaunchCfg& cfg, int mode, int64_t n, int64_t tile,
