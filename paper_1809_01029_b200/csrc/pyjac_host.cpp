@@ -106,13 +106,15 @@ void build_gather(const std::vector<std::vector<int32_t>>& lists, int stride, in
       segs.push_back({i, a, b - a, -2 - g.n_part++});
     }
   }
-  std::stable_sort(segs.begin(), segs.end(), [](const Seg& a, const Seg& b) { return a.len > b.len; });
+  // pieces of split lists (their sums go to shared memory) never join the narrow tail: its store path has no such case
+  auto eff_len = [&](const Seg& a) { return a.target <= -2 ? std::max(a.len, narrow_len + 1) : a.len; };
+  std::stable_sort(segs.begin(), segs.end(), [&](const Seg& a, const Seg& b) { return eff_len(a) > eff_len(b); });
   const int ns_ = (int)segs.size();
   // Wide super-groups of ELL_W segments first; the tail of short segments (<= narrow_len entries) goes into NARROW
   // super-groups of ELL_W_NARROW segments: a thread then owns 4x as many segments of a unit, so the fixed cost of a
   // unit (work counter, metadata, one exposed round trip for the first entries) is paid a quarter as often.
   int i_n = ns_;
-  for (int i = 0; i < ns_; ++i) if (segs[i].len <= narrow_len) { i_n = i; break; }
+  for (int i = 0; i < ns_; ++i) if (eff_len(segs[i]) <= narrow_len) { i_n = i; break; }
   g.n_wide = (i_n + ELL_W - 1) / ELL_W;
   const int rest = std::max(0, ns_ - g.n_wide * ELL_W);
   g.n_sg = g.n_wide + (rest + ELL_W_NARROW - 1) / ELL_W_NARROW;
@@ -161,7 +163,8 @@ void build_gather(const std::vector<std::vector<int32_t>>& lists, int stride, in
   int off = 0;
   for (int sg = 0; sg < g.n_sg; ++sg) {
     const int i0 = group_first(sg), EW = group_size(sg);
-    const int width = segs[i0].len;                   // sorted: the first segment of the group is the longest
+    int width = 0;                                    // the longest segment of the group
+    for (int w = 0; w < EW && i0 + w < ns_; ++w) width = std::max(width, segs[i0 + w].len);
     g.sg_meta.push_back(off); g.sg_meta.push_back(width);
     for (int p = 0; p < width; ++p)
       for (int w0 = 0; w0 < EW; w0 += 16) {

@@ -885,17 +885,21 @@ jacobian_kernel(const DevMech m, const DevPlan pl, int mode, int64_t n_states, i
       const uint32_t ent = (uint32_t)__ldg(e);
       v[0] += apply_sign(P[(ent & ~SIGN_BIT) * S + s], ent);
     };
-    auto posJ = [&](int slot) { return __ldg(pl.j_pos + slot); };
+    double* __restrict__ out_s = out + obase;
+    auto posJ = [&](int slot) { const int p = __ldg(pl.j_pos + slot); return valid || p < 0 ? p : -1; };   // ragged tail: store nothing
     auto storeJ = [&](int, int pos, const double (&v)[1]) {
-      if (pos >= 0) { if (valid) st_out(out + obase + (int64_t)pos * tile, v[0]); }
+      if (pos >= 0) st_out(out_s + (int64_t)pos * tile, v[0]);
       else if (pos <= -2) t.part[(-2 - pos) * S + s] = v[0];
+    };
+    auto storeN = [&](int, int pos, const double (&v)[1]) {      // narrow tail: whole lists only (see build_gather)
+      if (pos >= 0) st_out(out_s + (int64_t)pos * tile, v[0]);
     };
     const int2* metaJ = t.meta + m.cplan.n_sg;
     const int n_wide = pl.jplan.n_wide;
     gather<S, 1, 1, PYJAC_UJ, PYJAC_UNJ, ELL_W, int>(pl.jplan.ell_ent, metaJ, n_wide, 0, cnt + CNT_J, accJ, posJ, storeJ, side);
     // the narrow tail (lists of one or two entries: most nonzeros of a sparse mechanism): 16 segments per thread
     gather<S, 1, 1, 16, 1, ELL_W_NARROW, int>(pl.jplan.ell_ent, metaJ + n_wide, pl.jplan.n_sg - n_wide, n_wide * ELL_W,
-                                              cnt + CNT_J2, accJ, posJ, storeJ, side);
+                                              cnt + CNT_J2, accJ, posJ, storeN, side);
   }
   if (DENSE)                                      // whatever is left of the zero fill
     for (int z = next_chunk(cnt + CNT_Z); z < n_zslices; z = next_chunk(cnt + CNT_Z)) zero_slice(z);
