@@ -79,6 +79,10 @@ typedef struct {
                                                         chemically-activated bimolecular reaction (PAPER.md L143,
                                                         DESIGN.md R8): (A, beta, Ta) = k_inf and low_* = k_0 as for
                                                         falloff, P_r = k_0 [M] / k_inf, but k = k_0 F / (1 + P_r)   */
+  const double *rev_A, *rev_beta, *rev_Ta;           /* [Nr] each, or all NULL (= none).  rev_A[i] > 0 on a reversible
+                                                        reaction: explicit reverse rate constant k_r = A T^beta
+                                                        exp(-Ta/T) instead of k_f / K_c (R9); not for P-Log
+                                                        and Chebyshev reactions                                    */
 } pyjac_mech_desc;
 
 /* Step a0 (one-time, host): validate, sort reactions by type, pack device tables, build the exact
@@ -87,7 +91,7 @@ typedef struct {
  * PYJAC_EMECH: Ns < 2, Nr < 1, index out of range, nu outside 1..3, more than 3 species per side,
  * A <= 0, W <= 0, tmid <= 0, negative efficiency, P-Log with < 2 points or non-ascending pressures,
  * empty Chebyshev grid or Tmin >= Tmax or Pmin >= Pmax, unknown type, chem_activated on a reaction that is not of a
- * falloff type.  PYJAC_ECUDA: no such device.
+ * falloff type, explicit reverse parameters on an irreversible, P-Log or Chebyshev reaction or rev_A < 0.  PYJAC_ECUDA: no such device.
  * cuda_device = -1 builds a HOST-ONLY handle (pyjac_mech_dims / pyjac_sparsity work; every compute
  * call fails with PYJAC_ECUDA) -- there is no CPU compute path.  The compute calls launch on the
  * caller's current device, which must be the handle's device. */

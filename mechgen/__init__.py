@@ -11,6 +11,6 @@ A mechanism is a plain dict of numpy arrays ("desc arrays") whose keys mirror th
 from .mechanism import (CONFIGS, R_GAS, P_ATM, ELEMENTARY, THIRD_BODY, FALLOFF_LINDEMANN,
                         FALLOFF_TROE, FALLOFF_SRI, PLOG, CHEBYSHEV, CONP, CONV, CSR, CSC,
                         make_mechanism, config_mechanism, config_states, make_states, MechBuilder)
-from .hand import hand_ab, hand_four, hand_unbalanced, hand_all_types, hand_chem_activated
+from .hand import hand_ab, hand_four, hand_unbalanced, hand_all_types, hand_chem_activated, hand_rev_explicit
 
 __all__ = [n for n in dir() if not n.startswith("_")]

@@ -131,3 +131,26 @@ def hand_chem_activated():
                         chem_activated=chem, **hi)
     mb.add_reaction({C: 1}, {D: 1}, A=4.0e7, beta=0.2, Ta=6000.0, rev=True)
     return mb.build()
+
+
+def hand_rev_explicit():
+    """Five species and bath N (last): explicit reverse Arrhenius parameters (k_r given, not k_f / K_c) on an
+    elementary, a third-body, a Troe falloff and a chemically-activated Lindemann reaction, next to K_c-based ones."""
+    mb = MechBuilder()
+    W = [10.0, 10.0, 20.0, 20.0, 30.0, 28.0]
+    th = [_const_cp(2.6, 1.5e4, 5.0), _const_cp(2.9, 1.1e4, 5.5), _const_cp(3.6, 2.0e3, 7.0), _const_cp(3.9, 1.0e3, 7.5),
+          _const_cp(4.4, -2.0e3, 8.0), _const_cp(3.5, -1.0e3, 6.5)]
+    for w, t in zip(W, th):
+        mb.add_species(w, t)
+    A, B, C, D, E = 0, 1, 2, 3, 4
+    mb.add_reaction({A: 1, B: 1}, {C: 1}, A=2.0e9, beta=0.3, Ta=1500.0, rev=True, rev_params=(5.0e11, -0.2, 9000.0))
+    mb.add_reaction({A: 2}, {D: 1}, A=5.0e8, beta=-0.5, Ta=500.0, rev=True, type=THIRD_BODY, eff={C: 3.0, E: 0.5},
+                    rev_params=(2.0e10, 0.1, 7000.0))
+    mb.add_reaction({A: 1, C: 1}, {E: 1}, A=3.0e10, beta=0.4, Ta=2500.0, rev=True, type=FALLOFF_TROE,
+                    low=(7.0e11, -0.6, 1200.0), troe=(0.6, 200.0, 1800.0, 5000.0), eff={D: 2.0},
+                    rev_params=(8.0e12, 0.0, 15000.0))
+    mb.add_reaction({B: 1, D: 1}, {E: 1}, A=1.0e10, beta=0.2, Ta=1000.0, rev=True, type=FALLOFF_LINDEMANN,
+                    low=(3.0e11, -0.4, 800.0), chem_activated=True, rev_params=(4.0e12, -0.3, 12000.0))
+    mb.add_reaction({C: 1}, {D: 1}, A=4.0e7, beta=0.2, Ta=6000.0, rev=True)
+    mb.add_reaction({A: 1, B: 1}, {D: 1}, A=6.0e8, beta=0.1, Ta=2000.0, rev=True)
+    return mb.build()

@@ -43,12 +43,13 @@ class MechBuilder:
         return len(self.W) - 1
 
     def add_reaction(self, reac, prod, A=1.0, beta=0.0, Ta=0.0, rev=True, type=ELEMENTARY, eff=None,
-                     collider=-1, low=None, troe=None, sri=None, plog=None, cheb=None, chem_activated=False):
+                     collider=-1, low=None, troe=None, sri=None, plog=None, cheb=None, chem_activated=False, rev_params=None):
         """chem_activated (falloff types only): chemically-activated bimolecular reaction; (A, beta, Ta) stay the
-        high-pressure limit k_inf and `low` the low-pressure limit k_0, but k = k_0 F / (1 + P_r)."""
+        high-pressure limit k_inf and `low` the low-pressure limit k_0, but k = k_0 F / (1 + P_r).
+        rev_params = (A, beta, Ta): explicit reverse Arrhenius parameters, k_r = A T^beta exp(-Ta/T) instead of k_f / K_c."""
         self.reactions.append(dict(reac=dict(reac), prod=dict(prod), A=A, beta=beta, Ta=Ta, rev=rev,
                                    type=type, eff=dict(eff or {}), collider=collider, low=low,
-                                   troe=troe, sri=sri, plog=plog, cheb=cheb, chem_activated=bool(chem_activated)))
+                                   troe=troe, sri=sri, plog=plog, cheb=cheb, chem_activated=bool(chem_activated), rev_params=rev_params))
         return len(self.reactions) - 1
 
     def build(self):
@@ -122,6 +123,10 @@ class MechBuilder:
         d["cheb_Pmin"] = np.ascontiguousarray(lim[:, 2]); d["cheb_Pmax"] = np.ascontiguousarray(lim[:, 3])
         d["cheb_coef"] = np.array(coef, np.float64)
         d["chem_activated"] = np.array([1 if r["chem_activated"] else 0 for r in self.reactions], np.uint8)
+        rp = np.array([r["rev_params"] if r["rev_params"] is not None else (0.0, 0.0, 0.0) for r in self.reactions],
+                      np.float64).reshape(nr, 3)
+        d["rev_A"] = np.ascontiguousarray(rp[:, 0]); d["rev_beta"] = np.ascontiguousarray(rp[:, 1])
+        d["rev_Ta"] = np.ascontiguousarray(rp[:, 2])
         return d
 
 

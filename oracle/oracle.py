@@ -24,7 +24,7 @@ DESC_FIELDS = [
     ("plog_ptr", _I), ("plog_P", _D), ("plog_A", _D), ("plog_beta", _D), ("plog_Ta", _D),
     ("cheb_ptr", _I), ("cheb_nT", _I), ("cheb_nP", _I),
     ("cheb_Tmin", _D), ("cheb_Tmax", _D), ("cheb_Pmin", _D), ("cheb_Pmax", _D), ("cheb_coef", _D),
-    ("chem_activated", _U),
+    ("chem_activated", _U), ("rev_A", _D), ("rev_beta", _D), ("rev_Ta", _D),
 ]
 _NP = {_D: np.float64, _I: np.int32, _U: np.uint8}
 

@@ -62,6 +62,7 @@ struct Mech {
     std::vector<double> lowA, lowb, lowTa, troe;
     std::vector<int> troe_t2;
     std::vector<int> chem;                   // chemically-activated falloff (reading R8): k = k_0 F / (1 + P_r)
+    std::vector<double> revA, revb, revTa;   // explicit reverse Arrhenius parameters (reading R9); revA = 0: k_r = k_f / K_c
     std::vector<double> sri;
     std::vector<int> plog_ptr;
     std::vector<double> plogP, plogA, plogb, plogTa;
@@ -245,6 +246,11 @@ void eval_source(const Mech& m, int mode, const T* phi, const T& param, T* f, In
             if (snu < 0) Kc = Kc / ipow(pf, -snu);
             kr = kf / Kc;
             dlnKc = dh / (R_GAS * Tt * Tt) - double(snu) / Tt;
+            if (m.revA[i] > 0.0) {      // explicit reverse parameters (reading R9): K_c plays no role; the slot keeps k_f / k_r
+                kr = exp(std::log(m.revA[i]) + m.revb[i] * lnT - m.revTa[i] / Tt);
+                Kc = kf / kr;
+                dlnKc = lam_f - (m.revb[i] + m.revTa[i] / Tt) / Tt;
+            }
         }
         w.kr[i] = kr; w.Kc[i] = Kc; w.dlnKc_dT[i] = dlnKc;
         // a6: rates of progress by repeated multiplication
@@ -469,6 +475,7 @@ struct orc_desc {
     const int32_t *cheb_ptr, *cheb_nT, *cheb_nP;
     const double *cheb_Tmin, *cheb_Tmax, *cheb_Pmin, *cheb_Pmax, *cheb_coef;
     const uint8_t* chem_activated;            // [Nr] or NULL
+    const double *rev_A, *rev_beta, *rev_Ta;  // [Nr] or NULL; rev_A > 0: explicit reverse rate constant
 };
 
 void* orc_create2(const orc_desc* d, int approx) {
@@ -489,6 +496,8 @@ void* orc_create2(const orc_desc* d, int approx) {
     copy_in(m.lowA, d->low_A, nr); copy_in(m.lowb, d->low_beta, nr); copy_in(m.lowTa, d->low_Ta, nr);
     copy_in(m.troe, d->troe, 4 * nr); m.troe_t2.resize(nr); for (int i = 0; i < nr; ++i) m.troe_t2[i] = d->troe_has_T2[i];
     copy_in(m.sri, d->sri, 5 * nr);
+    m.revA.assign(nr, 0.0); m.revb.assign(nr, 0.0); m.revTa.assign(nr, 0.0);
+    if (d->rev_A) { copy_in(m.revA, d->rev_A, nr); copy_in(m.revb, d->rev_beta, nr); copy_in(m.revTa, d->rev_Ta, nr); }
     m.chem.assign(nr, 0); if (d->chem_activated) for (int i = 0; i < nr; ++i) m.chem[i] = d->chem_activated[i];
     copy_in(m.plog_ptr, d->plog_ptr, nr + 1);
     copy_in(m.plogP, d->plog_P, d->plog_ptr[nr]); copy_in(m.plogA, d->plog_A, d->plog_ptr[nr]);

@@ -30,7 +30,7 @@ _FIELDS = [
     ("plog_ptr", _I), ("plog_P", _D), ("plog_A", _D), ("plog_beta", _D), ("plog_Ta", _D),
     ("cheb_ptr", _I), ("cheb_nT", _I), ("cheb_nP", _I),
     ("cheb_Tmin", _D), ("cheb_Tmax", _D), ("cheb_Pmin", _D), ("cheb_Pmax", _D), ("cheb_coef", _D),
-    ("chem_activated", _U),
+    ("chem_activated", _U), ("rev_A", _D), ("rev_beta", _D), ("rev_Ta", _D),
 ]
 _NP = {_D: np.float64, _I: np.int32, _U: np.uint8}
 
@@ -86,8 +86,8 @@ def make_desc(mech):
     keep = []
     d.n_species = int(mech["n_species"]); d.n_reactions = int(mech["n_reactions"])
     for name, ct in _FIELDS:
-        if name == "chem_activated" and name not in mech:
-            continue                                     # optional: NULL = no chemically-activated reaction
+        if name in ("chem_activated", "rev_A", "rev_beta", "rev_Ta") and name not in mech:
+            continue                                     # optional fields: NULL = none
         a = np.ascontiguousarray(mech[name], dtype=_NP[ct])
         if a.size == 0:
             a = np.zeros(1, dtype=_NP[ct])

@@ -87,7 +87,7 @@ int pyjac_mech_create_ex(const pyjac_mech_desc* desc, int cuda_device, uint32_t 
     d.n_part_jac = h.n_part_jac; d.n_part_src = h.n_part_src;
 #define UP(field) if (int r_ = m->upload(h.field, &d.field)) return r_;
     UP(nasa) UP(wr) UP(lnA) UP(beta) UP(Ta) UP(dn) UP(info) UP(aux) UP(sp) UP(eff_ptr) UP(eff_sp) UP(eff_d)
-    UP(slot_base) UP(fall) UP(plog_ptr) UP(plog_P) UP(plog_lnP) UP(plog_lnA) UP(plog_b) UP(plog_Ta)
+    UP(slot_base) UP(rev_par) UP(fall) UP(plog_ptr) UP(plog_P) UP(plog_lnP) UP(plog_lnA) UP(plog_b) UP(plog_Ta)
     UP(cheb_meta) UP(cheb_lim) UP(cheb_coef)
 #undef UP
     if (int r_ = m->upload_plan(h.cplan, h.jplan.n_part, &d.cplan)) return r_;      // C partials follow the J partials

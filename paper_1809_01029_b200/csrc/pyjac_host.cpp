@@ -51,6 +51,11 @@ int validate(const pyjac_mech_desc* d, std::string& err) {
     if (ty <= PYJAC_FALLOFF_SRI && !(d->A[i] > 0.0)) MECH_FAIL("reaction " << i << ": A must be > 0 (ln A is tabulated)");
     if (d->chem_activated && d->chem_activated[i] && !(ty >= PYJAC_FALLOFF_LINDEMANN && ty <= PYJAC_FALLOFF_SRI))
       MECH_FAIL("reaction " << i << ": chem_activated needs a falloff type");
+    if (d->rev_A && d->rev_A[i] != 0.0) {
+      if (!(d->rev_A[i] > 0.0) || !d->rev_beta || !d->rev_Ta) MECH_FAIL("reaction " << i << ": explicit reverse parameters need rev_A > 0, rev_beta and rev_Ta");
+      if (!d->reversible[i] || ty == PYJAC_PLOG || ty == PYJAC_CHEBYSHEV)
+        MECH_FAIL("reaction " << i << ": explicit reverse parameters need a reversible reaction that is not P-Log / Chebyshev");
+    }
     if (ty >= PYJAC_FALLOFF_LINDEMANN && ty <= PYJAC_FALLOFF_SRI && !(d->low_A[i] > 0.0))
       MECH_FAIL("reaction " << i << ": low-pressure A must be > 0");
     if (d->collider[i] < -1 || d->collider[i] >= ns) MECH_FAIL("reaction " << i << ": collider index out of range");
@@ -323,6 +328,11 @@ int build_host_tables(const pyjac_mech_desc* d, bool approx, HostTables& h, std:
                (order_f << INFO_OF_SHIFT) | (order_r << INFO_OR_SHIFT);
     if (ty == PYJAC_FALLOFF_TROE && d->troe_has_T2[i]) info |= INFO_T2;
     if (chem) info |= INFO_CHEM;
+    if (rev && d->rev_A && d->rev_A[i] > 0.0) {
+      info |= INFO_REVX;
+      if (h.rev_par.empty()) h.rev_par.assign((size_t)nr * 3, 0.0);
+      h.rev_par[3 * r] = std::log(d->rev_A[i]); h.rev_par[3 * r + 1] = d->rev_beta[i]; h.rev_par[3 * r + 2] = d->rev_Ta[i];
+    }
     h.info[r] = info;
     // slots: 0 = T column, 1 = E column, then one per role
     int slot = h.slot_base[r] + 2;

@@ -19,6 +19,7 @@ constexpr int INFO_T2 = 1 << 4;      // Troe has T2
 constexpr int INFO_ADEF = 1 << 5;    // default third-body efficiency is 1 (mixture); 0: single collider
 constexpr int INFO_SIMPLE = 1 << 6;  // every stoichiometric coefficient is 1 (fast path, no powers)
 constexpr int INFO_CHEM = 1 << 7;    // chemically-activated falloff: Arrhenius columns hold k_0, the falloff record k_inf
+constexpr int INFO_REVX = 1 << 24;   // explicit reverse Arrhenius parameters (rev_par)
 constexpr int INFO_SNU_SHIFT = 8;    // bits 8-11: sum(nu) + 8
 constexpr int INFO_NREAC_SHIFT = 12; // bits 12-13: number of reactant entries
 constexpr int INFO_NPROD_SHIFT = 14; // bits 14-15: number of product entries
@@ -62,6 +63,7 @@ struct HostTables {
   std::vector<int32_t> eff_ptr, eff_sp;      // [nr+1], entries with alpha != default only
   std::vector<double> eff_d;                 // alpha - default
   std::vector<int32_t> slot_base;            // [nr+1] Jacobian slots: {T, E, reactant roles, product roles (rev), eff roles}
+  std::vector<double> rev_par;               // [nr*3] ln A_r, beta_r, Ta_r of reactions with INFO_REVX (else 0); empty if none
   std::vector<double> fall;                  // [nf*12]: lnA0, beta0, Ta0, pad, then 5 blend parameters
   std::vector<int32_t> plog_ptr;             // [npl+1]
   std::vector<double> plog_P, plog_lnP, plog_lnA, plog_b, plog_Ta;
@@ -107,6 +109,7 @@ struct DevMech {
   const int32_t *eff_ptr, *eff_sp;
   const double* eff_d;
   const int32_t* slot_base;
+  const double* rev_par;
   const double* fall;
   const int32_t* plog_ptr;
   const double *plog_P, *plog_lnP, *plog_lnA, *plog_b, *plog_Ta;

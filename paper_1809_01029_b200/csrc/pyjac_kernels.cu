@@ -430,8 +430,14 @@ __device__ __forceinline__ void phases01(const DevMech& m, Tile<S, JAC>& t, int 
     double kr = 0.0, lam_r = 0.0;
     if (rev) {      // a4: K_c from Gibbs polynomials; k_r = k_f / K_c = exp(ln k_f - ln K_c)
       const double snu = (double)(((info >> INFO_SNU_SHIFT) & 15) - 8);
-      kr = exp(lnkf + dg - snu * ln_patm_rt);
-      lam_r = lam_f - (dh - snu) * invT;
+      if (info & INFO_REVX) {        // explicit reverse Arrhenius parameters (R9): K_c plays no role
+        const double lAr = __ldg(m.rev_par + 3 * r), br = __ldg(m.rev_par + 3 * r + 1), Tar = __ldg(m.rev_par + 3 * r + 2);
+        kr = exp(lAr + br * lnT - Tar * invT);
+        lam_r = (br + Tar * invT) * invT;
+      } else {
+        kr = exp(lnkf + dg - snu * ln_patm_rt);
+        lam_r = lam_f - (dh - snu) * invT;
+      }
     }
     const double Rf = kf * Pif, Rr = kr * Pir, Rn = Rf - Rr;
     const double dRdT = lam_f * Rf - lam_r * Rr;

@@ -25,9 +25,9 @@ def test_library_exports_every_declared_symbol():
         assert hasattr(lib, n), n
 
 
-@pytest.mark.parametrize("name", ["four", "four_b", "all_types", "all_types_inert", "chem", "c1", "c2", "c3", "c4"])
+@pytest.mark.parametrize("name", ["four", "four_b", "all_types", "all_types_inert", "chem", "revx", "c1", "c2", "c3", "c4"])
 def test_pattern_bit_exact_vs_oracle(name):
-    m = {"four": lambda: mg.hand_four(), "four_b": lambda: mg.hand_four(order=(1, 2, 3, 0)), "chem": mg.hand_chem_activated,
+    m = {"four": lambda: mg.hand_four(), "four_b": lambda: mg.hand_four(order=(1, 2, 3, 0)), "chem": mg.hand_chem_activated, "revx": mg.hand_rev_explicit,
          "all_types": lambda: mg.hand_all_types(True, True), "all_types_inert": lambda: mg.hand_all_types(False, False)}.get(
         name, lambda: mg.config_mechanism(int(name[1:])))()
     M = pj.Mechanism(m, -1)
@@ -81,6 +81,8 @@ def test_mechanism_validation_errors():
     assert "type" in _bad(lambda m: m["type"].__setitem__(0, 9))
     assert "low-pressure" in _bad(lambda m: m["low_A"].__setitem__(2, 0.0))
     assert "chem_activated" in _bad(lambda m: m["chem_activated"].__setitem__(0, 1))       # reaction 0 is elementary
+    assert "explicit reverse" in _bad(lambda m: m["rev_A"].__setitem__(0, -1.0))
+    assert "explicit reverse" in _bad(lambda m: (m["rev_A"].__setitem__(0, 1.0), m["reversible"].__setitem__(0, 0)))
 
     def plog_bad(m):
         m["type"][0] = mg.PLOG

@@ -30,6 +30,8 @@ def setup(pj, name):
             m = mg.hand_four(); st = lambda n: mg.make_states(4, n, 22)
         elif name == "chem":
             m = mg.hand_chem_activated(); st = lambda n: mg.make_states(5, n, 23)
+        elif name == "revx":
+            m = mg.hand_rev_explicit(); st = lambda n: mg.make_states(6, n, 24)
         else:
             c = int(name[1:]); m = mg.config_mechanism(c); st = lambda n, c=c: mg.config_states(c, n)
         _CACHE[name] = (m, pj.Mechanism(m, 0), Oracle(m), st)
@@ -61,7 +63,7 @@ def run_gpu(pj, M, what, mode, fmt, states, ld=None, tile=None):
     return res
 
 
-SRC_CASES = [("four", 64), ("all_types", 300), ("chem", 200), ("c1", 1024), ("c2", 1500), ("c3", 700), ("c4", 96), ("c5", 96)]
+SRC_CASES = [("four", 64), ("all_types", 300), ("chem", 200), ("revx", 200), ("revx", 200), ("c1", 1024), ("c2", 1500), ("c3", 700), ("c4", 96), ("c5", 96)]
 
 
 @pytest.mark.parametrize("name,n", SRC_CASES)

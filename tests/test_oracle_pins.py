@@ -150,6 +150,7 @@ MECHS = {
     "all_types": lambda: (mg.hand_all_types(True, True), mg.make_states(6, 4, 11)),
     "all_types_inert": lambda: (mg.hand_all_types(False, False), mg.make_states(6, 4, 12)),
     "chem_activated": lambda: (mg.hand_chem_activated(), mg.make_states(5, 6, 13)),
+    "rev_explicit": lambda: (mg.hand_rev_explicit(), mg.make_states(6, 6, 14)),
     "c1": lambda: (mg.config_mechanism(1), mg.config_states(1, 16)),
     "c2": lambda: (mg.config_mechanism(2), mg.config_states(2, 16)),
     "c3": lambda: (mg.config_mechanism(3), mg.config_states(3, 16)),

@@ -196,3 +196,29 @@ def test_chem_activated_limits():
     T = 1300.0
     kinf = ARR["A"] * T ** ARR["beta"] * math.exp(-ARR["Ta"] / T)
     assert hi[1]["c"][0] * hi[1]["kf"][0] * hi[1]["M"][0] == pytest.approx(kinf, rel=1e-12)
+
+
+# ---- explicit reverse Arrhenius parameters (R9) ---------------------------------------------------------------
+@pytest.mark.parametrize("extra", [dict(), dict(type=mg.THIRD_BODY, eff={0: 2.0}),
+                                   dict(type=mg.FALLOFF_TROE, low=LOW, troe=(0.6, 200.0, 1800.0, 5000.0))])
+def test_explicit_reverse_equals_equilibrium_constant_for_constant_cp(extra):
+    """With constant c_p the Gibbs polynomial is g/RT = a0 (1 - ln T) + a5/T - a6, so K_c is itself of Arrhenius form:
+    k_f / K_c = A_f e^{da0 - da6} (R/P_atm)^{sum nu} T^{beta_f - da0 + sum nu} exp(-(Ta_f - da5)/T).  An explicit reverse
+    rate constant with exactly these parameters must reproduce the K_c-based source terms AND Jacobian."""
+    a0 = [2.6, 3.0, 3.8]; a5 = [15000.0, 9000.0, 4000.0]; a6 = [5.0, 4.0, 6.0]          # species of _two(): A + B <=> C
+    da0 = a0[2] - a0[0] - a0[1]; da5 = a5[2] - a5[0] - a5[1]; da6 = a6[2] - a6[0] - a6[1]; snu = -1
+    Ar = ARR["A"] * math.exp(da0 - da6) * (R / PATM) ** snu
+    rp = (Ar, ARR["beta"] - da0 + snu, ARR["Ta"] - da5)
+    ref = _run(_two(**extra, **ARR))
+    exp_ = _run(_two(rev_params=rp, **extra, **ARR))
+    assert exp_[1]["kr"][0] == pytest.approx(ref[1]["kr"][0], rel=1e-12)
+    np.testing.assert_allclose(exp_[2], ref[2], rtol=1e-11)
+    np.testing.assert_allclose(exp_[3], ref[3], rtol=1e-9, atol=1e-12 * np.abs(ref[3]).max())
+
+
+def test_explicit_reverse_value():
+    """k_r is the Arrhenius expression itself, whatever the thermo says."""
+    rp = (5.0e11, -0.2, 9000.0)
+    r = _run(_two(rev_params=rp, **ARR))
+    T = 1300.0
+    assert r[1]["kr"][0] == pytest.approx(rp[0] * T ** rp[1] * math.exp(-rp[2] / T), rel=1e-14)
