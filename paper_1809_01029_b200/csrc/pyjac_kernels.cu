@@ -800,13 +800,17 @@ jacobian_kernel(const DevMech m, const DevPlan pl, int mode, int64_t n_states, i
   };
   const bool zero_warp = DENSE && n_zslices >= ZERO_WARP_MIN_SLICES && (tid >> 5) >= NW - PYJAC_ZERO_WARPS;
   auto side = [&](const int* counter, int n) -> bool {
-    if (!DENSE || !zero_warp) return false;
-    while (*reinterpret_cast<const volatile int*>(counter) < n) {
-      const int z = next_chunk(cnt + CNT_Z);
-      if (z >= n_zslices) break;
-      zero_slice(z);
+    if constexpr (!DENSE) {
+      return false;
+    } else {
+      if (!zero_warp) return false;
+      while (*reinterpret_cast<const volatile int*>(counter) < n) {
+        const int z = next_chunk(cnt + CNT_Z);
+        if (z >= n_zslices) break;
+        zero_slice(z);
+      }
+      return true;
     }
-    return true;
   };
   phases01<S, true>(m, t, mode, [&](int e) { return phi[pbase + (int64_t)e * tile]; }, param[sg], cnt, tick_, side);
   TICK(2);
