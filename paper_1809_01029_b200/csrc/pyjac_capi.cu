@@ -2,6 +2,7 @@
 // kernel dispatch.  No torch types; plain pointers and sizes only.
 #include <cuda_runtime.h>
 
+#include <atomic>
 #include <cstdio>
 #include <cstring>
 #include <new>
@@ -28,6 +29,11 @@ struct pyjac_mech {
   DevMech dm{};
   DevPlan plan[4]{};
   std::vector<void*> allocs;
+  // tile-scheduler words of the persistent Jacobian kernel: a ring of N_SCHED zeroed pairs, one per launch in flight
+  // (the kernel resets its pair), so launches of one handle on different streams do not share a counter
+  static constexpr unsigned N_SCHED = 64;
+  unsigned long long* sched = nullptr;
+  mutable std::atomic<unsigned> sched_next{0};
   ~pyjac_mech() {
     for (void* p : allocs) cudaFree(p);
   }
@@ -81,6 +87,13 @@ int pyjac_mech_create_ex(const pyjac_mech_desc* desc, int cuda_device, uint32_t 
   auto body = [&]() -> int {
     CK(cudaSetDevice(cuda_device));
     if (int ea = set_kernel_attributes()) return cuda_fail((cudaError_t)ea, "cudaFuncSetAttribute");
+    {
+      void* p = nullptr;
+      CK(cudaMalloc(&p, pyjac_mech::N_SCHED * 2 * sizeof(unsigned long long)));
+      m->allocs.push_back(p);
+      CK(cudaMemset(p, 0, pyjac_mech::N_SCHED * 2 * sizeof(unsigned long long)));
+      m->sched = (unsigned long long*)p;
+    }
     HostTables& h = m->h;
     DevMech& d = m->dm;
     d.ns = h.ns; d.nr = h.nr; d.nvar = h.nvar; d.nslots = h.nslots;
@@ -183,7 +196,8 @@ static int run_jac(const char* fn, const pyjac_mech* mech, int mode, int ofmt, i
   if (n_states == 0) return PYJAC_OK;
   const LaunchCfg cfg = choose_cfg(mech->h, true, tile, n_states);
   if (cfg.smem > 227 * 1024) return fail(PYJAC_ENOMEM, std::string(fn) + ": mechanism too large for shared memory");
-  int e = launch_jacobian(mech->dm, mech->plan[ofmt], cfg, mode, n_states, ld, tile, d_phi, d_param, d_out, stream);
+  unsigned long long* sched = mech->sched + 2 * (mech->sched_next.fetch_add(1) % pyjac_mech::N_SCHED);
+  int e = launch_jacobian(mech->dm, mech->plan[ofmt], cfg, mode, n_states, ld, tile, d_phi, d_param, d_out, sched, stream);
   if (e) return cuda_fail((cudaError_t)e, "jacobian_kernel launch");
   return PYJAC_OK;
 }

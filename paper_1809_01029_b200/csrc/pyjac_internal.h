@@ -137,7 +137,9 @@ LaunchCfg choose_cfg(const HostTables& h, bool jac, int64_t tile, int64_t n_stat
 int launch_source(const DevMech& m, const LaunchCfg& cfg, int mode, int64_t n_states, int64_t ld, int64_t tile,
                   const double* phi, const double* param, double* out, void* stream);
 int launch_jacobian(const DevMech& m, const DevPlan& p, const LaunchCfg& cfg, int mode, int64_t n_states, int64_t ld,
-                    int64_t tile, const double* phi, const double* param, double* out, void* stream);
+                    int64_t tile, const double* phi, const double* param, double* out, unsigned long long* sched, void* stream);
+// sched: two zero-initialised 64-bit words in device memory (tile counter, finished CTAs) that no other launch in
+// flight uses; the kernel leaves them zero again.
 // first-order forward finite-difference Jacobian.  ofmt: OutFmt.  S = columns per pass.
 LaunchCfg choose_cfg_fd(const HostTables& h);
 int launch_fd(const DevMech& m, const LaunchCfg& cfg, int mode, int ofmt, int64_t n_e, double rel_step, double abs_step,

@@ -14,6 +14,8 @@
 // No tensor cores: nothing here is a dense contraction.  No fast-math.
 #include <cuda_runtime.h>
 
+#include <algorithm>
+
 #include "pyjac_internal.h"
 
 namespace pyjac {
@@ -66,7 +68,10 @@ __host__ __device__ inline size_t smem_doubles(int ns, int nr, int nslots, int n
   // C[ns+1] (C[ns] = 1: dummy species of unused stoichiometric entries), gh, ec [2(ns+1)] each, ck[ns], slots (+ zero slots)
   size_t per_state = NSC + 6 * (size_t)ns + 5 + (jac ? (size_t)nslots + nr : (size_t)nr) + N_ZERO_SLOTS;
   // n_part: partial sums of split gather lists; n_meta: (offset, width) of every ELL super-group (8 bytes each)
-  return (per_state + n_part) * S + (size_t)NW * NRED * S + n_meta;
+  // Jacobian kernel (persistent CTA): the NASA table [15*ns] and the prefetched state vector + parameter [(ns+2)*S]
+  // and a second c_k array (the second pass of tile n overlaps phase 0 of tile n+1, which rewrites c_k)
+  const size_t resident = jac ? 15 * (size_t)ns + (2 * (size_t)ns + 2) * S : 0;
+  return (per_state + n_part) * S + (size_t)NW * NRED * S + n_meta + resident;
 }
 
 // Dynamic work distribution inside a CTA: items are sorted by descending cost at create time and warps take the
@@ -187,9 +192,11 @@ struct Tile {
   double *sc, *C, *ck, *dE, *P, *red, *part;
   double2 *gh, *ec;
   int2* meta;     // (entry offset, width) of every ELL super-group of the plans this kernel gathers: read per unit
-  __device__ __forceinline__ Tile(double* smem, int ns, int nr, int nslots, int n_part) {
+  double *nasa, *phi;   // JAC only (persistent CTA): NASA table, loaded once; prefetched phi [nvar][S] and param [S]
+  __device__ __forceinline__ Tile(double* smem, int ns, int nr, int nslots, int n_part, int n_meta) {
     sc = smem; gh = reinterpret_cast<double2*>(sc + NSC * S); ec = gh + (ns + 1) * S; C = reinterpret_cast<double*>(ec + (ns + 1) * S); ck = C + (ns + 1) * S; dE = ck + ns * S; P = JAC ? dE + nr * S : dE; red = P + ((JAC ? nslots : nr) + N_ZERO_SLOTS) * S; part = red + NW * NRED * S;
     meta = reinterpret_cast<int2*>(part + n_part * S);
+    nasa = reinterpret_cast<double*>(meta + n_meta); phi = nasa + 15 * ns;
     // source kernel: dE unused, P[r] = q_r.  P[nslots ..] (JAC) / P[nr ..]: N_ZERO_SLOTS always-zero slots (ELL padding)
   }
 };
@@ -231,10 +238,12 @@ __device__ __forceinline__ void phases01(const DevMech& m, Tile<S, JAC>& t, int 
     const double T2 = T * T, T3 = T2 * T, T4 = T3 * T;
     // thermo of the LAST species, evaluated by every thread (cheap, warp-uniform loads): E~_k and c~_k fold the
     // last species in through mass conservation (R1/A1) and need it; saves a second pass and two barriers
+    // NASA table (coefficient-major): global memory, or the CTA's shared-memory copy in the persistent Jacobian kernel
+    auto nasa = [&](int i) -> double { if constexpr (JAC) return t.nasa[i]; else return __ldg(m.nasa + i); };
     double cL, dcL, eL;
     {
-      const double* __restrict__ a = m.nasa + L + ((T <= __ldg(m.nasa + L)) ? 1 : 8) * ns;   // table is coefficient-major
-      const double a0 = __ldg(a), a1 = __ldg(a + ns), a2 = __ldg(a + 2 * ns), a3 = __ldg(a + 3 * ns), a4 = __ldg(a + 4 * ns), a5 = __ldg(a + 5 * ns);
+      const int a = L + ((T <= nasa(L)) ? 1 : 8) * ns;
+      const double a0 = nasa(a), a1 = nasa(a + ns), a2 = nasa(a + 2 * ns), a3 = nasa(a + 3 * ns), a4 = nasa(a + 4 * ns), a5 = nasa(a + 5 * ns);
       const double cpR = a0 + a1 * T + a2 * T2 + a3 * T3 + a4 * T4;
       const double hRT = a0 + a1 * T * 0.5 + a2 * T2 * (1.0 / 3.0) + a3 * T3 * 0.25 + a4 * T4 * 0.2 + a5 * invT;
       cL = R_GAS * (mode == PYJAC_CONP ? cpR : cpR - 1.0);
@@ -247,14 +256,21 @@ __device__ __forceinline__ void phases01(const DevMech& m, Tile<S, JAC>& t, int 
       const int k = idx / S;
       // coefficient-major table (entry c of species k at nasa[c * ns + k]): consecutive lanes read consecutive
       // addresses, and BOTH ranges are requested before T is known, so the loads do not wait for the state load
-      const double* __restrict__ a = m.nasa + k;
-      double lo[7], hi[7];
-      const double tmid = __ldg(a);
+      double a0, a1, a2, a3, a4, a5, a6;
+      if constexpr (JAC) {                               // shared-memory table, T already on chip: read one range
+        const int b = k + (T <= t.nasa[k] ? 1 : 8) * ns; // low range iff T <= T_mid (R3)
+        a0 = t.nasa[b]; a1 = t.nasa[b + ns]; a2 = t.nasa[b + 2 * ns]; a3 = t.nasa[b + 3 * ns]; a4 = t.nasa[b + 4 * ns];
+        a5 = t.nasa[b + 5 * ns]; a6 = t.nasa[b + 6 * ns];
+      } else {
+        const double* __restrict__ a = m.nasa + k;
+        double lo[7], hi[7];
+        const double tmid = __ldg(a);
 #pragma unroll
-      for (int c = 0; c < 7; ++c) { lo[c] = __ldg(a + (1 + c) * ns); hi[c] = __ldg(a + (8 + c) * ns); }
-      const bool low = T <= tmid;                        // low range iff T <= T_mid (R3); per-lane select
-      const double a0 = low ? lo[0] : hi[0], a1 = low ? lo[1] : hi[1], a2 = low ? lo[2] : hi[2], a3 = low ? lo[3] : hi[3],
-                   a4 = low ? lo[4] : hi[4], a5 = low ? lo[5] : hi[5], a6 = low ? lo[6] : hi[6];
+        for (int c = 0; c < 7; ++c) { lo[c] = __ldg(a + (1 + c) * ns); hi[c] = __ldg(a + (8 + c) * ns); }
+        const bool low = T <= tmid;                      // low range iff T <= T_mid (R3); per-lane select
+        a0 = low ? lo[0] : hi[0]; a1 = low ? lo[1] : hi[1]; a2 = low ? lo[2] : hi[2]; a3 = low ? lo[3] : hi[3];
+        a4 = low ? lo[4] : hi[4]; a5 = low ? lo[5] : hi[5]; a6 = low ? lo[6] : hi[6];
+      }
       const double w = __ldg(m.wr + k);
       const double cpR = a0 + a1 * T + a2 * T2 + a3 * T3 + a4 * T4;
       const double dcpR = a1 + 2.0 * a2 * T + 3.0 * a3 * T2 + 4.0 * a4 * T3;
@@ -634,7 +650,7 @@ __global__ void __launch_bounds__(NT, 1)
 source_kernel(const DevMech m, int mode, int64_t n_states, int64_t tile, const double* __restrict__ phi,
               const double* __restrict__ param, double* __restrict__ out) {
   extern __shared__ __align__(16) double smem[];
-  Tile<S, false> t(smem, m.ns, m.nr, m.nslots, m.n_part_src);
+  Tile<S, false> t(smem, m.ns, m.nr, m.nslots, m.n_part_src, m.qplan.n_sg);
   load_meta(m.qplan, t.meta);
   const int64_t s0 = (int64_t)blockIdx.x * S;
   __shared__ int cnt[N_CNT];
@@ -686,7 +702,7 @@ __global__ void __launch_bounds__(NT, 1)
 fd_kernel(const DevMech m, int mode, int ofmt, double rel, double ab, int64_t tile, int64_t n_e,
           const double* __restrict__ phi, const double* __restrict__ param, double* __restrict__ out) {
   extern __shared__ __align__(16) double smem[];
-  Tile<S, false> t(smem, m.ns, m.nr, m.nslots, m.n_part_src);
+  Tile<S, false> t(smem, m.ns, m.nr, m.nslots, m.n_part_src, m.qplan.n_sg);
   load_meta(m.qplan, t.meta);
   double* __restrict__ f0 = reinterpret_cast<double*>(t.meta + m.qplan.n_sg);   // f(phi)           [nvar]
   double* __restrict__ fc = f0 + m.nvar;                      // f(phi + h_c e_c) [nvar][S]
@@ -759,12 +775,17 @@ fd_kernel(const DevMech m, int mode, int ofmt, double rel, double ab, int64_t ti
 template <int S, bool DENSE>
 __global__ void __launch_bounds__(NT, 1)
 jacobian_kernel(const DevMech m, const DevPlan pl, int mode, int64_t n_states, int64_t tile, const double* __restrict__ phi,
-                const double* __restrict__ param, double* __restrict__ out) {
+                const double* __restrict__ param, double* __restrict__ out, unsigned long long* __restrict__ sched) {
   extern __shared__ __align__(16) double smem[];
-  Tile<S, true> t(smem, m.ns, m.nr, m.nslots, m.n_part_jac);
+  Tile<S, true> t(smem, m.ns, m.nr, m.nslots, m.n_part_jac, m.cplan.n_sg + pl.jplan.n_sg);
+  // PERSISTENT CTA: the grid is one CTA per SM (x occupancy); a CTA starts with tile blockIdx.x and takes further
+  // tiles from a global counter (sched[0]; dynamic, because the SMs of the two dies do not run at the same speed when
+  // the output stream loads the memory system).  sched[1] counts finished CTAs: the last one resets both words.
+  // What does not depend on the state is brought on chip once (gather metadata, NASA table), and the state vector of
+  // the NEXT tile is prefetched with cp.async while the gathers of the current one run, so phase 0 never waits for
+  // DRAM (first capture of round 1b: 12.6 % of the kernel was phase 0, mostly that wait and the L2 reads of the table).
   load_meta(m.cplan, t.meta);
   load_meta(pl.jplan, t.meta + m.cplan.n_sg);
-  const int64_t s0 = (int64_t)blockIdx.x * S;
   __shared__ int cnt[N_CNT];
 #ifdef PYJAC_TIMING
   long long tick_ = clock64();
@@ -773,9 +794,33 @@ jacobian_kernel(const DevMech m, const DevPlan pl, int mode, int64_t n_states, i
 #endif
   const int tid = threadIdx.x, s = tid % S;
   const int L = m.ns - 1;
+  for (int i = tid; i < 15 * m.ns; i += NT) t.nasa[i] = __ldg(m.nasa + i);
+  const int64_t n_tiles = (n_states + S - 1) / S;
+  auto prefetch = [&](int64_t tl) {                // phi [nvar][S] and param [S] of tile tl -> t.phi (8-byte cp.async)
+    const int64_t sp = min(tl * S + s, n_states - 1);
+    const double* __restrict__ src = phi + state_base(sp, tile, m.nvar);
+    for (int idx = tid; idx < (m.nvar + 1) * S; idx += NT) {   // NT % S == 0: idx % S == s in every iteration
+      const int e = idx / S;
+      const double* g = e < m.nvar ? src + (int64_t)e * tile : param + sp;
+      asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" :: "r"((uint32_t)__cvta_generic_to_shared(t.phi + idx)), "l"(g) : "memory");
+    }
+    asm volatile("cp.async.commit_group;" ::: "memory");
+  };
+  prefetch(blockIdx.x);
+  asm volatile("cp.async.wait_all;" ::: "memory");
+  __syncthreads();
+  // Barriers per tile: two in phase 0, one after phase 1, one after the gathers.  There is none between the second
+  // pass of tile n and phase 0 of tile n+1: the two overlap (the only array both touch, c_k, is double-buffered).
+  double* const ck_buf[2] = {t.ck, t.phi + (m.nvar + 1) * S};
+  __shared__ long long next_tile;
+  int parity = 0;
+  for (int64_t tl = blockIdx.x, tl_next; tl < n_tiles; tl = tl_next, parity ^= 1) {
+  if (tid == 0) next_tile = (long long)gridDim.x + (long long)atomicAdd(sched, 1ull);   // published by the barriers of phase 0
+  t.ck = ck_buf[parity];
+  const int64_t s0 = tl * S;
   const bool valid = s0 + s < n_states;
   const int64_t sg = min(s0 + s, n_states - 1);   // ragged tail: recompute the last valid state, never store
-  const int64_t pbase = state_base(sg, tile, m.nvar), obase = state_base(sg, tile, pl.n_e);
+  const int64_t obase = state_base(sg, tile, pl.n_e);
   // dense output: structural zeros, each stored once (no memset pass), in slices of 32 bitmap words (1024 elements:
   // one coalesced mask load, then 32 coalesced predicated store instructions at S = 1).  For large matrices the
   // last warp streams the slices while the others compute (see NoSide above); what is left is shared at the end.
@@ -812,7 +857,9 @@ jacobian_kernel(const DevMech m, const DevPlan pl, int mode, int64_t n_states, i
       return true;
     }
   };
-  phases01<S, true>(m, t, mode, [&](int e) { return phi[pbase + (int64_t)e * tile]; }, param[sg], cnt, tick_, side);
+  phases01<S, true>(m, t, mode, [&](int e) { return t.phi[e * S + s]; }, t.phi[m.nvar * S + s], cnt, tick_, side);
+  tl_next = next_tile;
+  if (tl_next < n_tiles) prefetch(tl_next);                 // t.phi is not read after phase 0
   TICK(2);
   const double T = t.sc[SC_T * S + s], V = t.sc[SC_V * S + s], Pp = t.sc[SC_P * S + s], D = t.sc[SC_D * S + s];
   const double N = red_sum<S>(t.red, 0, s);
@@ -852,7 +899,7 @@ jacobian_kernel(const DevMech m, const DevPlan pl, int mode, int64_t n_states, i
       out[obase + (int64_t)pl.d_pos[3] * tile] = JEE;
     }
   };
-  if (S > 1) corners();
+  corners();     // before the gathers: that warp joins the dynamically scheduled gather a little late, no serial tail
   const double* __restrict__ P = t.P;
   // The T/E-row gather goes FIRST: it has few, long units; warps that finish it early move on to the many short
   // units of the species rows (no barrier in between), so its latency tail is hidden behind them.
@@ -914,8 +961,10 @@ jacobian_kernel(const DevMech m, const DevPlan pl, int mode, int64_t n_states, i
   if (DENSE)                                      // whatever is left of the zero fill
     for (int z = next_chunk(cnt + CNT_Z); z < n_zslices; z = next_chunk(cnt + CNT_Z)) zero_slice(z);
   TICK(6);
+  // every warp is done with the slots, and the prefetched phi of the next tile (issued after phase 1) has landed
+  asm volatile("cp.async.wait_all;" ::: "memory");
+  __syncthreads();
   if (pl.jplan.n_comb + m.cplan.n_comb) {
-    __syncthreads();
     // second pass over the split lists of both plans in ONE index space, with every table word (first partial,
     // count, output positions) requested before the partial sums are added: one L2 round trip for the whole pass
     const int nJ = pl.jplan.n_comb * S, nC = m.cplan.n_comb * S;
@@ -943,8 +992,9 @@ jacobian_kernel(const DevMech m, const DevPlan pl, int mode, int64_t n_states, i
       }
     }
   }
-  if (S == 1) corners();
   TICK(5);
+  }  // tiles of this CTA
+  if (tid == 0 && atomicAdd(sched + 1, 1ull) == (unsigned long long)gridDim.x - 1) { sched[0] = 0; sched[1] = 0; }
 }
 
 template <int S> int launch_source_S(const DevMech& m, const LaunchCfg& cfg, int mode, int64_t n, int64_t tile,
@@ -954,10 +1004,20 @@ template <int S> int launch_source_S(const DevMech& m, const LaunchCfg& cfg, int
   return (int)cudaGetLastError();
 }
 template <int S> int launch_jac_S(const DevMech& m, const DevPlan& p, const LaunchCfg& cfg, int mode, int64_t n, int64_t tile,
-                                  const double* phi, const double* param, double* out, cudaStream_t st) {
-  const int64_t blocks = (n + S - 1) / S;
-  if (p.nzmask != nullptr) jacobian_kernel<S, true><<<(unsigned)blocks, NT, cfg.smem, st>>>(m, p, mode, n, tile, phi, param, out);
-  else jacobian_kernel<S, false><<<(unsigned)blocks, NT, cfg.smem, st>>>(m, p, mode, n, tile, phi, param, out);
+                                  const double* phi, const double* param, double* out, unsigned long long* sched, cudaStream_t st) {
+  const int64_t tiles = (n + S - 1) / S;
+  if (tiles == 0) return 0;
+  // persistent grid: as many CTAs as are resident at once (one per SM with 512 threads x 128 registers)
+  int dev = 0, n_sm = 0, occ = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e == cudaSuccess) e = cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
+  if (e == cudaSuccess)
+    e = p.nzmask != nullptr ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, jacobian_kernel<S, true>, NT, cfg.smem)
+                            : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, jacobian_kernel<S, false>, NT, cfg.smem);
+  if (e != cudaSuccess) return (int)e;
+  const int64_t blocks = std::min<int64_t>(tiles, (int64_t)n_sm * (occ > 0 ? occ : 1));
+  if (p.nzmask != nullptr) jacobian_kernel<S, true><<<(unsigned)blocks, NT, cfg.smem, st>>>(m, p, mode, n, tile, phi, param, out, sched);
+  else jacobian_kernel<S, false><<<(unsigned)blocks, NT, cfg.smem, st>>>(m, p, mode, n, tile, phi, param, out, sched);
   return (int)cudaGetLastError();
 }
 
@@ -1024,16 +1084,16 @@ int launch_source(const DevMech& m, const LaunchCfg& cfg, int mode, int64_t n_st
 }
 
 int launch_jacobian(const DevMech& m, const DevPlan& p, const LaunchCfg& cfg, int mode, int64_t n_states, int64_t ld,
-                    int64_t tile, const double* phi, const double* param, double* out, void* stream) {
+                    int64_t tile, const double* phi, const double* param, double* out, unsigned long long* sched, void* stream) {
   (void)ld;
   cudaStream_t st = (cudaStream_t)stream;
   switch (cfg.S) {
-    case 1: return launch_jac_S<1>(m, p, cfg, mode, n_states, tile, phi, param, out, st);
-    case 2: return launch_jac_S<2>(m, p, cfg, mode, n_states, tile, phi, param, out, st);
-    case 4: return launch_jac_S<4>(m, p, cfg, mode, n_states, tile, phi, param, out, st);
-    case 8: return launch_jac_S<8>(m, p, cfg, mode, n_states, tile, phi, param, out, st);
-    case 16: return launch_jac_S<16>(m, p, cfg, mode, n_states, tile, phi, param, out, st);
-    default: return launch_jac_S<32>(m, p, cfg, mode, n_states, tile, phi, param, out, st);
+    case 1: return launch_jac_S<1>(m, p, cfg, mode, n_states, tile, phi, param, out, sched, st);
+    case 2: return launch_jac_S<2>(m, p, cfg, mode, n_states, tile, phi, param, out, sched, st);
+    case 4: return launch_jac_S<4>(m, p, cfg, mode, n_states, tile, phi, param, out, sched, st);
+    case 8: return launch_jac_S<8>(m, p, cfg, mode, n_states, tile, phi, param, out, sched, st);
+    case 16: return launch_jac_S<16>(m, p, cfg, mode, n_states, tile, phi, param, out, sched, st);
+    default: return launch_jac_S<32>(m, p, cfg, mode, n_states, tile, phi, param, out, sched, st);
   }
 }
 
