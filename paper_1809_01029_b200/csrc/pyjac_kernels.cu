@@ -59,7 +59,8 @@ namespace {
 #endif
 constexpr int NT = PYJAC_NT;      // threads per CTA
 constexpr int NW = NT / 32;
-constexpr int NRED = 8;           // reduction slots
+constexpr int NRED = 10;          // reduction slots: 0-6 reaction sums (phase 1), 7-9 species sums (phase 0)
+constexpr int RED0 = 7;
 // per-state scalars kept in shared memory
 enum { SC_T = 0, SC_V, SC_P, SC_CTOT, SC_SUMC, SC_SUMCC, SC_SUMCDC, SC_D, SC_DDDT, SC_CNS,
        SC_R0, SC_R1, SC_R2, SC_R3, SC_R4, SC_R5, SC_R6, SC_R7, SC_INVT, SC_LNT, SC_LNP, SC_LNPRT, NSC };
@@ -68,9 +69,9 @@ __host__ __device__ inline size_t smem_doubles(int ns, int nr, int nslots, int n
   // C[ns+1] (C[ns] = 1: dummy species of unused stoichiometric entries), gh, ec [2(ns+1)] each, ck[ns], slots (+ zero slots)
   size_t per_state = NSC + 6 * (size_t)ns + 5 + (jac ? (size_t)nslots + nr : (size_t)nr) + N_ZERO_SLOTS;
   // n_part: partial sums of split gather lists; n_meta: (offset, width) of every ELL super-group (8 bytes each)
-  // Jacobian kernel (persistent CTA): the NASA table [15*ns] and the prefetched state vector + parameter [(ns+2)*S]
+  // Jacobian kernel (persistent CTA): the NASA table [15*ns]
   // and a second c_k array (the second pass of tile n overlaps phase 0 of tile n+1, which rewrites c_k)
-  const size_t resident = jac ? 15 * (size_t)ns + (2 * (size_t)ns + 2) * S : 0;
+  const size_t resident = jac ? 15 * (size_t)ns + (size_t)ns * S : 0;
   return (per_state + n_part) * S + (size_t)NW * NRED * S + n_meta + resident;
 }
 
@@ -192,7 +193,7 @@ struct Tile {
   double *sc, *C, *ck, *dE, *P, *red, *part;
   double2 *gh, *ec;
   int2* meta;     // (entry offset, width) of every ELL super-group of the plans this kernel gathers: read per unit
-  double *nasa, *phi;   // JAC only (persistent CTA): NASA table, loaded once; prefetched phi [nvar][S] and param [S]
+  double *nasa, *phi;   // JAC only (persistent CTA): NASA table, loaded once; phi: the second c_k buffer [ns][S]
   __device__ __forceinline__ Tile(double* smem, int ns, int nr, int nslots, int n_part, int n_meta) {
     sc = smem; gh = reinterpret_cast<double2*>(sc + NSC * S); ec = gh + (ns + 1) * S; C = reinterpret_cast<double*>(ec + (ns + 1) * S); ck = C + (ns + 1) * S; dE = ck + ns * S; P = JAC ? dE + nr * S : dE; red = P + ((JAC ? nslots : nr) + N_ZERO_SLOTS) * S; part = red + NW * NRED * S;
     meta = reinterpret_cast<int2*>(part + n_part * S);
@@ -212,9 +213,13 @@ __device__ __forceinline__ int64_t state_base(int64_t s, int64_t tile, int64_t n
 // returns when the items are exhausted (*counter >= n) or the side job is finished.
 struct NoSide { __device__ __forceinline__ bool operator()(const int*, int) const { return false; } };
 
-template <int S, bool JAC, class PhiF, class SideF>
+// mid(): called by every thread between the two barriers of phase 0 (the persistent Jacobian kernel finishes the
+// previous tile there: its second pass needs a barrier after the gathers, and this one serves).
+struct NoMid { __device__ __forceinline__ void operator()() const {} };
+
+template <int S, bool JAC, class PhiF, class SideF, class MidF>
 __device__ __forceinline__ void phases01(const DevMech& m, Tile<S, JAC>& t, int mode, PhiF phi_of, double par_,
-                                         int* cnt, long long& tick_, SideF side) {
+                                         int* cnt, long long& tick_, SideF side, MidF mid) {
   (void)tick_;
   const int tid = threadIdx.x;
   const int ns = m.ns, nr = m.nr, L = ns - 1;
@@ -222,15 +227,13 @@ __device__ __forceinline__ void phases01(const DevMech& m, Tile<S, JAC>& t, int 
   // ---- phase 0: scalars, species (C_k = n_k / V, Eq. 6; NASA-7 thermo, R2) ------------------------
   // Every thread reads T, E and the parameter itself (same address for the lanes of a state: one broadcast
   // request) so that no barrier separates the state load from the species loop.
-  if (tid < N_CNT) cnt[tid] = 0;
+  // Nothing that the gathers of the PREVIOUS tile read (work counters, scalars, reaction sums) is written before
+  // the first barrier: in the persistent kernel warps enter here while others still gather (idempotent writes excepted).
   if (tid < N_ZERO_SLOTS * S) t.P[(JAC ? m.nslots : nr) * S + tid] = 0.0;   // always-zero slots (ELL padding)
   const double T = phi_of(0), E_ = phi_of(1);
   const double V = mode == PYJAC_CONP ? E_ : par_, Pp = mode == PYJAC_CONP ? par_ : E_;
   const double invT = 1.0 / T, lnT = log(T), RT = R_GAS * T, Ctot = Pp / RT;
   if (tid < S) {
-    t.sc[SC_T * S + s] = T; t.sc[SC_V * S + s] = V; t.sc[SC_P * S + s] = Pp; t.sc[SC_CTOT * S + s] = Ctot;
-    t.sc[SC_LNP * S + s] = log(Pp);
-    t.sc[SC_LNPRT * S + s] = log(P_ATM / RT);
     t.C[ns * S + s] = 1.0;                               // dummy species: unused stoichiometric entries
     t.gh[ns * S + s] = make_double2(0.0, 0.0); t.ec[ns * S + s] = make_double2(0.0, 0.0);
   }
@@ -293,19 +296,24 @@ __device__ __forceinline__ void phases01(const DevMech& m, Tile<S, JAC>& t, int 
 #pragma unroll
     for (int j = 0; j < 3; ++j) {
       const double v = group_sum<S>(acc[j]);
-      if (lane < S) t.red[(warp * NRED + j) * S + lane] = v;
+      if (lane < S) t.red[(warp * NRED + RED0 + j) * S + lane] = v;
     }
     __syncthreads();
+    if (tid >= NT - N_CNT) cnt[NT - 1 - tid] = 0;         // work counters of this tile (last warp: not the finishing threads)
     if (tid < S) {
+      t.sc[SC_T * S + s] = T; t.sc[SC_V * S + s] = V; t.sc[SC_P * S + s] = Pp; t.sc[SC_CTOT * S + s] = Ctot;
+      t.sc[SC_LNP * S + s] = log(Pp);
+      t.sc[SC_LNPRT * S + s] = log(P_ATM / RT);
       double sum[3] = {0.0, 0.0, 0.0};
       for (int w = 0; w < NW; ++w)
 #pragma unroll
-        for (int j = 0; j < 3; ++j) sum[j] += t.red[(w * NRED + j) * S + s];
+        for (int j = 0; j < 3; ++j) sum[j] += t.red[(w * NRED + RED0 + j) * S + s];
       const double CL = Ctot - sum[0];
       t.C[L * S + s] = CL;
       t.sc[SC_D * S + s] = sum[1] + CL * cL;
       t.sc[SC_DDDT * S + s] = sum[2] + CL * dcL;
     }
+    mid();
     __syncthreads();
   }
   TICK(0);
@@ -659,7 +667,7 @@ source_kernel(const DevMech m, int mode, int64_t n_states, int64_t tile, const d
   const bool valid = s0 + s < n_states;
   const int64_t sg = min(s0 + s, n_states - 1);   // ragged tail: recompute the last valid state, never store
   const int64_t pbase = state_base(sg, tile, m.nvar), obase = pbase;
-  phases01<S, false>(m, t, mode, [&](int e) { return phi[pbase + (int64_t)e * tile]; }, param[sg], cnt, tick_, NoSide());
+  phases01<S, false>(m, t, mode, [&](int e) { return phi[pbase + (int64_t)e * tile]; }, param[sg], cnt, tick_, NoSide(), NoMid());
   const double V = t.sc[SC_V * S + s];
   // a7: omega_k = sum_i nu_ki q_i (Eq. 4), dn_k/dt = V omega_k (Eq. 3)
   const double* __restrict__ P = t.P;
@@ -719,7 +727,7 @@ fd_kernel(const DevMech m, int mode, int ofmt, double rel, double ab, int64_t ti
     double x = 0.0, xp = 0.0;
     if (c >= 0) { x = phi[pbase + (int64_t)c * tile]; xp = x + fma(rel, fabs(x), ab); }
     phases01<S, false>(m, t, mode, [&](int e) { const double v = phi[pbase + (int64_t)e * tile]; return e == c ? xp : v; },
-                       par, cnt, tick_, NoSide());
+                       par, cnt, tick_, NoSide(), NoMid());
     const double V = t.sc[SC_V * S + s];
     const double* __restrict__ P = t.P;
     gather<S, 1, 1, PYJAC_UQ, 4, ELL_W, int>(m.qplan.ell_ent, t.meta, m.qplan.n_sg, 0, cnt + CNT_Q,
@@ -781,9 +789,13 @@ jacobian_kernel(const DevMech m, const DevPlan pl, int mode, int64_t n_states, i
   // PERSISTENT CTA: the grid is one CTA per SM (x occupancy); a CTA starts with tile blockIdx.x and takes further
   // tiles from a global counter (sched[0]; dynamic, because the SMs of the two dies do not run at the same speed when
   // the output stream loads the memory system).  sched[1] counts finished CTAs: the last one resets both words.
-  // What does not depend on the state is brought on chip once (gather metadata, NASA table), and the state vector of
-  // the NEXT tile is prefetched with cp.async while the gathers of the current one run, so phase 0 never waits for
-  // DRAM (first capture of round 1b: 12.6 % of the kernel was phase 0, mostly that wait and the L2 reads of the table).
+  // What does not depend on the state is brought on chip once (gather metadata, NASA table).  Each thread loads the
+  // state-vector elements it needs in phase 0 of the NEXT tile into registers right after phase 1, so their DRAM
+  // latency hides behind the gathers.  Three barriers per tile: two in phase 0, one after phase 1.  There is none after
+  // the gathers: a warp that runs out of gather units starts phase 0 of the next tile, and the second pass over the
+  // split lists of tile n runs between the two phase-0 barriers of tile n+1 (the first of them tells it that every
+  // partial sum is there).  Phase 0 therefore writes nothing the gathers read before its first barrier; c_k, which the
+  // T-row entries of the second pass need, is double-buffered.
   load_meta(m.cplan, t.meta);
   load_meta(pl.jplan, t.meta + m.cplan.n_sg);
   __shared__ int cnt[N_CNT];
@@ -796,26 +808,53 @@ jacobian_kernel(const DevMech m, const DevPlan pl, int mode, int64_t n_states, i
   const int L = m.ns - 1;
   for (int i = tid; i < 15 * m.ns; i += NT) t.nasa[i] = __ldg(m.nasa + i);
   const int64_t n_tiles = (n_states + S - 1) / S;
-  auto prefetch = [&](int64_t tl) {                // phi [nvar][S] and param [S] of tile tl -> t.phi (8-byte cp.async)
+  // this thread's inputs of phase 0: T, E, the parameter and the moles of species tid / S (first trip of the species loop)
+  const int e_mine = tid / S < L ? 2 + tid / S : 0;
+  double pT, pE, pPar, pN;
+  auto fetch_state = [&](int64_t tl) {
     const int64_t sp = min(tl * S + s, n_states - 1);
     const double* __restrict__ src = phi + state_base(sp, tile, m.nvar);
-    for (int idx = tid; idx < (m.nvar + 1) * S; idx += NT) {   // NT % S == 0: idx % S == s in every iteration
-      const int e = idx / S;
-      const double* g = e < m.nvar ? src + (int64_t)e * tile : param + sp;
-      asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" :: "r"((uint32_t)__cvta_generic_to_shared(t.phi + idx)), "l"(g) : "memory");
-    }
-    asm volatile("cp.async.commit_group;" ::: "memory");
+    pT = src[0]; pE = src[tile]; pN = src[(int64_t)e_mine * tile]; pPar = param[sp];
   };
-  prefetch(blockIdx.x);
-  asm volatile("cp.async.wait_all;" ::: "memory");
-  __syncthreads();
-  // Barriers per tile: two in phase 0, one after phase 1, one after the gathers.  There is none between the second
-  // pass of tile n and phase 0 of tile n+1: the two overlap (the only array both touch, c_k, is double-buffered).
-  double* const ck_buf[2] = {t.ck, t.phi + (m.nvar + 1) * S};
+  fetch_state(blockIdx.x);
+  double* const ck_buf[2] = {t.ck, reinterpret_cast<double*>(t.phi)};
   __shared__ long long next_tile;
   int parity = 0;
+  // context of the previous tile for its deferred second pass
+  bool prev_valid = false; int64_t prev_obase = 0; double prev_fT = 0.0, prev_iDV = 0.0, prev_cS = 0.0, prev_cT = 0.0, prev_cL = 0.0;
+  const double* prev_ck = t.ck;
+  const int nJ2 = pl.jplan.n_comb * S, nC2 = m.cplan.n_comb * S;
+  // second pass over the split lists of both plans in ONE index space, with every table word (first partial, count,
+  // output positions) requested before the partial sums are added
+  auto second_pass = [&]() {
+    const double* __restrict__ part = t.part;
+    for (int idx = tid; idx < nJ2 + nC2; idx += NT) {
+      if (idx < nJ2) {
+        const int c = idx / S;
+        const int first = pl.jplan.part_base + __ldg(pl.jplan.comb_first + c), n = __ldg(pl.jplan.comb_nseg + c);
+        const int pos = __ldg(pl.jc_pos + c);
+        double v = 0.0;
+        for (int q = 0; q < n; ++q) v += part[(first + q) * S + s];
+        if (prev_valid) st_out(out + prev_obase + (int64_t)pos * tile, v);
+      } else {
+        const int c = (idx - nJ2) / S;
+        const int first = m.cplan.part_base + 2 * __ldg(m.cplan.comb_first + c), n = __ldg(m.cplan.comb_nseg + c);
+        const int j = __ldg(m.cc_item + c);
+        const int2 pos = __ldg(reinterpret_cast<const int2*>(pl.cc_pos) + c);
+        double v0 = 0.0, v1 = 0.0;
+        for (int q = 0; q < n; ++q) { v0 += part[(first + 2 * q) * S + s]; v1 += part[(first + 2 * q + 1) * S + s]; }
+        if (prev_valid) {
+          const double JT = -(v0 + prev_fT * (prev_ck[j * S + s] - prev_cL)) * prev_iDV;
+          st_out(out + prev_obase + (int64_t)pos.x * tile, JT);
+          st_out(out + prev_obase + (int64_t)pos.y * tile, prev_cS * v1 + prev_cT * JT);
+        }
+      }
+    }
+  };
+  bool have_prev = false;
   for (int64_t tl = blockIdx.x, tl_next; tl < n_tiles; tl = tl_next, parity ^= 1) {
-  if (tid == 0) next_tile = (long long)gridDim.x + (long long)atomicAdd(sched, 1ull);   // published by the barriers of phase 0
+  unsigned long long ticket = 0;
+  if (tid == 0) ticket = atomicAdd(sched, 1ull);   // its latency hides behind the species loop; published in mid()
   t.ck = ck_buf[parity];
   const int64_t s0 = tl * S;
   const bool valid = s0 + s < n_states;
@@ -857,9 +896,23 @@ jacobian_kernel(const DevMech m, const DevPlan pl, int mode, int64_t n_states, i
       return true;
     }
   };
-  phases01<S, true>(m, t, mode, [&](int e) { return t.phi[e * S + s]; }, t.phi[m.nvar * S + s], cnt, tick_, side);
+  {
+    const double cT_ = pT, cE_ = pE, cN_ = pN, cPar_ = pPar;
+    phases01<S, true>(m, t, mode,
+        [&](int e) {
+          if (e == 0) return cT_;
+          if (e == 1) return cE_;
+          if (e == e_mine) return cN_;
+          return phi[state_base(sg, tile, m.nvar) + (int64_t)e * tile];     // species loops of more than one trip
+        },
+        cPar_, cnt, tick_, side,
+        [&]() {
+          if (tid == 0) next_tile = (long long)gridDim.x + (long long)ticket;
+          if (have_prev && nJ2 + nC2 > 0) second_pass();
+        });
+  }
   tl_next = next_tile;
-  if (tl_next < n_tiles) prefetch(tl_next);                 // t.phi is not read after phase 0
+  if (tl_next < n_tiles) fetch_state(tl_next);
   TICK(2);
   const double T = t.sc[SC_T * S + s], V = t.sc[SC_V * S + s], Pp = t.sc[SC_P * S + s], D = t.sc[SC_D * S + s];
   const double N = red_sum<S>(t.red, 0, s);
@@ -961,39 +1014,14 @@ jacobian_kernel(const DevMech m, const DevPlan pl, int mode, int64_t n_states, i
   if (DENSE)                                      // whatever is left of the zero fill
     for (int z = next_chunk(cnt + CNT_Z); z < n_zslices; z = next_chunk(cnt + CNT_Z)) zero_slice(z);
   TICK(6);
-  // every warp is done with the slots, and the prefetched phi of the next tile (issued after phase 1) has landed
-  asm volatile("cp.async.wait_all;" ::: "memory");
-  __syncthreads();
-  if (pl.jplan.n_comb + m.cplan.n_comb) {
-    // second pass over the split lists of both plans in ONE index space, with every table word (first partial,
-    // count, output positions) requested before the partial sums are added: one L2 round trip for the whole pass
-    const int nJ = pl.jplan.n_comb * S, nC = m.cplan.n_comb * S;
-    const double* __restrict__ part = t.part;
-    for (int idx = tid; idx < nJ + nC; idx += NT) {
-      if (idx < nJ) {
-        const int c = idx / S;
-        const int first = pl.jplan.part_base + __ldg(pl.jplan.comb_first + c), n = __ldg(pl.jplan.comb_nseg + c);
-        const int pos = __ldg(pl.jc_pos + c);
-        double v = 0.0;
-        for (int q = 0; q < n; ++q) v += part[(first + q) * S + s];
-        if (valid) st_out(out + obase + (int64_t)pos * tile, v);
-      } else {
-        const int c = (idx - nJ) / S;
-        const int first = m.cplan.part_base + 2 * __ldg(m.cplan.comb_first + c), n = __ldg(m.cplan.comb_nseg + c);
-        const int j = __ldg(m.cc_item + c);
-        const int2 pos = __ldg(reinterpret_cast<const int2*>(pl.cc_pos) + c);
-        double v0 = 0.0, v1 = 0.0;
-        for (int q = 0; q < n; ++q) { v0 += part[(first + 2 * q) * S + s]; v1 += part[(first + 2 * q + 1) * S + s]; }
-        if (valid) {
-          const double JT = -(v0 + fT * (t.ck[j * S + s] - cL)) * iDV;
-          st_out(out + obase + (int64_t)pos.x * tile, JT);
-          st_out(out + obase + (int64_t)pos.y * tile, cS * v1 + cT * JT);
-        }
-      }
-    }
-  }
+  have_prev = true; prev_valid = valid; prev_obase = obase; prev_fT = fT; prev_iDV = iDV; prev_cS = cS; prev_cT = cT; prev_cL = cL;
+  prev_ck = t.ck;
   TICK(5);
   }  // tiles of this CTA
+  if (have_prev && nJ2 + nC2 > 0) {            // the last tile's second pass
+    __syncthreads();
+    second_pass();
+  }
   if (tid == 0 && atomicAdd(sched + 1, 1ull) == (unsigned long long)gridDim.x - 1) { sched[0] = 0; sched[1] = 0; }
 }
 
