@@ -817,6 +817,7 @@ jacobian_kernel(const DevMech m, const DevPlan pl, int mode, int64_t n_states, i
     pT = src[0]; pE = src[tile]; pN = src[(int64_t)e_mine * tile]; pPar = param[sp];
   };
   fetch_state(blockIdx.x);
+  __syncthreads();                                 // NASA table and gather metadata are in place
   double* const ck_buf[2] = {t.ck, reinterpret_cast<double*>(t.phi)};
   __shared__ long long next_tile;
   int parity = 0;
