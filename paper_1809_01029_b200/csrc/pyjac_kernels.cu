@@ -94,6 +94,42 @@ template <int S> __device__ __forceinline__ double group_sum(double v) {
   return v;
 }
 
+// Eight per-state sums at once: in the rounds with offset 16, 8, 4 (those >= S) a lane keeps half of its values and
+// hands the other half to its partner, so the eight sums cost 4 + 2 + 1 + 1 + 1 = 9 shuffles instead of 40 (S = 1).
+// Afterwards a lane holds the sums j0 .. j0 + n - 1 of state lane % S (n = 1 for S <= 4, 2 / 4 / 8 for S = 8 / 16 / 32);
+// store(j, value) is called by exactly one lane per (j, state).
+template <int S, class StoreF>
+__device__ __forceinline__ void group_sum8(double (&v)[8], StoreF store) {
+  const int lane = threadIdx.x & 31;
+  int j0 = 0;
+  constexpr int N16 = S <= 16 ? 4 : 8, N8 = S <= 8 ? N16 / 2 : N16, N4 = S <= 4 ? N8 / 2 : N8;
+  if constexpr (S <= 16) {
+    const bool up = lane & 16;
+#pragma unroll
+    for (int i = 0; i < 4; ++i) { const double send = up ? v[i] : v[i + 4], keep = up ? v[i + 4] : v[i]; v[i] = keep + __shfl_xor_sync(0xffffffffu, send, 16); }
+    j0 += up ? 4 : 0;
+  }
+  if constexpr (S <= 8) {
+    const bool up = lane & 8;
+#pragma unroll
+    for (int i = 0; i < 2; ++i) { const double send = up ? v[i] : v[i + 2], keep = up ? v[i + 2] : v[i]; v[i] = keep + __shfl_xor_sync(0xffffffffu, send, 8); }
+    j0 += up ? 2 : 0;
+  }
+  if constexpr (S <= 4) {
+    const bool up = lane & 4;
+    const double send = up ? v[0] : v[1], keep = up ? v[1] : v[0];
+    v[0] = keep + __shfl_xor_sync(0xffffffffu, send, 4);
+    j0 += up ? 1 : 0;
+  }
+  if constexpr (S <= 2) v[0] += __shfl_xor_sync(0xffffffffu, v[0], 2);
+  if constexpr (S <= 1) v[0] += __shfl_xor_sync(0xffffffffu, v[0], 1);
+  constexpr int PLAIN = (S <= 2 ? 2 : 0) | (S <= 1 ? 1 : 0);     // lane bits summed over without splitting
+  if ((lane & PLAIN) == 0) {
+#pragma unroll
+    for (int i = 0; i < N4; ++i) store(j0 + i, v[i]);
+  }
+}
+
 // sum over the warps of reduction slot j of state s (partials written by phases01)
 template <int S> __device__ __forceinline__ double red_sum(const double* red, int j, int s) {
   double t = 0.0;
@@ -563,10 +599,15 @@ __device__ __forceinline__ void phases01(const DevMech& m, Tile<S, JAC>& t, int 
   // Consumers add the NW partials themselves (red_sum), which saves the second reduction stage and its barrier.
   {
     const int lane = tid & 31, warp = tid >> 5;
+    if constexpr (JAC) {
+      double v8[8] = {acc[0], acc[1], acc[2], acc[3], acc[4], acc[5], acc[6], 0.0};
+      group_sum8<S>(v8, [&](int j, double v) { if (j < 7) t.red[(warp * NRED + j) * S + (lane % S)] = v; });
+    } else {
 #pragma unroll
-    for (int j = 0; j < (JAC ? 7 : 2); ++j) {
-      const double v = group_sum<S>(acc[j]);
-      if (lane < S) t.red[(warp * NRED + j) * S + lane] = v;
+      for (int j = 0; j < 2; ++j) {
+        const double v = group_sum<S>(acc[j]);
+        if (lane < S) t.red[(warp * NRED + j) * S + lane] = v;
+      }
     }
   }
   __syncthreads();
