@@ -27,7 +27,7 @@ constexpr int INFO_OF_SHIFT = 16;    // bits 16-19: forward order  sum nu'
 constexpr int INFO_OR_SHIFT = 20;    // bits 20-23: reverse order  sum nu''
 constexpr uint32_t SIGN_BIT = 0x80000000u;
 constexpr int N_ZERO_SLOTS = 16;             // always-zero slots after the real ones: ELL padding, one per 8-byte bank
-constexpr int SEG_LEN_DEFAULT = 32;   // gather lists longer than this are split into segments (env PYJAC_SEG_LEN)
+constexpr int SEG_LEN_DEFAULT = 24;   // gather lists longer than this are split into segments (env PYJAC_SEG_LEN)
 
 enum OutFmt { OUT_CSR = 0, OUT_CSC = 1, OUT_DENSE_C = 2, OUT_DENSE_F = 3 };
 

@@ -43,7 +43,7 @@ namespace {
 #define PYJAC_UJ 4
 #endif
 #ifndef PYJAC_UC
-#define PYJAC_UC 1
+#define PYJAC_UC 2
 #endif
 #ifndef PYJAC_UNJ
 #define PYJAC_UNJ 4
