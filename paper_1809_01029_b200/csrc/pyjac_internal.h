@@ -32,8 +32,14 @@ constexpr int SEG_LEN_DEFAULT = 24;   // gather lists longer than this are split
 enum OutFmt { OUT_CSR = 0, OUT_CSC = 1, OUT_DENSE_C = 2, OUT_DENSE_F = 3 };
 
 constexpr int ELL_W = 128;           // items per ELL super-group (4 items per lane at one state per CTA)
-constexpr int ELL_W_NARROW = 512;    // items per NARROW super-group (segments of <= NARROW_LEN entries; species rows only)
-constexpr int NARROW_LEN = 2;
+#ifndef PYJAC_ELL_W_NARROW
+#define PYJAC_ELL_W_NARROW 512
+#endif
+#ifndef PYJAC_NARROW_LEN
+#define PYJAC_NARROW_LEN 2
+#endif
+constexpr int ELL_W_NARROW = PYJAC_ELL_W_NARROW;   // items per NARROW super-group (segments of <= NARROW_LEN entries; species rows only)
+constexpr int NARROW_LEN = PYJAC_NARROW_LEN;
 
 struct GatherPlan {
   int stride = 1;                            // ints per entry
