@@ -51,6 +51,9 @@ namespace {
 #ifndef PYJAC_UNC
 #define PYJAC_UNC 4
 #endif
+#ifndef PYJAC_UN1
+#define PYJAC_UN1 8     // narrow gather at one state per CTA: 8 segments per thread (two units per super-group: finer tail)
+#endif
 #ifndef PYJAC_ZERO_WARPS
 #define PYJAC_ZERO_WARPS 1
 #endif
@@ -1050,7 +1053,7 @@ jacobian_kernel(const DevMech m, const DevPlan pl, int mode, int64_t n_states, i
     const int n_wide = pl.jplan.n_wide;
     gather<S, 1, 1, PYJAC_UJ, PYJAC_UNJ, ELL_W, int>(pl.jplan.ell_ent, metaJ, n_wide, 0, cnt + CNT_J, accJ, posJ, storeJ, side);
     // the narrow tail (lists of one or two entries: most nonzeros of a sparse mechanism): 16 segments per thread
-    gather<S, 1, 1, ELL_W_NARROW / 32, 1, ELL_W_NARROW, int>(pl.jplan.ell_ent, metaJ + n_wide, pl.jplan.n_sg - n_wide, n_wide * ELL_W,
+    gather<S, 1, 1, (S == 1 && !DENSE ? PYJAC_UN1 : ELL_W_NARROW / 32), 1, ELL_W_NARROW, int>(pl.jplan.ell_ent, metaJ + n_wide, pl.jplan.n_sg - n_wide, n_wide * ELL_W,
                                               cnt + CNT_J2, accJ, posJ, storeN, side);
   }
   if (DENSE)                                      // whatever is left of the zero fill
