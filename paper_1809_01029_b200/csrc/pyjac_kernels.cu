@@ -904,7 +904,7 @@ jacobian_kernel(const DevMech m, const DevPlan pl, int mode, int64_t n_states, i
   // (with several states per CTA the sparse kernel derives these again after phase 1 instead of keeping them in
   // registers across it: C2 -2.7 %, C3 -3.6 %; at one state per CTA the same change cost 0.4 %)
   const int64_t s0_a = tl * S;
-  const bool valid_a = s0_a + s < n_states;
+  const bool valid_a = S == 1 || s0_a + s < n_states;   // one state per tile: every tile is a valid state
   const int64_t sg = min(s0_a + s, n_states - 1);   // ragged tail: recompute the last valid state, never store
   constexpr bool REDERIVE = !DENSE && S > 1;
   const int64_t obase_a = REDERIVE ? 0 : state_base(sg, tile, pl.n_e);
