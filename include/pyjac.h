@@ -157,6 +157,22 @@ int pyjac_eval_host(const pyjac_mech *mech, int what, int mode, int fmt, int64_t
 int pyjac_launch_info(const pyjac_mech *mech, int what, int32_t *states_per_cta, int32_t *threads,
                       int64_t *smem_bytes);
 
+/* Shape of the Jacobian kernel's gather plan, for reporting: info[0] = H (reaction blocks per
+ * state pair), [1] = value slots of the largest block, [2] = partial-sum slots, [3] = gather entries, [4] = stored
+ * entries (with ELL padding), [5] = groups, [6] = piece slots, [7] = lists cut into more than one piece. */
+int pyjac_plan_info(const pyjac_mech *mech, int64_t info[8]);
+
+/* Machine peaks measured on `cuda_device` (the denominators of the rooflines bench.py reports; SURVEY.md section
+ * 8d asks for a measured DFMA rate and a measured write-only stream instead of datasheet figures).  Each figure is
+ * timed with CUDA events around `reps` back-to-back launches after one warm-up launch; the call allocates its own
+ * scratch (up to 8 GiB for the copy) and synchronises.  *value: DFMA per second (PYJAC_PEAK_DFMA: 8 independent
+ * chains per thread, 2048 threads per SM) or bytes per second (the others: 4 GiB streams with 16-byte accesses;
+ * PYJAC_PEAK_L2_READ: every CTA sweeps one L2-resident 32 MiB window with ld.global.cg; PYJAC_PEAK_LDS:
+ * conflict-free 16-byte shared-memory loads). */
+enum { PYJAC_PEAK_DFMA = 0, PYJAC_PEAK_HBM_WRITE = 1, PYJAC_PEAK_HBM_READ = 2, PYJAC_PEAK_HBM_COPY = 3,
+       PYJAC_PEAK_L2_READ = 4, PYJAC_PEAK_LDS = 5 };
+int pyjac_measure_peak(int kind, int cuda_device, int reps, double *value);
+
 const char *pyjac_last_error(void); /* thread-local, never NULL */
 
 #ifdef __cplusplus

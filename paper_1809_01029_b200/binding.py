@@ -71,6 +71,8 @@ def lib():
         L.pyjac_jacobian_fd.argtypes = [vp, i32, i32, C.c_double, C.c_double, i64, i64, i64, vp, vp, vp, vp]
         L.pyjac_eval_host.argtypes = [vp, i32, i32, i32, i64, i64, i64, vp, vp, vp]
         L.pyjac_launch_info.argtypes = [vp, i32, _I, _I, C.POINTER(i64)]
+        L.pyjac_measure_peak.argtypes = [i32, i32, i32, _D]
+        L.pyjac_plan_info.argtypes = [vp, C.POINTER(i64)]
         _lib = L
     return _lib
 
@@ -160,6 +162,24 @@ def pyjac_launch_info(h, what):
     S, nt, sm = C.c_int32(), C.c_int32(), C.c_int64()
     _check(lib().pyjac_launch_info(h, what, C.byref(S), C.byref(nt), C.byref(sm)))
     return S.value, nt.value, sm.value
+
+
+def pyjac_plan_info(h):
+    """dict with the shape of the Jacobian kernel's gather plan (reporting only)."""
+    a = (C.c_int64 * 8)()
+    _check(lib().pyjac_plan_info(h, a))
+    return dict(zip(("blocks", "slots_per_block", "partial_slots", "entries", "stored_entries", "groups", "piece_slots",
+                     "split_lists"), [int(x) for x in a]))
+
+
+PEAK_DFMA, PEAK_HBM_WRITE, PEAK_HBM_READ, PEAK_HBM_COPY, PEAK_L2_READ, PEAK_LDS = range(6)
+
+
+def pyjac_measure_peak(kind, cuda_device=0, reps=5):
+    """DFMA/s (PEAK_DFMA) or bytes/s of the machine, measured with the library's own microbenchmarks."""
+    v = C.c_double()
+    _check(lib().pyjac_measure_peak(int(kind), int(cuda_device), int(reps), C.byref(v)))
+    return v.value
 
 
 class Mechanism:

@@ -3,6 +3,7 @@
 #include <cuda_runtime.h>
 
 #include <atomic>
+#include <mutex>
 #include <cstdio>
 #include <cstring>
 #include <new>
@@ -25,17 +26,26 @@ int cuda_fail(cudaError_t e, const char* what) {
 
 struct pyjac_mech {
   int device = 0;
+  int n_sm = 0;
   HostTables h;
+  JacTables j;
   DevMech dm{};
-  DevPlan plan[4]{};
+  DevJac dj{};
+  DevJacOut jout[4]{};
   std::vector<void*> allocs;
-  // tile-scheduler words of the persistent Jacobian kernel: a ring of N_SCHED zeroed pairs, one per launch in flight
-  // (the kernel resets its pair), so launches of one handle on different streams do not share a counter
+  // tile-scheduler words of the persistent Jacobian kernel: a ring of N_SCHED zeroed pairs (tile counter, finished
+  // CTAs; the kernel leaves its pair zero again).  A launch takes the next pair; the event recorded behind the launch
+  // that used the pair before tells whether that launch is still in flight (another stream), in which case the new
+  // launch is ordered behind it: two kernels in flight never share a counter.
   static constexpr unsigned N_SCHED = 64;
   unsigned long long* sched = nullptr;
-  mutable std::atomic<unsigned> sched_next{0};
+  mutable cudaEvent_t sched_ev[N_SCHED] = {};
+  mutable bool sched_used[N_SCHED] = {};
+  mutable unsigned sched_next = 0;
+  mutable std::mutex sched_mu;
   ~pyjac_mech() {
     for (void* p : allocs) cudaFree(p);
+    for (cudaEvent_t e : sched_ev) if (e) cudaEventDestroy(e);
   }
   int upload_plan(const GatherPlan& g, int part_base, DevGather* out) {
     out->n_sg = g.n_sg; out->n_wide = g.n_wide; out->n_comb = (int)g.comb_item.size(); out->part_base = part_base;
@@ -72,6 +82,7 @@ int pyjac_mech_create_ex(const pyjac_mech_desc* desc, int cuda_device, uint32_t 
   if (!m) return fail(PYJAC_ENOMEM, "out of host memory");
   std::string err;
   int rc = build_host_tables(desc, (flags & PYJAC_APPROX_JACOBIAN) != 0, m->h, err);
+  if (rc == PYJAC_OK) rc = build_jac_tables(m->h, m->j, err);
   if (rc != PYJAC_OK) { delete m; return fail(rc, err); }
   if (cuda_device == -1) { m->device = -1; *out = m; return PYJAC_OK; }   // host-only handle: pattern and dims only
   int ndev = 0;
@@ -87,6 +98,9 @@ int pyjac_mech_create_ex(const pyjac_mech_desc* desc, int cuda_device, uint32_t 
   auto body = [&]() -> int {
     CK(cudaSetDevice(cuda_device));
     if (int ea = set_kernel_attributes()) return cuda_fail((cudaError_t)ea, "cudaFuncSetAttribute");
+    if (int ea = set_kernel_attributes_jac()) return cuda_fail((cudaError_t)ea, "cudaFuncSetAttribute");
+    CK(cudaDeviceGetAttribute(&m->n_sm, cudaDevAttrMultiProcessorCount, cuda_device));
+    for (unsigned q = 0; q < pyjac_mech::N_SCHED; ++q) CK(cudaEventCreateWithFlags(&m->sched_ev[q], cudaEventDisableTiming));
     {
       void* p = nullptr;
       CK(cudaMalloc(&p, pyjac_mech::N_SCHED * 2 * sizeof(unsigned long long)));
@@ -112,21 +126,43 @@ int pyjac_mech_create_ex(const pyjac_mech_desc* desc, int cuda_device, uint32_t 
     if (int r_ = m->upload(h.csc_ptr, &d.csc_ptr)) return r_;
     if (int r_ = m->upload(h.csc_idx, &d.csc_idx)) return r_;
     if (int r_ = m->upload(h.csc2csr, &d.csc2csr)) return r_;
-    DevGather jplan;
-    if (int r_ = m->upload_plan(h.jplan, 0, &jplan)) return r_;
     const uint32_t* mask[2];
     for (int p = 0; p < 2; ++p)
       if (int r_ = m->upload(h.nzmask[p], &mask[p])) return r_;
-    for (int f = 0; f < 4; ++f) {
-      DevPlan& pl = m->plan[f];
-      pl.n_e = f < 2 ? h.nnz : (int64_t)h.nvar * h.nvar;
-      pl.jplan = jplan;
-      if (int r_ = m->upload(h.j_pos[f], &pl.j_pos)) return r_;
-      if (int r_ = m->upload(h.c_pos[f], &pl.c_pos)) return r_;
-      if (int r_ = m->upload(h.jc_pos[f], &pl.jc_pos)) return r_;
-      if (int r_ = m->upload(h.cc_pos[f], &pl.cc_pos)) return r_;
-      for (int j = 0; j < 4; ++j) pl.d_pos[j] = h.d_pos[f][j];
-      pl.nzmask = f < 2 ? nullptr : mask[f & 1];
+    // the Jacobian kernel's own tables (block order) and plan
+    {
+      const JacTables& j = m->j;
+      DevJac& q = m->dj;
+      q.ns = j.ns; q.nr = j.nr; q.nvar = j.nvar; q.H = j.H; q.ns_max = j.ns_max; q.n_val = j.n_val; q.max_nrb = j.max_nrb;
+      q.n_groups = (int)j.groups.size();
+      for (int b = 0; b <= j.H; ++b) q.blk_r0[b] = j.blk_r0[b];
+      for (int b = 0; b <= j.H + 1; ++b) q.blk_g0[b] = j.blk_g0[b];
+#define UPJ(field) if (int r_ = m->upload(j.field, &q.field)) return r_;
+      UPJ(lnA) UPJ(beta) UPJ(Ta) UPJ(dn) UPJ(info) UPJ(sp) UPJ(ext) UPJ(groups) UPJ(ent) UPJ(pidx) UPJ(item) UPJ(nplus)
+#undef UPJ
+      q.nasa = d.nasa; q.eff_sp = d.eff_sp; q.eff_d = d.eff_d; q.rev_par = d.rev_par; q.fall = d.fall;
+      q.plog_ptr = d.plog_ptr; q.plog_P = d.plog_P; q.plog_lnP = d.plog_lnP; q.plog_lnA = d.plog_lnA; q.plog_b = d.plog_b; q.plog_Ta = d.plog_Ta;
+      q.cheb_meta = d.cheb_meta; q.cheb_lim = d.cheb_lim; q.cheb_coef = d.cheb_coef;
+      for (int f = 0; f < 4; ++f) {
+        DevJacOut& jo = m->jout[f];
+        jo.n_e = f < 2 ? h.nnz : (int64_t)h.nvar * h.nvar;
+        jo.pos16 = f < 2 && h.nnz < 65535;            // 16-bit output positions (0xffff = none)
+        if (jo.pos16) {
+          std::vector<uint16_t> a(j.posA[f].size()), b(j.posB[f].size());
+          for (size_t e = 0; e < a.size(); ++e) { a[e] = (uint16_t)j.posA[f][e]; b[e] = (uint16_t)j.posB[f][e]; }   // J_NOPOS -> 0xffff
+          const uint16_t *pa = nullptr, *pb = nullptr;
+          if (int r_ = m->upload(a, &pa)) return r_;
+          if (int r_ = m->upload(b, &pb)) return r_;
+          jo.posA = pa; jo.posB = pb;
+        } else {
+          const uint32_t *pa = nullptr, *pb = nullptr;
+          if (int r_ = m->upload(j.posA[f], &pa)) return r_;
+          if (int r_ = m->upload(j.posB[f], &pb)) return r_;
+          jo.posA = pa; jo.posB = pb;
+        }
+        for (int c = 0; c < 4; ++c) jo.d_pos[c] = j.d_pos[f][c];
+        jo.nzmask = f < 2 ? nullptr : mask[f & 1];
+      }
     }
     CK(cudaDeviceSynchronize());
     return PYJAC_OK;
@@ -194,11 +230,17 @@ static int run_jac(const char* fn, const pyjac_mech* mech, int mode, int ofmt, i
                    const double* d_phi, const double* d_param, double* d_out, void* stream) {
   if (int rc = check_common(fn, mech, mode, n_states, ld, tile, d_phi, d_param, d_out)) return rc;
   if (n_states == 0) return PYJAC_OK;
-  const LaunchCfg cfg = choose_cfg(mech->h, true, tile, n_states);
-  if (cfg.smem > 227 * 1024) return fail(PYJAC_ENOMEM, std::string(fn) + ": mechanism too large for shared memory");
-  unsigned long long* sched = mech->sched + 2 * (mech->sched_next.fetch_add(1) % pyjac_mech::N_SCHED);
-  int e = launch_jacobian(mech->dm, mech->plan[ofmt], cfg, mode, n_states, ld, tile, d_phi, d_param, d_out, sched, stream);
-  if (e) return cuda_fail((cudaError_t)e, "jacobian_kernel launch");
+  const LaunchCfg cfg = choose_cfg_jac(mech->j, tile, n_states, mech->n_sm);
+  if (cfg.smem > J_SMEM_LIMIT) return fail(PYJAC_ENOMEM, std::string(fn) + ": mechanism too large for shared memory");
+  std::lock_guard<std::mutex> lock(mech->sched_mu);
+  const unsigned slot = mech->sched_next++ % pyjac_mech::N_SCHED;
+  if (mech->sched_used[slot] && cudaEventQuery(mech->sched_ev[slot]) == cudaErrorNotReady)
+    CK(cudaStreamWaitEvent((cudaStream_t)stream, mech->sched_ev[slot], 0));     // the pair's previous launch is still in flight
+  (void)cudaGetLastError();                                                       // cudaErrorNotReady is not an error
+  int e = launch_jacobian2(mech->dj, mech->jout[ofmt], cfg, mech->n_sm, mode, n_states, tile, d_phi, d_param, d_out, mech->sched + 2 * slot, stream);
+  if (e) return cuda_fail((cudaError_t)e, "jacobian kernel launch");
+  CK(cudaEventRecord(mech->sched_ev[slot], (cudaStream_t)stream));
+  mech->sched_used[slot] = true;
   return PYJAC_OK;
 }
 
@@ -236,10 +278,20 @@ int pyjac_jacobian_fd(const pyjac_mech* mech, int mode, int fmt, double rel_step
 
 int pyjac_launch_info(const pyjac_mech* mech, int what, int32_t* states_per_cta, int32_t* threads, int64_t* smem_bytes) {
   if (!mech) return fail(PYJAC_EINVAL, "pyjac_launch_info: null handle");
-  const LaunchCfg cfg = what == 3 ? choose_cfg_fd(mech->h) : choose_cfg(mech->h, what != 0, (int64_t)1 << 40, (int64_t)1 << 40);
+  const LaunchCfg cfg = what == 3 ? choose_cfg_fd(mech->h)
+                      : (what == 0 ? choose_cfg(mech->h, false, (int64_t)1 << 40, (int64_t)1 << 40)
+                                   : choose_cfg_jac(mech->j, (int64_t)1 << 40, (int64_t)1 << 40, mech->n_sm > 0 ? mech->n_sm : 148));
   if (states_per_cta) *states_per_cta = cfg.S;
   if (threads) *threads = cfg.threads;
   if (smem_bytes) *smem_bytes = (int64_t)cfg.smem;
+  return PYJAC_OK;
+}
+
+int pyjac_plan_info(const pyjac_mech* mech, int64_t info[8]) {
+  if (!mech || !info) return fail(PYJAC_EINVAL, "pyjac_plan_info: null argument");
+  const JacTables& j = mech->j;
+  info[0] = j.H; info[1] = j.ns_max; info[2] = j.n_part; info[3] = j.n_entries; info[4] = j.n_padded;
+  info[5] = (int64_t)j.groups.size(); info[6] = j.n_pieces; info[7] = j.n_span;
   return PYJAC_OK;
 }
 

@@ -487,6 +487,12 @@ int build_host_tables(const pyjac_mech_desc* d, bool approx, HostTables& h, std:
   for (int k = 0; k < L; ++k)
     for (auto& kv : rowmap[k]) { jitems.push_back({2 + k, 2 + kv.first}); jlists.push_back(kv.second); }
   h.nA = (int)jitems.size();
+  // raw gather lists (old slot numbering) for the block-partitioned plan of the Jacobian kernel (pyjac_plan.cpp)
+  h.raw_blk = jlists;
+  for (const Item& it : jitems) { h.blk_r.push_back(it.r); h.blk_c.push_back(it.c); }
+  h.raw_col = bl;
+  h.raw_row = cl;
+  h.csr2csc.assign(csr2csc.begin(), csr2csc.end());
   for (int col = 0; col < 2; ++col)
     for (int k = 0; k < L; ++k) {
       std::vector<int32_t> l = bl[k];

@@ -93,12 +93,76 @@ struct HostTables {
   std::vector<uint32_t> nzmask[2];           // dense bitmaps, bit e set iff dense element e ('C' / 'F' order) is in the pattern
   int nslots = 0;                            // total Jacobian slots
   int max_eff = 0;
+  // raw gather lists in the slot numbering above, consumed by build_jac_tables (pyjac_plan.cpp)
+  std::vector<std::vector<int32_t>> raw_blk;  // [nA] species-block nonzero -> entries (slot | sign), |nu| copies
+  std::vector<int32_t> blk_r, blk_c;          // [nA] matrix row / column of the nonzero
+  std::vector<std::vector<int32_t>> raw_col;  // [Ns-1] species k -> entries (slot_base[r] | sign): T and E columns
+  std::vector<std::vector<int32_t>> raw_row;  // [Ns-1] species j -> pairs (slot | sign, reaction): T and E rows
+  std::vector<int32_t> csr2csc;               // [nnz] CSC value position of CSR entry p
 };
 
 // returns PYJAC_OK or an error code with a message in err
 // approx: the "approximate" Jacobian of PAPER.md L313-317 (derivatives through the last species' concentration with
 // respect to the other species' moles are ignored: sparser pattern, inexact values)
 int build_host_tables(const pyjac_mech_desc* d, bool approx, HostTables& h, std::string& err);
+
+// ---- analytical Jacobian kernel (pyjac_jacobian.cuh): block-partitioned plan -----------------------------------
+// A thread owns one item for a PAIR of states (double2 everywhere).  The reactions are cut into H blocks so that the
+// per-reaction partials ("slots") of one block and two states fit in shared memory; a gather list is cut into PIECES,
+// one per (block, segment of <= J_SEG entries).  Pieces of one block are packed in groups of J_GW (ELL, padded,
+// entry-pair-major); a group is homogeneous in kind and class and stores its plus entries before its minus entries.
+constexpr int J_GW = 128;             // pieces per group
+constexpr int J_GW1 = 256;            // pieces per group of kind JK_BLK1 (lists of exactly one entry)
+constexpr int J_SEG = 24;             // longest piece (entries)
+constexpr int J_NZERO = 16;           // always-zero value slots: ELL padding points at the first 8 (one per 16-byte bank group); the JK_COL gather also reads slot + 8
+constexpr uint32_t J_NOPOS = 0xffffffffu;
+// kind of a piece: species-block nonzero; the same with exactly one entry; T and E columns of a species row (two
+// sums, slots v and v + 8); T and E rows of a species column (two sums weighted by dE~_i, dn~_i of the entry's
+// reaction); JK_ROWC: combine of T/E-row partial sums (gathers like JK_COL, finishes like JK_ROW)
+enum JKind { JK_BLK = 0, JK_BLK1 = 1, JK_COL = 2, JK_ROW = 3, JK_ROWC = 4 };
+// class of a piece: store the finished value; partial = sum; partial += sum; store partial + sum
+enum JCls { JC_OUT = 0, JC_FIRST = 1, JC_ADD = 2, JC_LAST = 3 };
+// nP2 / nM2: pair steps of plus / minus entries (JK_ROW; JK_BLK1: 1 / 0 or 0 / 1); JK_BLK, JK_COL, JK_ROWC: nP2 = pair
+// steps of the longest piece, nM2 = 0, and every piece has its own boundary (JacTables::nplus)
+struct JGroup { uint32_t ent_off, piece_off; uint8_t nP2, nM2, cls, kind; uint32_t cost; };   // 16 bytes
+// bits of JacTables::info
+constexpr uint32_t JI_TYPE_MASK = 7, JI_REV = 1u << 3, JI_T2 = 1u << 4, JI_ADEF = 1u << 5, JI_FAST = 1u << 6, JI_CHEM = 1u << 7;
+constexpr int JI_SNU_SHIFT = 8;       // bits 8-12: sum(nu) + 16
+constexpr int JI_NREAC_SHIFT = 13, JI_NPROD_SHIFT = 15, JI_OF_SHIFT = 17, JI_OR_SHIFT = 21;
+constexpr uint32_t JI_REVX = 1u << 25, JI_HASL = 1u << 26;
+
+struct JacTables {
+  int ns = 0, nr = 0, nvar = 0, H = 1;
+  std::vector<int32_t> old_of_new;           // new reaction index -> index in the HostTables order
+  std::vector<int32_t> blk_r0;               // [H+1] first reaction of every block
+  std::vector<double> lnA, beta, Ta, dn;     // [nr]
+  std::vector<uint32_t> info;                // [nr]
+  std::vector<uint32_t> sp;                  // [nr*4]: species 0|1, 2|3, 4|5 (16 bits each; unused = ns), slot base | nu bits << 16
+  std::vector<int32_t> ext;                  // [nr*4]: aux, first efficiency, number of efficiencies, HostTables index
+  int ns_max = 0;                            // value slots of the largest block (multiple of 8)
+  int n_part = 0;                            // partial-sum slots
+  int n_val = 0;                             // value space: ns_max + J_NZERO + n_part   (<= 65535: 16-bit entries)
+  int max_nrb = 0;                           // reactions of the largest block
+  std::vector<JGroup> groups;                // block by block, descending cost inside a block
+  std::vector<int32_t> blk_g0;               // [H+2]; block H = the final combine wave
+  std::vector<uint32_t> ent;                 // entries
+  std::vector<uint32_t> posA[4], posB[4];    // [OutFmt][piece slot] output element (J_NOPOS: none)
+  std::vector<uint16_t> pidx, item;          // [piece slot] partial slot; species column (JK_ROW, JK_ROWC)
+  std::vector<uint8_t> nplus;                // [piece slot] JK_BLK / JK_COL / JK_ROWC: pair steps of plus entries (then minus)
+  int n_pieces = 0;
+  int32_t d_pos[4][4];
+  int64_t n_entries = 0, n_padded = 0;       // real / stored entries
+  int n_span = 0;                            // lists with more than one piece
+};
+constexpr int J_NT = 512, J_NW = J_NT / 32;   // threads / warps of the Jacobian kernel
+constexpr int J_NSC = 24;                     // per-pair scalars kept in shared memory
+constexpr int J_NRED = 12;                    // reduction words per warp: 0-6 reaction sums, 8-10 species sums
+constexpr int J_MAXH = 8;
+// bytes of dynamic shared memory of the Jacobian kernel with LS state pairs per item
+size_t jac_smem_bytes(const JacTables& j, int LS);
+constexpr size_t J_SMEM_LIMIT = 227 * 1024 - 256;   // dynamic part; the rest: static counters
+// builds the plan with the smallest H whose footprint at one state pair per item fits; PYJAC_ENOMEM if none does
+int build_jac_tables(const HostTables& h, JacTables& j, std::string& err);
 
 // ---- device views ------------------------------------------------------------------------------
 struct DevGather {
@@ -134,6 +198,36 @@ struct DevPlan {
   const uint32_t* nzmask;    // dense only (else nullptr)
 };
 
+// device view of JacTables (+ the type-specific parameter tables it shares with DevMech)
+struct DevJac {
+  int ns, nr, nvar, H, ns_max, n_val, max_nrb, n_groups;
+  int blk_r0[J_MAXH + 1], blk_g0[J_MAXH + 2];
+  const double *lnA, *beta, *Ta, *dn;
+  const uint32_t* info;
+  const uint32_t* sp;         // uint4 per reaction
+  const int32_t* ext;         // int4 per reaction
+  const JGroup* groups;
+  const uint32_t* ent;
+  const uint16_t *pidx, *item;
+  const uint8_t* nplus;
+  const double* nasa;
+  const int32_t* eff_sp;
+  const double* eff_d;
+  const double* rev_par;
+  const double* fall;
+  const int32_t* plog_ptr;
+  const double *plog_P, *plog_lnP, *plog_lnA, *plog_b, *plog_Ta;
+  const int32_t* cheb_meta;
+  const double *cheb_lim, *cheb_coef;
+};
+struct DevJacOut {
+  int64_t n_e;                // elements per state in the output (nnz or nvar^2)
+  const void *posA, *posB;    // uint16_t (pos16) or uint32_t per piece slot
+  int pos16;
+  int32_t d_pos[4];
+  const uint32_t* nzmask;     // dense only (else nullptr)
+};
+
 struct LaunchCfg { int S, threads; size_t smem; };
 
 // what: 0 source, 1 jacobian.  Chooses states-per-CTA from the shared-memory footprint and `tile`.
@@ -144,6 +238,11 @@ int launch_source(const DevMech& m, const LaunchCfg& cfg, int mode, int64_t n_st
                   const double* phi, const double* param, double* out, void* stream);
 int launch_jacobian(const DevMech& m, const DevPlan& p, const LaunchCfg& cfg, int mode, int64_t n_states, int64_t ld,
                     int64_t tile, const double* phi, const double* param, double* out, unsigned long long* sched, void* stream);
+// the pair-of-states Jacobian kernel (pyjac_jacobian.cuh).  LS = state pairs per item (1, 2 or 4: 2 LS states per CTA)
+LaunchCfg choose_cfg_jac(const JacTables& j, int64_t tile, int64_t n_states, int n_sm);
+int launch_jacobian2(const DevJac& m, const DevJacOut& o, const LaunchCfg& cfg, int n_sm, int mode, int64_t n_states, int64_t tile,
+                     const double* phi, const double* param, double* out, unsigned long long* sched, void* stream);
+int set_kernel_attributes_jac();
 // sched: two zero-initialised 64-bit words in device memory (tile counter, finished CTAs) that no other launch in
 // flight uses; the kernel leaves them zero again.
 // first-order forward finite-difference Jacobian.  ofmt: OutFmt.  S = columns per pass.

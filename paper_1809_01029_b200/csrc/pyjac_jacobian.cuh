@@ -1,0 +1,773 @@
+// Analytical Jacobian kernel for sm_100a (steps a1-a6, a8-a11 of SURVEY.md section 8a), fp64.
+//
+// A CTA owns a tile of S = 2 LS states and keeps every per-state intermediate on chip.  A THREAD OWNS ONE ITEM FOR A
+// PAIR OF STATES: every value is a double2, so table words, plan entries, indices and addresses are decoded once per
+// two states, shared memory is read with 16-byte loads and every nonzero leaves the SM as one 16-byte store.
+//   phase 0  items = species         : concentrations (Eq. 6-7), NASA-7 thermo, D = sum C_k c_k
+//   for every reaction block b (the reactions are cut into H blocks so that one block's partials fit, pyjac_plan.cpp):
+//     phase 1  items = reactions     : k_f, K_c, k_r, third body / falloff, rates of progress and the per-reaction
+//                                      partials dq_i/dT, dq_i/dE, dQ_i/dC_j -> value slots in shared memory
+//     phase 2  items = list pieces   : every Jacobian nonzero gathers its static list of slots (plus entries, then minus
+//                                      entries: no per-entry sign arithmetic); a list inside one block is finished in
+//                                      registers and stored ONCE, a list that spans blocks carries a partial sum
+//   final wave: lists with several segments per block are combined from their partial sums
+// Replaces the paper's zero-fill + "J[idx] += ..." read-modify-write and its run-time index search
+// (PAPER.md L345).  No tensor cores (nothing here is a dense contraction), no fast-math.
+#pragma once
+#include <cuda_runtime.h>
+
+#include "pyjac_internal.h"
+
+namespace pyjac {
+namespace jac2 {
+
+constexpr int NT = J_NT, NW = J_NW;
+
+struct D2 { double a, b; };
+__device__ __forceinline__ D2 mk(double a, double b) { D2 r; r.a = a; r.b = b; return r; }
+__device__ __forceinline__ D2 mk(double a) { return mk(a, a); }
+__device__ __forceinline__ D2 operator+(D2 x, D2 y) { return mk(x.a + y.a, x.b + y.b); }
+__device__ __forceinline__ D2 operator-(D2 x, D2 y) { return mk(x.a - y.a, x.b - y.b); }
+__device__ __forceinline__ D2 operator*(D2 x, D2 y) { return mk(x.a * y.a, x.b * y.b); }
+__device__ __forceinline__ D2 operator*(D2 x, double y) { return mk(x.a * y, x.b * y); }
+__device__ __forceinline__ D2 operator*(double y, D2 x) { return mk(x.a * y, x.b * y); }
+__device__ __forceinline__ D2 operator+(D2 x, double y) { return mk(x.a + y, x.b + y); }
+__device__ __forceinline__ D2 operator-(D2 x, double y) { return mk(x.a - y, x.b - y); }
+__device__ __forceinline__ D2 operator-(D2 x) { return mk(-x.a, -x.b); }
+__device__ __forceinline__ D2& operator+=(D2& x, D2 y) { x.a += y.a; x.b += y.b; return x; }
+__device__ __forceinline__ D2& operator-=(D2& x, D2 y) { x.a -= y.a; x.b -= y.b; return x; }
+__device__ __forceinline__ D2 fma2(D2 x, D2 y, D2 z) { return mk(fma(x.a, y.a, z.a), fma(x.b, y.b, z.b)); }
+__device__ __forceinline__ D2 fma2(double x, D2 y, D2 z) { return mk(fma(x, y.a, z.a), fma(x, y.b, z.b)); }
+__device__ __forceinline__ D2 exp2_(D2 x) { return mk(exp(x.a), exp(x.b)); }
+__device__ __forceinline__ D2 ld2(const D2* p) { const double2 v = *reinterpret_cast<const double2*>(p); return mk(v.x, v.y); }
+__device__ __forceinline__ void st2(D2* p, D2 v) { *reinterpret_cast<double2*>(p) = make_double2(v.a, v.b); }
+__device__ __forceinline__ D2 shfl_xor2(D2 v, int o) { return mk(__shfl_xor_sync(0xffffffffu, v.a, o), __shfl_xor_sync(0xffffffffu, v.b, o)); }
+
+// per-pair scalars in shared memory
+enum { SC_T = 0, SC_V, SC_P, SC_INVT, SC_LNT, SC_CTOT, SC_RT, SC_LNP, SC_LNPRT, SC_EL, SC_CL, SC_DCL, SC_D, SC_DDDT, NSC_USED };
+static_assert(NSC_USED <= J_NSC, "scalar area too small");
+
+__device__ __forceinline__ int next_chunk(int* counter) {
+  int c = 0;
+  if ((threadIdx.x & 31) == 0) c = atomicAdd(counter, 1);
+  return __shfl_sync(0xffffffffu, c, 0);
+}
+
+__device__ __forceinline__ int64_t state_base(int64_t s, int64_t tile, int64_t n_e) { return (s / tile) * (n_e * tile) + (s % tile); }
+
+__device__ __forceinline__ double ipow(double x, int n) {   // n in 0..3
+  double r = 1.0;
+  if (n >= 1) r = x;
+  if (n >= 2) r *= x;
+  if (n >= 3) r *= x;
+  return r;
+}
+__device__ __forceinline__ double dpow(double x, int n) {   // n x^(n-1)
+  return n == 0 ? 0.0 : (n == 1 ? 1.0 : (n == 2 ? 2.0 * x : 3.0 * x * x));
+}
+
+struct Blend { double F, dF_dPr, dF_dT; };
+// Troe / SRI blending function and its partial derivatives (R2, R4-5)
+static __device__ __noinline__ Blend blend(int type, bool hasT2, const double* __restrict__ fp, double T, double invT, double lnT, double Pr_in) {
+  Blend b; b.F = 1.0; b.dF_dPr = 0.0; b.dF_dT = 0.0;
+  const double LN10 = 2.302585092994045684, ILN10 = 0.434294481903251828;
+  const double Pr = fmax(Pr_in, 1e-300);
+  if (type == PYJAC_FALLOFF_TROE) {
+    const double a = fp[4], iT3 = 1.0 / fp[5], iT1 = 1.0 / fp[6], T2 = fp[7];
+    const double e3 = exp(-T * iT3), e1 = exp(-T * iT1);
+    double Fc = (1.0 - a) * e3 + a * e1;
+    double dFc = -(1.0 - a) * iT3 * e3 - a * iT1 * e1;
+    if (hasT2) { const double e2 = exp(-T2 * invT); Fc += e2; dFc += T2 * invT * invT * e2; }
+    const double L = log(Pr) * ILN10, Lc = log(Fc) * ILN10;
+    const double n = 0.75 - 1.27 * Lc;
+    const double A = L - 0.4 - 0.67 * Lc;
+    const double B = n - 0.14 * A;
+    const double iB = 1.0 / B;
+    const double f = A * iB;
+    const double g = 1.0 / (1.0 + f * f);
+    b.F = exp(LN10 * Lc * g);
+    const double dlogF_df = -2.0 * Lc * f * g * g;
+    const double df_dL = n * iB * iB;
+    const double df_dLc = (-0.67 * B + 1.1762 * A) * iB * iB;
+    b.dF_dPr = b.F * dlogF_df * df_dL / Pr;
+    b.dF_dT = b.F * (g + dlogF_df * df_dLc) * dFc / Fc;
+  } else if (type == PYJAC_FALLOFF_SRI) {
+    const double a = fp[4], bb = fp[5], ic = 1.0 / fp[6], d = fp[7], e = fp[8];
+    const double L = log(Pr) * ILN10;
+    const double X = 1.0 / (1.0 + L * L);
+    const double eb = exp(-bb * invT), ec = exp(-T * ic);
+    const double base = a * eb + ec;
+    const double dbase = a * bb * invT * invT * eb - ec * ic;
+    const double lb = log(base);
+    b.F = d * exp(X * lb + e * lnT);
+    b.dF_dPr = b.F * lb * (-2.0 * L * X * X) * ILN10 / Pr;
+    b.dF_dT = b.F * (X * dbase / base + e * invT);
+  }
+  return b;
+}
+
+// shared-memory carve-up (units of D2 unless noted); every per-pair array is [index][LS]
+template <int LS>
+struct Smem {
+  D2 *sc, *C, *G, *Hh, *K, *dE, *V, *red;
+  double* dn;
+  int4* grp;
+  __device__ __forceinline__ Smem(unsigned char* raw, const DevJac& m) {
+    sc = reinterpret_cast<D2*>(raw);
+    C = sc + J_NSC * LS; G = C + (m.ns + 1) * LS; Hh = G + (m.ns + 1) * LS; K = Hh + (m.ns + 1) * LS;
+    dE = K + (m.ns + 1) * LS; V = dE + m.max_nrb * LS; red = V + m.n_val * LS;
+    dn = reinterpret_cast<double*>(red + NW * J_NRED * LS);
+    grp = reinterpret_cast<int4*>(dn + ((m.nr + 1) & ~1));
+  }
+};
+
+// where this thread's pair of states lives in the output
+struct Out {
+  double *pa, *pb;     // element 0 of state a / b
+  int64_t tile;
+  bool va, vb, vec;    // state valid; 16-byte store possible (tile even: the two states are adjacent)
+  __device__ __forceinline__ void store(uint32_t pos, D2 v) const {
+    const int64_t off = (int64_t)pos * tile;
+    if (vec) {
+      if (vb) __stcs(reinterpret_cast<double2*>(pa + off), make_double2(v.a, v.b));
+      else if (va) __stcs(pa + off, v.a);
+    } else {
+      if (va) __stcs(pa + off, v.a);
+      if (vb) __stcs(pb + off, v.b);
+    }
+  }
+};
+
+template <class PosT> __device__ __forceinline__ bool has_pos(PosT p) { return p != (PosT)~(PosT)0; }
+
+// ---------------------------------------------------------------------------------------------------
+// phase 2: the gather engine.  A unit = U x (32 / LS) pieces of one group; a thread owns U pieces (U independent
+// chains of loads per step) for its pair of states.
+// ---------------------------------------------------------------------------------------------------
+template <int LS, class PosT>
+__device__ __forceinline__ void gather_unit(const DevJac& m, const DevJacOut& o, const Smem<LS>& sm, const JGroup g, int sub,
+                                            const Out& out, bool conp, int blk_r0) {
+  constexpr int IPW = 32 / LS, U = 4;
+  const int lane = threadIdx.x & 31, pr = lane % LS, il = lane / LS;
+  const D2* __restrict__ V = sm.V + pr;
+  const PosT* __restrict__ posA = reinterpret_cast<const PosT*>(o.posA) + g.piece_off;
+  const PosT* __restrict__ posB = reinterpret_cast<const PosT*>(o.posB) + g.piece_off;
+  const uint16_t* __restrict__ pidx = m.pidx + g.piece_off;
+  const uint8_t* __restrict__ nplus = m.nplus + g.piece_off;
+  const int cls = g.cls;
+  if (g.kind == JK_BLK1) {
+    // lists of exactly one entry: J_GW1 pieces per group, 2 U per thread and unit
+    constexpr int U1 = 2 * U;
+    const int p0 = sub * (U1 * IPW) + il;
+    const uint16_t* __restrict__ e = reinterpret_cast<const uint16_t*>(m.ent + g.ent_off) + p0;
+    uint32_t idx[U1]; PosT pos[U1];
+#pragma unroll
+    for (int u = 0; u < U1; ++u) { idx[u] = __ldg(e + u * IPW); pos[u] = __ldg(posA + p0 + u * IPW); }
+    const bool minus = g.nM2 != 0;
+#pragma unroll
+    for (int u = 0; u < U1; ++u) {
+      D2 v = ld2(V + idx[u] * LS);
+      if (minus) v = -v;
+      if (has_pos(pos[u])) out.store(pos[u], v);
+    }
+    return;
+  }
+  const int p0 = sub * (U * IPW) + il;
+  const int nP2 = g.nP2, nM2 = g.nM2;
+  if (g.kind == JK_BLK) {
+    const uint32_t* __restrict__ e = m.ent + g.ent_off + p0;
+    PosT pos[U]; uint32_t pi[U];
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+      pos[u] = (cls == JC_OUT || cls == JC_LAST) ? __ldg(posA + p0 + u * IPW) : (PosT)0;
+      pi[u] = cls != JC_OUT ? __ldg(pidx + p0 + u * IPW) : 0u;
+    }
+    D2 v[U];
+    int np[U];
+#pragma unroll
+    for (int u = 0; u < U; ++u) { v[u] = mk(0.0); np[u] = __ldg(nplus + p0 + u * IPW); }
+    // entries 2 s and 2 s + 1 of a piece have one sign: plus while s < nplus, then minus (a multiplier of +-1 in the
+    // DFMA: no sign arithmetic on the values)
+#pragma unroll 2
+    for (int s = 0; s < nP2; ++s) {
+      uint32_t w[U];
+#pragma unroll
+      for (int u = 0; u < U; ++u) w[u] = __ldg(e + s * J_GW + u * IPW);
+#pragma unroll
+      for (int u = 0; u < U; ++u) {
+        const double sg = s < np[u] ? 1.0 : -1.0;
+        v[u] = fma2(sg, ld2(V + (w[u] & 0xffffu) * LS), v[u]);
+        v[u] = fma2(sg, ld2(V + (w[u] >> 16) * LS), v[u]);
+      }
+    }
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+      D2* part = sm.V + pi[u] * LS + pr;
+      if (cls == JC_OUT) { if (has_pos(pos[u])) out.store(pos[u], v[u]); }
+      else if (cls == JC_FIRST) st2(part, v[u]);
+      else if (cls == JC_ADD) st2(part, ld2(part) + v[u]);
+      else if (has_pos(pos[u])) out.store(pos[u], v[u] + ld2(part));
+    }
+    return;
+  }
+  // two sums per piece
+  PosT pa[U], pb[U]; uint32_t pi[U], it[U];
+#pragma unroll
+  for (int u = 0; u < U; ++u) {
+    const bool fin = cls == JC_OUT || cls == JC_LAST;
+    pa[u] = fin ? __ldg(posA + p0 + u * IPW) : (PosT)0;
+    pb[u] = fin ? __ldg(posB + p0 + u * IPW) : (PosT)0;
+    pi[u] = cls != JC_OUT ? __ldg(pidx + p0 + u * IPW) : 0u;
+    it[u] = fin && g.kind != JK_COL ? __ldg(m.item + g.piece_off + p0 + u * IPW) : 0u;
+  }
+  D2 v0[U], v1[U];
+#pragma unroll
+  for (int u = 0; u < U; ++u) { v0[u] = mk(0.0); v1[u] = mk(0.0); }
+  if (g.kind == JK_ROW) {
+    // J[T][j] ~ sum_i dE~_i g_ij, J[E][j] ~ sum_i dn~_i g_ij: entry = slot | reaction-in-block << 16
+    const uint2* __restrict__ e = reinterpret_cast<const uint2*>(m.ent + g.ent_off) + p0;
+    const D2* __restrict__ dE = sm.dE + pr;
+    const double* __restrict__ dn = sm.dn + blk_r0;
+    auto acc = [&](uint32_t w, int u, bool minus) {
+      const D2 x = ld2(V + (w & 0xffffu) * LS);
+      const D2 de = ld2(dE + (w >> 16) * LS);
+      const double d = dn[w >> 16];
+      if (!minus) { v0[u] = fma2(de, x, v0[u]); v1[u] = fma2(d, x, v1[u]); }
+      else { v0[u] = fma2(-de, x, v0[u]); v1[u] = fma2(-d, x, v1[u]); }
+    };
+    for (int s = 0; s < nP2; ++s) {
+      uint2 w[U];
+#pragma unroll
+      for (int u = 0; u < U; ++u) w[u] = __ldg(e + s * J_GW + u * IPW);
+#pragma unroll
+      for (int u = 0; u < U; ++u) { acc(w[u].x, u, false); acc(w[u].y, u, false); }
+    }
+    e += nP2 * J_GW;
+    for (int s = 0; s < nM2; ++s) {
+      uint2 w[U];
+#pragma unroll
+      for (int u = 0; u < U; ++u) w[u] = __ldg(e + s * J_GW + u * IPW);
+#pragma unroll
+      for (int u = 0; u < U; ++u) { acc(w[u].x, u, true); acc(w[u].y, u, true); }
+    }
+  } else {
+    // JK_COL: J[k][T] = sum_i nu_ki slotT_i, J[k][E] = sum_i nu_ki slotE_i (slot E = slot T + 8); JK_ROWC: partial sums
+    const uint32_t* __restrict__ e = m.ent + g.ent_off + p0;
+    const D2* __restrict__ V8 = V + 8 * LS;
+    int np[U];
+#pragma unroll
+    for (int u = 0; u < U; ++u) np[u] = __ldg(nplus + p0 + u * IPW);
+    for (int s = 0; s < nP2; ++s) {
+      uint32_t w[U];
+#pragma unroll
+      for (int u = 0; u < U; ++u) w[u] = __ldg(e + s * J_GW + u * IPW);
+#pragma unroll
+      for (int u = 0; u < U; ++u) {
+        const uint32_t i0 = (w[u] & 0xffffu) * LS, i1 = (w[u] >> 16) * LS;
+        const double sg = s < np[u] ? 1.0 : -1.0;
+        v0[u] = fma2(sg, ld2(V + i0), v0[u]); v1[u] = fma2(sg, ld2(V8 + i0), v1[u]);
+        v0[u] = fma2(sg, ld2(V + i1), v0[u]); v1[u] = fma2(sg, ld2(V8 + i1), v1[u]);
+      }
+    }
+  }
+  // factors of the T / E rows (only units that finish such rows get here with kind != JK_COL: a few per tile)
+  D2 fT = mk(0.0), iDV = mk(0.0), cS = mk(0.0), cT = mk(0.0), cL = mk(0.0);
+  if (g.kind != JK_COL && (cls == JC_OUT || cls == JC_LAST)) {
+    D2 N = mk(0.0);
+    for (int w = 0; w < NW; ++w) N += ld2(sm.red + (w * J_NRED + 0) * LS + pr);
+    const D2 D = ld2(sm.sc + SC_D * LS + pr), T = ld2(sm.sc + SC_T * LS + pr), V_ = ld2(sm.sc + SC_V * LS + pr), Pp = ld2(sm.sc + SC_P * LS + pr);
+    fT = mk(-N.a / D.a, -N.b / D.b);
+    iDV = mk(1.0 / (D.a * V_.a), 1.0 / (D.b * V_.b));
+    cS = conp ? mk(T.a * R_GAS / Pp.a, T.b * R_GAS / Pp.b) : mk(T.a * R_GAS / V_.a, T.b * R_GAS / V_.b);
+    cT = conp ? mk(V_.a / T.a, V_.b / T.b) : mk(Pp.a / T.a, Pp.b / T.b);
+    cL = ld2(sm.sc + SC_CL * LS + pr);
+  }
+#pragma unroll
+  for (int u = 0; u < U; ++u) {
+    D2* part = sm.V + pi[u] * LS + pr;
+    if (cls == JC_FIRST) { st2(part, v0[u]); st2(part + 8 * LS, v1[u]); continue; }
+    if (cls == JC_ADD) { st2(part, ld2(part) + v0[u]); st2(part + 8 * LS, ld2(part + 8 * LS) + v1[u]); continue; }
+    if (cls == JC_LAST) { v0[u] += ld2(part); v1[u] += ld2(part + 8 * LS); }
+    if (!has_pos(pa[u])) continue;
+    if (g.kind == JK_COL) { out.store(pa[u], v0[u]); out.store(pb[u], v1[u]); }
+    else {
+      // a10: J[T][j] = -(sum_i dE~_i g_ij + f_T (c_j - c_Ns)) / (D V);  J[E][j] = cS sum_i dn~_i g_ij + cT J[T][j]
+      const D2 cj = ld2(sm.K + it[u] * LS + pr);
+      const D2 JT = -((v0[u] + fT * (cj - cL)) * iDV);
+      out.store(pa[u], JT);
+      out.store(pb[u], cS * v1[u] + cT * JT);
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------
+// phase 1, general path (any reaction type, any coefficients, the last species in any role): one STATE at a time,
+// scalar code.  Shared arrays are addressed as doubles: element (i, pair, st) at ((i * LS + pr) * 2 + st).
+// Returns the reaction's contributions to the seven reaction sums in inc[].
+// ---------------------------------------------------------------------------------------------------
+template <int LS>
+__device__ __forceinline__ void reaction_general(const DevJac& m, const Smem<LS>& sm, int r, int lr, int pr, int st, bool conp,
+                                              uint32_t info, uint4 spw, double (&inc)[7]) {
+  const int ns = m.ns, L = ns - 1;
+  const double* __restrict__ scd = reinterpret_cast<const double*>(sm.sc);
+  auto sc = [&](int i) { return scd[(i * LS + pr) * 2 + st]; };
+  auto sp_arr = [&](const D2* a, int k) { return reinterpret_cast<const double*>(a)[(k * LS + pr) * 2 + st]; };
+  const double T = sc(SC_T), V = sc(SC_V), Pp = sc(SC_P), invT = sc(SC_INVT), lnT = sc(SC_LNT), Ctot = sc(SC_CTOT), RT = sc(SC_RT);
+  const double lnP = sc(SC_LNP), ln_patm_rt = sc(SC_LNPRT), eL = sc(SC_EL), cL = sc(SC_CL);
+  const double ctot_T = Ctot * invT;
+  const int type = info & JI_TYPE_MASK;
+  const bool rev = info & JI_REV;
+  const int4 ext = __ldg(reinterpret_cast<const int4*>(m.ext) + r);
+  const int rx_aux = ext.x, e0 = ext.y, e1 = ext.y + ext.z;
+  const double rx_lnA = __ldg(m.lnA + r), rx_beta = __ldg(m.beta + r), rx_Ta = __ldg(m.Ta + r), dn = sm.dn[r];
+  // a3: forward rate constant
+  double lnkf, lam_f, dlnk_dP = 0.0;
+  if (type <= PYJAC_FALLOFF_SRI) {
+    lnkf = rx_lnA + rx_beta * lnT - rx_Ta * invT;
+    lam_f = (rx_beta + rx_Ta * invT) * invT;
+  } else if (type == PYJAC_PLOG) {
+    const int p0 = __ldg(m.plog_ptr + rx_aux), np = __ldg(m.plog_ptr + rx_aux + 1) - p0;
+    int cnt_le = 0;                                   // number of table pressures <= P
+    for (int q = 0; q < np; ++q) cnt_le += __ldg(m.plog_P + p0 + q) <= Pp ? 1 : 0;
+    // P <= P_0: first point; P >= P_last: last point; else interval j = last j with P_j <= P (S4)
+    const bool interp = cnt_le >= 1 && cnt_le < np && !(cnt_le == 1 && Pp <= __ldg(m.plog_P + p0));
+    const int j = cnt_le >= np ? np - 1 : (cnt_le >= 1 ? cnt_le - 1 : 0);
+    const int j1 = interp ? j + 1 : j;
+    const double b0 = __ldg(m.plog_b + p0 + j), Ta0 = __ldg(m.plog_Ta + p0 + j), lA0 = __ldg(m.plog_lnA + p0 + j), lP0 = __ldg(m.plog_lnP + p0 + j);
+    const double b1 = __ldg(m.plog_b + p0 + j1), Ta1 = __ldg(m.plog_Ta + p0 + j1), lA1 = __ldg(m.plog_lnA + p0 + j1), lP1 = __ldg(m.plog_lnP + p0 + j1);
+    const double l0 = lA0 + b0 * lnT - Ta0 * invT;
+    const double lam0 = (b0 + Ta0 * invT) * invT;
+    lnkf = l0; lam_f = lam0;
+    if (interp) {
+      const double l1 = lA1 + b1 * lnT - Ta1 * invT;
+      const double lam1 = (b1 + Ta1 * invT) * invT;
+      const double idl = 1.0 / (lP1 - lP0);
+      const double w = (lnP - lP0) * idl;
+      lnkf = l0 + (l1 - l0) * w;
+      lam_f = (1.0 - w) * lam0 + w * lam1;
+      dlnk_dP = (l1 - l0) * idl / Pp;
+    }
+  } else {
+    const double LN10 = 2.302585092994045684, ILN10 = 0.434294481903251828;
+    const int4 cm = __ldg(reinterpret_cast<const int4*>(m.cheb_meta) + rx_aux);          // nT, nP, coefficient offset
+    const double2 cl0 = __ldg(reinterpret_cast<const double2*>(m.cheb_lim) + 2 * rx_aux);
+    const double2 cl1 = __ldg(reinterpret_cast<const double2*>(m.cheb_lim) + 2 * rx_aux + 1);
+    const int nP = cm.y, n_coef = cm.x * cm.y;
+    const double* __restrict__ eta = m.cheb_coef + cm.z;
+    const double iTmin = cl0.x, iTmax = cl0.y, lPmin = cl1.x, lPmax = cl1.y;
+    const double Tr = (2.0 * invT - iTmin - iTmax) / (iTmax - iTmin);
+    const double Pr_ = (2.0 * lnP * ILN10 - lPmin - lPmax) / (lPmax - lPmin);
+    double lg = 0.0, dlg_dT = 0.0, dlg_dP = 0.0;
+    // the row-major coefficients are consumed in order by a running pair of three-term recurrences
+    double cT = 1.0, cTm = 0.0, dT = 0.0, dTm = 0.0;       // T_a(Tr), T_{a-1}, derivatives
+    double cP = 1.0, cPm = 0.0, dP = 0.0, dPm = 0.0;
+    int ia = 0, ib = 0;
+    for (int q = 0; q < n_coef; ++q) {
+      const double e = __ldg(eta + q);
+      lg += e * cT * cP; dlg_dT += e * dT * cP; dlg_dP += e * cT * dP;
+      if (++ib == nP) {                    // next row: advance T_a, restart T_b
+        ib = 0; ++ia;
+        if (ia == 1) { cTm = 1.0; cT = Tr; dTm = 0.0; dT = 1.0; }
+        else { const double n1 = 2.0 * Tr * cT - cTm, d1 = 2.0 * cT + 2.0 * Tr * dT - dTm; cTm = cT; cT = n1; dTm = dT; dT = d1; }
+        cP = 1.0; cPm = 0.0; dP = 0.0; dPm = 0.0;
+      } else if (ib == 1) { cPm = 1.0; cP = Pr_; dPm = 0.0; dP = 1.0; }
+      else { const double n1 = 2.0 * Pr_ * cP - cPm, d1 = 2.0 * cP + 2.0 * Pr_ * dP - dPm; cPm = cP; cP = n1; dPm = dP; dP = d1; }
+    }
+    lnkf = LN10 * lg;
+    lam_f = LN10 * dlg_dT * (-2.0 * invT * invT / (iTmax - iTmin));
+    dlnk_dP = dlg_dP * 2.0 / (Pp * (lPmax - lPmin));
+  }
+  const double kf = exp(lnkf);
+  // stoichiometry: concentrations, powers and one-factor-removed products (no division by C_k: DESIGN.md S7).
+  // Unused entries point at the dummy species ns (C = 1, thermo = 0).
+  const uint32_t spk[6] = {spw.x & 0xffffu, spw.x >> 16, spw.y & 0xffffu, spw.y >> 16, spw.z & 0xffffu, spw.z >> 16};
+  const uint32_t nu_bits = spw.w >> 16;
+  double pw[6], pm[6];
+  double dg = 0.0, dh = 0.0, dc = 0.0;
+#pragma unroll
+  for (int a = 0; a < 6; ++a) {
+    const int k = (int)spk[a], nu = (int)((nu_bits >> (2 * a)) & 3u);
+    const double Ck = sp_arr(sm.C, k);
+    pw[a] = ipow(Ck, nu); pm[a] = dpow(Ck, nu);
+    const double snu = a < 3 ? -(double)nu : (double)nu;
+    dg += snu * sp_arr(sm.G, k); dh += snu * sp_arr(sm.Hh, k); dc += snu * sp_arr(sm.K, k);
+  }
+  const double Pif = pw[0] * pw[1] * pw[2], Pir = pw[3] * pw[4] * pw[5];
+  const double snu = (double)((int)((info >> JI_SNU_SHIFT) & 31u) - 16);
+  double kr = 0.0, lam_r = 0.0;
+  if (rev) {      // a4: K_c from Gibbs polynomials; k_r = k_f / K_c = exp(ln k_f - ln K_c)
+    if (info & JI_REVX) {        // explicit reverse Arrhenius parameters (R9): K_c plays no role
+      const int ro = ext.w;
+      const double lAr = __ldg(m.rev_par + 3 * ro), br = __ldg(m.rev_par + 3 * ro + 1), Tar = __ldg(m.rev_par + 3 * ro + 2);
+      kr = exp(lAr + br * lnT - Tar * invT);
+      lam_r = (br + Tar * invT) * invT;
+    } else {
+      kr = exp(lnkf + dg - snu * ln_patm_rt);
+      lam_r = lam_f - (dh - snu) * invT;
+    }
+  }
+  const double Rf = kf * Pif, Rr = kr * Pir, Rn = Rf - Rr;
+  const double dRdT = lam_f * Rf - lam_r * Rr;
+  // a5: third body / falloff
+  double c = 1.0, X = 0.0, GT = dRdT, MdcdM_R = 0.0;
+  const double adef = (info & JI_ADEF) ? 1.0 : 0.0;
+  if (type >= PYJAC_THIRD_BODY && type <= PYJAC_FALLOFF_SRI) {
+    double M = adef * Ctot;                       // sum_k C_k == C_tot by construction of C_Ns
+    for (int eb = e0; eb < e1; ++eb) M += __ldg(m.eff_d + eb) * sp_arr(sm.C, __ldg(m.eff_sp + eb));
+    if (type == PYJAC_THIRD_BODY) {
+      c = M; X = Rn; GT = M * dRdT; MdcdM_R = M * Rn;
+    } else {
+      double fp[10];
+      {
+        const double2* __restrict__ f2 = reinterpret_cast<const double2*>(m.fall + 12 * rx_aux);
+#pragma unroll
+        for (int q = 0; q < 5; ++q) { const double2 v2 = __ldg(f2 + q); fp[2 * q] = v2.x; fp[2 * q + 1] = v2.y; }
+      }
+      // falloff: the record holds k_0 and lnkf = ln k_inf.  Chemically activated (R8): the record holds k_inf and
+      // lnkf = ln k_0, so the ratio k_0 / k_inf and its temperature derivative change sign in the exponent, and
+      // c = F / (1 + Pr) instead of F Pr / (1 + Pr).
+      const bool chem = (info & JI_CHEM) != 0;
+      const double b0 = fp[1], Ta0 = fp[2];
+      const double lnrat = fp[0] + b0 * lnT - Ta0 * invT - lnkf;
+      const double k0_kinf = exp(chem ? -lnrat : lnrat);
+      const double Pr = k0_kinf * M;
+      const Blend bl = blend(type, info & JI_T2, fp, T, invT, lnT, Pr);
+      const double i1p = 1.0 / (1.0 + Pr);
+      const double cF = chem ? i1p : Pr * i1p;            // dc/dF
+      c = bl.F * cF;
+      const double dc_dPr = (chem ? -bl.F : bl.F) * i1p * i1p + cF * bl.dF_dPr;
+      const double dlnrat_dT = (b0 - rx_beta + (Ta0 - rx_Ta) * invT) * invT;
+      const double dPr_dT = Pr * (chem ? -dlnrat_dT : dlnrat_dT);
+      X = dc_dPr * k0_kinf * Rn;
+      GT = (dc_dPr * dPr_dT + cF * bl.dF_dT) * Rn + c * dRdT;
+      MdcdM_R = Pr * dc_dPr * Rn;
+    }
+  }
+  const double q = c * Rn;
+  // reaction sums (R4-7/8): dE~_i = sum_k nu_ki (E_k - w_k E_Ns) = RT (sum nu_k e_k - e_Ns sum nu_k w_k) with
+  // sum_k nu_ki w_k = sum(nu) - dn~_i; likewise dc~_i
+  const double conv = conp ? 0.0 : 1.0;
+  const double dEt = RT * (dh - conv * snu - eL * (snu - dn));
+  const double dct = dc - cL * (snu - dn);
+  // a8: per-reaction partials -> value slots (slot i at base + 8 i)
+  double* __restrict__ Vd = reinterpret_cast<double*>(sm.V);
+  const int sbase = (int)(spw.w & 0xffffu);
+  auto slot = [&](int i) -> double& { return Vd[((sbase + 8 * i) * LS + pr) * 2 + st]; };
+  const int nre = (info >> JI_NREAC_SHIFT) & 3, npr = (info >> JI_NPROD_SHIFT) & 3;
+  const double a_ = c * kf, b_ = c * kr;
+  double GL = adef * X;                          // full dQ_i/dC_Ns
+  const double df[3] = {a_ * pm[0] * pw[1] * pw[2], a_ * pw[0] * pm[1] * pw[2], a_ * pw[0] * pw[1] * pm[2]};
+  const double dr[3] = {-b_ * pm[3] * pw[4] * pw[5], -b_ * pw[3] * pm[4] * pw[5], -b_ * pw[3] * pw[4] * pm[5]};
+  int si = 2;
+#pragma unroll
+  for (int a = 0; a < 3; ++a)
+    if (a < nre) { slot(si++) = df[a]; if ((int)spk[a] == L) GL += df[a]; }
+  if (rev) {
+#pragma unroll
+    for (int a = 0; a < 3; ++a)
+      if (a < npr) { slot(si++) = dr[a]; if ((int)spk[3 + a] == L) GL += dr[a]; }
+  }
+  for (int eb = e0; eb < e1; ++eb) {
+    const double v = __ldg(m.eff_d + eb) * X;
+    slot(si++) = v;
+    if (__ldg(m.eff_sp + eb) == L) GL += v;
+  }
+  // chain rule to the state variables (R4-2); E column in Euler-homogeneity form (R4-6)
+  const double slotT = V * (GT - ctot_T * GL);
+  double slotE;
+  if (conp) {
+    const int of = (info >> JI_OF_SHIFT) & 15, orv = (info >> JI_OR_SHIFT) & 15;
+    slotE = q - c * ((double)of * Rf - (double)orv * Rr) - MdcdM_R + Ctot * GL;
+  } else {
+    slotE = V * (c * dlnk_dP * Rn + GL / RT);
+  }
+  slot(0) = slotT;
+  slot(1) = slotE;
+  reinterpret_cast<double*>(sm.dE)[(lr * LS + pr) * 2 + st] = dEt;
+  inc[0] = dEt * q; inc[1] = dn * q; inc[2] = dEt * slotT; inc[3] = dn * slotT; inc[4] = dEt * slotE; inc[5] = dn * slotE; inc[6] = dct * q;
+}
+
+// ---------------------------------------------------------------------------------------------------
+// the kernel
+// ---------------------------------------------------------------------------------------------------
+template <int LS, bool DENSE, class PosT>
+__global__ void __launch_bounds__(NT, 1)
+jacobian2_kernel(const DevJac m, const DevJacOut o, int mode, int64_t n_states, int64_t tile, const double* __restrict__ phi,
+                 const double* __restrict__ param, double* __restrict__ out, unsigned long long* __restrict__ sched) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  constexpr int S = 2 * LS, IPW = 32 / LS;
+  const Smem<LS> sm(smem_raw, m);
+  __shared__ int cnt[4];
+  __shared__ long long next_tile;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, pr = tid % LS;
+  const int ns = m.ns, L = ns - 1, nvar = m.nvar;
+  const bool conp = mode == PYJAC_CONP;
+  const double conv = conp ? 0.0 : 1.0;
+  // ---- once per CTA: what does not depend on the state ------------------------------------------------------------
+  for (int i = tid; i < m.nr; i += NT) sm.dn[i] = __ldg(m.dn + i);
+  for (int i = tid; i < m.n_groups; i += NT) sm.grp[i] = __ldg(reinterpret_cast<const int4*>(m.groups) + i);
+  if (tid < J_NZERO * LS) st2(sm.V + m.ns_max * LS + tid, mk(0.0));
+  if (tid < LS) { st2(sm.C + ns * LS + tid, mk(1.0)); st2(sm.G + ns * LS + tid, mk(0.0)); st2(sm.Hh + ns * LS + tid, mk(0.0)); st2(sm.K + ns * LS + tid, mk(0.0)); }
+  if (tid < 4) cnt[tid] = 0;
+  const int64_t n_tiles = (n_states + S - 1) / S;
+  const bool vec = (tile & 1) == 0;
+  const int n2 = nvar * nvar;
+  const int n_zslices = DENSE ? (n2 + 1023) / 1024 : 0;
+  __syncthreads();
+  for (int64_t tl = blockIdx.x; tl < n_tiles;) {
+    unsigned long long ticket = 0;
+    if (tid == 0) ticket = atomicAdd(sched, 1ull);
+    const int64_t s0 = tl * S + 2 * pr;
+    const bool va = s0 < n_states, vb = s0 + 1 < n_states;
+    const int64_t sa = min(s0, n_states - 1), sb = min(s0 + 1, n_states - 1);   // ragged tail: recompute the last state, never store
+    const double* __restrict__ pha = phi + state_base(sa, tile, nvar);
+    const double* __restrict__ phb = phi + state_base(sb, tile, nvar);
+    Out og;
+    og.pa = out + state_base(sa, tile, o.n_e); og.pb = out + state_base(sb, tile, o.n_e);
+    og.tile = tile; og.va = va; og.vb = vb; og.vec = vec;
+    // ---- phase 0a: per-pair scalars, by the first warp ------------------------------------------------------------
+    if (warp == 0) {
+      const D2 T = mk(pha[0], phb[0]), E_ = mk(pha[tile], phb[tile]), par = mk(param[sa], param[sb]);
+      const D2 V = conp ? E_ : par, Pp = conp ? par : E_;
+      if (lane < LS) {
+        const D2 invT = mk(1.0 / T.a, 1.0 / T.b), lnT = mk(log(T.a), log(T.b)), RT = T * R_GAS;
+        const D2 Ctot = mk(Pp.a / RT.a, Pp.b / RT.b);
+        st2(sm.sc + SC_T * LS + pr, T); st2(sm.sc + SC_V * LS + pr, V); st2(sm.sc + SC_P * LS + pr, Pp);
+        st2(sm.sc + SC_INVT * LS + pr, invT); st2(sm.sc + SC_LNT * LS + pr, lnT); st2(sm.sc + SC_CTOT * LS + pr, Ctot);
+        st2(sm.sc + SC_RT * LS + pr, RT); st2(sm.sc + SC_LNP * LS + pr, mk(log(Pp.a), log(Pp.b)));
+        st2(sm.sc + SC_LNPRT * LS + pr, mk(log(P_ATM / RT.a), log(P_ATM / RT.b)));
+      }
+      if (tid == 0) { next_tile = (long long)gridDim.x + (long long)ticket; cnt[2] = 0; cnt[3] = 0; }
+    }
+    __syncthreads();
+    const int64_t tl_next = next_tile;
+    // ---- phase 0b: species (C_k = n_k / V, Eq. 6; NASA-7 thermo, R2) ------------------------------------
+    {
+      const D2 T = ld2(sm.sc + SC_T * LS + pr), V = ld2(sm.sc + SC_V * LS + pr);
+      const D2 invT = ld2(sm.sc + SC_INVT * LS + pr), lnT = ld2(sm.sc + SC_LNT * LS + pr);
+      const D2 T2 = T * T, T3 = T2 * T, T4 = T3 * T;
+      const D2 invV = mk(1.0 / V.a, 1.0 / V.b);
+      D2 acc0 = mk(0.0), acc1 = mk(0.0), acc2 = mk(0.0);
+      for (int idx = tid; idx < ns * LS; idx += NT) {
+        const int k = idx / LS;
+        const double* __restrict__ tab = m.nasa + k;               // coefficient-major: tmid, lo[7], hi[7]
+        const double tmid = __ldg(tab);
+        const bool la = T.a <= tmid, lb = T.b <= tmid;             // low range iff T <= T_mid (R3)
+        double ca[7], cb[7];
+        if (la == lb) {
+#pragma unroll
+          for (int c = 0; c < 7; ++c) { ca[c] = __ldg(tab + (size_t)((la ? 1 : 8) + c) * ns); cb[c] = ca[c]; }
+        } else {
+#pragma unroll
+          for (int c = 0; c < 7; ++c) { const double lo = __ldg(tab + (size_t)(1 + c) * ns), hi = __ldg(tab + (size_t)(8 + c) * ns); ca[c] = la ? lo : hi; cb[c] = lb ? lo : hi; }
+        }
+        auto thermo = [&](const double (&a)[7], double t, double t2, double t3, double t4, double it, double lt, double& cpR, double& dcpR, double& hRT, double& sR) {
+          cpR = a[0] + a[1] * t + a[2] * t2 + a[3] * t3 + a[4] * t4;
+          dcpR = a[1] + 2.0 * a[2] * t + 3.0 * a[3] * t2 + 4.0 * a[4] * t3;
+          hRT = a[0] + a[1] * t * 0.5 + a[2] * t2 * (1.0 / 3.0) + a[3] * t3 * 0.25 + a[4] * t4 * 0.2 + a[5] * it;
+          sR = a[0] * lt + a[1] * t + a[2] * t2 * 0.5 + a[3] * t3 * (1.0 / 3.0) + a[4] * t4 * 0.25 + a[6];
+        };
+        D2 cpR, dcpR, hRT, sR;
+        thermo(ca, T.a, T2.a, T3.a, T4.a, invT.a, lnT.a, cpR.a, dcpR.a, hRT.a, sR.a);
+        thermo(cb, T.b, T2.b, T3.b, T4.b, invT.b, lnT.b, cpR.b, dcpR.b, hRT.b, sR.b);
+        const D2 c = (cpR - conv) * R_GAS;                            // c_p or c_v = c_p - R
+        st2(sm.G + idx, hRT - sR);
+        st2(sm.Hh + idx, hRT);
+        st2(sm.K + idx, c);
+        if (k < L) {
+          const D2 Ck = mk(pha[(int64_t)(2 + k) * tile], phb[(int64_t)(2 + k) * tile]) * invV;
+          st2(sm.C + idx, Ck);
+          acc0 += Ck; acc1 = fma2(Ck, c, acc1); acc2 = fma2(Ck, dcpR * R_GAS, acc2);
+        } else {
+          st2(sm.sc + SC_EL * LS + pr, hRT - conv); st2(sm.sc + SC_CL * LS + pr, c); st2(sm.sc + SC_DCL * LS + pr, dcpR * R_GAS);
+        }
+      }
+#pragma unroll
+      for (int off = 16; off >= LS; off >>= 1) { acc0 += shfl_xor2(acc0, off); acc1 += shfl_xor2(acc1, off); acc2 += shfl_xor2(acc2, off); }
+      if (lane < LS) { st2(sm.red + (warp * J_NRED + 8) * LS + lane, acc0); st2(sm.red + (warp * J_NRED + 9) * LS + lane, acc1); st2(sm.red + (warp * J_NRED + 10) * LS + lane, acc2); }
+      // reaction sums of this tile start at zero (per-warp partials, summed by their consumers)
+      if (lane < 8 * LS) st2(sm.red + warp * J_NRED * LS + lane, mk(0.0));
+    }
+    __syncthreads();
+    if (tid < LS) {
+      // the last species: C_Ns from the ideal-gas law
+      D2 s0_ = mk(0.0), s1_ = mk(0.0), s2_ = mk(0.0);
+      for (int w = 0; w < NW; ++w) { s0_ += ld2(sm.red + (w * J_NRED + 8) * LS + tid); s1_ += ld2(sm.red + (w * J_NRED + 9) * LS + tid); s2_ += ld2(sm.red + (w * J_NRED + 10) * LS + tid); }
+      const D2 CL = ld2(sm.sc + SC_CTOT * LS + tid) - s0_;
+      st2(sm.C + L * LS + tid, CL);
+      st2(sm.sc + SC_D * LS + tid, s1_ + CL * ld2(sm.sc + SC_CL * LS + tid));
+      st2(sm.sc + SC_DDDT * LS + tid, s2_ + CL * ld2(sm.sc + SC_DCL * LS + tid));
+    }
+    __syncthreads();
+    for (int b = 0; b <= m.H; ++b) {
+      if (b < m.H) {
+        // ---- phase 1: reactions of block b ------------------------------------------------------------------------
+        const D2 V = ld2(sm.sc + SC_V * LS + pr), invT = ld2(sm.sc + SC_INVT * LS + pr), lnT = ld2(sm.sc + SC_LNT * LS + pr);
+        const D2 Ctot = ld2(sm.sc + SC_CTOT * LS + pr), RT = ld2(sm.sc + SC_RT * LS + pr), ln_patm_rt = ld2(sm.sc + SC_LNPRT * LS + pr);
+        const D2 eL = ld2(sm.sc + SC_EL * LS + pr), cL = ld2(sm.sc + SC_CL * LS + pr);
+        const D2 ctot_T = Ctot * invT;
+        const int r0 = m.blk_r0[b], nrb = m.blk_r0[b + 1] - r0;
+        D2 acc[7];
+#pragma unroll
+        for (int q = 0; q < 7; ++q) acc[q] = mk(0.0);
+        const int n_chunks = (nrb * LS + 31) / 32;
+        for (int chunk = next_chunk(cnt + 0); chunk < n_chunks; chunk = next_chunk(cnt + 0)) {
+          const int lr = chunk * IPW + lane / LS;
+          if (lr >= nrb) continue;
+          const int r = r0 + lr;
+          const uint32_t info = __ldg(m.info + r);
+          const uint4 spw = __ldg(reinterpret_cast<const uint4*>(m.sp) + r);
+          if (!(info & JI_FAST)) {
+#pragma unroll 1
+            for (int st = 0; st < 2; ++st) {
+              double inc[7];
+              reaction_general<LS>(m, sm, r, lr, pr, st, conp, info, spw, inc);
+#pragma unroll
+              for (int q = 0; q < 7; ++q) { if (st == 0) acc[q].a += inc[q]; else acc[q].b += inc[q]; }
+            }
+            continue;
+          }
+          // fast path: elementary or third-body reaction, all coefficients 1, <= 2 species per side, the last
+          // species in no role; both states at once
+          const double rx_lnA = __ldg(m.lnA + r), rx_beta = __ldg(m.beta + r), rx_Ta = __ldg(m.Ta + r), dn = sm.dn[r];
+          const int k0 = spw.x & 0xffffu, k1 = spw.x >> 16, k2 = spw.y >> 16, k3 = spw.z & 0xffffu;   // reactants 0, 1; products 3, 4
+          const D2 C0 = ld2(sm.C + k0 * LS + pr), C1 = ld2(sm.C + k1 * LS + pr), C2 = ld2(sm.C + k2 * LS + pr), C3 = ld2(sm.C + k3 * LS + pr);
+          const D2 dh = (ld2(sm.Hh + k2 * LS + pr) + ld2(sm.Hh + k3 * LS + pr)) - (ld2(sm.Hh + k0 * LS + pr) + ld2(sm.Hh + k1 * LS + pr));
+          const D2 dc = (ld2(sm.K + k2 * LS + pr) + ld2(sm.K + k3 * LS + pr)) - (ld2(sm.K + k0 * LS + pr) + ld2(sm.K + k1 * LS + pr));
+          const D2 lnkf = fma2(rx_beta, lnT, mk(rx_lnA)) - rx_Ta * invT;
+          const D2 lam_f = fma2(rx_Ta, invT, mk(rx_beta)) * invT;
+          const D2 kf = exp2_(lnkf);
+          const double snu = (double)((int)((info >> JI_SNU_SHIFT) & 31u) - 16);
+          const bool rev = info & JI_REV;
+          D2 kr = mk(0.0), lam_r = mk(0.0);
+          if (rev) {
+            const D2 dg = (ld2(sm.G + k2 * LS + pr) + ld2(sm.G + k3 * LS + pr)) - (ld2(sm.G + k0 * LS + pr) + ld2(sm.G + k1 * LS + pr));
+            kr = exp2_(lnkf + dg - snu * ln_patm_rt);
+            lam_r = lam_f - (dh - snu) * invT;
+          }
+          const D2 Rf = kf * (C0 * C1), Rr = kr * (C2 * C3), Rn = Rf - Rr;
+          const D2 dRdT = lam_f * Rf - lam_r * Rr;
+          D2* __restrict__ Vp = sm.V + (spw.w & 0xffffu) * LS + pr;
+          const int nre = (info >> JI_NREAC_SHIFT) & 3, npr = (info >> JI_NPROD_SHIFT) & 3;
+          D2 c = mk(1.0), GT = dRdT, MdcdM_R = mk(0.0), GL = mk(0.0);
+          int si = 2 + nre + (rev ? npr : 0);
+          if ((info & JI_TYPE_MASK) == PYJAC_THIRD_BODY) {
+            const int4 ext = __ldg(reinterpret_cast<const int4*>(m.ext) + r);
+            const double adef = (info & JI_ADEF) ? 1.0 : 0.0;
+            D2 M = Ctot * adef;
+            for (int q = 0; q < ext.z; ++q) {
+              const int esp = __ldg(m.eff_sp + ext.y + q);
+              const double ed = __ldg(m.eff_d + ext.y + q);
+              M = fma2(ed, ld2(sm.C + esp * LS + pr), M);
+              st2(Vp + (si + q) * 8 * LS, Rn * ed);            // dQ/dC_e through [M]: alpha' X, X = R_n
+            }
+            c = M; GT = M * dRdT; MdcdM_R = M * Rn; GL = Rn * adef;
+          }
+          const D2 q = c * Rn;
+          const D2 a_ = c * kf, b_ = c * kr;
+          st2(Vp + 2 * 8 * LS, a_ * C1);
+          if (nre == 2) st2(Vp + 3 * 8 * LS, a_ * C0);
+          if (rev) {
+            st2(Vp + (2 + nre) * 8 * LS, -(b_ * C3));
+            if (npr == 2) st2(Vp + (3 + nre) * 8 * LS, -(b_ * C2));
+          }
+          const D2 slotT = V * (GT - ctot_T * GL);
+          D2 slotE;
+          if (conp) {
+            const double of = (double)((info >> JI_OF_SHIFT) & 15), orv = (double)((info >> JI_OR_SHIFT) & 15);
+            slotE = q - c * (Rf * of - Rr * orv) - MdcdM_R + Ctot * GL;
+          } else {
+            slotE = V * mk(GL.a / RT.a, GL.b / RT.b);
+          }
+          st2(Vp, slotT);
+          st2(Vp + 8 * LS, slotE);
+          const D2 dEt = RT * (dh - conv * snu - eL * (snu - dn));
+          const D2 dct = dc - cL * (snu - dn);
+          st2(sm.dE + lr * LS + pr, dEt);
+          acc[0] = fma2(dEt, q, acc[0]); acc[1] = fma2(dn, q, acc[1]); acc[2] = fma2(dEt, slotT, acc[2]); acc[3] = fma2(dn, slotT, acc[3]);
+          acc[4] = fma2(dEt, slotE, acc[4]); acc[5] = fma2(dn, slotE, acc[5]); acc[6] = fma2(dct, q, acc[6]);
+        }
+        // per-warp partial reaction sums (the barrier below publishes them together with the slots)
+#pragma unroll
+        for (int q = 0; q < 7; ++q) {
+          D2 v = acc[q];
+#pragma unroll
+          for (int off = 16; off >= LS; off >>= 1) v += shfl_xor2(v, off);
+          if (lane < LS) { D2* p = sm.red + (warp * J_NRED + q) * LS + lane; st2(p, ld2(p) + v); }
+        }
+        __syncthreads();
+        if (tid == 0) cnt[0] = 0;
+        if (b == m.H - 1) {
+          // every reaction is done.  a10: the four corner entries from the reaction sums (R4-7), by the last warp
+          if (warp == NW - 1 && lane < LS) {
+            const D2 T = ld2(sm.sc + SC_T * LS + pr), Pp = ld2(sm.sc + SC_P * LS + pr), D = ld2(sm.sc + SC_D * LS + pr);
+            D2 sums[7];
+#pragma unroll
+            for (int q = 0; q < 7; ++q) { sums[q] = mk(0.0); for (int w = 0; w < NW; ++w) sums[q] += ld2(sm.red + (w * J_NRED + q) * LS + pr); }
+            const D2 dDdT0 = ld2(sm.sc + SC_DDDT * LS + pr);
+            D2 JTT, JTE, JET, JEE;
+            auto corner = [&](double T, double V, double Pp, double Ctot, double D, double cL, double dDdT0, double fT, double N, double Ssum,
+                              double AT, double BT, double AE, double BE, double sumcw, double& JTT, double& JTE, double& JET, double& JEE) {
+              const double iV = 1.0 / V;
+              const double dN_dT = AT * iV + sumcw;
+              const double dD_dT = dDdT0 - cL * Ctot / T;
+              JTT = -(dN_dT + fT * dD_dT) / D;
+              const double dS_dT = BT * iV;
+              double dN_dE, dD_dE, dS_dE;
+              if (conp) {
+                const double fE = V * (T * R_GAS / Pp * Ssum + fT / T);
+                dN_dE = (AE - N) * iV; dD_dE = -(D - Ctot * cL) * iV; dS_dE = (BE - Ssum) * iV;
+                JTE = -(dN_dE + fT * dD_dE) / D;
+                JET = V * (T * R_GAS / Pp * dS_dT + JTT / T) + V * (R_GAS * Ssum / Pp - fT / (T * T));
+                JEE = V * (T * R_GAS / Pp * dS_dE + JTE / T) + fE * iV;
+              } else {
+                dN_dE = AE * iV; dD_dE = cL / (R_GAS * T); dS_dE = BE * iV;
+                JTE = -(dN_dE + fT * dD_dE) / D;
+                JET = T * R_GAS * dS_dT + Pp / T * JTT + R_GAS * Ssum - Pp * fT / (T * T);
+                JEE = T * R_GAS * dS_dE + Pp / T * JTE + fT / T;
+              }
+            };
+            const D2 fT = mk(-sums[0].a / D.a, -sums[0].b / D.b);        // f_T = -N / D (Eq. 5)
+            corner(T.a, V.a, Pp.a, Ctot.a, D.a, cL.a, dDdT0.a, fT.a, sums[0].a, sums[1].a, sums[2].a, sums[3].a, sums[4].a, sums[5].a, sums[6].a, JTT.a, JTE.a, JET.a, JEE.a);
+            corner(T.b, V.b, Pp.b, Ctot.b, D.b, cL.b, dDdT0.b, fT.b, sums[0].b, sums[1].b, sums[2].b, sums[3].b, sums[4].b, sums[5].b, sums[6].b, JTT.b, JTE.b, JET.b, JEE.b);
+            og.store((uint32_t)o.d_pos[0], JTT); og.store((uint32_t)o.d_pos[1], JTE); og.store((uint32_t)o.d_pos[2], JET); og.store((uint32_t)o.d_pos[3], JEE);
+          }
+        }
+      }
+      // ---- phase 2: pieces of block b (b == H: the final combine wave) -----------------------------------------------
+      const int g0 = m.blk_g0[b], n_units = (m.blk_g0[b + 1] - g0) * LS;
+      int* counter = cnt + (b < m.H ? 1 : 2);
+      if (n_units > 0) {
+        int unit = next_chunk(counter);
+        while (unit < n_units) {
+          const int next = next_chunk(counter);
+          const int4 gw = sm.grp[g0 + unit / LS];
+          JGroup g;
+          g.ent_off = (uint32_t)gw.x; g.piece_off = (uint32_t)gw.y;
+          g.nP2 = (uint8_t)(gw.z & 0xff); g.nM2 = (uint8_t)((gw.z >> 8) & 0xff); g.cls = (uint8_t)((gw.z >> 16) & 0xff); g.kind = (uint8_t)((uint32_t)gw.z >> 24);
+          gather_unit<LS, PosT>(m, o, sm, g, unit % LS, og, conp, b < m.H ? m.blk_r0[b] : 0);
+          unit = next;
+        }
+      }
+      if (DENSE && b == m.H) {
+        // structural zeros, each stored once (no memset pass): slices of 1024 elements, one coalesced mask load each
+        for (int z = next_chunk(cnt + 3); z < n_zslices; z = next_chunk(cnt + 3)) {
+          const int w0 = z * 32, n_words = (n2 + 31) / 32;
+          const uint32_t mine = w0 + lane < n_words ? __ldg(o.nzmask + w0 + lane) : 0xffffffffu;
+          for (int q = lane / LS; q < 1024; q += IPW) {
+            const uint32_t wj = __shfl_sync(0xffffffffu, mine, q >> 5);
+            const int e = z * 1024 + q;
+            if (!((wj >> (q & 31)) & 1u) && e < n2) og.store((uint32_t)e, mk(0.0));
+          }
+        }
+      }
+      __syncthreads();
+      if (tid == 0 && b < m.H) cnt[1] = 0;
+    }
+    tl = tl_next;
+  }
+  if (tid == 0 && atomicAdd(sched + 1, 1ull) == (unsigned long long)gridDim.x - 1) { sched[0] = 0; sched[1] = 0; }
+}
+
+}  // namespace jac2
+}  // namespace pyjac
