@@ -104,7 +104,11 @@ int pyjac_mech_create(const pyjac_mech_desc *desc, int cuda_device, pyjac_mech *
  * efficiency of the last species disappear; pyjac_sparsity returns the sparser pattern; the T and E columns, the
  * source terms and everything else are unchanged.  For mechanisms whose last species is inert with default
  * efficiencies the two Jacobians are identical. */
-enum { PYJAC_APPROX_JACOBIAN = 1 };
+enum { PYJAC_APPROX_JACOBIAN = 1, PYJAC_PAIR_KERNEL = 2 };
+/* PYJAC_PAIR_KERNEL: evaluate the Jacobian with the pair-of-states kernel (a thread owns an item for
+ * two states, the reactions are cut into blocks so that the per-reaction partials of one block fit on chip).  It is
+ * chosen automatically for mechanisms whose partials do not fit in one SM's shared memory all at once; the flag forces it
+ * for any mechanism (same results within the tolerances; tests and benchmarks). */
 int pyjac_mech_create_ex(const pyjac_mech_desc *desc, int cuda_device, uint32_t flags, pyjac_mech **out);
 void pyjac_mech_destroy(pyjac_mech *mech);
 

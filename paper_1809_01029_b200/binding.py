@@ -16,6 +16,7 @@ PYJAC_OK, PYJAC_EINVAL, PYJAC_EMECH, PYJAC_ECUDA, PYJAC_ENOMEM = range(5)
 PYJAC_CONP, PYJAC_CONV = 0, 1
 PYJAC_CSR, PYJAC_CSC = 0, 1
 PYJAC_APPROX_JACOBIAN = 1
+PYJAC_PAIR_KERNEL = 2
 WHAT_SOURCE, WHAT_SPARSE, WHAT_DENSE = 0, 1, 2
 
 _D = C.POINTER(C.c_double)

@@ -30,8 +30,10 @@ struct pyjac_mech {
   HostTables h;
   JacTables j;
   DevMech dm{};
-  DevJac dj{};
+  DevPlan plan[4]{};          // tile kernel (jacobian_kernel, pyjac_kernels.cu)
+  DevJac dj{};                // pair kernel (jacobian2_kernel, pyjac_jacobian.cuh)
   DevJacOut jout[4]{};
+  bool pair_only = false;     // the tile kernel's intermediates do not fit in shared memory, or PYJAC_PAIR_KERNEL
   std::vector<void*> allocs;
   // tile-scheduler words of the persistent Jacobian kernel: a ring of N_SCHED zeroed pairs (tile counter, finished
   // CTAs; the kernel leaves its pair zero again).  A launch takes the next pair; the event recorded behind the launch
@@ -76,13 +78,16 @@ int pyjac_mech_create(const pyjac_mech_desc* desc, int cuda_device, pyjac_mech**
 
 int pyjac_mech_create_ex(const pyjac_mech_desc* desc, int cuda_device, uint32_t flags, pyjac_mech** out) {
   if (!desc || !out) return fail(PYJAC_EINVAL, "pyjac_mech_create: null argument");
-  if (flags & ~(uint32_t)PYJAC_APPROX_JACOBIAN) return fail(PYJAC_EINVAL, "pyjac_mech_create_ex: unknown flag");
+  if (flags & ~(uint32_t)(PYJAC_APPROX_JACOBIAN | PYJAC_PAIR_KERNEL)) return fail(PYJAC_EINVAL, "pyjac_mech_create_ex: unknown flag");
   *out = nullptr;
   pyjac_mech* m = new (std::nothrow) pyjac_mech();
   if (!m) return fail(PYJAC_ENOMEM, "out of host memory");
   std::string err;
   int rc = build_host_tables(desc, (flags & PYJAC_APPROX_JACOBIAN) != 0, m->h, err);
   if (rc == PYJAC_OK) rc = build_jac_tables(m->h, m->j, err);
+  // the tile kernel keeps ALL per-reaction partials of a state on chip; when they do not fit (or on request) the pair
+  // kernel, which cuts the reactions into blocks, evaluates the Jacobian
+  m->pair_only = (flags & PYJAC_PAIR_KERNEL) != 0 || choose_cfg(m->h, true, (int64_t)1 << 40, (int64_t)1 << 40).smem > (size_t)(227 * 1024 - 64);
   if (rc != PYJAC_OK) { delete m; return fail(rc, err); }
   if (cuda_device == -1) { m->device = -1; *out = m; return PYJAC_OK; }   // host-only handle: pattern and dims only
   int ndev = 0;
@@ -129,13 +134,29 @@ int pyjac_mech_create_ex(const pyjac_mech_desc* desc, int cuda_device, uint32_t 
     const uint32_t* mask[2];
     for (int p = 0; p < 2; ++p)
       if (int r_ = m->upload(h.nzmask[p], &mask[p])) return r_;
-    // the Jacobian kernel's own tables (block order) and plan
+    {
+      DevGather jplan;
+      if (int r_ = m->upload_plan(h.jplan, 0, &jplan)) return r_;
+      for (int f = 0; f < 4; ++f) {
+        DevPlan& pl = m->plan[f];
+        pl.n_e = f < 2 ? h.nnz : (int64_t)h.nvar * h.nvar;
+        pl.jplan = jplan;
+        if (int r_ = m->upload(h.j_pos[f], &pl.j_pos)) return r_;
+        if (int r_ = m->upload(h.c_pos[f], &pl.c_pos)) return r_;
+        if (int r_ = m->upload(h.jc_pos[f], &pl.jc_pos)) return r_;
+        if (int r_ = m->upload(h.cc_pos[f], &pl.cc_pos)) return r_;
+        for (int c = 0; c < 4; ++c) pl.d_pos[c] = h.d_pos[f][c];
+        pl.nzmask = f < 2 ? nullptr : mask[f & 1];
+      }
+    }
+    // the pair kernel's own tables (block order) and plan
     {
       const JacTables& j = m->j;
       DevJac& q = m->dj;
       q.ns = j.ns; q.nr = j.nr; q.nvar = j.nvar; q.H = j.H; q.ns_max = j.ns_max; q.n_val = j.n_val; q.max_nrb = j.max_nrb;
       q.n_groups = (int)j.groups.size();
       for (int b = 0; b <= j.H; ++b) q.blk_r0[b] = j.blk_r0[b];
+      for (int b = 0; b < j.H; ++b) q.blk_ng[b] = j.blk_ng[b];
       for (int b = 0; b <= j.H + 1; ++b) q.blk_g0[b] = j.blk_g0[b];
 #define UPJ(field) if (int r_ = m->upload(j.field, &q.field)) return r_;
       UPJ(lnA) UPJ(beta) UPJ(Ta) UPJ(dn) UPJ(info) UPJ(sp) UPJ(ext) UPJ(groups) UPJ(ent) UPJ(pidx) UPJ(item) UPJ(nplus)
@@ -230,14 +251,17 @@ static int run_jac(const char* fn, const pyjac_mech* mech, int mode, int ofmt, i
                    const double* d_phi, const double* d_param, double* d_out, void* stream) {
   if (int rc = check_common(fn, mech, mode, n_states, ld, tile, d_phi, d_param, d_out)) return rc;
   if (n_states == 0) return PYJAC_OK;
-  const LaunchCfg cfg = choose_cfg_jac(mech->j, tile, n_states, mech->n_sm);
+  const LaunchCfg cfg = mech->pair_only ? choose_cfg_jac(mech->j, tile, n_states, mech->n_sm) : choose_cfg(mech->h, true, tile, n_states);
   if (cfg.smem > J_SMEM_LIMIT) return fail(PYJAC_ENOMEM, std::string(fn) + ": mechanism too large for shared memory");
   std::lock_guard<std::mutex> lock(mech->sched_mu);
   const unsigned slot = mech->sched_next++ % pyjac_mech::N_SCHED;
   if (mech->sched_used[slot] && cudaEventQuery(mech->sched_ev[slot]) == cudaErrorNotReady)
     CK(cudaStreamWaitEvent((cudaStream_t)stream, mech->sched_ev[slot], 0));     // the pair's previous launch is still in flight
   (void)cudaGetLastError();                                                       // cudaErrorNotReady is not an error
-  int e = launch_jacobian2(mech->dj, mech->jout[ofmt], cfg, mech->n_sm, mode, n_states, tile, d_phi, d_param, d_out, mech->sched + 2 * slot, stream);
+  unsigned long long* sched = mech->sched + 2 * slot;
+  const int e = mech->pair_only
+                    ? launch_jacobian2(mech->dj, mech->jout[ofmt], cfg, mech->n_sm, mode, n_states, tile, d_phi, d_param, d_out, sched, stream)
+                    : launch_jacobian(mech->dm, mech->plan[ofmt], cfg, mode, n_states, ld, tile, d_phi, d_param, d_out, sched, stream);
   if (e) return cuda_fail((cudaError_t)e, "jacobian kernel launch");
   CK(cudaEventRecord(mech->sched_ev[slot], (cudaStream_t)stream));
   mech->sched_used[slot] = true;
@@ -280,7 +304,8 @@ int pyjac_launch_info(const pyjac_mech* mech, int what, int32_t* states_per_cta,
   if (!mech) return fail(PYJAC_EINVAL, "pyjac_launch_info: null handle");
   const LaunchCfg cfg = what == 3 ? choose_cfg_fd(mech->h)
                       : (what == 0 ? choose_cfg(mech->h, false, (int64_t)1 << 40, (int64_t)1 << 40)
-                                   : choose_cfg_jac(mech->j, (int64_t)1 << 40, (int64_t)1 << 40, mech->n_sm > 0 ? mech->n_sm : 148));
+                                   : (mech->pair_only ? choose_cfg_jac(mech->j, (int64_t)1 << 40, (int64_t)1 << 40, mech->n_sm > 0 ? mech->n_sm : 148)
+                                                      : choose_cfg(mech->h, true, (int64_t)1 << 40, (int64_t)1 << 40)));
   if (states_per_cta) *states_per_cta = cfg.S;
   if (threads) *threads = cfg.threads;
   if (smem_bytes) *smem_bytes = (int64_t)cfg.smem;

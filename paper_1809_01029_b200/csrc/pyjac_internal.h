@@ -124,7 +124,8 @@ enum JKind { JK_BLK = 0, JK_BLK1 = 1, JK_COL = 2, JK_ROW = 3, JK_ROWC = 4 };
 enum JCls { JC_OUT = 0, JC_FIRST = 1, JC_ADD = 2, JC_LAST = 3 };
 // nP2 / nM2: pair steps of plus / minus entries (JK_ROW; JK_BLK1: 1 / 0 or 0 / 1); JK_BLK, JK_COL, JK_ROWC: nP2 = pair
 // steps of the longest piece, nM2 = 0, and every piece has its own boundary (JacTables::nplus)
-struct JGroup { uint32_t ent_off, piece_off; uint8_t nP2, nM2, cls, kind; uint32_t cost; };   // 16 bytes
+// qsteps: byte q = pair steps (of plus entries for JK_ROW) needed by pieces 32 q .. 32 q + 31
+struct JGroup { uint32_t ent_off, piece_off; uint8_t nP2, nM2, cls, kind; uint32_t qsteps; };   // 16 bytes
 // bits of JacTables::info
 constexpr uint32_t JI_TYPE_MASK = 7, JI_REV = 1u << 3, JI_T2 = 1u << 4, JI_ADEF = 1u << 5, JI_FAST = 1u << 6, JI_CHEM = 1u << 7;
 constexpr int JI_SNU_SHIFT = 8;       // bits 8-12: sum(nu) + 16
@@ -135,6 +136,7 @@ struct JacTables {
   int ns = 0, nr = 0, nvar = 0, H = 1;
   std::vector<int32_t> old_of_new;           // new reaction index -> index in the HostTables order
   std::vector<int32_t> blk_r0;               // [H+1] first reaction of every block
+  std::vector<int32_t> blk_ng;               // [H] reactions of the block that take the general path of phase 1 (they come first)
   std::vector<double> lnA, beta, Ta, dn;     // [nr]
   std::vector<uint32_t> info;                // [nr]
   std::vector<uint32_t> sp;                  // [nr*4]: species 0|1, 2|3, 4|5 (16 bits each; unused = ns), slot base | nu bits << 16
@@ -201,7 +203,7 @@ struct DevPlan {
 // device view of JacTables (+ the type-specific parameter tables it shares with DevMech)
 struct DevJac {
   int ns, nr, nvar, H, ns_max, n_val, max_nrb, n_groups;
-  int blk_r0[J_MAXH + 1], blk_g0[J_MAXH + 2];
+  int blk_r0[J_MAXH + 1], blk_ng[J_MAXH], blk_g0[J_MAXH + 2];
   const double *lnA, *beta, *Ta, *dn;
   const uint32_t* info;
   const uint32_t* sp;         // uint4 per reaction

@@ -21,6 +21,7 @@
 namespace pyjac {
 namespace jac2 {
 
+
 constexpr int NT = J_NT, NW = J_NW;
 
 struct D2 { double a, b; };
@@ -38,10 +39,71 @@ __device__ __forceinline__ D2& operator+=(D2& x, D2 y) { x.a += y.a; x.b += y.b;
 __device__ __forceinline__ D2& operator-=(D2& x, D2 y) { x.a -= y.a; x.b -= y.b; return x; }
 __device__ __forceinline__ D2 fma2(D2 x, D2 y, D2 z) { return mk(fma(x.a, y.a, z.a), fma(x.b, y.b, z.b)); }
 __device__ __forceinline__ D2 fma2(double x, D2 y, D2 z) { return mk(fma(x, y.a, z.a), fma(x, y.b, z.b)); }
-__device__ __forceinline__ D2 exp2_(D2 x) { return mk(exp(x.a), exp(x.b)); }
+// The library exponential and logarithm are ~100 instructions each when inlined; the kernel's instruction working set has
+// to fit the instruction caches (16 warps in different phases fetch different code), so every use shares one copy.
+static __device__ __noinline__ double exp_lib(double x) { return exp(x); }
+static __device__ __noinline__ double log_lib(double x) { return log(x); }
+__device__ __forceinline__ D2 exp2_(D2 x) { return mk(exp_lib(x.a), exp_lib(x.b)); }
+// exp(x), |x| < 700 (callers fall back to the library routine otherwise): n = rint(x log2 e), r = x - n ln 2 in two
+// steps, Taylor polynomial of degree 13 (truncation 4e-18) by Estrin's scheme -- a dependency chain of 5 DFMAs instead
+// of Horner's 13, which is what phase 1 waits for with 16 warps per SM -- scaled by 2^n through the exponent field.
+__device__ __forceinline__ double exp_core(double x) {
+  const double t = fma(x, 1.4426950408889634074, 6755399441055744.0);
+  const int n = __double2loint(t);
+  const double nf = t - 6755399441055744.0;
+  double r = fma(nf, -6.93147180559945286227e-01, x);
+  r = fma(nf, -2.31904681384629955842e-17, r);
+  const double r2 = r * r, r4 = r2 * r2, r8 = r4 * r4;
+  const double p01 = 1.0 + r;
+  const double p23 = fma(r, 1.0 / 6.0, 0.5);
+  const double p45 = fma(r, 1.0 / 120.0, 1.0 / 24.0);
+  const double p67 = fma(r, 1.0 / 5040.0, 1.0 / 720.0);
+  const double p89 = fma(r, 1.0 / 362880.0, 1.0 / 40320.0);
+  const double pab = fma(r, 1.0 / 39916800.0, 1.0 / 3628800.0);
+  const double pcd = fma(r, 1.0 / 6227020800.0, 1.0 / 479001600.0);
+  const double q0 = fma(r2, p23, p01), q1 = fma(r2, p67, p45), q2 = fma(r2, pab, p89);
+  const double s0 = fma(r4, q1, q0), s1 = fma(r4, pcd, q2);
+  const double p = fma(r8, s1, s0);
+  return __hiloint2double(__double2hiint(p) + (n << 20), __double2loint(p));
+}
+__device__ __forceinline__ bool exp_in_range(double x) { return fabs(x) < 700.0; }
+__device__ __forceinline__ D2 exp2_fast(D2 x) {
+  D2 e = mk(exp_core(x.a), exp_core(x.b));
+  if (!(exp_in_range(x.a) && exp_in_range(x.b))) e = exp2_(x);
+  return e;
+}
 __device__ __forceinline__ D2 ld2(const D2* p) { const double2 v = *reinterpret_cast<const double2*>(p); return mk(v.x, v.y); }
 __device__ __forceinline__ void st2(D2* p, D2 v) { *reinterpret_cast<double2*>(p) = make_double2(v.a, v.b); }
 __device__ __forceinline__ D2 shfl_xor2(D2 v, int o) { return mk(__shfl_xor_sync(0xffffffffu, v.a, o), __shfl_xor_sync(0xffffffffu, v.b, o)); }
+
+// Sums N per-lane values over the lanes that agree in their low log2(KEEP) bits by recursive halving: in every round
+// with more than one value left a lane keeps half of its values and hands the other half to its partner, so 16 values
+// cost 8 + 4 + 2 + 1 + 1 exchanges instead of 16 x 5.  store(j, sum) is called by exactly one lane per (j, low bits).
+template <int N, int OFF, int KEEP>
+struct WarpSum {
+  template <class F>
+  static __device__ __forceinline__ void run(double (&v)[N], int j0, bool owner, F store) {
+    const int lane = threadIdx.x & 31;
+    if constexpr (OFF < KEEP || OFF == 0) {
+      if (owner) {
+#pragma unroll
+        for (int i = 0; i < N; ++i) store(j0 + i, v[i]);
+      }
+    } else if constexpr (N > 1) {
+      const bool up = (lane & OFF) != 0;
+      double h[N / 2];
+#pragma unroll
+      for (int i = 0; i < N / 2; ++i) {
+        const double send = up ? v[i] : v[i + N / 2], keep = up ? v[i + N / 2] : v[i];
+        h[i] = keep + __shfl_xor_sync(0xffffffffu, send, OFF);
+      }
+      WarpSum<N / 2, OFF / 2, KEEP>::run(h, j0 + (up ? N / 2 : 0), owner, store);
+    } else {
+      double h[1] = {v[0] + __shfl_xor_sync(0xffffffffu, v[0], OFF)};
+      WarpSum<1, OFF / 2, KEEP>::run(h, j0, owner && !(lane & OFF), store);
+    }
+  }
+};
 
 // per-pair scalars in shared memory
 enum { SC_T = 0, SC_V, SC_P, SC_INVT, SC_LNT, SC_CTOT, SC_RT, SC_LNP, SC_LNPRT, SC_EL, SC_CL, SC_DCL, SC_D, SC_DDDT, NSC_USED };
@@ -53,7 +115,11 @@ __device__ __forceinline__ int next_chunk(int* counter) {
   return __shfl_sync(0xffffffffu, c, 0);
 }
 
-__device__ __forceinline__ int64_t state_base(int64_t s, int64_t tile, int64_t n_e) { return (s / tile) * (n_e * tile) + (s % tile); }
+// element offset of (element 0, state s) in the library layout (s / tile) * (n_e * tile) + s % tile.  tile is a power of
+// two (shift >= 0) or equal to ld (shift < 0: one tile holds every state), so no 64-bit division is needed.
+__device__ __forceinline__ int64_t state_base(int64_t s, int shift, int64_t n_e) {
+  return shift < 0 ? s : (((s >> shift) * n_e) << shift) + (s & (((int64_t)1 << shift) - 1));
+}
 
 __device__ __forceinline__ double ipow(double x, int n) {   // n in 0..3
   double r = 1.0;
@@ -74,18 +140,18 @@ static __device__ __noinline__ Blend blend(int type, bool hasT2, const double* _
   const double Pr = fmax(Pr_in, 1e-300);
   if (type == PYJAC_FALLOFF_TROE) {
     const double a = fp[4], iT3 = 1.0 / fp[5], iT1 = 1.0 / fp[6], T2 = fp[7];
-    const double e3 = exp(-T * iT3), e1 = exp(-T * iT1);
+    const double e3 = exp_lib(-T * iT3), e1 = exp_lib(-T * iT1);
     double Fc = (1.0 - a) * e3 + a * e1;
     double dFc = -(1.0 - a) * iT3 * e3 - a * iT1 * e1;
-    if (hasT2) { const double e2 = exp(-T2 * invT); Fc += e2; dFc += T2 * invT * invT * e2; }
-    const double L = log(Pr) * ILN10, Lc = log(Fc) * ILN10;
+    if (hasT2) { const double e2 = exp_lib(-T2 * invT); Fc += e2; dFc += T2 * invT * invT * e2; }
+    const double L = log_lib(Pr) * ILN10, Lc = log_lib(Fc) * ILN10;
     const double n = 0.75 - 1.27 * Lc;
     const double A = L - 0.4 - 0.67 * Lc;
     const double B = n - 0.14 * A;
     const double iB = 1.0 / B;
     const double f = A * iB;
     const double g = 1.0 / (1.0 + f * f);
-    b.F = exp(LN10 * Lc * g);
+    b.F = exp_lib(LN10 * Lc * g);
     const double dlogF_df = -2.0 * Lc * f * g * g;
     const double df_dL = n * iB * iB;
     const double df_dLc = (-0.67 * B + 1.1762 * A) * iB * iB;
@@ -93,13 +159,13 @@ static __device__ __noinline__ Blend blend(int type, bool hasT2, const double* _
     b.dF_dT = b.F * (g + dlogF_df * df_dLc) * dFc / Fc;
   } else if (type == PYJAC_FALLOFF_SRI) {
     const double a = fp[4], bb = fp[5], ic = 1.0 / fp[6], d = fp[7], e = fp[8];
-    const double L = log(Pr) * ILN10;
+    const double L = log_lib(Pr) * ILN10;
     const double X = 1.0 / (1.0 + L * L);
-    const double eb = exp(-bb * invT), ec = exp(-T * ic);
+    const double eb = exp_lib(-bb * invT), ec = exp_lib(-T * ic);
     const double base = a * eb + ec;
     const double dbase = a * bb * invT * invT * eb - ec * ic;
-    const double lb = log(base);
-    b.F = d * exp(X * lb + e * lnT);
+    const double lb = log_lib(base);
+    b.F = d * exp_lib(X * lb + e * lnT);
     b.dF_dPr = b.F * lb * (-2.0 * L * X * X) * ILN10 / Pr;
     b.dF_dT = b.F * (X * dbase / base + e * invT);
   }
@@ -114,7 +180,7 @@ struct Smem {
   int4* grp;
   __device__ __forceinline__ Smem(unsigned char* raw, const DevJac& m) {
     sc = reinterpret_cast<D2*>(raw);
-    C = sc + J_NSC * LS; G = C + (m.ns + 1) * LS; Hh = G + (m.ns + 1) * LS; K = Hh + (m.ns + 1) * LS;
+    C = sc + 2 * J_NSC * LS; G = C + (m.ns + 1) * LS; Hh = G + (m.ns + 1) * LS; K = Hh + (m.ns + 1) * LS;
     dE = K + (m.ns + 1) * LS; V = dE + m.max_nrb * LS; red = V + m.n_val * LS;
     dn = reinterpret_cast<double*>(red + NW * J_NRED * LS);
     grp = reinterpret_cast<int4*>(dn + ((m.nr + 1) & ~1));
@@ -125,16 +191,16 @@ struct Smem {
 struct Out {
   double *pa, *pb;     // element 0 of state a / b
   int64_t tile;
-  bool va, vb, vec;    // state valid; 16-byte store possible (tile even: the two states are adjacent)
-  __device__ __forceinline__ void store(uint32_t pos, D2 v) const {
+  bool full;           // both states valid and adjacent in memory (tile even): one 16-byte store
+  bool va, vb;         // state valid (the slow path: ragged last pair, odd tile)
+  __device__ __noinline__ void store_slow(uint32_t pos, double a, double b) const {
     const int64_t off = (int64_t)pos * tile;
-    if (vec) {
-      if (vb) __stcs(reinterpret_cast<double2*>(pa + off), make_double2(v.a, v.b));
-      else if (va) __stcs(pa + off, v.a);
-    } else {
-      if (va) __stcs(pa + off, v.a);
-      if (vb) __stcs(pb + off, v.b);
-    }
+    if (va) __stcs(pa + off, a);
+    if (vb) __stcs(pb + off, b);
+  }
+  __device__ __forceinline__ void store(uint32_t pos, D2 v) const {
+    if (full) __stcs(reinterpret_cast<double2*>(pa + (int64_t)pos * tile), make_double2(v.a, v.b));
+    else store_slow(pos, v.a, v.b);
   }
 };
 
@@ -147,7 +213,7 @@ template <class PosT> __device__ __forceinline__ bool has_pos(PosT p) { return p
 template <int LS, class PosT>
 __device__ __forceinline__ void gather_unit(const DevJac& m, const DevJacOut& o, const Smem<LS>& sm, const JGroup g, int sub,
                                             const Out& out, bool conp, int blk_r0) {
-  constexpr int IPW = 32 / LS, U = 4;
+  constexpr int IPW = 32 / LS, U = 4, R = 1, RR = 1;   // pair steps requested at once: R (one word per step), RR (JK_ROW: two)
   const int lane = threadIdx.x & 31, pr = lane % LS, il = lane / LS;
   const D2* __restrict__ V = sm.V + pr;
   const PosT* __restrict__ posA = reinterpret_cast<const PosT*>(o.posA) + g.piece_off;
@@ -174,6 +240,11 @@ __device__ __forceinline__ void gather_unit(const DevJac& m, const DevJacOut& o,
   }
   const int p0 = sub * (U * IPW) + il;
   const int nP2 = g.nP2, nM2 = g.nM2;
+  // pair steps needed by the quarter of the group that this thread's u-th piece belongs to (warp-uniform, descending)
+  int nb[U];
+#pragma unroll
+  for (int u = 0; u < U; ++u) nb[u] = (int)((g.qsteps >> (8 * ((sub * U + u) / LS))) & 0xffu);
+  (void)nP2;
   if (g.kind == JK_BLK) {
     const uint32_t* __restrict__ e = m.ent + g.ent_off + p0;
     PosT pos[U]; uint32_t pi[U];
@@ -188,17 +259,25 @@ __device__ __forceinline__ void gather_unit(const DevJac& m, const DevJacOut& o,
     for (int u = 0; u < U; ++u) { v[u] = mk(0.0); np[u] = __ldg(nplus + p0 + u * IPW); }
     // entries 2 s and 2 s + 1 of a piece have one sign: plus while s < nplus, then minus (a multiplier of +-1 in the
     // DFMA: no sign arithmetic on the values)
-#pragma unroll 2
-    for (int s = 0; s < nP2; ++s) {
-      uint32_t w[U];
+    // rounds of R pair steps: every entry word of a round is requested before the first one is used (one exposed L2
+    // round trip per round instead of one per step: the gathers are latency bound)
+#pragma unroll 1
+    for (int s0 = 0; s0 < nb[0]; s0 += R) {
+      uint32_t w[R][U];
 #pragma unroll
-      for (int u = 0; u < U; ++u) w[u] = __ldg(e + s * J_GW + u * IPW);
+      for (int q = 0; q < R; ++q)
 #pragma unroll
-      for (int u = 0; u < U; ++u) {
-        const double sg = s < np[u] ? 1.0 : -1.0;
-        v[u] = fma2(sg, ld2(V + (w[u] & 0xffffu) * LS), v[u]);
-        v[u] = fma2(sg, ld2(V + (w[u] >> 16) * LS), v[u]);
-      }
+        for (int u = 0; u < U; ++u) w[q][u] = s0 + q < nb[u] ? __ldg(e + (s0 + q) * J_GW + u * IPW) : 0u;
+#pragma unroll
+      for (int q = 0; q < R; ++q)
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+          if (s0 + q < nb[u]) {
+            const double sg = s0 + q < np[u] ? 1.0 : -1.0;
+            v[u] = fma2(sg, ld2(V + (w[q][u] & 0xffffu) * LS), v[u]);
+            v[u] = fma2(sg, ld2(V + (w[q][u] >> 16) * LS), v[u]);
+          }
+        }
     }
 #pragma unroll
     for (int u = 0; u < U; ++u) {
@@ -235,12 +314,17 @@ __device__ __forceinline__ void gather_unit(const DevJac& m, const DevJacOut& o,
       if (!minus) { v0[u] = fma2(de, x, v0[u]); v1[u] = fma2(d, x, v1[u]); }
       else { v0[u] = fma2(-de, x, v0[u]); v1[u] = fma2(-d, x, v1[u]); }
     };
-    for (int s = 0; s < nP2; ++s) {
-      uint2 w[U];
+#pragma unroll 1
+    for (int s0 = 0; s0 < nb[0]; s0 += RR) {
+      uint2 w[RR][U];
 #pragma unroll
-      for (int u = 0; u < U; ++u) w[u] = __ldg(e + s * J_GW + u * IPW);
+      for (int q = 0; q < RR; ++q)
 #pragma unroll
-      for (int u = 0; u < U; ++u) { acc(w[u].x, u, false); acc(w[u].y, u, false); }
+        for (int u = 0; u < U; ++u) w[q][u] = s0 + q < nb[u] ? __ldg(e + (s0 + q) * J_GW + u * IPW) : make_uint2(0u, 0u);
+#pragma unroll
+      for (int q = 0; q < RR; ++q)
+#pragma unroll
+        for (int u = 0; u < U; ++u) if (s0 + q < nb[u]) { acc(w[q][u].x, u, false); acc(w[q][u].y, u, false); }
     }
     e += nP2 * J_GW;
     for (int s = 0; s < nM2; ++s) {
@@ -257,17 +341,24 @@ __device__ __forceinline__ void gather_unit(const DevJac& m, const DevJacOut& o,
     int np[U];
 #pragma unroll
     for (int u = 0; u < U; ++u) np[u] = __ldg(nplus + p0 + u * IPW);
-    for (int s = 0; s < nP2; ++s) {
-      uint32_t w[U];
+#pragma unroll 1
+    for (int s0 = 0; s0 < nb[0]; s0 += R) {
+      uint32_t w[R][U];
 #pragma unroll
-      for (int u = 0; u < U; ++u) w[u] = __ldg(e + s * J_GW + u * IPW);
+      for (int q = 0; q < R; ++q)
 #pragma unroll
-      for (int u = 0; u < U; ++u) {
-        const uint32_t i0 = (w[u] & 0xffffu) * LS, i1 = (w[u] >> 16) * LS;
-        const double sg = s < np[u] ? 1.0 : -1.0;
-        v0[u] = fma2(sg, ld2(V + i0), v0[u]); v1[u] = fma2(sg, ld2(V8 + i0), v1[u]);
-        v0[u] = fma2(sg, ld2(V + i1), v0[u]); v1[u] = fma2(sg, ld2(V8 + i1), v1[u]);
-      }
+        for (int u = 0; u < U; ++u) w[q][u] = s0 + q < nb[u] ? __ldg(e + (s0 + q) * J_GW + u * IPW) : 0u;
+#pragma unroll
+      for (int q = 0; q < R; ++q)
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+          if (s0 + q < nb[u]) {
+            const uint32_t i0 = (w[q][u] & 0xffffu) * LS, i1 = (w[q][u] >> 16) * LS;
+            const double sg = s0 + q < np[u] ? 1.0 : -1.0;
+            v0[u] = fma2(sg, ld2(V + i0), v0[u]); v1[u] = fma2(sg, ld2(V8 + i0), v1[u]);
+            v0[u] = fma2(sg, ld2(V + i1), v0[u]); v1[u] = fma2(sg, ld2(V8 + i1), v1[u]);
+          }
+        }
     }
   }
   // factors of the T / E rows (only units that finish such rows get here with kind != JK_COL: a few per tile)
@@ -377,7 +468,7 @@ __device__ __forceinline__ void reaction_general(const DevJac& m, const Smem<LS>
     lam_f = LN10 * dlg_dT * (-2.0 * invT * invT / (iTmax - iTmin));
     dlnk_dP = dlg_dP * 2.0 / (Pp * (lPmax - lPmin));
   }
-  const double kf = exp(lnkf);
+  const double kf = exp_lib(lnkf);
   // stoichiometry: concentrations, powers and one-factor-removed products (no division by C_k: DESIGN.md S7).
   // Unused entries point at the dummy species ns (C = 1, thermo = 0).
   const uint32_t spk[6] = {spw.x & 0xffffu, spw.x >> 16, spw.y & 0xffffu, spw.y >> 16, spw.z & 0xffffu, spw.z >> 16};
@@ -395,14 +486,14 @@ __device__ __forceinline__ void reaction_general(const DevJac& m, const Smem<LS>
   const double Pif = pw[0] * pw[1] * pw[2], Pir = pw[3] * pw[4] * pw[5];
   const double snu = (double)((int)((info >> JI_SNU_SHIFT) & 31u) - 16);
   double kr = 0.0, lam_r = 0.0;
-  if (rev) {      // a4: K_c from Gibbs polynomials; k_r = k_f / K_c = exp(ln k_f - ln K_c)
+  if (rev) {      // a4: K_c from Gibbs polynomials; k_r = k_f / K_c = exp_lib(ln k_f - ln K_c)
     if (info & JI_REVX) {        // explicit reverse Arrhenius parameters (R9): K_c plays no role
       const int ro = ext.w;
       const double lAr = __ldg(m.rev_par + 3 * ro), br = __ldg(m.rev_par + 3 * ro + 1), Tar = __ldg(m.rev_par + 3 * ro + 2);
-      kr = exp(lAr + br * lnT - Tar * invT);
+      kr = exp_lib(lAr + br * lnT - Tar * invT);
       lam_r = (br + Tar * invT) * invT;
     } else {
-      kr = exp(lnkf + dg - snu * ln_patm_rt);
+      kr = exp_lib(lnkf + dg - snu * ln_patm_rt);
       lam_r = lam_f - (dh - snu) * invT;
     }
   }
@@ -429,7 +520,7 @@ __device__ __forceinline__ void reaction_general(const DevJac& m, const Smem<LS>
       const bool chem = (info & JI_CHEM) != 0;
       const double b0 = fp[1], Ta0 = fp[2];
       const double lnrat = fp[0] + b0 * lnT - Ta0 * invT - lnkf;
-      const double k0_kinf = exp(chem ? -lnrat : lnrat);
+      const double k0_kinf = exp_lib(chem ? -lnrat : lnrat);
       const double Pr = k0_kinf * M;
       const Blend bl = blend(type, info & JI_T2, fp, T, invT, lnT, Pr);
       const double i1p = 1.0 / (1.0 + Pr);
@@ -492,11 +583,11 @@ __device__ __forceinline__ void reaction_general(const DevJac& m, const Smem<LS>
 // ---------------------------------------------------------------------------------------------------
 template <int LS, bool DENSE, class PosT>
 __global__ void __launch_bounds__(NT, 1)
-jacobian2_kernel(const DevJac m, const DevJacOut o, int mode, int64_t n_states, int64_t tile, const double* __restrict__ phi,
+jacobian2_kernel(const DevJac m, const DevJacOut o, int mode, int64_t n_states, int64_t tile, int tshift, const double* __restrict__ phi,
                  const double* __restrict__ param, double* __restrict__ out, unsigned long long* __restrict__ sched) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   constexpr int S = 2 * LS, IPW = 32 / LS;
-  const Smem<LS> sm(smem_raw, m);
+  Smem<LS> sm(smem_raw, m);
   __shared__ int cnt[4];
   __shared__ long long next_tile;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, pr = tid % LS;
@@ -513,34 +604,49 @@ jacobian2_kernel(const DevJac m, const DevJacOut o, int mode, int64_t n_states, 
   const bool vec = (tile & 1) == 0;
   const int n2 = nvar * nvar;
   const int n_zslices = DENSE ? (n2 + 1023) / 1024 : 0;
+  // per-pair scalars of a tile, by the first warp (T, E and the parameter already in registers): double-buffered,
+  // the scalars of tile n + 1 are computed while tile n is gathered
+  auto write_scalars = [&](D2* sc, D2 T, D2 E_, D2 par) {
+    const D2 V = conp ? E_ : par, Pp = conp ? par : E_;
+    if (lane < LS) {
+      const D2 invT = mk(1.0 / T.a, 1.0 / T.b), lnT = mk(log_lib(T.a), log_lib(T.b)), RT = T * R_GAS;
+      const D2 Ctot = mk(Pp.a / RT.a, Pp.b / RT.b);
+      st2(sc + SC_T * LS + pr, T); st2(sc + SC_V * LS + pr, V); st2(sc + SC_P * LS + pr, Pp);
+      st2(sc + SC_INVT * LS + pr, invT); st2(sc + SC_LNT * LS + pr, lnT); st2(sc + SC_CTOT * LS + pr, Ctot);
+      st2(sc + SC_RT * LS + pr, RT); st2(sc + SC_LNP * LS + pr, mk(log_lib(Pp.a), log_lib(Pp.b)));
+      st2(sc + SC_LNPRT * LS + pr, mk(log_lib(P_ATM / RT.a), log_lib(P_ATM / RT.b)));
+    }
+  };
+  // this thread's pair of states in tile t (ragged tail: the last state is recomputed, never stored)
+  auto pair_of = [&](int64_t t, int64_t& sa, int64_t& sb) { const int64_t s0 = t * S + 2 * pr; sa = min(s0, n_states - 1); sb = min(s0 + 1, n_states - 1); };
+  // moles of the species this thread handles in the first trip of the species loop
+  const int k_mine = tid / LS;
+  auto fetch_moles = [&](int64_t t) {
+    int64_t sa, sb; pair_of(t, sa, sb);
+    if (k_mine < L) return mk(phi[state_base(sa, tshift, nvar) + (int64_t)(2 + k_mine) * tile], phi[state_base(sb, tshift, nvar) + (int64_t)(2 + k_mine) * tile]);
+    return mk(0.0);
+  };
+  D2* sc_other = sm.sc + J_NSC * LS;
+  D2 pn = mk(0.0);
+  if ((int64_t)blockIdx.x < n_tiles) {
+    pn = fetch_moles(blockIdx.x);
+    if (warp == 0) {
+      int64_t sa, sb; pair_of(blockIdx.x, sa, sb);
+      const double *pha = phi + state_base(sa, tshift, nvar), *phb = phi + state_base(sb, tshift, nvar);
+      write_scalars(sm.sc, mk(pha[0], phb[0]), mk(pha[tile], phb[tile]), mk(param[sa], param[sb]));
+    }
+  }
   __syncthreads();
   for (int64_t tl = blockIdx.x; tl < n_tiles;) {
-    unsigned long long ticket = 0;
-    if (tid == 0) ticket = atomicAdd(sched, 1ull);
+    if (tid == 0) { next_tile = (long long)gridDim.x + (long long)atomicAdd(sched, 1ull); cnt[2] = 0; cnt[3] = 0; }   // read after the next barrier
     const int64_t s0 = tl * S + 2 * pr;
     const bool va = s0 < n_states, vb = s0 + 1 < n_states;
-    const int64_t sa = min(s0, n_states - 1), sb = min(s0 + 1, n_states - 1);   // ragged tail: recompute the last state, never store
-    const double* __restrict__ pha = phi + state_base(sa, tile, nvar);
-    const double* __restrict__ phb = phi + state_base(sb, tile, nvar);
+    const int64_t sa = min(s0, n_states - 1), sb = min(s0 + 1, n_states - 1);
+    const double* __restrict__ pha = phi + state_base(sa, tshift, nvar);
+    const double* __restrict__ phb = phi + state_base(sb, tshift, nvar);
     Out og;
-    og.pa = out + state_base(sa, tile, o.n_e); og.pb = out + state_base(sb, tile, o.n_e);
-    og.tile = tile; og.va = va; og.vb = vb; og.vec = vec;
-    // ---- phase 0a: per-pair scalars, by the first warp ------------------------------------------------------------
-    if (warp == 0) {
-      const D2 T = mk(pha[0], phb[0]), E_ = mk(pha[tile], phb[tile]), par = mk(param[sa], param[sb]);
-      const D2 V = conp ? E_ : par, Pp = conp ? par : E_;
-      if (lane < LS) {
-        const D2 invT = mk(1.0 / T.a, 1.0 / T.b), lnT = mk(log(T.a), log(T.b)), RT = T * R_GAS;
-        const D2 Ctot = mk(Pp.a / RT.a, Pp.b / RT.b);
-        st2(sm.sc + SC_T * LS + pr, T); st2(sm.sc + SC_V * LS + pr, V); st2(sm.sc + SC_P * LS + pr, Pp);
-        st2(sm.sc + SC_INVT * LS + pr, invT); st2(sm.sc + SC_LNT * LS + pr, lnT); st2(sm.sc + SC_CTOT * LS + pr, Ctot);
-        st2(sm.sc + SC_RT * LS + pr, RT); st2(sm.sc + SC_LNP * LS + pr, mk(log(Pp.a), log(Pp.b)));
-        st2(sm.sc + SC_LNPRT * LS + pr, mk(log(P_ATM / RT.a), log(P_ATM / RT.b)));
-      }
-      if (tid == 0) { next_tile = (long long)gridDim.x + (long long)ticket; cnt[2] = 0; cnt[3] = 0; }
-    }
-    __syncthreads();
-    const int64_t tl_next = next_tile;
+    og.pa = out + state_base(sa, tshift, o.n_e); og.pb = out + state_base(sb, tshift, o.n_e);
+    og.tile = tile; og.va = va; og.vb = vb; og.full = vec && vb;
     // ---- phase 0b: species (C_k = n_k / V, Eq. 6; NASA-7 thermo, R2) ------------------------------------
     {
       const D2 T = ld2(sm.sc + SC_T * LS + pr), V = ld2(sm.sc + SC_V * LS + pr);
@@ -575,7 +681,7 @@ jacobian2_kernel(const DevJac m, const DevJacOut o, int mode, int64_t n_states, 
         st2(sm.Hh + idx, hRT);
         st2(sm.K + idx, c);
         if (k < L) {
-          const D2 Ck = mk(pha[(int64_t)(2 + k) * tile], phb[(int64_t)(2 + k) * tile]) * invV;
+          const D2 Ck = (idx == tid ? pn : mk(pha[(int64_t)(2 + k) * tile], phb[(int64_t)(2 + k) * tile])) * invV;
           st2(sm.C + idx, Ck);
           acc0 += Ck; acc1 = fma2(Ck, c, acc1); acc2 = fma2(Ck, dcpR * R_GAS, acc2);
         } else {
@@ -589,6 +695,7 @@ jacobian2_kernel(const DevJac m, const DevJacOut o, int mode, int64_t n_states, 
       if (lane < 8 * LS) st2(sm.red + warp * J_NRED * LS + lane, mk(0.0));
     }
     __syncthreads();
+    const int64_t tl_next = next_tile;
     if (tid < LS) {
       // the last species: C_Ns from the ideal-gas law
       D2 s0_ = mk(0.0), s1_ = mk(0.0), s2_ = mk(0.0);
@@ -602,98 +709,113 @@ jacobian2_kernel(const DevJac m, const DevJacOut o, int mode, int64_t n_states, 
     for (int b = 0; b <= m.H; ++b) {
       if (b < m.H) {
         // ---- phase 1: reactions of block b ------------------------------------------------------------------------
-        const D2 V = ld2(sm.sc + SC_V * LS + pr), invT = ld2(sm.sc + SC_INVT * LS + pr), lnT = ld2(sm.sc + SC_LNT * LS + pr);
-        const D2 Ctot = ld2(sm.sc + SC_CTOT * LS + pr), RT = ld2(sm.sc + SC_RT * LS + pr), ln_patm_rt = ld2(sm.sc + SC_LNPRT * LS + pr);
-        const D2 eL = ld2(sm.sc + SC_EL * LS + pr), cL = ld2(sm.sc + SC_CL * LS + pr);
-        const D2 ctot_T = Ctot * invT;
-        const int r0 = m.blk_r0[b], nrb = m.blk_r0[b + 1] - r0;
-        D2 acc[7];
+        // One lane per (reaction, pair, STATE): scalar code, half the registers of a two-state formulation, so that 16
+        // warps fit without spills (phase 1 is bound by dependent fp64 latency: it needs the warps, not the sharing of
+        // table words between the two states).  16 / LS reactions per chunk; the reactions of the general path come
+        // first in the block (they are the expensive ones: longest-processing-time-first).
+        const int prs = (lane >> 1) % LS, st = lane & 1;                 // this lane's pair and state
+        const double* __restrict__ scd = reinterpret_cast<const double*>(sm.sc);
+        auto scv = [&](int i) { return scd[(i * LS + prs) * 2 + st]; };
+        const double V = scv(SC_V), invT = scv(SC_INVT), lnT = scv(SC_LNT), Ctot = scv(SC_CTOT), RT = scv(SC_RT), ln_patm_rt = scv(SC_LNPRT);
+        const double eL = scv(SC_EL), cL = scv(SC_CL);
+        const double ctot_T = Ctot * invT;
+        const int r0 = m.blk_r0[b], nrb = m.blk_r0[b + 1] - r0, ng = m.blk_ng[b];
+        constexpr int RPC = 16 / LS;                                     // reactions per chunk
+        const int n_gchunks = (ng + RPC - 1) / RPC, n_chunks = n_gchunks + (nrb - ng + RPC - 1) / RPC;
+        double acc[8];
 #pragma unroll
-        for (int q = 0; q < 7; ++q) acc[q] = mk(0.0);
-        const int n_chunks = (nrb * LS + 31) / 32;
+        for (int q = 0; q < 8; ++q) acc[q] = 0.0;
+        const double* __restrict__ Cd = reinterpret_cast<const double*>(sm.C) + prs * 2 + st;
+        const double* __restrict__ Gd = reinterpret_cast<const double*>(sm.G) + prs * 2 + st;
+        const double* __restrict__ Hd = reinterpret_cast<const double*>(sm.Hh) + prs * 2 + st;
+        const double* __restrict__ Kd = reinterpret_cast<const double*>(sm.K) + prs * 2 + st;
+        double* __restrict__ Vd = reinterpret_cast<double*>(sm.V) + prs * 2 + st;
         for (int chunk = next_chunk(cnt + 0); chunk < n_chunks; chunk = next_chunk(cnt + 0)) {
-          const int lr = chunk * IPW + lane / LS;
-          if (lr >= nrb) continue;
+          const bool general = chunk < n_gchunks;
+          const int lr = general ? chunk * RPC + lane / (2 * LS) : ng + (chunk - n_gchunks) * RPC + lane / (2 * LS);
+          if (lr >= (general ? ng : nrb)) continue;
           const int r = r0 + lr;
           const uint32_t info = __ldg(m.info + r);
           const uint4 spw = __ldg(reinterpret_cast<const uint4*>(m.sp) + r);
-          if (!(info & JI_FAST)) {
-#pragma unroll 1
-            for (int st = 0; st < 2; ++st) {
-              double inc[7];
-              reaction_general<LS>(m, sm, r, lr, pr, st, conp, info, spw, inc);
+          if (general) {
+            double inc[7];
+            reaction_general<LS>(m, sm, r, lr, prs, st, conp, info, spw, inc);
 #pragma unroll
-              for (int q = 0; q < 7; ++q) { if (st == 0) acc[q].a += inc[q]; else acc[q].b += inc[q]; }
-            }
+            for (int q = 0; q < 7; ++q) acc[q] += inc[q];
             continue;
           }
           // fast path: elementary or third-body reaction, all coefficients 1, <= 2 species per side, the last
-          // species in no role; both states at once
+          // species in no role
           const double rx_lnA = __ldg(m.lnA + r), rx_beta = __ldg(m.beta + r), rx_Ta = __ldg(m.Ta + r), dn = sm.dn[r];
-          const int k0 = spw.x & 0xffffu, k1 = spw.x >> 16, k2 = spw.y >> 16, k3 = spw.z & 0xffffu;   // reactants 0, 1; products 3, 4
-          const D2 C0 = ld2(sm.C + k0 * LS + pr), C1 = ld2(sm.C + k1 * LS + pr), C2 = ld2(sm.C + k2 * LS + pr), C3 = ld2(sm.C + k3 * LS + pr);
-          const D2 dh = (ld2(sm.Hh + k2 * LS + pr) + ld2(sm.Hh + k3 * LS + pr)) - (ld2(sm.Hh + k0 * LS + pr) + ld2(sm.Hh + k1 * LS + pr));
-          const D2 dc = (ld2(sm.K + k2 * LS + pr) + ld2(sm.K + k3 * LS + pr)) - (ld2(sm.K + k0 * LS + pr) + ld2(sm.K + k1 * LS + pr));
-          const D2 lnkf = fma2(rx_beta, lnT, mk(rx_lnA)) - rx_Ta * invT;
-          const D2 lam_f = fma2(rx_Ta, invT, mk(rx_beta)) * invT;
-          const D2 kf = exp2_(lnkf);
+          const int k0 = (spw.x & 0xffffu) * (2 * LS), k1 = (spw.x >> 16) * (2 * LS), k2 = (spw.y >> 16) * (2 * LS), k3 = (spw.z & 0xffffu) * (2 * LS);   // reactants 0, 1; products 3, 4
+          const double C0 = Cd[k0], C1 = Cd[k1], C2 = Cd[k2], C3 = Cd[k3];
+          const double dh = (Hd[k2] + Hd[k3]) - (Hd[k0] + Hd[k1]);
+          const double dc = (Kd[k2] + Kd[k3]) - (Kd[k0] + Kd[k1]);
+          const double lnkf = fma(rx_beta, lnT, rx_lnA) - rx_Ta * invT;
+          const double lam_f = fma(rx_Ta, invT, rx_beta) * invT;
           const double snu = (double)((int)((info >> JI_SNU_SHIFT) & 31u) - 16);
           const bool rev = info & JI_REV;
-          D2 kr = mk(0.0), lam_r = mk(0.0);
+          // a4: K_c from the Gibbs polynomials, k_r = k_f / K_c = exp(ln k_f - ln K_c); both exponentials together
+          double arg_r = lnkf, lam_r = 0.0;
           if (rev) {
-            const D2 dg = (ld2(sm.G + k2 * LS + pr) + ld2(sm.G + k3 * LS + pr)) - (ld2(sm.G + k0 * LS + pr) + ld2(sm.G + k1 * LS + pr));
-            kr = exp2_(lnkf + dg - snu * ln_patm_rt);
+            const double dg = (Gd[k2] + Gd[k3]) - (Gd[k0] + Gd[k1]);
+            arg_r = lnkf + dg - snu * ln_patm_rt;
             lam_r = lam_f - (dh - snu) * invT;
           }
-          const D2 Rf = kf * (C0 * C1), Rr = kr * (C2 * C3), Rn = Rf - Rr;
-          const D2 dRdT = lam_f * Rf - lam_r * Rr;
-          D2* __restrict__ Vp = sm.V + (spw.w & 0xffffu) * LS + pr;
+          double kf = exp_core(lnkf), kr = exp_core(arg_r);
+          if (!(exp_in_range(lnkf) && exp_in_range(arg_r))) { kf = exp_lib(lnkf); kr = exp_lib(arg_r); }
+          if (!rev) kr = 0.0;
+          const double Rf = kf * (C0 * C1), Rr = kr * (C2 * C3), Rn = Rf - Rr;
+          const double dRdT = lam_f * Rf - lam_r * Rr;
+          double* __restrict__ Vp = Vd + (spw.w & 0xffffu) * (2 * LS);
+          constexpr int SL = 8 * 2 * LS;                                 // doubles between consecutive slots of a reaction
           const int nre = (info >> JI_NREAC_SHIFT) & 3, npr = (info >> JI_NPROD_SHIFT) & 3;
-          D2 c = mk(1.0), GT = dRdT, MdcdM_R = mk(0.0), GL = mk(0.0);
-          int si = 2 + nre + (rev ? npr : 0);
+          double c = 1.0, GT = dRdT, MdcdM_R = 0.0, GL = 0.0;
           if ((info & JI_TYPE_MASK) == PYJAC_THIRD_BODY) {
             const int4 ext = __ldg(reinterpret_cast<const int4*>(m.ext) + r);
             const double adef = (info & JI_ADEF) ? 1.0 : 0.0;
-            D2 M = Ctot * adef;
-            for (int q = 0; q < ext.z; ++q) {
-              const int esp = __ldg(m.eff_sp + ext.y + q);
-              const double ed = __ldg(m.eff_d + ext.y + q);
-              M = fma2(ed, ld2(sm.C + esp * LS + pr), M);
-              st2(Vp + (si + q) * 8 * LS, Rn * ed);            // dQ/dC_e through [M]: alpha' X, X = R_n
+            const int si = 2 + nre + (rev ? npr : 0);
+            double M = Ctot * adef;
+            for (int q0 = 0; q0 < ext.z; q0 += 4) {                       // efficiency list, 4 entries per round trip
+              int esp[4]; double ed[4];
+#pragma unroll
+              for (int q = 0; q < 4; ++q) { esp[q] = q0 + q < ext.z ? __ldg(m.eff_sp + ext.y + q0 + q) : ns; ed[q] = q0 + q < ext.z ? __ldg(m.eff_d + ext.y + q0 + q) : 0.0; }
+#pragma unroll
+              for (int q = 0; q < 4; ++q) {
+                M = fma(ed[q], Cd[esp[q] * (2 * LS)], M);
+                if (q0 + q < ext.z) Vp[(si + q0 + q) * SL] = Rn * ed[q];     // dQ/dC_e through [M]: alpha' X, X = R_n
+              }
             }
             c = M; GT = M * dRdT; MdcdM_R = M * Rn; GL = Rn * adef;
           }
-          const D2 q = c * Rn;
-          const D2 a_ = c * kf, b_ = c * kr;
-          st2(Vp + 2 * 8 * LS, a_ * C1);
-          if (nre == 2) st2(Vp + 3 * 8 * LS, a_ * C0);
+          const double q = c * Rn;
+          const double a_ = c * kf, b_ = c * kr;
+          Vp[2 * SL] = a_ * C1;
+          if (nre == 2) Vp[3 * SL] = a_ * C0;
           if (rev) {
-            st2(Vp + (2 + nre) * 8 * LS, -(b_ * C3));
-            if (npr == 2) st2(Vp + (3 + nre) * 8 * LS, -(b_ * C2));
+            Vp[(2 + nre) * SL] = -(b_ * C3);
+            if (npr == 2) Vp[(3 + nre) * SL] = -(b_ * C2);
           }
-          const D2 slotT = V * (GT - ctot_T * GL);
-          D2 slotE;
+          const double slotT = V * (GT - ctot_T * GL);
+          double slotE;
           if (conp) {
             const double of = (double)((info >> JI_OF_SHIFT) & 15), orv = (double)((info >> JI_OR_SHIFT) & 15);
             slotE = q - c * (Rf * of - Rr * orv) - MdcdM_R + Ctot * GL;
           } else {
-            slotE = V * mk(GL.a / RT.a, GL.b / RT.b);
+            slotE = V * (GL / RT);
           }
-          st2(Vp, slotT);
-          st2(Vp + 8 * LS, slotE);
-          const D2 dEt = RT * (dh - conv * snu - eL * (snu - dn));
-          const D2 dct = dc - cL * (snu - dn);
-          st2(sm.dE + lr * LS + pr, dEt);
-          acc[0] = fma2(dEt, q, acc[0]); acc[1] = fma2(dn, q, acc[1]); acc[2] = fma2(dEt, slotT, acc[2]); acc[3] = fma2(dn, slotT, acc[3]);
-          acc[4] = fma2(dEt, slotE, acc[4]); acc[5] = fma2(dn, slotE, acc[5]); acc[6] = fma2(dct, q, acc[6]);
+          Vp[0] = slotT;
+          Vp[SL] = slotE;
+          const double dEt = RT * (dh - conv * snu - eL * (snu - dn));
+          const double dct = dc - cL * (snu - dn);
+          reinterpret_cast<double*>(sm.dE)[(lr * LS + prs) * 2 + st] = dEt;
+          acc[0] = fma(dEt, q, acc[0]); acc[1] = fma(dn, q, acc[1]); acc[2] = fma(dEt, slotT, acc[2]); acc[3] = fma(dn, slotT, acc[3]);
+          acc[4] = fma(dEt, slotE, acc[4]); acc[5] = fma(dn, slotE, acc[5]); acc[6] = fma(dct, q, acc[6]);
         }
         // per-warp partial reaction sums (the barrier below publishes them together with the slots)
-#pragma unroll
-        for (int q = 0; q < 7; ++q) {
-          D2 v = acc[q];
-#pragma unroll
-          for (int off = 16; off >= LS; off >>= 1) v += shfl_xor2(v, off);
-          if (lane < LS) { D2* p = sm.red + (warp * J_NRED + q) * LS + lane; st2(p, ld2(p) + v); }
+        {
+          double* __restrict__ redd = reinterpret_cast<double*>(sm.red + warp * J_NRED * LS);
+          WarpSum<8, 16, 2 * LS>::run(acc, 0, true, [&](int jv, double x) { if (jv < 7) redd[(jv * LS + prs) * 2 + st] += x; });
         }
         __syncthreads();
         if (tid == 0) cnt[0] = 0;
@@ -701,40 +823,55 @@ jacobian2_kernel(const DevJac m, const DevJacOut o, int mode, int64_t n_states, 
           // every reaction is done.  a10: the four corner entries from the reaction sums (R4-7), by the last warp
           if (warp == NW - 1 && lane < LS) {
             const D2 T = ld2(sm.sc + SC_T * LS + pr), Pp = ld2(sm.sc + SC_P * LS + pr), D = ld2(sm.sc + SC_D * LS + pr);
+            const D2 V = ld2(sm.sc + SC_V * LS + pr), Ctot = ld2(sm.sc + SC_CTOT * LS + pr), cL = ld2(sm.sc + SC_CL * LS + pr);
             D2 sums[7];
 #pragma unroll
             for (int q = 0; q < 7; ++q) { sums[q] = mk(0.0); for (int w = 0; w < NW; ++w) sums[q] += ld2(sm.red + (w * J_NRED + q) * LS + pr); }
             const D2 dDdT0 = ld2(sm.sc + SC_DDDT * LS + pr);
-            D2 JTT, JTE, JET, JEE;
-            auto corner = [&](double T, double V, double Pp, double Ctot, double D, double cL, double dDdT0, double fT, double N, double Ssum,
-                              double AT, double BT, double AE, double BE, double sumcw, double& JTT, double& JTE, double& JET, double& JEE) {
-              const double iV = 1.0 / V;
-              const double dN_dT = AT * iV + sumcw;
-              const double dD_dT = dDdT0 - cL * Ctot / T;
-              JTT = -(dN_dT + fT * dD_dT) / D;
-              const double dS_dT = BT * iV;
-              double dN_dE, dD_dE, dS_dE;
-              if (conp) {
-                const double fE = V * (T * R_GAS / Pp * Ssum + fT / T);
-                dN_dE = (AE - N) * iV; dD_dE = -(D - Ctot * cL) * iV; dS_dE = (BE - Ssum) * iV;
-                JTE = -(dN_dE + fT * dD_dE) / D;
-                JET = V * (T * R_GAS / Pp * dS_dT + JTT / T) + V * (R_GAS * Ssum / Pp - fT / (T * T));
-                JEE = V * (T * R_GAS / Pp * dS_dE + JTE / T) + fE * iV;
-              } else {
-                dN_dE = AE * iV; dD_dE = cL / (R_GAS * T); dS_dE = BE * iV;
-                JTE = -(dN_dE + fT * dD_dE) / D;
-                JET = T * R_GAS * dS_dT + Pp / T * JTT + R_GAS * Ssum - Pp * fT / (T * T);
-                JEE = T * R_GAS * dS_dE + Pp / T * JTE + fT / T;
-              }
-            };
             const D2 fT = mk(-sums[0].a / D.a, -sums[0].b / D.b);        // f_T = -N / D (Eq. 5)
-            corner(T.a, V.a, Pp.a, Ctot.a, D.a, cL.a, dDdT0.a, fT.a, sums[0].a, sums[1].a, sums[2].a, sums[3].a, sums[4].a, sums[5].a, sums[6].a, JTT.a, JTE.a, JET.a, JEE.a);
-            corner(T.b, V.b, Pp.b, Ctot.b, D.b, cL.b, dDdT0.b, fT.b, sums[0].b, sums[1].b, sums[2].b, sums[3].b, sums[4].b, sums[5].b, sums[6].b, JTT.b, JTE.b, JET.b, JEE.b);
+            D2 JTT, JTE, JET, JEE;
+#pragma unroll 1
+            for (int h2 = 0; h2 < 2; ++h2) {
+              auto pick = [&](D2 x) { return h2 ? x.b : x.a; };
+              const double T_ = pick(T), V_ = pick(V), Pp_ = pick(Pp), Ctot_ = pick(Ctot), D_ = pick(D), cL_ = pick(cL), fT_ = pick(fT);
+              const double N = pick(sums[0]), Ssum = pick(sums[1]), AT = pick(sums[2]), BT = pick(sums[3]), AE = pick(sums[4]), BE = pick(sums[5]), sumcw = pick(sums[6]);
+              const double iV = 1.0 / V_;
+              const double dN_dT = AT * iV + sumcw;
+              const double dD_dT = pick(dDdT0) - cL_ * Ctot_ / T_;
+              const double jTT = -(dN_dT + fT_ * dD_dT) / D_;
+              const double dS_dT = BT * iV;
+              double dN_dE, dD_dE, dS_dE, jTE, jET, jEE;
+              if (conp) {
+                const double fE = V_ * (T_ * R_GAS / Pp_ * Ssum + fT_ / T_);
+                dN_dE = (AE - N) * iV; dD_dE = -(D_ - Ctot_ * cL_) * iV; dS_dE = (BE - Ssum) * iV;
+                jTE = -(dN_dE + fT_ * dD_dE) / D_;
+                jET = V_ * (T_ * R_GAS / Pp_ * dS_dT + jTT / T_) + V_ * (R_GAS * Ssum / Pp_ - fT_ / (T_ * T_));
+                jEE = V_ * (T_ * R_GAS / Pp_ * dS_dE + jTE / T_) + fE * iV;
+              } else {
+                dN_dE = AE * iV; dD_dE = cL_ / (R_GAS * T_); dS_dE = BE * iV;
+                jTE = -(dN_dE + fT_ * dD_dE) / D_;
+                jET = T_ * R_GAS * dS_dT + Pp_ / T_ * jTT + R_GAS * Ssum - Pp_ * fT_ / (T_ * T_);
+                jEE = T_ * R_GAS * dS_dE + Pp_ / T_ * jTE + fT_ / T_;
+              }
+              if (h2) { JTT.b = jTT; JTE.b = jTE; JET.b = jET; JEE.b = jEE; } else { JTT.a = jTT; JTE.a = jTE; JET.a = jET; JEE.a = jEE; }
+            }
             og.store((uint32_t)o.d_pos[0], JTT); og.store((uint32_t)o.d_pos[1], JTE); og.store((uint32_t)o.d_pos[2], JET); og.store((uint32_t)o.d_pos[3], JEE);
           }
         }
       }
       // ---- phase 2: pieces of block b (b == H: the final combine wave) -----------------------------------------------
+      // The state of the NEXT tile is requested before the last block is gathered: its DRAM latency hides behind the
+      // gathers, and the first warp turns T, E and the parameter into the next tile's scalars when it runs out of units.
+      D2 nT = mk(1.0), nE = mk(1.0), nPar = mk(1.0);
+      const bool fetch_next = b == m.H - 1 && tl_next < n_tiles;
+      if (fetch_next) {
+        pn = fetch_moles(tl_next);
+        if (warp == 0) {
+          int64_t na, nb_; pair_of(tl_next, na, nb_);
+          const double *qa = phi + state_base(na, tshift, nvar), *qb = phi + state_base(nb_, tshift, nvar);
+          nT = mk(qa[0], qb[0]); nE = mk(qa[tile], qb[tile]); nPar = mk(param[na], param[nb_]);
+        }
+      }
       const int g0 = m.blk_g0[b], n_units = (m.blk_g0[b + 1] - g0) * LS;
       int* counter = cnt + (b < m.H ? 1 : 2);
       if (n_units > 0) {
@@ -745,10 +882,12 @@ jacobian2_kernel(const DevJac m, const DevJacOut o, int mode, int64_t n_states, 
           JGroup g;
           g.ent_off = (uint32_t)gw.x; g.piece_off = (uint32_t)gw.y;
           g.nP2 = (uint8_t)(gw.z & 0xff); g.nM2 = (uint8_t)((gw.z >> 8) & 0xff); g.cls = (uint8_t)((gw.z >> 16) & 0xff); g.kind = (uint8_t)((uint32_t)gw.z >> 24);
+          g.qsteps = (uint32_t)gw.w;
           gather_unit<LS, PosT>(m, o, sm, g, unit % LS, og, conp, b < m.H ? m.blk_r0[b] : 0);
           unit = next;
         }
       }
+      if (fetch_next && warp == 0) write_scalars(sc_other, nT, nE, nPar);
       if (DENSE && b == m.H) {
         // structural zeros, each stored once (no memset pass): slices of 1024 elements, one coalesced mask load each
         for (int z = next_chunk(cnt + 3); z < n_zslices; z = next_chunk(cnt + 3)) {
@@ -765,6 +904,7 @@ jacobian2_kernel(const DevJac m, const DevJacOut o, int mode, int64_t n_states, 
       if (tid == 0 && b < m.H) cnt[1] = 0;
     }
     tl = tl_next;
+    { D2* t_ = sm.sc; sm.sc = sc_other; sc_other = t_; }
   }
   if (tid == 0 && atomicAdd(sched + 1, 1ull) == (unsigned long long)gridDim.x - 1) { sched[0] = 0; sched[1] = 0; }
 }

@@ -18,9 +18,11 @@ template <int LS> int jac2_launch(const DevJac& m, const DevJacOut& o, size_t sm
   const int64_t tiles = (n_states + 2 * LS - 1) / (2 * LS);
   if (tiles == 0) return 0;
   const unsigned blocks = (unsigned)std::min<int64_t>(tiles, (int64_t)n_sm);   // persistent: one CTA per SM
-  if (o.nzmask != nullptr) jac2::jacobian2_kernel<LS, true, uint32_t><<<blocks, J_NT, smem, st>>>(m, o, mode, n_states, tile, phi, param, out, sched);
-  else if (o.pos16) jac2::jacobian2_kernel<LS, false, uint16_t><<<blocks, J_NT, smem, st>>>(m, o, mode, n_states, tile, phi, param, out, sched);
-  else jac2::jacobian2_kernel<LS, false, uint32_t><<<blocks, J_NT, smem, st>>>(m, o, mode, n_states, tile, phi, param, out, sched);
+  int tshift = -1;                                  // log2(tile) if tile is a power of two, else tile == ld
+  if ((tile & (tile - 1)) == 0) { tshift = 0; while (((int64_t)1 << tshift) < tile) ++tshift; }
+  if (o.nzmask != nullptr) jac2::jacobian2_kernel<LS, true, uint32_t><<<blocks, J_NT, smem, st>>>(m, o, mode, n_states, tile, tshift, phi, param, out, sched);
+  else if (o.pos16) jac2::jacobian2_kernel<LS, false, uint16_t><<<blocks, J_NT, smem, st>>>(m, o, mode, n_states, tile, tshift, phi, param, out, sched);
+  else jac2::jacobian2_kernel<LS, false, uint32_t><<<blocks, J_NT, smem, st>>>(m, o, mode, n_states, tile, tshift, phi, param, out, sched);
   return (int)cudaGetLastError();
 }
 

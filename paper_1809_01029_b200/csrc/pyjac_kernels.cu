@@ -242,7 +242,12 @@ struct Tile {
 };
 
 // element offset of (element e, state s) in the library layout; base_s precomputed per thread
-__device__ __forceinline__ int64_t state_base(int64_t s, int64_t tile, int64_t n_e) { return (s / tile) * (n_e * tile) + (s % tile); }
+// tile is a power of two, or tile == ld (then one tile holds every state: s / tile == 0): no 64-bit division
+__device__ __forceinline__ int64_t state_base(int64_t s, int64_t tile, int64_t n_e) {
+  if (tile & (tile - 1)) return s;
+  const int sh = __ffsll((long long)tile) - 1;
+  return (((s >> sh) * n_e) << sh) + (s & (tile - 1));
+}
 
 // phi_of(e): element e of the state vector of THIS thread's lane (tid % S); par_: that lane's parameter.  The
 // analytical kernels read the caller's arrays; the finite-difference kernel adds the perturbation of its column.

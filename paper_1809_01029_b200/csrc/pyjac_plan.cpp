@@ -8,8 +8,6 @@
 #include <algorithm>
 #include <array>
 #include <cstring>
-#include <cstdio>
-#include <cstdlib>
 #include <functional>
 #include <map>
 #include <numeric>
@@ -34,7 +32,7 @@ int len2(size_t n) { return (int)((n + 1) / 2); }
 }  // namespace
 
 size_t jac_smem_bytes(const JacTables& j, int LS) {
-  const size_t pair16 = (size_t)J_NSC + 4 * (size_t)(j.ns + 1) + (size_t)j.max_nrb + (size_t)j.n_val + (size_t)J_NW * J_NRED;
+  const size_t pair16 = 2 * (size_t)J_NSC + 4 * (size_t)(j.ns + 1) + (size_t)j.max_nrb + (size_t)j.n_val + (size_t)J_NW * J_NRED;
   return 16 * (size_t)LS * pair16 + 8 * (size_t)((j.nr + 1) & ~1) + 16 * j.groups.size();
 }
 
@@ -71,14 +69,28 @@ static int build_with_blocks(const HostTables& h, int H, JacTables& j, std::stri
       run += nslots_of(order[q]);
     }
   }
-  // inside a block: the HostTables order (descending cost class, bank-friendly inside a class) is kept
+  // inside a block: the reactions of the general path of phase 1 first (the kernel gives them a lane per STATE and
+  // hands them out first: they are the expensive ones), then the fast-path reactions; inside each part the HostTables
+  // order (descending cost class, bank-friendly inside a class) is kept
+  auto is_fast = [&](int ro) {
+    const int oi = h.info[ro];
+    const int type = oi & INFO_TYPE_MASK, nre = (oi >> INFO_NREAC_SHIFT) & 3, npr = (oi >> INFO_NPROD_SHIFT) & 3;
+    bool hasL = false;
+    for (int a = 0; a < 6; ++a) hasL |= species_of(ro, a) == L;
+    for (int e = h.eff_ptr[ro]; e < h.eff_ptr[ro + 1]; ++e) hasL |= h.eff_sp[e] == L;
+    return (type == PYJAC_ELEMENTARY || type == PYJAC_THIRD_BODY) && (oi & INFO_SIMPLE) && nre <= 2 && npr <= 2 && !(oi & INFO_REVX) && !hasL;
+  };
   std::vector<std::vector<int>> members(H);
-  for (int r = 0; r < nr; ++r) members[blk_of_old[r]].push_back(r);
+  for (int pass = 0; pass < 2; ++pass)
+    for (int r = 0; r < nr; ++r)
+      if ((int)is_fast(r) == pass) members[blk_of_old[r]].push_back(r);
   j.blk_r0.assign(1, 0);
   std::vector<int> new_of_old(nr, 0);
   for (int b = 0; b < H; ++b) {
-    for (int r : members[b]) { new_of_old[r] = (int)j.old_of_new.size(); j.old_of_new.push_back(r); }
+    int ng = 0;
+    for (int r : members[b]) { new_of_old[r] = (int)j.old_of_new.size(); j.old_of_new.push_back(r); ng += is_fast(r) ? 0 : 1; }
     j.blk_r0.push_back((int)j.old_of_new.size());
+    j.blk_ng.push_back(ng);
     j.max_nrb = std::max(j.max_nrb, (int)members[b].size());
   }
   for (int b = 0; b < H; ++b)
@@ -128,8 +140,7 @@ static int build_with_blocks(const HostTables& h, int H, JacTables& j, std::stri
     for (int e = h.eff_ptr[ro]; e < h.eff_ptr[ro + 1]; ++e) hasL |= h.eff_sp[e] == L;
     // fast path of phase 1: elementary or third body, every coefficient 1, at most two species per side, K_c-based
     // reverse rate, the last species not involved in any role
-    const bool fast = (type == PYJAC_ELEMENTARY || type == PYJAC_THIRD_BODY) && (oi & INFO_SIMPLE) && nre <= 2 && npr <= 2 &&
-                      !(oi & INFO_REVX) && !hasL;
+    const bool fast = is_fast(ro);
     uint32_t info = (uint32_t)type | ((oi & INFO_REV) ? JI_REV : 0u) | ((oi & INFO_T2) ? JI_T2 : 0u) | ((oi & INFO_ADEF) ? JI_ADEF : 0u) |
                     ((oi & INFO_CHEM) ? JI_CHEM : 0u) | (fast ? JI_FAST : 0u) | ((uint32_t)(snu + 16) << JI_SNU_SHIFT) |
                     ((uint32_t)nre << JI_NREAC_SHIFT) | ((uint32_t)npr << JI_NPROD_SHIFT) | ((uint32_t)of << JI_OF_SHIFT) |
@@ -283,7 +294,7 @@ static int build_with_blocks(const HostTables& h, int H, JacTables& j, std::stri
       return false;
     });
     std::vector<JGroup> gb;
-    struct Built { JGroup g; std::vector<uint32_t> ent; std::vector<int> members; std::vector<uint8_t> nplus; };
+    struct Built { JGroup g; std::vector<uint32_t> ent; std::vector<int> members; std::vector<uint8_t> nplus; int cost = 0; };
     std::vector<Built> built;
     size_t i0 = 0;
     while (i0 < mine.size()) {
@@ -388,14 +399,27 @@ static int build_with_blocks(const HostTables& h, int H, JacTables& j, std::stri
           for (int p = 0; p < GW; ++p) B.ent[(size_t)s2 * GW + p] = (sched[p][2 * s2] & 0xffffu) | (sched[p][2 * s2 + 1] << 16);
         j.n_padded += (int64_t)n_steps * GW;
       }
+      // pair steps actually needed by every quarter of the group (32 pieces; the pieces are sorted by descending
+      // length): the kernel stops a quarter's lanes there instead of running them to the group's longest piece
+      B.g.qsteps = 0;
+      int work = 0;
+      for (int q = 0; q < 4; ++q) {
+        int mx = 0;
+        for (int p = 32 * q; p < std::min<int>(32 * q + 32, (int)B.members.size()); ++p) {
+          const Piece& pc = pieces[B.members[p]];
+          mx = std::max(mx, own_boundary ? len2(pc.P.size()) + len2(pc.M.size()) : len2(pc.P.size()));
+        }
+        B.g.qsteps |= (uint32_t)mx << (8 * q);
+        work += mx + nM2;
+      }
+      j.n_padded -= first.kind == JK_BLK1 ? 0 : (int64_t)n_steps * GW - 64 * (int64_t)work;    // count what is gathered
       // descending cost: work per piece ~ entries x (loads per entry) + fixed epilogue
       const int wk = first.kind == JK_BLK || first.kind == JK_BLK1 ? 2 : (first.kind == JK_ROW ? 5 : 3);
-      B.g.cost = (uint32_t)((n_steps * wk + 8) * (first.kind == JK_BLK1 ? 2 : 1));
-      if (getenv("PYJAC_PLAN_DEBUG")) { int real = 0; for (int m : B.members) real += (int)(pieces[m].P.size() + pieces[m].M.size()); fprintf(stderr, "blk %d kind %d cls %d nP2 %d nM2 %d members %zu real %d stored %d\n", b, (int)B.g.kind, (int)B.g.cls, nP2, nM2, B.members.size(), real, n_steps * GW); }
+      B.cost = first.kind == JK_BLK1 ? 40 : work * wk + 16;
       built.push_back(std::move(B));
       i0 = i1;
     }
-    std::stable_sort(built.begin(), built.end(), [](const Built& a, const Built& c) { return a.g.cost > c.g.cost; });
+    std::stable_sort(built.begin(), built.end(), [](const Built& a, const Built& c) { return a.cost > c.cost; });
     for (Built& B : built) {
       const int GW = B.g.kind == JK_BLK1 ? J_GW1 : J_GW;
       if (j.ent.size() & 1) j.ent.push_back(0);                   // 8-byte alignment (JK_ROW reads uint2)
