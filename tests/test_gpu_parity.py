@@ -63,7 +63,7 @@ def run_gpu(pj, M, what, mode, fmt, states, ld=None, tile=None):
     return res
 
 
-SRC_CASES = [("four", 64), ("all_types", 300), ("chem", 200), ("revx", 200), ("revx", 200), ("c1", 1024), ("c2", 1500), ("c3", 700), ("c4", 96), ("c5", 96)]
+SRC_CASES = [("four", 64), ("all_types", 300), ("chem", 200), ("revx", 200), ("c1", 1024), ("c2", 1500), ("c3", 700), ("c4", 96), ("c5", 96)]
 
 
 @pytest.mark.parametrize("name,n", SRC_CASES)
@@ -76,7 +76,7 @@ def test_source_terms(pj, name, n, mode):
     assert source_ok(got, ref) <= 1.0
 
 
-JAC_CASES = [("four", 64), ("all_types", 300), ("chem", 200), ("c1", 1024), ("c2", 600), ("c3", 200), ("c4", 24), ("c5", 24)]
+JAC_CASES = [("four", 64), ("all_types", 300), ("chem", 200), ("revx", 200), ("c1", 1024), ("c2", 600), ("c3", 200), ("c4", 24), ("c5", 24)]
 
 
 @pytest.mark.parametrize("name,n", JAC_CASES)

@@ -222,3 +222,54 @@ def test_explicit_reverse_value():
     r = _run(_two(rev_params=rp, **ARR))
     T = 1300.0
     assert r[1]["kr"][0] == pytest.approx(rp[0] * T ** rp[1] * math.exp(-rp[2] / T), rel=1e-14)
+
+
+# ---- the blending functions BY VALUE (PAPER.md L143 / L430): the textbook Troe and SRI
+# formulas are evaluated here in plain Python with the constants written out again (0.75, 1.27, 0.4, 0.67, 0.14) and
+# compared with the oracle's F; c and q follow by closed form.  Non-degenerate parameters: F is far from 1. ----
+def _troe_F(T, Pr, a, T3, T1, T2):
+    Fc = (1.0 - a) * math.exp(-T / T3) + a * math.exp(-T / T1) + (math.exp(-T2 / T) if T2 is not None else 0.0)
+    lc = math.log10(Fc)
+    n = 0.75 - 1.27 * lc
+    cc = -0.4 - 0.67 * lc
+    x = (math.log10(Pr) + cc) / (n - 0.14 * (math.log10(Pr) + cc))
+    return 10.0 ** (lc / (1.0 + x * x))
+
+
+def _sri_F(T, Pr, a, b, c, d, e):
+    X = 1.0 / (1.0 + math.log10(Pr) ** 2)
+    return d * (a * math.exp(-b / T) + math.exp(-T / c)) ** X * T ** e
+
+
+BLEND_CASES = [
+    ("troe", (0.6, 250.0, 1800.0, None), (6e15, -1.0, 20000.0), dict(T=1300.0)),
+    ("troe", (0.35, 90.0, 4200.0, 5200.0), (6e16, -1.2, 19000.0), dict(T=900.0, P=12 * PATM)),
+    ("troe", (0.82, 700.0, 950.0, 2600.0), (2e14, -0.4, 21000.0), dict(T=2100.0, P=0.7 * PATM)),
+    ("sri", (0.9, 350.0, 1200.0, 1.4, 0.0), (6e15, -1.0, 20000.0), dict(T=1300.0)),
+    ("sri", (1.6, 800.0, 600.0, 0.8, 0.15), (6e16, -1.2, 19000.0), dict(T=1700.0, P=25 * PATM)),
+    ("sri", (0.45, 150.0, 3000.0, 1.3, -0.1), (2e14, -0.4, 21000.0), dict(T=850.0, P=0.5 * PATM)),
+]
+
+
+@pytest.mark.parametrize("kind,par,low,st", BLEND_CASES)
+def test_blend_value_against_textbook_formula(kind, par, low, st):
+    if kind == "troe":
+        m = _three(type=mg.FALLOFF_TROE, low=low, troe=par, **ARR)
+    else:
+        m = _three(type=mg.FALLOFF_SRI, low=low, sri=par, **ARR)
+    o, it, f, _ = _run(m, **st)
+    T = st.get("T", 1300.0); P = st.get("P", 3 * PATM)
+    Ctot = P / (R * T)
+    k0 = low[0] * T ** low[1] * math.exp(-low[2] / T)
+    kinf = ARR["A"] * T ** ARR["beta"] * math.exp(-ARR["Ta"] / T)
+    Pr = k0 * Ctot / kinf                                  # default efficiencies: [M] = C_tot
+    assert it["Pr"][0] == pytest.approx(Pr, rel=1e-13)
+    F = _troe_F(T, Pr, *par) if kind == "troe" else _sri_F(T, Pr, *par)
+    assert abs(F - 1.0) > 0.02                             # a non-degenerate case
+    assert it["F"][0] == pytest.approx(F, rel=1e-13)
+    c = F * Pr / (1.0 + Pr)                                # c_i = F P_r / (1 + P_r)
+    assert it["c"][0] == pytest.approx(c, rel=1e-13)
+    CA = 0.3 * Ctot; CB = 0.2 * Ctot; CC = 0.1 * Ctot     # mole fractions of _state
+    q = c * (kinf * CA - it["kr"][0] * CB * CC)            # q = c (k_inf C_A - k_r C_B C_C)
+    assert it["q"][0] == pytest.approx(q, rel=1e-12)
+    assert f[2] == pytest.approx(-0.05 * q, rel=1e-12)     # dn_A/dt = -V q (V = 0.05)
