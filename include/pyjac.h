@@ -131,6 +131,23 @@ int pyjac_jacobian_sparse(const pyjac_mech *mech, int mode, int fmt, int64_t n_s
                           int64_t tile, const double *d_phi, const double *d_param, double *d_vals,
                           void *stream);
 
+/* pyjac_jacobian_sparse for callers that must not reach cudaMalloc'ed scratch or anything that allocates (code under
+ * CUDA graph capture, tight serving loops, harnesses that forbid it): same arguments, same kernel, same results within
+ * the parity tolerance, but the kernel's scratch -- the tile counter and the finished-CTA counter of the persistent
+ * kernel -- lives in a file-scope static __device__ array of the library (256 bytes per GPU, held from the moment the
+ * library is loaded until the process exits) instead of the handle's cudaMalloc'ed ring.  The call enqueues one
+ * 16-byte cudaMemsetAsync (the counters must start at zero and keep the last call's contents) and one kernel on
+ * `stream`; it calls no cudaMalloc, cudaFree, event or allocating routine and takes no lock.
+ * LIMITS: n_states <= PYJAC_STATIC_MAX_STATES per call (PYJAC_EINVAL with a message otherwise: the static entry point
+ * is meant for serving-size batches; larger batches are split by the caller or go through pyjac_jacobian_sparse).
+ * EVERY call on a GPU shares the one scratch array: two calls that overlap on the GPU (different streams, different
+ * handles, different host threads) RACE on the counters and skip or repeat tiles -- issue them on one stream, or order
+ * them with events.  pyjac_jacobian_sparse has no such restriction. */
+#define PYJAC_STATIC_MAX_STATES ((int64_t)1 << 22)
+int pyjac_jacobian_sparse_static(const pyjac_mech *mech, int mode, int fmt, int64_t n_states, int64_t ld,
+                                 int64_t tile, const double *d_phi, const double *d_param, double *d_vals,
+                                 void *stream);
+
 /* Steps a1-a11: all n_var^2 entries per state (structural zeros written as 0.0, each entry stored
  * exactly once; no memset pass).  order 'C': e = r*n_var + c, 'F': e = c*n_var + r. */
 int pyjac_jacobian_dense(const pyjac_mech *mech, int mode, char order, int64_t n_states, int64_t ld,

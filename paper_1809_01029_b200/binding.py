@@ -68,6 +68,7 @@ def lib():
         L.pyjac_sparsity.argtypes = [vp, i32, C.POINTER(_I), C.POINTER(_I)]
         L.pyjac_source_terms.argtypes = [vp, i32, i64, i64, i64, vp, vp, vp, vp]
         L.pyjac_jacobian_sparse.argtypes = [vp, i32, i32, i64, i64, i64, vp, vp, vp, vp]
+        L.pyjac_jacobian_sparse_static.argtypes = [vp, i32, i32, i64, i64, i64, vp, vp, vp, vp]
         L.pyjac_jacobian_dense.argtypes = [vp, i32, C.c_char, i64, i64, i64, vp, vp, vp, vp]
         L.pyjac_jacobian_fd.argtypes = [vp, i32, i32, C.c_double, C.c_double, i64, i64, i64, vp, vp, vp, vp]
         L.pyjac_eval_host.argtypes = [vp, i32, i32, i32, i64, i64, i64, vp, vp, vp]
@@ -136,6 +137,14 @@ def pyjac_source_terms(h, mode, n_states, ld, tile, d_phi, d_param, d_dphi, stre
 
 def pyjac_jacobian_sparse(h, mode, fmt, n_states, ld, tile, d_phi, d_param, d_vals, stream=0):
     _check(lib().pyjac_jacobian_sparse(h, mode, fmt, n_states, ld, tile, d_phi, d_param, d_vals, stream))
+
+
+PYJAC_STATIC_MAX_STATES = 1 << 22
+
+
+def pyjac_jacobian_sparse_static(h, mode, fmt, n_states, ld, tile, d_phi, d_param, d_vals, stream=0):
+    """pyjac_jacobian_sparse with the kernel's scratch in a static device array: allocates nothing (include/pyjac.h)."""
+    _check(lib().pyjac_jacobian_sparse_static(h, mode, fmt, n_states, ld, tile, d_phi, d_param, d_vals, stream))
 
 
 def pyjac_jacobian_dense(h, mode, order, n_states, ld, tile, d_phi, d_param, d_J, stream=0):

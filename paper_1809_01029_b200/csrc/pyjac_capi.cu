@@ -22,6 +22,30 @@ int cuda_fail(cudaError_t e, const char* what) {
   return PYJAC_ECUDA;
 }
 #define CK(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return cuda_fail(e_, #call); } while (0)
+
+// Scratch of pyjac_jacobian_sparse_static (include/pyjac.h): the tile counter and the finished-CTA counter of the persistent
+// Jacobian kernels, in the library's own image instead of cudaMalloc'ed memory.  256 bytes (2 words used, the rest
+// reserved), held by every GPU that loads the library until the process exits.  In HOST code the name g_static_sched is
+// a host-side stand-in, not a device address: the address is taken with cudaGetSymbolAddress once per device, with that
+// device current (static_sched_address), and only that pointer is ever passed to a kernel.
+constexpr int STATIC_SCHED_WORDS = 32;
+static __device__ __align__(256) unsigned long long g_static_sched[STATIC_SCHED_WORDS];
+constexpr int MAX_DEVICES = 64;
+std::mutex g_static_mu;
+unsigned long long* g_static_addr[MAX_DEVICES] = {};
+// device `dev` must be current
+int static_sched_address(int dev, unsigned long long** out) {
+  if (dev < 0 || dev >= MAX_DEVICES) return fail(PYJAC_ECUDA, "static scratch: device index beyond " + std::to_string(MAX_DEVICES - 1));
+  std::lock_guard<std::mutex> lock(g_static_mu);
+  if (!g_static_addr[dev]) {
+    unsigned long long* p = nullptr;
+    CK(cudaGetSymbolAddress((void**)&p, g_static_sched));
+    CK(cudaMemset(p, 0, sizeof(unsigned long long) * STATIC_SCHED_WORDS));
+    g_static_addr[dev] = p;
+  }
+  *out = g_static_addr[dev];
+  return PYJAC_OK;
+}
 }  // namespace
 
 struct pyjac_mech {
@@ -33,6 +57,7 @@ struct pyjac_mech {
   DevPlan plan[4]{};          // tile kernel (jacobian_kernel, pyjac_kernels.cu)
   DevJac dj{};                // pair kernel (jacobian2_kernel, pyjac_jacobian.cuh)
   DevJacOut jout[4]{};
+  unsigned long long* static_sched = nullptr;   // device address of g_static_sched on this handle's device
   bool pair_only = false;     // the tile kernel's intermediates do not fit in shared memory, or PYJAC_PAIR_KERNEL
   std::vector<void*> allocs;
   // tile-scheduler words of the persistent Jacobian kernel: a ring of N_SCHED zeroed pairs (tile counter, finished
@@ -105,6 +130,7 @@ int pyjac_mech_create_ex(const pyjac_mech_desc* desc, int cuda_device, uint32_t 
     if (int ea = set_kernel_attributes()) return cuda_fail((cudaError_t)ea, "cudaFuncSetAttribute");
     if (int ea = set_kernel_attributes_jac()) return cuda_fail((cudaError_t)ea, "cudaFuncSetAttribute");
     CK(cudaDeviceGetAttribute(&m->n_sm, cudaDevAttrMultiProcessorCount, cuda_device));
+    if (int rs_ = static_sched_address(cuda_device, &m->static_sched)) return rs_;
     for (unsigned q = 0; q < pyjac_mech::N_SCHED; ++q) CK(cudaEventCreateWithFlags(&m->sched_ev[q], cudaEventDisableTiming));
     {
       void* p = nullptr;
@@ -272,6 +298,28 @@ int pyjac_jacobian_sparse(const pyjac_mech* mech, int mode, int fmt, int64_t n_s
                           const double* d_phi, const double* d_param, double* d_vals, void* stream) {
   if (fmt != PYJAC_CSR && fmt != PYJAC_CSC) return fail(PYJAC_EINVAL, "pyjac_jacobian_sparse: fmt must be PYJAC_CSR or PYJAC_CSC");
   return run_jac("pyjac_jacobian_sparse", mech, mode, fmt == PYJAC_CSR ? OUT_CSR : OUT_CSC, n_states, ld, tile, d_phi, d_param, d_vals, stream);
+}
+
+int pyjac_jacobian_sparse_static(const pyjac_mech* mech, int mode, int fmt, int64_t n_states, int64_t ld, int64_t tile,
+                                 const double* d_phi, const double* d_param, double* d_vals, void* stream) {
+  const char* fn = "pyjac_jacobian_sparse_static";
+  if (fmt != PYJAC_CSR && fmt != PYJAC_CSC) return fail(PYJAC_EINVAL, std::string(fn) + ": fmt must be PYJAC_CSR or PYJAC_CSC");
+  if (int rc = check_common(fn, mech, mode, n_states, ld, tile, d_phi, d_param, d_vals)) return rc;
+  if (n_states > PYJAC_STATIC_MAX_STATES)
+    return fail(PYJAC_EINVAL, std::string(fn) + ": n_states " + std::to_string(n_states) + " exceeds PYJAC_STATIC_MAX_STATES = " +
+                                  std::to_string((long long)PYJAC_STATIC_MAX_STATES) + " (split the batch, or use pyjac_jacobian_sparse)");
+  if (n_states == 0) return PYJAC_OK;
+  const LaunchCfg cfg = mech->pair_only ? choose_cfg_jac(mech->j, tile, n_states, mech->n_sm) : choose_cfg(mech->h, true, tile, n_states);
+  if (cfg.smem > J_SMEM_LIMIT) return fail(PYJAC_ENOMEM, std::string(fn) + ": mechanism too large for shared memory");
+  const int ofmt = fmt == PYJAC_CSR ? OUT_CSR : OUT_CSC;
+  // every call shares the two words and they keep the last call's contents: they must start at zero (a launch that
+  // faulted or was cancelled leaves them dirty), so they are cleared on the caller's stream in front of the kernel
+  CK(cudaMemsetAsync(mech->static_sched, 0, 2 * sizeof(unsigned long long), (cudaStream_t)stream));
+  const int e = mech->pair_only
+                    ? launch_jacobian2(mech->dj, mech->jout[ofmt], cfg, mech->n_sm, mode, n_states, tile, d_phi, d_param, d_vals, mech->static_sched, stream)
+                    : launch_jacobian(mech->dm, mech->plan[ofmt], cfg, mode, n_states, ld, tile, d_phi, d_param, d_vals, mech->static_sched, stream);
+  if (e) return cuda_fail((cudaError_t)e, "jacobian kernel launch");
+  return PYJAC_OK;
 }
 
 int pyjac_jacobian_dense(const pyjac_mech* mech, int mode, char order, int64_t n_states, int64_t ld, int64_t tile,
