@@ -154,6 +154,22 @@ int pyjac_jacobian_dense(const pyjac_mech *mech, int mode, char order, int64_t n
                          int64_t tile, const double *d_phi, const double *d_param, double *d_J,
                          void *stream);
 
+/* Conversions between the common mass / mole fractions and the state vector ("conversion to/from the
+ * more-common mass/mole fractions and moles is straightforward"; Eq. 1).  d_frac holds ALL Ns fractions per
+ * state in the library layout with n_e = Ns; d_T, d_P, d_V, d_param are plain [ld] arrays.
+ *   from fractions:  X_k = (Y_k / W_k) / sum_j (Y_j / W_j) (mass fractions only);  n_k = X_k P V / (R T), k < Ns;
+ *                    phi = [T, V | P, n_1 .. n_{Ns-1}], param = P | V.  The fractions need not be normalised for
+ *                    kind = MASS (only ratios enter); for kind = MOLE they are used as given.
+ *   from state:      X_k = n_k R T / (P V), k < Ns;  X_Ns = 1 - sum_{k<Ns} X_k (the last species' moles follow from the
+ *                    ideal-gas law);  Y_k = X_k W_k / sum_j X_j W_j.
+ * One elementwise kernel each on `stream`; no allocation, no synchronisation. */
+enum { PYJAC_MOLE_FRACTION = 0, PYJAC_MASS_FRACTION = 1 };
+int pyjac_state_from_fractions(const pyjac_mech *mech, int mode, int kind, int64_t n_states, int64_t ld, int64_t tile,
+                               const double *d_T, const double *d_P, const double *d_V, const double *d_frac,
+                               double *d_phi, double *d_param, void *stream);
+int pyjac_fractions_from_state(const pyjac_mech *mech, int mode, int kind, int64_t n_states, int64_t ld, int64_t tile,
+                               const double *d_phi, const double *d_param, double *d_frac, void *stream);
+
 /* First-order forward finite-difference Jacobian: the paper's own comparison baseline (Fig. 12;
  * "implemented for comparison purposes only").  The paper gives no step rule; R7:
  *     xp_c = fl(phi_c + fma(rel_step, |phi_c|, abs_step)),  h_c = fl(xp_c - phi_c),

@@ -55,6 +55,8 @@ def _load():
         lib.orc_intermediates.argtypes = [C.c_void_p, C.c_int, _D, C.c_double] + [_D] * 17
         lib.orc_fd_jacobian.argtypes = [C.c_void_p, C.c_int, _D, C.c_double, C.c_double, _D, _D]
         lib.orc_cs_jacobian.argtypes = [C.c_void_p, C.c_int, _D, C.c_double, C.c_double, _D, _D]
+        lib.orc_state_from_fractions.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int64, _D, _D, _D, _D, _D, _D]
+        lib.orc_fractions_from_state.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int64, _D, _D, _D]
         lib.orc_fd1_jacobian.argtypes = [C.c_void_p, C.c_int, C.c_int64, _D, _D, C.c_double, C.c_double, _D]
         _lib = lib
     return _lib
@@ -120,6 +122,21 @@ class Oracle:
         v = np.empty((phi.shape[0], self.nnz))
         _lib.orc_jacobian_sparse(self._h, mode, fmt, phi.shape[0], _p(phi), _p(param), _p(v))
         return v
+
+    def state_from_fractions(self, mode, kind, T, P, V, frac):
+        """kind 0: mole fractions, 1: mass fractions; frac [n][ns] -> (phi [n][nvar], param [n])."""
+        T, P, V = (np.ascontiguousarray(a, np.float64).reshape(-1) for a in (T, P, V))
+        frac = np.ascontiguousarray(frac, np.float64).reshape(-1, self.ns)
+        phi = np.empty((T.shape[0], self.nvar)); param = np.empty(T.shape[0])
+        _lib.orc_state_from_fractions(self._h, mode, kind, T.shape[0], _p(T), _p(P), _p(V), _p(frac), _p(phi), _p(param))
+        return phi, param
+
+    def fractions_from_state(self, mode, kind, phi, param):
+        phi = np.ascontiguousarray(phi, np.float64).reshape(-1, self.nvar)
+        param = np.ascontiguousarray(param, np.float64).reshape(-1)
+        frac = np.empty((phi.shape[0], self.ns))
+        _lib.orc_fractions_from_state(self._h, mode, kind, phi.shape[0], _p(phi), _p(param), _p(frac))
+        return frac
 
     def intermediates(self, mode, phi, param):
         phi = np.ascontiguousarray(phi, np.float64).reshape(self.nvar)

@@ -171,20 +171,36 @@ void eval_source(const Mech& m, int mode, const T* phi, const T& param, T* f, In
         const int ty = m.type[i];
         T kf, lam_f, dlnk_dP = T(0.0);
         if (ty == T_PLOG) {
+            // Entries with EQUAL pressures form one pressure LEVEL whose rate constant is the SUM of the entries'
+            // Arrhenius rates (reading R10, the CHEMKIN convention for several P-Log lines per pressure); ln k is
+            // interpolated linearly in ln P between neighbouring levels, constant outside the table (S4).
             const int p0 = m.plog_ptr[i], np_ = m.plog_ptr[i + 1] - p0;
-            auto lnk = [&](int j) { return std::log(m.plogA[p0 + j]) + m.plogb[p0 + j] * lnT - m.plogTa[p0 + j] / Tt; };
-            auto lam = [&](int j) { return (m.plogb[p0 + j] + m.plogTa[p0 + j] / Tt) / Tt; };
+            std::vector<int> first;                                   // first entry of every level, then np_
+            for (int j = 0; j < np_; ++j) if (j == 0 || m.plogP[p0 + j] != m.plogP[p0 + j - 1]) first.push_back(j);
+            const int nl = (int)first.size();
+            first.push_back(np_);
+            auto level = [&](int l, T& lnk, T& lam) {                  // ln k and d ln k / dT of level l
+                auto lnk1 = [&](int j) { return std::log(m.plogA[p0 + j]) + m.plogb[p0 + j] * lnT - m.plogTa[p0 + j] / Tt; };
+                auto lam1 = [&](int j) { return (m.plogb[p0 + j] + m.plogTa[p0 + j] / Tt) / Tt; };
+                if (first[l + 1] - first[l] == 1) { lnk = lnk1(first[l]); lam = lam1(first[l]); return; }
+                T ksum = T(0.0), dsum = T(0.0);
+                for (int j = first[l]; j < first[l + 1]; ++j) { T kj = exp(lnk1(j)); ksum += kj; dsum += kj * lam1(j); }
+                lnk = log(ksum); lam = dsum / ksum;
+            };
+            auto Pl = [&](int l) { return m.plogP[p0 + first[l]]; };
             const double Pre = re(P);
-            if (Pre <= m.plogP[p0]) { kf = exp(lnk(0)); lam_f = lam(0); }
-            else if (Pre >= m.plogP[p0 + np_ - 1]) { kf = exp(lnk(np_ - 1)); lam_f = lam(np_ - 1); }
+            T l0, lam0;
+            if (Pre <= Pl(0)) { level(0, l0, lam0); kf = exp(l0); lam_f = lam0; }
+            else if (Pre >= Pl(nl - 1)) { level(nl - 1, l0, lam0); kf = exp(l0); lam_f = lam0; }
             else {
                 int j = 0;
-                while (j + 2 < np_ && m.plogP[p0 + j + 1] <= Pre) ++j;       // last j with P_j <= P (S4)
-                const double dlnP = std::log(m.plogP[p0 + j + 1]) - std::log(m.plogP[p0 + j]);
-                T wgt = (log(P) - std::log(m.plogP[p0 + j])) / dlnP;
-                T l0 = lnk(j), l1 = lnk(j + 1);
+                while (j + 2 < nl && Pl(j + 1) <= Pre) ++j;            // last level with P_j <= P (S4)
+                const double dlnP = std::log(Pl(j + 1)) - std::log(Pl(j));
+                T wgt = (log(P) - std::log(Pl(j))) / dlnP;
+                T l1, lam1v;
+                level(j, l0, lam0); level(j + 1, l1, lam1v);
                 kf = exp(l0 + (l1 - l0) * wgt);
-                lam_f = (1.0 - wgt) * lam(j) + wgt * lam(j + 1);
+                lam_f = (1.0 - wgt) * lam0 + wgt * lam1v;
                 dlnk_dP = (l1 - l0) / (dlnP * P);
             }
         } else if (ty == T_CHEB) {
@@ -550,6 +566,48 @@ void orc_source(void* hv, int mode, int64_t n, const double* phi, const double* 
         Inter<double> w; w.resize(m.ns, m.nr);
 #pragma omp for schedule(static)
         for (int64_t s = 0; s < n; ++s) eval_source(m, mode, phi + s * nvar, param[s], f + s * nvar, w);
+    }
+}
+
+// ---- conversions between the common mass / mole fractions and the paper's state vector ("conversion
+// to/from the more-common mass/mole fractions and moles is straightforward"; Eq. 1).  Plain definitions:
+//   mole fractions from mass fractions:  X_k = (Y_k / W_k) / sum_j (Y_j / W_j)
+//   moles:                               n_k = X_k n_tot,  n_tot = P V / (R T)   (ideal-gas law), k = 1 .. Ns-1
+//   back:                                X_k = n_k / n_tot (k < Ns), X_Ns = 1 - sum_{k<Ns} X_k  (the last species'
+//                                        moles follow from the ideal-gas law);  Y_k = X_k W_k / sum_j X_j W_j
+// kind 0: mole fractions, 1: mass fractions.  State-major arrays: frac [n][ns], phi [n][nvar], T, P, V, param [n].
+void orc_state_from_fractions(void* hv, int mode, int kind, int64_t n, const double* Tt, const double* P, const double* V,
+                              const double* frac, double* phi, double* param) {
+    Handle* h = (Handle*)hv; const Mech& m = h->m; const int ns = m.ns, nvar = ns + 1;
+    for (int64_t s = 0; s < n; ++s) {
+        std::vector<double> X(frac + s * ns, frac + (s + 1) * ns);
+        if (kind == 1) {
+            double sum = 0.0;
+            for (int k = 0; k < ns; ++k) sum += frac[s * ns + k] / m.W[k];
+            for (int k = 0; k < ns; ++k) X[k] = (frac[s * ns + k] / m.W[k]) / sum;
+        }
+        const double ntot = P[s] * V[s] / (R_GAS * Tt[s]);
+        phi[s * nvar] = Tt[s];
+        phi[s * nvar + 1] = mode == 0 ? V[s] : P[s];
+        param[s] = mode == 0 ? P[s] : V[s];
+        for (int k = 0; k < ns - 1; ++k) phi[s * nvar + 2 + k] = X[k] * ntot;
+    }
+}
+
+void orc_fractions_from_state(void* hv, int mode, int kind, int64_t n, const double* phi, const double* param, double* frac) {
+    Handle* h = (Handle*)hv; const Mech& m = h->m; const int ns = m.ns, nvar = ns + 1;
+    for (int64_t s = 0; s < n; ++s) {
+        const double Tt = phi[s * nvar];
+        const double V = mode == 0 ? phi[s * nvar + 1] : param[s], P = mode == 0 ? param[s] : phi[s * nvar + 1];
+        const double ntot = P * V / (R_GAS * Tt);
+        std::vector<double> X(ns);
+        double sum = 0.0;
+        for (int k = 0; k < ns - 1; ++k) { X[k] = phi[s * nvar + 2 + k] / ntot; sum += X[k]; }
+        X[ns - 1] = 1.0 - sum;
+        if (kind == 0) { for (int k = 0; k < ns; ++k) frac[s * ns + k] = X[k]; continue; }
+        double wbar = 0.0;
+        for (int k = 0; k < ns; ++k) wbar += X[k] * m.W[k];
+        for (int k = 0; k < ns; ++k) frac[s * ns + k] = X[k] * m.W[k] / wbar;
     }
 }
 

@@ -70,6 +70,8 @@ def lib():
         L.pyjac_jacobian_sparse.argtypes = [vp, i32, i32, i64, i64, i64, vp, vp, vp, vp]
         L.pyjac_jacobian_sparse_static.argtypes = [vp, i32, i32, i64, i64, i64, vp, vp, vp, vp]
         L.pyjac_jacobian_dense.argtypes = [vp, i32, C.c_char, i64, i64, i64, vp, vp, vp, vp]
+        L.pyjac_state_from_fractions.argtypes = [vp, i32, i32, i64, i64, i64, vp, vp, vp, vp, vp, vp, vp]
+        L.pyjac_fractions_from_state.argtypes = [vp, i32, i32, i64, i64, i64, vp, vp, vp, vp]
         L.pyjac_jacobian_fd.argtypes = [vp, i32, i32, C.c_double, C.c_double, i64, i64, i64, vp, vp, vp, vp]
         L.pyjac_eval_host.argtypes = [vp, i32, i32, i32, i64, i64, i64, vp, vp, vp]
         L.pyjac_launch_info.argtypes = [vp, i32, _I, _I, C.POINTER(i64)]
@@ -150,6 +152,17 @@ def pyjac_jacobian_sparse_static(h, mode, fmt, n_states, ld, tile, d_phi, d_para
 def pyjac_jacobian_dense(h, mode, order, n_states, ld, tile, d_phi, d_param, d_J, stream=0):
     _check(lib().pyjac_jacobian_dense(h, mode, order.encode() if isinstance(order, str) else order, n_states, ld, tile,
                                       d_phi, d_param, d_J, stream))
+
+
+PYJAC_MOLE_FRACTION, PYJAC_MASS_FRACTION = 0, 1
+
+
+def pyjac_state_from_fractions(h, mode, kind, n_states, ld, tile, d_T, d_P, d_V, d_frac, d_phi, d_param, stream=0):
+    _check(lib().pyjac_state_from_fractions(h, mode, kind, n_states, ld, tile, d_T, d_P, d_V, d_frac, d_phi, d_param, stream))
+
+
+def pyjac_fractions_from_state(h, mode, kind, n_states, ld, tile, d_phi, d_param, d_frac, stream=0):
+    _check(lib().pyjac_fractions_from_state(h, mode, kind, n_states, ld, tile, d_phi, d_param, d_frac, stream))
 
 
 def pyjac_jacobian_fd(h, mode, fmt, rel_step, abs_step, n_states, ld, tile, d_phi, d_param, d_out, stream=0):

@@ -46,6 +46,59 @@ int static_sched_address(int dev, unsigned long long** out) {
   *out = g_static_addr[dev];
   return PYJAC_OK;
 }
+
+// ---- fraction <-> state conversions (Eq. 1; include/pyjac.h) ---------------------------------------
+// One thread per state, the species loop inside: with the state index fastest in memory (tile > 1) every load and store
+// of a warp is a contiguous run.  wr[k] = W_k / W_Ns: only ratios of molecular weights enter.
+__device__ __forceinline__ int64_t conv_base(int64_t s, int64_t tile, int64_t n_e) {
+  if (tile & (tile - 1)) return s;                       // tile == ld: one tile holds every state
+  const int sh = __ffsll((long long)tile) - 1;
+  return (((s >> sh) * n_e) << sh) + (s & (tile - 1));
+}
+__global__ void __launch_bounds__(256) state_from_fractions_kernel(int ns, int mode, int kind, int64_t n, int64_t tile,
+                                                                   const double* __restrict__ wr, const double* __restrict__ T,
+                                                                   const double* __restrict__ P, const double* __restrict__ V,
+                                                                   const double* __restrict__ frac, double* __restrict__ phi,
+                                                                   double* __restrict__ param) {
+  const int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (s >= n) return;
+  const double* __restrict__ f = frac + conv_base(s, tile, ns);
+  double* __restrict__ o = phi + conv_base(s, tile, ns + 1);
+  double scale = P[s] * V[s] / (R_GAS * T[s]);            // n_tot = P V / (R T)
+  if (kind == PYJAC_MASS_FRACTION) {                      // X_k = (Y_k / W_k) / sum_j (Y_j / W_j)
+    double sum = 0.0;
+    for (int k = 0; k < ns; ++k) sum += f[(int64_t)k * tile] / __ldg(wr + k);
+    scale /= sum;
+  }
+  o[0] = T[s];
+  o[tile] = mode == PYJAC_CONP ? V[s] : P[s];
+  param[s] = mode == PYJAC_CONP ? P[s] : V[s];
+  for (int k = 0; k < ns - 1; ++k) {
+    const double x = kind == PYJAC_MASS_FRACTION ? f[(int64_t)k * tile] / __ldg(wr + k) : f[(int64_t)k * tile];
+    o[(int64_t)(2 + k) * tile] = x * scale;
+  }
+}
+__global__ void __launch_bounds__(256) fractions_from_state_kernel(int ns, int mode, int kind, int64_t n, int64_t tile,
+                                                                   const double* __restrict__ wr, const double* __restrict__ phi,
+                                                                   const double* __restrict__ param, double* __restrict__ frac) {
+  const int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (s >= n) return;
+  const double* __restrict__ p = phi + conv_base(s, tile, ns + 1);
+  double* __restrict__ f = frac + conv_base(s, tile, ns);
+  const double T = p[0], E = p[tile], par = param[s];
+  const double V = mode == PYJAC_CONP ? E : par, P = mode == PYJAC_CONP ? par : E;
+  const double inv_ntot = R_GAS * T / (P * V);
+  double sum = 0.0, wbar = 0.0;                           // sum of X_k and of X_k W_k / W_Ns over k < Ns
+  for (int k = 0; k < ns - 1; ++k) { const double x = p[(int64_t)(2 + k) * tile] * inv_ntot; sum += x; wbar += x * __ldg(wr + k); }
+  const double xl = 1.0 - sum;                            // the last species closes the ideal-gas law
+  wbar += xl;                                             // wr[Ns-1] = 1
+  const double iw = kind == PYJAC_MASS_FRACTION ? 1.0 / wbar : 1.0;
+  for (int k = 0; k < ns - 1; ++k) {
+    const double x = p[(int64_t)(2 + k) * tile] * inv_ntot;
+    f[(int64_t)k * tile] = kind == PYJAC_MASS_FRACTION ? x * __ldg(wr + k) * iw : x;
+  }
+  f[(int64_t)(ns - 1) * tile] = xl * iw;
+}
 }  // namespace
 
 struct pyjac_mech {
@@ -145,7 +198,7 @@ int pyjac_mech_create_ex(const pyjac_mech_desc* desc, int cuda_device, uint32_t 
     d.n_part_jac = h.n_part_jac; d.n_part_src = h.n_part_src;
 #define UP(field) if (int r_ = m->upload(h.field, &d.field)) return r_;
     UP(nasa) UP(wr) UP(lnA) UP(beta) UP(Ta) UP(dn) UP(info) UP(aux) UP(sp) UP(eff_ptr) UP(eff_sp) UP(eff_d)
-    UP(slot_base) UP(rev_par) UP(fall) UP(plog_ptr) UP(plog_P) UP(plog_lnP) UP(plog_lnA) UP(plog_b) UP(plog_Ta)
+    UP(slot_base) UP(rev_par) UP(fall) UP(plog_ptr) UP(plog_ent) UP(plog_P) UP(plog_lnP) UP(plog_lnA) UP(plog_b) UP(plog_Ta)
     UP(cheb_meta) UP(cheb_lim) UP(cheb_coef)
 #undef UP
     if (int r_ = m->upload_plan(h.cplan, h.jplan.n_part, &d.cplan)) return r_;      // C partials follow the J partials
@@ -188,7 +241,7 @@ int pyjac_mech_create_ex(const pyjac_mech_desc* desc, int cuda_device, uint32_t 
       UPJ(lnA) UPJ(beta) UPJ(Ta) UPJ(dn) UPJ(info) UPJ(sp) UPJ(ext) UPJ(groups) UPJ(ent) UPJ(pidx) UPJ(item) UPJ(nplus)
 #undef UPJ
       q.nasa = d.nasa; q.eff_sp = d.eff_sp; q.eff_d = d.eff_d; q.rev_par = d.rev_par; q.fall = d.fall;
-      q.plog_ptr = d.plog_ptr; q.plog_P = d.plog_P; q.plog_lnP = d.plog_lnP; q.plog_lnA = d.plog_lnA; q.plog_b = d.plog_b; q.plog_Ta = d.plog_Ta;
+      q.plog_ptr = d.plog_ptr; q.plog_ent = d.plog_ent; q.plog_P = d.plog_P; q.plog_lnP = d.plog_lnP; q.plog_lnA = d.plog_lnA; q.plog_b = d.plog_b; q.plog_Ta = d.plog_Ta;
       q.cheb_meta = d.cheb_meta; q.cheb_lim = d.cheb_lim; q.cheb_coef = d.cheb_coef;
       for (int f = 0; f < 4; ++f) {
         DevJacOut& jo = m->jout[f];
@@ -357,6 +410,42 @@ int pyjac_launch_info(const pyjac_mech* mech, int what, int32_t* states_per_cta,
   if (states_per_cta) *states_per_cta = cfg.S;
   if (threads) *threads = cfg.threads;
   if (smem_bytes) *smem_bytes = (int64_t)cfg.smem;
+  return PYJAC_OK;
+}
+
+static int check_conv(const char* fn, const pyjac_mech* mech, int mode, int kind, int64_t n_states, int64_t ld, int64_t tile) {
+  if (!mech) return fail(PYJAC_EINVAL, std::string(fn) + ": null handle");
+  if (mech->device < 0) return fail(PYJAC_ECUDA, std::string(fn) + ": host-only handle (created with cuda_device = -1) cannot compute");
+  if (mode != PYJAC_CONP && mode != PYJAC_CONV) return fail(PYJAC_EINVAL, std::string(fn) + ": mode must be PYJAC_CONP or PYJAC_CONV");
+  if (kind != PYJAC_MOLE_FRACTION && kind != PYJAC_MASS_FRACTION) return fail(PYJAC_EINVAL, std::string(fn) + ": kind must be PYJAC_MOLE_FRACTION or PYJAC_MASS_FRACTION");
+  if (n_states < 0 || ld < n_states) return fail(PYJAC_EINVAL, std::string(fn) + ": bad n_states / ld");
+  if (tile < 1 || (tile != ld && (tile & (tile - 1)) != 0) || (n_states > 0 && ld % tile != 0))
+    return fail(PYJAC_EINVAL, std::string(fn) + ": tile must be a power of two dividing ld, or equal to ld");
+  return PYJAC_OK;
+}
+
+int pyjac_state_from_fractions(const pyjac_mech* mech, int mode, int kind, int64_t n_states, int64_t ld, int64_t tile,
+                               const double* d_T, const double* d_P, const double* d_V, const double* d_frac, double* d_phi,
+                               double* d_param, void* stream) {
+  const char* fn = "pyjac_state_from_fractions";
+  if (int rc = check_conv(fn, mech, mode, kind, n_states, ld, tile)) return rc;
+  if (n_states == 0) return PYJAC_OK;
+  if (!d_T || !d_P || !d_V || !d_frac || !d_phi || !d_param) return fail(PYJAC_EINVAL, std::string(fn) + ": null buffer");
+  state_from_fractions_kernel<<<(unsigned)((n_states + 255) / 256), 256, 0, (cudaStream_t)stream>>>(
+      mech->h.ns, mode, kind, n_states, tile, mech->dm.wr, d_T, d_P, d_V, d_frac, d_phi, d_param);
+  CK(cudaGetLastError());
+  return PYJAC_OK;
+}
+
+int pyjac_fractions_from_state(const pyjac_mech* mech, int mode, int kind, int64_t n_states, int64_t ld, int64_t tile,
+                               const double* d_phi, const double* d_param, double* d_frac, void* stream) {
+  const char* fn = "pyjac_fractions_from_state";
+  if (int rc = check_conv(fn, mech, mode, kind, n_states, ld, tile)) return rc;
+  if (n_states == 0) return PYJAC_OK;
+  if (!d_phi || !d_param || !d_frac) return fail(PYJAC_EINVAL, std::string(fn) + ": null buffer");
+  fractions_from_state_kernel<<<(unsigned)((n_states + 255) / 256), 256, 0, (cudaStream_t)stream>>>(
+      mech->h.ns, mode, kind, n_states, tile, mech->dm.wr, d_phi, d_param, d_frac);
+  CK(cudaGetLastError());
   return PYJAC_OK;
 }
 

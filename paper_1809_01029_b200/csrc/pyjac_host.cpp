@@ -65,11 +65,13 @@ int validate(const pyjac_mech_desc* d, std::string& err) {
     }
     if (ty == PYJAC_PLOG) {
       const int n = d->plog_ptr[i + 1] - d->plog_ptr[i];
-      if (n < 2) MECH_FAIL("reaction " << i << ": P-Log needs >= 2 pressure points");
+      int levels = 0;
       for (int j = d->plog_ptr[i]; j < d->plog_ptr[i + 1]; ++j) {
         if (!(d->plog_P[j] > 0.0) || !(d->plog_A[j] > 0.0)) MECH_FAIL("reaction " << i << ": P-Log P and A must be > 0");
-        if (j > d->plog_ptr[i] && !(d->plog_P[j] > d->plog_P[j - 1])) MECH_FAIL("reaction " << i << ": P-Log pressures must be strictly ascending");
+        if (j > d->plog_ptr[i] && !(d->plog_P[j] >= d->plog_P[j - 1])) MECH_FAIL("reaction " << i << ": P-Log pressures must be ascending");
+        if (j == d->plog_ptr[i] || d->plog_P[j] != d->plog_P[j - 1]) ++levels;      // equal pressures: one level, rates summed (R10)
       }
+      if (n < 2 || levels < 2) MECH_FAIL("reaction " << i << ": P-Log needs >= 2 distinct pressures");
     }
     if (ty == PYJAC_CHEBYSHEV) {
       if (d->cheb_nT[i] < 1 || d->cheb_nP[i] < 1) MECH_FAIL("reaction " << i << ": empty Chebyshev grid");
@@ -364,12 +366,17 @@ int build_host_tables(const pyjac_mech_desc* d, bool approx, HostTables& h, std:
       if (ty == PYJAC_FALLOFF_SRI) for (int j = 0; j < 5; ++j) f[4 + j] = d->sri[5 * i + j];
       h.fall.insert(h.fall.end(), f, f + 12);
     } else if (ty == PYJAC_PLOG) {
-      if (h.plog_ptr.empty()) h.plog_ptr.push_back(0);
+      // pressure LEVELS: entries of equal pressure form one level whose rate is the sum of theirs (R10)
+      if (h.plog_ptr.empty()) { h.plog_ptr.push_back(0); h.plog_ent.push_back(0); }
       h.aux[r] = (int)h.plog_ptr.size() - 1;
       for (int j = d->plog_ptr[i]; j < d->plog_ptr[i + 1]; ++j) {
-        h.plog_P.push_back(d->plog_P[j]); h.plog_lnP.push_back(std::log(d->plog_P[j]));
+        if (j == d->plog_ptr[i] || d->plog_P[j] != d->plog_P[j - 1]) {
+          if (j > d->plog_ptr[i]) h.plog_ent.push_back((int)h.plog_lnA.size());
+          h.plog_P.push_back(d->plog_P[j]); h.plog_lnP.push_back(std::log(d->plog_P[j]));
+        }
         h.plog_lnA.push_back(std::log(d->plog_A[j])); h.plog_b.push_back(d->plog_beta[j]); h.plog_Ta.push_back(d->plog_Ta[j]);
       }
+      h.plog_ent.push_back((int)h.plog_lnA.size());
       h.plog_ptr.push_back((int)h.plog_P.size());
     } else if (ty == PYJAC_CHEBYSHEV) {
       h.aux[r] = (int)(h.cheb_meta.size() / 4);

@@ -71,8 +71,10 @@ struct HostTables {
   std::vector<int32_t> slot_base;            // [nr+1] Jacobian slots: {T, E, reactant roles, product roles (rev), eff roles}
   std::vector<double> rev_par;               // [nr*3] ln A_r, beta_r, Ta_r of reactions with INFO_REVX (else 0); empty if none
   std::vector<double> fall;                  // [nf*12]: lnA0, beta0, Ta0, pad, then 5 blend parameters
-  std::vector<int32_t> plog_ptr;             // [npl+1]
-  std::vector<double> plog_P, plog_lnP, plog_lnA, plog_b, plog_Ta;
+  std::vector<int32_t> plog_ptr;             // [npl+1] pressure LEVELS of every P-Log reaction
+  std::vector<int32_t> plog_ent;             // [n_levels+1] entries of every level (equal-pressure entries: rates summed, R10)
+  std::vector<double> plog_P, plog_lnP;      // [n_levels]
+  std::vector<double> plog_lnA, plog_b, plog_Ta;   // [n_entries]
   std::vector<int32_t> cheb_meta;            // [nc*4]: nT, nP, coef offset, 0
   std::vector<double> cheb_lim, cheb_coef;   // [nc*4]: 1/Tmin, 1/Tmax, log10 Pmin, log10 Pmax
   // pattern
@@ -183,7 +185,7 @@ struct DevMech {
   const int32_t* slot_base;
   const double* rev_par;
   const double* fall;
-  const int32_t* plog_ptr;
+  const int32_t *plog_ptr, *plog_ent;
   const double *plog_P, *plog_lnP, *plog_lnA, *plog_b, *plog_Ta;
   const int32_t* cheb_meta;
   const double *cheb_lim, *cheb_coef;
@@ -217,7 +219,7 @@ struct DevJac {
   const double* eff_d;
   const double* rev_par;
   const double* fall;
-  const int32_t* plog_ptr;
+  const int32_t *plog_ptr, *plog_ent;
   const double *plog_P, *plog_lnP, *plog_lnA, *plog_b, *plog_Ta;
   const int32_t* cheb_meta;
   const double *cheb_lim, *cheb_coef;

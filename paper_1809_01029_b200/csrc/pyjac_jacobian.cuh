@@ -424,14 +424,28 @@ __device__ __forceinline__ void reaction_general(const DevJac& m, const Smem<LS>
     const bool interp = cnt_le >= 1 && cnt_le < np && !(cnt_le == 1 && Pp <= __ldg(m.plog_P + p0));
     const int j = cnt_le >= np ? np - 1 : (cnt_le >= 1 ? cnt_le - 1 : 0);
     const int j1 = interp ? j + 1 : j;
-    const double b0 = __ldg(m.plog_b + p0 + j), Ta0 = __ldg(m.plog_Ta + p0 + j), lA0 = __ldg(m.plog_lnA + p0 + j), lP0 = __ldg(m.plog_lnP + p0 + j);
-    const double b1 = __ldg(m.plog_b + p0 + j1), Ta1 = __ldg(m.plog_Ta + p0 + j1), lA1 = __ldg(m.plog_lnA + p0 + j1), lP1 = __ldg(m.plog_lnP + p0 + j1);
-    const double l0 = lA0 + b0 * lnT - Ta0 * invT;
-    const double lam0 = (b0 + Ta0 * invT) * invT;
+    // a pressure level is one entry, or several entries of equal pressure whose rates are summed (R10)
+    auto level = [&](int l, double& lnk, double& lam) {
+      const int q0 = __ldg(m.plog_ent + p0 + l), q1 = __ldg(m.plog_ent + p0 + l + 1);
+      const double bq = __ldg(m.plog_b + q0), Taq = __ldg(m.plog_Ta + q0), lAq = __ldg(m.plog_lnA + q0);
+      lnk = lAq + bq * lnT - Taq * invT;
+      lam = (bq + Taq * invT) * invT;
+      if (q1 - q0 > 1) {
+        double ksum = exp_lib(lnk), dsum = ksum * lam;
+        for (int e = q0 + 1; e < q1; ++e) {
+          const double be = __ldg(m.plog_b + e), Tae = __ldg(m.plog_Ta + e);
+          const double ke = exp_lib(__ldg(m.plog_lnA + e) + be * lnT - Tae * invT);
+          ksum += ke; dsum += ke * ((be + Tae * invT) * invT);
+        }
+        lnk = log_lib(ksum); lam = dsum / ksum;
+      }
+    };
+    const double lP0 = __ldg(m.plog_lnP + p0 + j), lP1 = __ldg(m.plog_lnP + p0 + j1);
+    double l0, lam0, l1 = 0.0, lam1 = 0.0;
+    level(j, l0, lam0);
+    if (interp) level(j1, l1, lam1);
     lnkf = l0; lam_f = lam0;
     if (interp) {
-      const double l1 = lA1 + b1 * lnT - Ta1 * invT;
-      const double lam1 = (b1 + Ta1 * invT) * invT;
       const double idl = 1.0 / (lP1 - lP0);
       const double w = (lnP - lP0) * idl;
       lnkf = l0 + (l1 - l0) * w;

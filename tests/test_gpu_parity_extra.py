@@ -224,3 +224,77 @@ def test_held_back_stream_and_ring_wraparound(pj, flags):
         assert np.isfinite(got).all()                         # a skipped tile would leave NaN behind
         # launches differ in the last bits (dynamic chunk order); entries that cancel may differ by more
         assert np.all(np.abs(got - ref) <= 1e-9 * np.abs(ref) + 1e-13 * np.abs(ref).max(axis=1, keepdims=True))
+
+
+# ---- several P-Log entries per pressure (R10): summed rates, both Jacobian kernels and the source kernel ----
+@pytest.mark.parametrize("flags", [0, 2])
+def test_plog_several_entries_per_pressure_on_gpu(pj, flags):
+    from mechgen import MechBuilder
+    from oracle import Oracle
+    PATM = 101325.0
+    cp = lambda a0, a5, a6: [a0, 0, 0, 0, 0, a5, a6]
+    mb = MechBuilder()
+    mb.add_species(30.0, cp(4.0, 1000.0, 5.0)); mb.add_species(10.0, cp(3.0, 9000.0, 4.0))
+    mb.add_species(20.0, cp(3.5, 4000.0, 6.0)); mb.add_species(28.0, cp(3.5, -1000.0, 6.5))
+    pts = [(1.0 * PATM, 1e10, 0.0, 5000.0), (1.0 * PATM, 3e7, 0.9, 2500.0), (10.0 * PATM, 1e12, 0.5, 8000.0),
+           (10.0 * PATM, 5e9, 0.2, 3000.0), (10.0 * PATM, 2e11, -0.3, 6000.0), (50.0 * PATM, 4e12, 0.1, 9000.0)]
+    mb.add_reaction({0: 1}, {1: 1, 2: 1}, 1.0, 0.0, 0.0, rev=True, type=mg.PLOG, plog=pts)
+    mb.add_reaction({1: 1, 2: 1}, {0: 1}, 3e9, 0.4, 1500.0, rev=False)
+    mb.add_reaction({0: 2}, {1: 2, 2: 2}, 1.0, 0.0, 0.0, rev=False, type=mg.PLOG, plog=pts[2:4] + pts[5:])
+    m = mb.build()
+    M = pj.Mechanism(m, 0, flags)
+    o = Oracle(m)
+    states = mg.make_states(4, 24, 91)
+    P = states["P"]
+    P[:8] = np.array([0.3, 1.0, 2.0, 10.0, 30.0, 50.0, 90.0, 9.999999]) * PATM
+    for mode in (mg.CONP, mg.CONV):
+        phi, par = o.pack(states, mode)
+        fr = o.source(mode, phi, par); Jr = o.jacobian_dense(mode, phi, par)
+        assert source_ok(run_gpu(pj, M, pj.WHAT_SOURCE, mode, 0, states), fr) <= 1.0
+        ptr, idx = M.sparsity(mg.CSR)
+        got = run_gpu(pj, M, pj.WHAT_SPARSE, mode, mg.CSR, states, 24, 2)
+        bad = jac_ok_dense(dense_from_sparse(got, ptr, idx, mg.CSR, M.nvar), Jr)
+        assert not bad.any(), np.argwhere(bad)[:8]
+
+
+# ---- fraction <-> state conversion kernels against the oracle, every layout kind ----
+@pytest.mark.parametrize("name,n,ld,tile", [("c1", 1000, 1024, 1024), ("c3", 333, 336, 8), ("c2", 77, 77, 1), ("c5", 200, 200, 200)])
+def test_fraction_conversions(pj, name, n, ld, tile):
+    m, M, o, st = setup(pj, name)
+    states = st(n)
+    ns = M.ns
+
+    def to_dev(a, n_e):          # [n][n_e] -> library layout
+        full = np.zeros((ld, n_e)); full[:n] = a
+        return torch.from_numpy(np.ascontiguousarray(full.reshape(ld // tile, tile, n_e).transpose(0, 2, 1)).reshape(-1)).cuda()
+
+    def vec(a):
+        v = np.ones(ld); v[:n] = a
+        return torch.from_numpy(v).cuda()
+
+    s_ = torch.cuda.current_stream().cuda_stream
+    for mode in (mg.CONP, mg.CONV):
+        phi0, par0 = o.pack(states, mode)
+        for kind in (pj.PYJAC_MOLE_FRACTION, pj.PYJAC_MASS_FRACTION):
+            ref = o.fractions_from_state(mode, kind, phi0, par0)
+            d_phi = to_dev(phi0, M.nvar); d_par = vec(par0)
+            d_f = torch.full((ns * ld,), float("nan"), dtype=torch.float64, device="cuda")
+            pj.pyjac_fractions_from_state(M.h, mode, kind, n, ld, tile, d_phi.data_ptr(), d_par.data_ptr(), d_f.data_ptr(), s_)
+            torch.cuda.synchronize()
+            got = unpack(d_f.cpu().numpy(), ns, n, ld, tile)
+            assert np.all(np.abs(got - ref) <= 1e-12 * np.abs(ref) + 1e-15)      # X_Ns = 1 - sum X_k: absolute floor
+            # and back: state from the fractions
+            pref, parref = o.state_from_fractions(mode, kind, states["T"], states["P"], states["V"], ref)
+            d_T, d_P, d_V = vec(states["T"]), vec(states["P"]), vec(states["V"])
+            d_out = torch.full((M.nvar * ld,), float("nan"), dtype=torch.float64, device="cuda")
+            d_po = torch.full((ld,), float("nan"), dtype=torch.float64, device="cuda")
+            pj.pyjac_state_from_fractions(M.h, mode, kind, n, ld, tile, d_T.data_ptr(), d_P.data_ptr(), d_V.data_ptr(),
+                                          to_dev(ref, ns).data_ptr(), d_out.data_ptr(), d_po.data_ptr(), s_)
+            torch.cuda.synchronize()
+            got = unpack(d_out.cpu().numpy(), M.nvar, n, ld, tile)
+            np.testing.assert_allclose(got, pref, rtol=1e-13, atol=0)
+            assert d_po.cpu().numpy()[:n].tobytes() == parref.tobytes()
+            if ld > n:
+                assert np.isnan(d_po.cpu().numpy()[n:]).all()
+    with pytest.raises(pj.PyjacError):
+        pj.pyjac_fractions_from_state(M.h, 0, 5, n, ld, tile, d_phi.data_ptr(), d_par.data_ptr(), d_f.data_ptr(), s_)

@@ -273,3 +273,39 @@ def test_blend_value_against_textbook_formula(kind, par, low, st):
     q = c * (kinf * CA - it["kr"][0] * CB * CC)            # q = c (k_inf C_A - k_r C_B C_C)
     assert it["q"][0] == pytest.approx(q, rel=1e-12)
     assert f[2] == pytest.approx(-0.05 * q, rel=1e-12)     # dn_A/dt = -V q (V = 0.05)
+
+
+# ---- several P-Log entries per pressure (reading R10: the rates of equal-pressure entries are summed) ----
+def test_plog_several_entries_per_pressure():
+    T = 1300.0
+    arr = lambda A, b, Ta: A * T ** b * math.exp(-Ta / T)
+    e1a, e1b = (1e10, 0.0, 5000.0), (3e7, 0.9, 2500.0)
+    e2a, e2b, e2c = (1e12, 0.5, 8000.0), (5e9, 0.2, 3000.0), (2e11, -0.3, 6000.0)
+    pts = [(1.0 * PATM,) + e1a, (1.0 * PATM,) + e1b, (10.0 * PATM,) + e2a, (10.0 * PATM,) + e2b, (10.0 * PATM,) + e2c]
+    m = _three(type=mg.PLOG, plog=pts)
+    k1 = arr(*e1a) + arr(*e1b); k2 = arr(*e2a) + arr(*e2b) + arr(*e2c)
+    # on the nodes and outside the table: the SUM at that pressure
+    for P, k in ((1.0 * PATM, k1), (0.3 * PATM, k1), (10.0 * PATM, k2), (55.0 * PATM, k2)):
+        _, it, _, _ = _run(m, P=P)
+        assert it["kf"][0] == pytest.approx(k, rel=1e-13)
+    # between the levels: log-log interpolation of the sums
+    _, it, _, _ = _run(m, P=math.sqrt(10.0) * PATM)
+    assert it["kf"][0] == pytest.approx(math.sqrt(k1 * k2), rel=1e-12)
+    w = math.log(2.0) / math.log(10.0)
+    _, it, _, _ = _run(m, P=2.0 * PATM)
+    assert it["kf"][0] == pytest.approx(k1 ** (1 - w) * k2 ** w, rel=1e-12)
+    # two identical entries = one entry with 2A: source terms and Jacobian, inside and outside the table
+    twice = [(p * PATM, A, b, Ta) for (p, A, b, Ta) in ((1.0, 1e10, 0.0, 5000.0), (10.0, 1e12, 0.5, 8000.0)) for _ in range(2)]
+    once = [(1.0 * PATM, 2e10, 0.0, 5000.0), (10.0 * PATM, 2e12, 0.5, 8000.0)]
+    for P in (0.5 * PATM, 1.0 * PATM, 3.0 * PATM, 10.0 * PATM, 40.0 * PATM):
+        a = _run(_three(type=mg.PLOG, plog=twice), P=P); b = _run(_three(type=mg.PLOG, plog=once), P=P)
+        np.testing.assert_allclose(a[2], b[2], rtol=1e-13)
+        np.testing.assert_allclose(a[3], b[3], rtol=1e-11, atol=1e-300)
+    # the analytical Jacobian of the summed form against the complex step of the oracle's own source terms
+    o = Oracle(m)
+    for P in (0.3 * PATM, 2.0 * PATM, 10.0 * PATM, 70.0 * PATM):
+        phi, Pp = _state(P=P)
+        J = o.jacobian_dense(mg.CONP, phi, [Pp])[0]
+        Jc = o.cs_jacobian(mg.CONP, phi, Pp)
+        tol = np.maximum(1e-11 * np.abs(Jc), 1e-15 * np.abs(Jc).max(axis=1, keepdims=True))
+        assert np.all(np.abs(J - Jc) <= tol)
