@@ -182,17 +182,23 @@ int pyjac_fractions_from_state(const pyjac_mech *mech, int mode, int kind, int64
 int pyjac_jacobian_fd(const pyjac_mech *mech, int mode, int fmt, double rel_step, double abs_step, int64_t n_states,
                       int64_t ld, int64_t tile, const double *d_phi, const double *d_param, double *d_out, void *stream);
 
-/* End-to-end convenience calls on HOST buffers (same layouts): allocate device scratch, copy in,
- * run, copy out, synchronise.  what: 0 = source terms, 1 = sparse Jacobian (fmt), 2 = dense Jacobian
- * (fmt = 'C' or 'F').  h_out must hold n_e * ld doubles. */
+/* End-to-end convenience call on HOST buffers (same layouts): copy in, run, copy out, synchronise -- chunks of <= 8192
+ * states double-buffered over two streams, so that with PINNED host buffers the copies overlap the kernels.  The
+ * device staging buffers and the two streams belong to the handle: they are created by the first call (and grown if a
+ * later call needs more) and freed by pyjac_mech_destroy, so repeated calls allocate nothing.  One pyjac_eval_host call
+ * per handle at a time (calls from several threads serialise).  what: 0 = source terms, 1 = sparse Jacobian (fmt),
+ * 2 = dense Jacobian (fmt = 'C' or 'F').  h_out must hold n_e * ld doubles. */
 int pyjac_eval_host(const pyjac_mech *mech, int what, int mode, int fmt, int64_t n_states, int64_t ld,
                     int64_t tile, const double *h_phi, const double *h_param, double *h_out);
 
-/* Launch geometry chosen for a call (for DESIGN/bench reporting): states per CTA, threads per CTA,
- * dynamic shared memory bytes.  what as in pyjac_eval_host; 3 = finite-difference Jacobian (states_per_cta is then
- * the number of perturbed columns one CTA evaluates per pass over its single state). */
-int pyjac_launch_info(const pyjac_mech *mech, int what, int32_t *states_per_cta, int32_t *threads,
-                      int64_t *smem_bytes);
+/* Launch geometry the library chooses for a call with these n_states and tile (the ONE launch policy; bench.py and
+ * the tests ask here): states per CTA, threads per CTA, dynamic shared memory bytes.  what as in pyjac_eval_host;
+ * 3 = finite-difference Jacobian (states_per_cta is then the number of perturbed columns one CTA evaluates per pass
+ * over its single state).  n_states <= 0 means "a large batch", tile <= 0 "any layout".  States per CTA: the largest
+ * power of two whose intermediates fit in shared memory, that does not exceed `tile`, and that still leaves two tiles
+ * per SM of the handle's device. */
+int pyjac_launch_info(const pyjac_mech *mech, int what, int64_t n_states, int64_t tile, int32_t *states_per_cta,
+                      int32_t *threads, int64_t *smem_bytes);
 
 /* Shape of the Jacobian kernel's gather plan, for reporting: info[0] = H (reaction blocks per
  * state pair), [1] = value slots of the largest block, [2] = partial-sum slots, [3] = gather entries, [4] = stored

@@ -74,7 +74,7 @@ def lib():
         L.pyjac_fractions_from_state.argtypes = [vp, i32, i32, i64, i64, i64, vp, vp, vp, vp]
         L.pyjac_jacobian_fd.argtypes = [vp, i32, i32, C.c_double, C.c_double, i64, i64, i64, vp, vp, vp, vp]
         L.pyjac_eval_host.argtypes = [vp, i32, i32, i32, i64, i64, i64, vp, vp, vp]
-        L.pyjac_launch_info.argtypes = [vp, i32, _I, _I, C.POINTER(i64)]
+        L.pyjac_launch_info.argtypes = [vp, i32, i64, i64, _I, _I, C.POINTER(i64)]
         L.pyjac_measure_peak.argtypes = [i32, i32, i32, _D]
         L.pyjac_plan_info.argtypes = [vp, C.POINTER(i64)]
         _lib = L
@@ -181,9 +181,10 @@ def pyjac_eval_host(h, what, mode, fmt, n_states, ld, tile, h_phi, h_param, h_ou
                                  h_out.ctypes.data))
 
 
-def pyjac_launch_info(h, what):
+def pyjac_launch_info(h, what, n_states=0, tile=0):
+    """(states per CTA, threads, shared-memory bytes) the library uses for a call with these n_states and tile."""
     S, nt, sm = C.c_int32(), C.c_int32(), C.c_int64()
-    _check(lib().pyjac_launch_info(h, what, C.byref(S), C.byref(nt), C.byref(sm)))
+    _check(lib().pyjac_launch_info(h, what, int(n_states), int(tile), C.byref(S), C.byref(nt), C.byref(sm)))
     return S.value, nt.value, sm.value
 
 

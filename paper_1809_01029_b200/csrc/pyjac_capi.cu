@@ -110,6 +110,15 @@ struct pyjac_mech {
   DevPlan plan[4]{};          // tile kernel (jacobian_kernel, pyjac_kernels.cu)
   DevJac dj{};                // pair kernel (jacobian2_kernel, pyjac_jacobian.cuh)
   DevJacOut jout[4]{};
+  // pyjac_eval_host: two streams and two sets of staging buffers, created on first use and kept (grown when a call needs
+  // more): the copy-inclusive path allocates nothing in steady state.  One eval_host call per handle at a time.
+  struct HostStage {
+    cudaStream_t st[2] = {nullptr, nullptr};
+    double *phi[2] = {nullptr, nullptr}, *param[2] = {nullptr, nullptr}, *out[2] = {nullptr, nullptr};
+    size_t phi_bytes = 0, param_bytes = 0, out_bytes = 0;
+  };
+  mutable HostStage stage;
+  mutable std::mutex stage_mu;
   unsigned long long* static_sched = nullptr;   // device address of g_static_sched on this handle's device
   bool pair_only = false;     // the tile kernel's intermediates do not fit in shared memory, or PYJAC_PAIR_KERNEL
   std::vector<void*> allocs;
@@ -126,6 +135,10 @@ struct pyjac_mech {
   ~pyjac_mech() {
     for (void* p : allocs) cudaFree(p);
     for (cudaEvent_t e : sched_ev) if (e) cudaEventDestroy(e);
+    for (int b = 0; b < 2; ++b) {
+      if (stage.st[b]) cudaStreamDestroy(stage.st[b]);
+      cudaFree(stage.phi[b]); cudaFree(stage.param[b]); cudaFree(stage.out[b]);
+    }
   }
   int upload_plan(const GatherPlan& g, int part_base, DevGather* out) {
     out->n_sg = g.n_sg; out->n_wide = g.n_wide; out->n_comb = (int)g.comb_item.size(); out->part_base = part_base;
@@ -165,7 +178,7 @@ int pyjac_mech_create_ex(const pyjac_mech_desc* desc, int cuda_device, uint32_t 
   if (rc == PYJAC_OK) rc = build_jac_tables(m->h, m->j, err);
   // the tile kernel keeps ALL per-reaction partials of a state on chip; when they do not fit (or on request) the pair
   // kernel, which cuts the reactions into blocks, evaluates the Jacobian
-  m->pair_only = (flags & PYJAC_PAIR_KERNEL) != 0 || choose_cfg(m->h, true, (int64_t)1 << 40, (int64_t)1 << 40).smem > (size_t)(227 * 1024 - 64);
+  m->pair_only = (flags & PYJAC_PAIR_KERNEL) != 0 || choose_cfg(m->h, true, (int64_t)1 << 40, (int64_t)1 << 40, 148).smem > SMEM_LIMIT;
   if (rc != PYJAC_OK) { delete m; return fail(rc, err); }
   if (cuda_device == -1) { m->device = -1; *out = m; return PYJAC_OK; }   // host-only handle: pattern and dims only
   int ndev = 0;
@@ -312,6 +325,10 @@ static int check_common(const char* fn, const pyjac_mech* mech, int mode, int64_
   if (n_states > 0 && ld % tile != 0) return fail(PYJAC_EINVAL, std::string(fn) + ": ld must be a multiple of tile");
   if (n_states > 0 && (!phi || !param || !out)) return fail(PYJAC_EINVAL, std::string(fn) + ": null buffer");
   if (((uintptr_t)phi | (uintptr_t)param | (uintptr_t)out) & 15) return fail(PYJAC_EINVAL, std::string(fn) + ": buffers must be 16-byte aligned");
+  int cur = -1;
+  if (cudaGetDevice(&cur) != cudaSuccess || cur != mech->device)
+    return fail(PYJAC_EINVAL, std::string(fn) + ": the current CUDA device (" + std::to_string(cur) + ") is not the handle's device (" +
+                                  std::to_string(mech->device) + ")");
   return PYJAC_OK;
 }
 
@@ -319,8 +336,8 @@ int pyjac_source_terms(const pyjac_mech* mech, int mode, int64_t n_states, int64
                        const double* d_param, double* d_dphi, void* stream) {
   if (int rc = check_common("pyjac_source_terms", mech, mode, n_states, ld, tile, d_phi, d_param, d_dphi)) return rc;
   if (n_states == 0) return PYJAC_OK;
-  const LaunchCfg cfg = choose_cfg(mech->h, false, tile, n_states);
-  if (cfg.smem > 227 * 1024) return fail(PYJAC_ENOMEM, "pyjac_source_terms: mechanism too large for shared memory");
+  const LaunchCfg cfg = choose_cfg(mech->h, false, tile, n_states, mech->n_sm);
+  if (cfg.smem > SMEM_LIMIT) return fail(PYJAC_ENOMEM, "pyjac_source_terms: mechanism too large for shared memory");
   int e = launch_source(mech->dm, cfg, mode, n_states, ld, tile, d_phi, d_param, d_dphi, stream);
   if (e) return cuda_fail((cudaError_t)e, "source_kernel launch");
   return PYJAC_OK;
@@ -330,7 +347,7 @@ static int run_jac(const char* fn, const pyjac_mech* mech, int mode, int ofmt, i
                    const double* d_phi, const double* d_param, double* d_out, void* stream) {
   if (int rc = check_common(fn, mech, mode, n_states, ld, tile, d_phi, d_param, d_out)) return rc;
   if (n_states == 0) return PYJAC_OK;
-  const LaunchCfg cfg = mech->pair_only ? choose_cfg_jac(mech->j, tile, n_states, mech->n_sm) : choose_cfg(mech->h, true, tile, n_states);
+  const LaunchCfg cfg = mech->pair_only ? choose_cfg_jac(mech->j, tile, n_states, mech->n_sm) : choose_cfg(mech->h, true, tile, n_states, mech->n_sm);
   if (cfg.smem > J_SMEM_LIMIT) return fail(PYJAC_ENOMEM, std::string(fn) + ": mechanism too large for shared memory");
   std::lock_guard<std::mutex> lock(mech->sched_mu);
   const unsigned slot = mech->sched_next++ % pyjac_mech::N_SCHED;
@@ -362,7 +379,7 @@ int pyjac_jacobian_sparse_static(const pyjac_mech* mech, int mode, int fmt, int6
     return fail(PYJAC_EINVAL, std::string(fn) + ": n_states " + std::to_string(n_states) + " exceeds PYJAC_STATIC_MAX_STATES = " +
                                   std::to_string((long long)PYJAC_STATIC_MAX_STATES) + " (split the batch, or use pyjac_jacobian_sparse)");
   if (n_states == 0) return PYJAC_OK;
-  const LaunchCfg cfg = mech->pair_only ? choose_cfg_jac(mech->j, tile, n_states, mech->n_sm) : choose_cfg(mech->h, true, tile, n_states);
+  const LaunchCfg cfg = mech->pair_only ? choose_cfg_jac(mech->j, tile, n_states, mech->n_sm) : choose_cfg(mech->h, true, tile, n_states, mech->n_sm);
   if (cfg.smem > J_SMEM_LIMIT) return fail(PYJAC_ENOMEM, std::string(fn) + ": mechanism too large for shared memory");
   const int ofmt = fmt == PYJAC_CSR ? OUT_CSR : OUT_CSC;
   // every call shares the two words and they keep the last call's contents: they must start at zero (a launch that
@@ -394,19 +411,23 @@ int pyjac_jacobian_fd(const pyjac_mech* mech, int mode, int fmt, double rel_step
   if (int rc = check_common("pyjac_jacobian_fd", mech, mode, n_states, ld, tile, d_phi, d_param, d_out)) return rc;
   if (n_states == 0) return PYJAC_OK;
   const LaunchCfg cfg = choose_cfg_fd(mech->h);
-  if (cfg.smem > 227 * 1024) return fail(PYJAC_ENOMEM, "pyjac_jacobian_fd: mechanism too large for shared memory");
+  if (cfg.smem > SMEM_LIMIT) return fail(PYJAC_ENOMEM, "pyjac_jacobian_fd: mechanism too large for shared memory");
   const int64_t n_e = ofmt < OUT_DENSE_C ? mech->h.nnz : (int64_t)mech->h.nvar * mech->h.nvar;
   int e = launch_fd(mech->dm, cfg, mode, ofmt, n_e, rel_step, abs_step, n_states, ld, tile, d_phi, d_param, d_out, stream);
   if (e) return cuda_fail((cudaError_t)e, "fd_kernel launch");
   return PYJAC_OK;
 }
 
-int pyjac_launch_info(const pyjac_mech* mech, int what, int32_t* states_per_cta, int32_t* threads, int64_t* smem_bytes) {
+int pyjac_launch_info(const pyjac_mech* mech, int what, int64_t n_states, int64_t tile, int32_t* states_per_cta, int32_t* threads,
+                      int64_t* smem_bytes) {
   if (!mech) return fail(PYJAC_EINVAL, "pyjac_launch_info: null handle");
+  if (what < 0 || what > 3) return fail(PYJAC_EINVAL, "pyjac_launch_info: what must be 0..3");
+  if (n_states <= 0) n_states = (int64_t)1 << 40;          // "a large batch"
+  if (tile <= 0) tile = (int64_t)1 << 40;                  // "any layout"
+  const int n_sm = mech->n_sm > 0 ? mech->n_sm : 148;       // host-only handle: a B200's SM count, for reporting
   const LaunchCfg cfg = what == 3 ? choose_cfg_fd(mech->h)
-                      : (what == 0 ? choose_cfg(mech->h, false, (int64_t)1 << 40, (int64_t)1 << 40)
-                                   : (mech->pair_only ? choose_cfg_jac(mech->j, (int64_t)1 << 40, (int64_t)1 << 40, mech->n_sm > 0 ? mech->n_sm : 148)
-                                                      : choose_cfg(mech->h, true, (int64_t)1 << 40, (int64_t)1 << 40)));
+                      : (what == 0 ? choose_cfg(mech->h, false, tile, n_states, n_sm)
+                                   : (mech->pair_only ? choose_cfg_jac(mech->j, tile, n_states, n_sm) : choose_cfg(mech->h, true, tile, n_states, n_sm)));
   if (states_per_cta) *states_per_cta = cfg.S;
   if (threads) *threads = cfg.threads;
   if (smem_bytes) *smem_bytes = (int64_t)cfg.smem;
@@ -505,16 +526,25 @@ int pyjac_eval_host(const pyjac_mech* mech, int what, int mode, int fmt, int64_t
   const int64_t tile_dev = tile == ld ? chunk : tile;
   int prev = 0;
   cudaGetDevice(&prev);
-  double *d_phi[2] = {nullptr, nullptr}, *d_param[2] = {nullptr, nullptr}, *d_out[2] = {nullptr, nullptr};
-  cudaStream_t st[2] = {nullptr, nullptr};
+  std::lock_guard<std::mutex> stage_lock(mech->stage_mu);
+  pyjac_mech::HostStage& sg = mech->stage;
+  double **d_phi = sg.phi, **d_param = sg.param, **d_out = sg.out;
+  cudaStream_t* st = sg.st;
   auto body = [&]() -> int {
     CK(cudaSetDevice(mech->device));
-    for (int b = 0; b < 2; ++b) {
-      CK(cudaStreamCreateWithFlags(&st[b], cudaStreamNonBlocking));
-      CK(cudaMalloc(&d_phi[b], sizeof(double) * nvar * chunk));
-      CK(cudaMalloc(&d_param[b], sizeof(double) * chunk));
-      CK(cudaMalloc(&d_out[b], sizeof(double) * n_e * chunk));
-    }
+    auto grow = [&](double** buf, size_t& have, size_t need) -> int {
+      if (need <= have) return PYJAC_OK;
+      for (int b = 0; b < 2; ++b) { CK(cudaFree(buf[b])); buf[b] = nullptr; }
+      have = 0;
+      for (int b = 0; b < 2; ++b) CK(cudaMalloc(&buf[b], need));
+      have = need;
+      return PYJAC_OK;
+    };
+    for (int b = 0; b < 2; ++b)
+      if (!st[b]) CK(cudaStreamCreateWithFlags(&st[b], cudaStreamNonBlocking));
+    if (int rg = grow(d_phi, sg.phi_bytes, sizeof(double) * nvar * chunk)) return rg;
+    if (int rg = grow(d_param, sg.param_bytes, sizeof(double) * chunk)) return rg;
+    if (int rg = grow(d_out, sg.out_bytes, sizeof(double) * n_e * chunk)) return rg;
     int b = 0;
     for (int64_t c0 = 0; c0 < n_states; c0 += chunk, b ^= 1) {
       const int64_t n_c = n_states - c0 < chunk ? n_states - c0 : chunk;
@@ -532,10 +562,8 @@ int pyjac_eval_host(const pyjac_mech* mech, int what, int mode, int fmt, int64_t
     return PYJAC_OK;
   };
   int rc = body();
-  for (int b = 0; b < 2; ++b) {
-    if (st[b]) { cudaStreamSynchronize(st[b]); cudaStreamDestroy(st[b]); }
-    cudaFree(d_phi[b]); cudaFree(d_param[b]); cudaFree(d_out[b]);
-  }
+  for (int b = 0; b < 2; ++b)
+    if (st[b]) cudaStreamSynchronize(st[b]);
   cudaSetDevice(prev);
   return rc;
 }

@@ -7,7 +7,6 @@
 #include <array>
 #include <functional>
 #include <cmath>
-#include <cstdlib>
 #include <cstring>
 #include <map>
 #include <numeric>
@@ -28,6 +27,14 @@ int validate(const pyjac_mech_desc* d, std::string& err) {
   if (ns < 2) MECH_FAIL("n_species must be >= 2, got " << ns);
   if (nr < 1) MECH_FAIL("n_reactions must be >= 1, got " << nr);
   if (ns > 32767) MECH_FAIL("n_species > 32767 unsupported");
+  if (!d->mol_weight || !d->nasa_tmid || !d->nasa_lo || !d->nasa_hi || !d->reac_ptr || !d->reac_species || !d->reac_nu || !d->prod_ptr ||
+      !d->prod_species || !d->prod_nu || !d->reversible || !d->type || !d->A || !d->beta || !d->Ta || !d->eff_ptr || !d->collider)
+    MECH_FAIL("a required array of the mechanism description is NULL");
+  for (int i = 0; i < nr; ++i) {
+    if (d->reac_ptr[i + 1] < d->reac_ptr[i] || d->prod_ptr[i + 1] < d->prod_ptr[i] || d->eff_ptr[i + 1] < d->eff_ptr[i])
+      MECH_FAIL("reaction " << i << ": pointer arrays must be non-decreasing");
+    if (d->eff_ptr[i + 1] > d->eff_ptr[i] && (!d->eff_species || !d->eff_value)) MECH_FAIL("efficiency arrays are NULL");
+  }
   for (int k = 0; k < ns; ++k) {
     if (!(d->mol_weight[k] > 0.0)) MECH_FAIL("species " << k << ": molecular weight must be > 0");
     if (!(d->nasa_tmid[k] > 0.0)) MECH_FAIL("species " << k << ": T_mid must be > 0");
@@ -48,6 +55,18 @@ int validate(const pyjac_mech_desc* d, std::string& err) {
           if (sp[l] == sp[j]) MECH_FAIL("reaction " << i << ": species " << sp[j] << " listed twice on one side");
       }
     }
+    {
+      int snu = 0;
+      for (int j = d->reac_ptr[i]; j < d->reac_ptr[i + 1]; ++j) snu -= d->reac_nu[j];
+      for (int j = d->prod_ptr[i]; j < d->prod_ptr[i + 1]; ++j) snu += d->prod_nu[j];
+      if (snu < -7 || snu > 7) MECH_FAIL("reaction " << i << ": |sum of stoichiometric coefficients| = " << (snu < 0 ? -snu : snu) << " exceeds 7");
+    }
+    if (ty >= PYJAC_FALLOFF_LINDEMANN && ty <= PYJAC_FALLOFF_SRI && (!d->low_A || !d->low_beta || !d->low_Ta)) MECH_FAIL("reaction " << i << ": falloff arrays are NULL");
+    if (ty == PYJAC_FALLOFF_TROE && (!d->troe || !d->troe_has_T2)) MECH_FAIL("reaction " << i << ": Troe arrays are NULL");
+    if (ty == PYJAC_FALLOFF_SRI && !d->sri) MECH_FAIL("reaction " << i << ": SRI array is NULL");
+    if (ty == PYJAC_PLOG && (!d->plog_ptr || !d->plog_P || !d->plog_A || !d->plog_beta || !d->plog_Ta)) MECH_FAIL("reaction " << i << ": P-Log arrays are NULL");
+    if (ty == PYJAC_CHEBYSHEV && (!d->cheb_ptr || !d->cheb_nT || !d->cheb_nP || !d->cheb_Tmin || !d->cheb_Tmax || !d->cheb_Pmin || !d->cheb_Pmax || !d->cheb_coef))
+      MECH_FAIL("reaction " << i << ": Chebyshev arrays are NULL");
     if (ty <= PYJAC_FALLOFF_SRI && !(d->A[i] > 0.0)) MECH_FAIL("reaction " << i << ": A must be > 0 (ln A is tabulated)");
     if (d->chem_activated && d->chem_activated[i] && !(ty >= PYJAC_FALLOFF_LINDEMANN && ty <= PYJAC_FALLOFF_SRI))
       MECH_FAIL("reaction " << i << ": chem_activated needs a falloff type");
@@ -89,14 +108,8 @@ int validate(const pyjac_mech_desc* d, std::string& err) {
 // consecutive entries and a thread keeps several independent loads in flight.  A list that fits one segment is
 // stored straight to the output; the segments of a split list leave partial sums in shared memory which a short
 // second pass combines.  stride = ints per entry.
-int seg_len() {
-  const char* e = std::getenv("PYJAC_SEG_LEN");
-  const int v = e ? std::atoi(e) : SEG_LEN_DEFAULT;
-  return v > 0 ? v : SEG_LEN_DEFAULT;
-}
-
 void build_gather(const std::vector<std::vector<int32_t>>& lists, int stride, int zero_slot, int narrow_len, GatherPlan& g) {
-  const int SEG = seg_len();
+  const int SEG = SEG_LEN;
   const int n = (int)lists.size();
   g = GatherPlan();
   g.stride = stride;
@@ -123,6 +136,9 @@ void build_gather(const std::vector<std::vector<int32_t>>& lists, int stride, in
   int i_n = ns_;
   for (int i = 0; i < ns_; ++i) if (eff_len(segs[i]) <= narrow_len) { i_n = i; break; }
   g.n_wide = (i_n + ELL_W - 1) / ELL_W;
+  // plans whose kernels walk wide groups only (narrow_len == 0: T/E rows, source terms) get no narrow groups, however
+  // many empty lists there are (inert species still need their stores)
+  if (narrow_len == 0) g.n_wide = (ns_ + ELL_W - 1) / ELL_W;
   const int rest = std::max(0, ns_ - g.n_wide * ELL_W);
   g.n_sg = g.n_wide + (rest + ELL_W_NARROW - 1) / ELL_W_NARROW;
   auto group_first = [&](int sg) { return sg < g.n_wide ? sg * ELL_W : g.n_wide * ELL_W + (sg - g.n_wide) * ELL_W_NARROW; };

@@ -27,19 +27,13 @@ constexpr int INFO_OF_SHIFT = 16;    // bits 16-19: forward order  sum nu'
 constexpr int INFO_OR_SHIFT = 20;    // bits 20-23: reverse order  sum nu''
 constexpr uint32_t SIGN_BIT = 0x80000000u;
 constexpr int N_ZERO_SLOTS = 16;             // always-zero slots after the real ones: ELL padding, one per 8-byte bank
-constexpr int SEG_LEN_DEFAULT = 24;   // gather lists longer than this are split into segments (env PYJAC_SEG_LEN)
+constexpr int SEG_LEN = 24;           // gather lists longer than this are split into segments
 
 enum OutFmt { OUT_CSR = 0, OUT_CSC = 1, OUT_DENSE_C = 2, OUT_DENSE_F = 3 };
 
 constexpr int ELL_W = 128;           // items per ELL super-group (4 items per lane at one state per CTA)
-#ifndef PYJAC_ELL_W_NARROW
-#define PYJAC_ELL_W_NARROW 512
-#endif
-#ifndef PYJAC_NARROW_LEN
-#define PYJAC_NARROW_LEN 2
-#endif
-constexpr int ELL_W_NARROW = PYJAC_ELL_W_NARROW;   // items per NARROW super-group (segments of <= NARROW_LEN entries; species rows only)
-constexpr int NARROW_LEN = PYJAC_NARROW_LEN;
+constexpr int ELL_W_NARROW = 512;   // items per NARROW super-group (segments of <= NARROW_LEN entries; species rows only)
+constexpr int NARROW_LEN = 2;
 
 struct GatherPlan {
   int stride = 1;                            // ints per entry
@@ -235,7 +229,9 @@ struct DevJacOut {
 struct LaunchCfg { int S, threads; size_t smem; };
 
 // what: 0 source, 1 jacobian.  Chooses states-per-CTA from the shared-memory footprint and `tile`.
-LaunchCfg choose_cfg(const HostTables& h, bool jac, int64_t tile, int64_t n_states);
+constexpr size_t SMEM_LIMIT = 227 * 1024 - 64;   // dynamic shared memory of the tile kernels; 64 B left for static counters
+// n_sm: SMs of the handle's device (states per CTA are reduced until there are two tiles per SM)
+LaunchCfg choose_cfg(const HostTables& h, bool jac, int64_t tile, int64_t n_states, int n_sm);
 
 // kernel launchers (pyjac_kernels.cu); return cudaError_t as int
 int launch_source(const DevMech& m, const LaunchCfg& cfg, int mode, int64_t n_states, int64_t ld, int64_t tile,

@@ -20,47 +20,17 @@
 
 namespace pyjac {
 
-#ifdef PYJAC_TIMING   // debug build only (tuning): per-phase clock64() sums over all CTAs, see _work/
-__device__ unsigned long long g_timing[16];
-#define TICK(i) do { __syncthreads(); if (threadIdx.x == 0) { const long long c_ = clock64(); atomicAdd(&g_timing[i], (unsigned long long)(c_ - tick_)); tick_ = c_; } } while (0)
-#define TICK_INIT long long tick_ = clock64()
-extern "C" int pyjac_debug_timing(unsigned long long* out, int reset) {
-  if (out) cudaMemcpyFromSymbol(out, g_timing, sizeof(g_timing));
-  if (reset) { unsigned long long z[16] = {0}; cudaMemcpyToSymbol(g_timing, z, sizeof(z)); }
-  return 0;
-}
-#else
-#define TICK(i) do { } while (0)
-#define TICK_INIT do { } while (0)
-#endif
-
 namespace {
 
-#ifndef PYJAC_NT
-#define PYJAC_NT 512
-#endif
-#ifndef PYJAC_UJ
-#define PYJAC_UJ 4
-#endif
-#ifndef PYJAC_UC
-#define PYJAC_UC 2
-#endif
-#ifndef PYJAC_UNJ
-#define PYJAC_UNJ 4
-#endif
-#ifndef PYJAC_UNC
-#define PYJAC_UNC 4
-#endif
-#ifndef PYJAC_UN1
-#define PYJAC_UN1 8     // narrow gather at one state per CTA: 8 segments per thread (two units per super-group: finer tail)
-#endif
-#ifndef PYJAC_ZERO_WARPS
-#define PYJAC_ZERO_WARPS 1
-#endif
-#ifndef PYJAC_UQ
-#define PYJAC_UQ 1
-#endif
-constexpr int NT = PYJAC_NT;      // threads per CTA
+// unroll factors / segments per thread of the gathers (measured on C5 / C2 / C3, profiles/r01_sweeps.md)
+#define PYJAC_UJ 4          // species-row gather, wide groups: segments per thread
+#define PYJAC_UC 2          // T/E-row gather: segments per thread
+#define PYJAC_UNJ 4         // entry-loop unroll of the species-row gather
+#define PYJAC_UNC 4         // entry-loop unroll of the T/E-row gather
+#define PYJAC_UN1 8         // narrow gather at one state per CTA: segments per thread
+#define PYJAC_UQ 1          // source-term gather: segments per thread
+constexpr int ZERO_WARPS = 1;   // warps that stream the zero fill of large dense matrices
+constexpr int NT = 512;            // threads per CTA
 constexpr int NW = NT / 32;
 constexpr int NRED = 10;          // reduction slots: 0-6 reaction sums (phase 1), 7-9 species sums (phase 0)
 constexpr int RED0 = 7;
@@ -263,8 +233,7 @@ struct NoMid { __device__ __forceinline__ void operator()() const {} };
 
 template <int S, bool JAC, class PhiF, class SideF, class MidF>
 __device__ __forceinline__ void phases01(const DevMech& m, Tile<S, JAC>& t, int mode, PhiF phi_of, double par_,
-                                         int* cnt, long long& tick_, SideF side, MidF mid) {
-  (void)tick_;
+                                         int* cnt, SideF side, MidF mid) {
   const int tid = threadIdx.x;
   const int ns = m.ns, nr = m.nr, L = ns - 1;
   const int s = tid % S;                        // NT % S == 0: a thread keeps its state in every loop
@@ -360,7 +329,6 @@ __device__ __forceinline__ void phases01(const DevMech& m, Tile<S, JAC>& t, int 
     mid();
     __syncthreads();
   }
-  TICK(0);
   // ---- phase 1: reactions ----------------------------------------------------------------------------
   const double lnP = t.sc[SC_LNP * S + s];
   const double ln_patm_rt = t.sc[SC_LNPRT * S + s];
@@ -615,7 +583,6 @@ __device__ __forceinline__ void phases01(const DevMech& m, Tile<S, JAC>& t, int 
       acc[2] += dEt * slotT; acc[3] += dn * slotT; acc[4] += dEt * slotE; acc[5] += dn * slotE; acc[6] += dct * q;
     }
   }
-  TICK(1);
   // reaction sums: only the per-warp partials are written here; the single barrier below also publishes the slots.
   // Consumers add the NW partials themselves (red_sum), which saves the second reduction stage and its barrier.
   {
@@ -724,12 +691,11 @@ source_kernel(const DevMech m, int mode, int64_t n_states, int64_t tile, const d
   load_meta(m.qplan, t.meta);
   const int64_t s0 = (int64_t)blockIdx.x * S;
   __shared__ int cnt[N_CNT];
-  long long tick_ = 0;
   const int s = threadIdx.x % S;
   const bool valid = s0 + s < n_states;
   const int64_t sg = min(s0 + s, n_states - 1);   // ragged tail: recompute the last valid state, never store
   const int64_t pbase = state_base(sg, tile, m.nvar), obase = pbase;
-  phases01<S, false>(m, t, mode, [&](int e) { return phi[pbase + (int64_t)e * tile]; }, param[sg], cnt, tick_, NoSide(), NoMid());
+  phases01<S, false>(m, t, mode, [&](int e) { return phi[pbase + (int64_t)e * tile]; }, param[sg], cnt, NoSide(), NoMid());
   const double V = t.sc[SC_V * S + s];
   // a7: omega_k = sum_i nu_ki q_i (Eq. 4), dn_k/dt = V omega_k (Eq. 3)
   const double* __restrict__ P = t.P;
@@ -777,7 +743,6 @@ fd_kernel(const DevMech m, int mode, int ofmt, double rel, double ab, int64_t ti
   double* __restrict__ f0 = reinterpret_cast<double*>(t.meta + m.qplan.n_sg);   // f(phi)           [nvar]
   double* __restrict__ fc = f0 + m.nvar;                      // f(phi + h_c e_c) [nvar][S]
   __shared__ int cnt[N_CNT];
-  long long tick_ = 0;
   const int tid = threadIdx.x, s = tid % S, nvar = m.nvar;
   const int64_t sg = blockIdx.x;
   const int64_t pbase = state_base(sg, tile, nvar), obase = state_base(sg, tile, n_e);
@@ -789,7 +754,7 @@ fd_kernel(const DevMech m, int mode, int ofmt, double rel, double ab, int64_t ti
     double x = 0.0, xp = 0.0;
     if (c >= 0) { x = phi[pbase + (int64_t)c * tile]; xp = x + fma(rel, fabs(x), ab); }
     phases01<S, false>(m, t, mode, [&](int e) { const double v = phi[pbase + (int64_t)e * tile]; return e == c ? xp : v; },
-                       par, cnt, tick_, NoSide(), NoMid());
+                       par, cnt, NoSide(), NoMid());
     const double V = t.sc[SC_V * S + s];
     const double* __restrict__ P = t.P;
     gather<S, 1, 1, PYJAC_UQ, 4, ELL_W, int>(m.qplan.ell_ent, t.meta, m.qplan.n_sg, 0, cnt + CNT_Q,
@@ -861,11 +826,6 @@ jacobian_kernel(const DevMech m, const DevPlan pl, int mode, int64_t n_states, i
   load_meta(m.cplan, t.meta);
   load_meta(pl.jplan, t.meta + m.cplan.n_sg);
   __shared__ int cnt[N_CNT];
-#ifdef PYJAC_TIMING
-  long long tick_ = clock64();
-#else
-  long long tick_ = 0;
-#endif
   const int tid = threadIdx.x, s = tid % S;
   const int L = m.ns - 1;
   for (int i = tid; i < 15 * m.ns; i += NT) t.nasa[i] = __ldg(m.nasa + i);
@@ -949,7 +909,7 @@ jacobian_kernel(const DevMech m, const DevPlan pl, int mode, int64_t n_states, i
       }
     }
   };
-  const bool zero_warp = DENSE && n_zslices >= ZERO_WARP_MIN_SLICES && (tid >> 5) >= NW - PYJAC_ZERO_WARPS;
+  const bool zero_warp = DENSE && n_zslices >= ZERO_WARP_MIN_SLICES && (tid >> 5) >= NW - ZERO_WARPS;
   auto side = [&](const int* counter, int n) -> bool {
     if constexpr (!DENSE) {
       return false;
@@ -972,7 +932,7 @@ jacobian_kernel(const DevMech m, const DevPlan pl, int mode, int64_t n_states, i
           if (e == e_mine) return cN_;
           return phi[state_base(sg, tile, m.nvar) + (int64_t)e * tile];     // species loops of more than one trip
         },
-        cPar_, cnt, tick_, side,
+        cPar_, cnt, side,
         [&]() {
           if (tid == 0) next_tile = (long long)gridDim.x + (long long)ticket;
           if (have_prev && nJ2 + nC2 > 0) second_pass();
@@ -987,11 +947,9 @@ jacobian_kernel(const DevMech m, const DevPlan pl, int mode, int64_t n_states, i
     valid = sb < n_states;
     obase = state_base(min(sb, n_states - 1), tile, pl.n_e);
   }
-  TICK(2);
   const double T = t.sc[SC_T * S + s], V = t.sc[SC_V * S + s], Pp = t.sc[SC_P * S + s], D = t.sc[SC_D * S + s];
   const double N = red_sum<S>(t.red, 0, s);
   const double fT = -N / D;
-  TICK(3);
   const double cL = t.ck[L * S + s];
   // a10: the four corner entries from the phase-1 reductions (R4-7), by the last warp (it has no item of
   // the second pass).  With several states per CTA they are done BEFORE the gathers (that warp joins the dynamically
@@ -1060,7 +1018,6 @@ jacobian_kernel(const DevMech m, const DevPlan pl, int mode, int64_t n_states, i
           t.part[pi * S + s] = v[0]; t.part[(pi + 1) * S + s] = v[1];
         }
       }, side);
-  TICK(4);
   // a9: species rows.  Block entries J[k][j] = sum_i nu_ki (Ghat^j_i - Ghat^Ns_i); T and E columns
   // J[k][T] = sum_i nu_ki slotT_i, J[k][E] = sum_i nu_ki slotE_i.  Every nonzero is finished in a register and
   // stored once.
@@ -1087,10 +1044,8 @@ jacobian_kernel(const DevMech m, const DevPlan pl, int mode, int64_t n_states, i
   }
   if (DENSE)                                      // whatever is left of the zero fill
     for (int z = next_chunk(cnt + CNT_Z); z < n_zslices; z = next_chunk(cnt + CNT_Z)) zero_slice(z);
-  TICK(6);
   have_prev = true; prev_valid = valid; prev_obase = obase; prev_fT = fT; prev_iDV = iDV; prev_cS = cS; prev_cT = cT; prev_cL = cL;
   prev_ck = t.ck;
-  TICK(5);
   }  // tiles of this CTA
   if (have_prev && nJ2 + nC2 > 0) {            // the last tile's second pass
     __syncthreads();
@@ -1129,18 +1084,17 @@ template <int S> int launch_fd_S(const DevMech& m, const LaunchCfg& cfg, int mod
   return (int)cudaGetLastError();
 }
 
-constexpr size_t SMEM_LIMIT = 227 * 1024 - 64;   // dynamic part; 64 B left for the static work counters
 
 }  // namespace
 
-LaunchCfg choose_cfg(const HostTables& h, bool jac, int64_t tile, int64_t n_states) {
+LaunchCfg choose_cfg(const HostTables& h, bool jac, int64_t tile, int64_t n_states, int n_sm) {
   LaunchCfg cfg{1, NT, 0};
   for (int S = 32; S >= 1; S >>= 1) {
     const size_t bytes = smem_doubles(h.ns, h.nr, h.nslots, jac ? h.n_part_jac : h.n_part_src, jac ? h.jplan.n_sg + h.cplan.n_sg : h.qplan.n_sg, S, jac) * sizeof(double);
     cfg.S = S; cfg.smem = bytes;
     if (bytes > SMEM_LIMIT) continue;
     if ((int64_t)S > tile) continue;                       // lanes of one item must stay inside one tile
-    if (S > 1 && (n_states + S - 1) / S < 2 * 148) continue;  // small batches: spread over the 148 SMs first
+    if (S > 1 && (n_states + S - 1) / S < 2 * (int64_t)n_sm) continue;  // small batches: spread over the SMs first
     break;
   }
   return cfg;

@@ -99,3 +99,36 @@ def test_mechanism_validation_errors():
 def test_graft_entry_build_imports():
     import __graft_entry__ as g
     assert callable(g.build) and callable(g.smoke)
+
+
+def test_validation_rejects_what_the_tables_cannot_hold():
+    """|sum nu| > 7 does not fit the packed reaction word; NULL required arrays and decreasing pointer arrays."""
+    from mechgen import MechBuilder
+    cp = [3.5, 0, 0, 0, 0, 0.0, 1.0]
+    mb = MechBuilder()
+    for w in (90.0, 10.0, 10.0, 10.0, 28.0):
+        mb.add_species(w, cp)
+    mb.add_reaction({0: 1}, {1: 3, 2: 3, 3: 3}, 1e5, 0.0, 1000.0, rev=False)       # sum nu = +8
+    with pytest.raises(pj.PyjacError) as ei:
+        pj.Mechanism(mb.build(), -1)
+    assert ei.value.code == pj.PYJAC_EMECH and "exceeds 7" in str(ei.value)
+    m = dict(mg.config_mechanism(1))
+    bad = dict(m); p = np.array(m["reac_ptr"]).copy(); p[3] = p[2] - 1; bad["reac_ptr"] = p
+    with pytest.raises(pj.PyjacError) as ei:
+        pj.Mechanism(bad, -1)
+    assert ei.value.code == pj.PYJAC_EMECH
+    d, keep = pj.make_desc(m)
+    d.nasa_lo = None
+    h = ctypes.c_void_p()
+    rc = pj.lib().pyjac_mech_create(ctypes.byref(d), -1, ctypes.byref(h))
+    assert rc == pj.PYJAC_EMECH and b"NULL" in pj.lib().pyjac_last_error()
+
+
+def test_launch_info_is_the_one_launch_policy():
+    M = pj.Mechanism(mg.config_mechanism(2), -1)
+    S_big, nt, smem = pj.pyjac_launch_info(M.h, pj.WHAT_SPARSE)
+    assert S_big == 8 and nt == 512 and 0 < smem <= 227 * 1024
+    assert pj.pyjac_launch_info(M.h, pj.WHAT_SPARSE, 1 << 17, 4)[0] == 4          # never more states than the layout tile
+    assert pj.pyjac_launch_info(M.h, pj.WHAT_SPARSE, 296 * 8, 8)[0] == 8          # two tiles per SM (148 on a host-only handle)
+    assert pj.pyjac_launch_info(M.h, pj.WHAT_SPARSE, 296 * 8 - 8, 8)[0] == 4
+    assert pj.pyjac_launch_info(M.h, pj.WHAT_SPARSE, 100, 1 << 20)[0] == 1

@@ -298,3 +298,31 @@ def test_fraction_conversions(pj, name, n, ld, tile):
                 assert np.isnan(d_po.cpu().numpy()[n:]).all()
     with pytest.raises(pj.PyjacError):
         pj.pyjac_fractions_from_state(M.h, 0, 5, n, ld, tile, d_phi.data_ptr(), d_par.data_ptr(), d_f.data_ptr(), s_)
+
+
+# ---- many inert species: more than 128 empty gather lists in the T/E-row and source-term plans (their
+# outputs -- an explicit 0 for dn_k/dt, the f_T (c_j - c_Ns) term of J[T][j] -- must still be stored) ----
+def test_many_inert_species(pj):
+    from mechgen import MechBuilder
+    from oracle import Oracle
+    rng = np.random.default_rng(5)
+    mb = MechBuilder()
+    ns = 340
+    for k in range(ns):
+        mb.add_species(10.0 + 0.1 * k, [3.0 + 0.002 * k, 1e-4, 0, 0, 0, -500.0 * (k % 7), 4.0])
+    mb.add_reaction({0: 1, 1: 1}, {2: 1, 3: 1}, 4e9, 0.3, 4000.0, rev=True)
+    mb.add_reaction({2: 1}, {0: 1}, 2e7, 0.0, 3000.0, rev=False)
+    mb.add_reaction({3: 1, 4: 1}, {1: 1, 5: 1}, 6e9, -0.2, 2500.0, rev=True, type=mg.THIRD_BODY, eff={7: 2.5, 200: 0.4})
+    m = mb.build()
+    M = pj.Mechanism(m, 0); o = Oracle(m)
+    states = mg.make_states(ns, 40, 17)
+    for mode in (mg.CONP, mg.CONV):
+        phi, par = o.pack(states, mode)
+        fr = o.source(mode, phi, par); Jr = o.jacobian_dense(mode, phi, par)
+        got = run_gpu(pj, M, pj.WHAT_SOURCE, mode, 0, states)
+        assert np.isfinite(got).all() and source_ok(got, fr) <= 1.0
+        assert np.all(got[:, 2 + 10:] == 0.0)                        # inert species: an explicit zero
+        ptr, idx = M.sparsity(mg.CSR)
+        got = run_gpu(pj, M, pj.WHAT_SPARSE, mode, mg.CSR, states, 40, 1)
+        assert np.isfinite(got).all()
+        assert not jac_ok_dense(dense_from_sparse(got, ptr, idx, mg.CSR, M.nvar), Jr).any()
