@@ -6,9 +6,11 @@ Default workload = BASELINE.json configs[4] (C5): synthetic 360-species / 2172-r
 path (steps a1-a11: concentrations, thermo, rate constants, falloff, rates of progress, per-reaction
 partials, species rows, T/E rows, store) over the batch = one pyjac_jacobian_sparse call.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 5] [--impl reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 5] [--impl reference] [--peaks]
 
-Prints ONE JSON line.  `--impl reference` times the CPU oracle (oracle/) on the host cores instead.
+Prints ONE JSON line.  `--impl reference` times the CPU oracle (oracle/) on the host cores instead.  `--gpus N` with
+N > 1 outside torchrun spawns N ranks itself (one process per GPU).  `--peaks` prints the machine peaks measured by the
+library's own microbenchmarks (pyjac_measure_peak: DFMA/s, HBM write / read / copy, L2 read, shared-memory load).
 """
 from __future__ import annotations
 
@@ -40,16 +42,57 @@ def measured_peaks():
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
-def ncu_traffic(config):
-    """dram bytes (read + write) per launch of the timed kernel from the committed ncu summary
-    profiles/r01_traffic.csv (columns: config,n_states,dram_bytes_per_launch), scaled to this run's states."""
-    p = os.path.join(ROOT, "profiles", "r01_traffic.csv")
+TRAFFIC_CSV = os.path.join("profiles", "r02_traffic.csv")
+
+
+def ncu_traffic(config, kernel):
+    """dram bytes (read + write) per launch of the timed kernel from the committed ncu summary profiles/r02_traffic.csv
+    (columns: config,kernel,n_states,dram_bytes_per_launch,capture), scaled to this run's states by the caller.  It is
+    a constant from an earlier `ncu --set full` capture, NOT measured by this run: `traffic_source` says which."""
+    p = os.path.join(ROOT, TRAFFIC_CSV)
     if os.path.exists(p):
         for line in open(p):
             f = line.strip().split(",")
-            if f and f[0] == "c%d" % config:
-                return {"n_states": int(f[1]), "dram_bytes": float(f[2])}
+            if len(f) >= 5 and f[0] == "c%d" % config and f[1] == kernel:
+                return {"n_states": int(f[2]), "dram_bytes": float(f[3]), "source": "%s, ncu --set full capture %s" % (TRAFFIC_CSV, f[4])}
     return None
+
+
+def fp64_model_ops(mech, what):
+    """A-priori DFMA-equivalent count per state from the mechanism alone (SURVEY.md section 8d "Algorithmic FP64 ops";
+    DESIGN.md section 8): not from the kernel's SASS.  exp = 24, log = 28, divide = 10 DFMA slots.
+    what: "source" | "sparse" | "dense" (the Jacobian count includes everything the source terms need)."""
+    EXP, LOG, DIV = 24, 28, 10
+    ns, nr = int(mech["n_species"]), int(mech["n_reactions"])
+    ty = np.asarray(mech["type"]); rev = np.asarray(mech["reversible"]).astype(bool)
+    jac = what != "source"
+    ops = (15 + (4 if jac else 0)) * ns + 2 * LOG
+    n_re = np.diff(mech["reac_ptr"]); n_pr = np.diff(mech["prod_ptr"])
+    n_eff = np.diff(mech["eff_ptr"])
+    for i in range(nr):
+        o = 2 + EXP + 5 + 4                                   # k_f, mass action, omega
+        if rev[i]:
+            o += 5 + EXP
+        t = int(ty[i])
+        if t in (2, 3, 4):
+            o += EXP + 2 * DIV
+        if t == 3:
+            o += 4 * EXP + 2 * LOG + EXP
+        if t == 4:
+            o += 2 * EXP + 2 * LOG + EXP
+        if t == 5:
+            o += 15
+        if t == 6:
+            o += 50
+        if t in (1, 2, 3, 4):
+            o += 2 * int(n_eff[i])
+        if jac:
+            rows = int(len(set(mech["reac_species"][mech["reac_ptr"][i]:mech["reac_ptr"][i + 1]]) |
+                           set(mech["prod_species"][mech["prod_ptr"][i]:mech["prod_ptr"][i + 1]])))
+            cols = int(n_re[i]) + (int(n_pr[i]) if rev[i] else 0) + (int(n_eff[i]) if t in (1, 2, 3, 4) else 0)
+            o += 19 + rows * (cols + 2) + 2 * (cols + 2)
+        ops += o
+    return int(ops)
 
 
 class ClockSampler:
@@ -154,16 +197,7 @@ def workload_config(c, what, tile, S, N=None, mode=None):
         "l2": "inputs+outputs larger than L2 (no flush needed)" if N * 8 * 1000 > 126e6 else "l2_flush_between_steps"}
 
 
-def states_per_cta(S_max, tile, N):
-    """Mirror of the library's launch choice (choose_cfg): largest power of two <= S_max that fits inside a layout
-    tile and still leaves two CTAs per SM."""
-    S = S_max
-    while S > 1 and (S > tile or (N + S - 1) // S < 2 * 148):
-        S //= 2
-    return S
-
-
-def main():
+def parse_args(argv=None):
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=10)
@@ -173,10 +207,62 @@ def main():
     ap.add_argument("--states", type=int, default=None, help="override states per GPU (sweeps)")
     ap.add_argument("--tile", type=int, default=None, help="override layout tile (default: states per CTA)")
     ap.add_argument("--mode", choices=["conp", "conv"], default=None, help="override the config's mode (sweeps)")
+    ap.add_argument("--pair-kernel", action="store_true", help="force the pair-of-states Jacobian kernel (PYJAC_PAIR_KERNEL)")
+    ap.add_argument("--peaks", action="store_true", help="print the machine peaks measured by pyjac_measure_peak and exit")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-fd", action="store_true", help="skip the finite-difference comparison")
-    args = ap.parse_args()
+    return ap.parse_args(argv)
+
+
+PEAK_NAMES = ("dfma_per_s", "hbm_write_Bps", "hbm_read_Bps", "hbm_copy_Bps", "l2_read_Bps", "lds_Bps")
+
+
+def measure_peaks(pj, device, kinds=range(6), reps=5, tries=3):
+    """best of `tries` x (`reps` back-to-back launches, CUDA-event timed inside the library)"""
+    return {PEAK_NAMES[k]: max(pj.pyjac_measure_peak(k, device, reps) for _ in range(tries)) for k in kinds}
+
+
+def run_peaks(args):
+    import torch
+    import paper_1809_01029_b200 as pj
+    assert torch.cuda.is_available(), "bench.py --peaks needs a CUDA device"
+    with ClockSampler(0) as clk:
+        peaks = measure_peaks(pj, 0)
+    sm = torch.cuda.get_device_properties(0).multi_processor_count
+    mhz = clk.summary().get("sm_mhz") or 0.0
+    line = {"peaks": peaks, "n_sm": sm, "clocks": clk.summary(),
+            "dfma_per_clk_per_sm": peaks["dfma_per_s"] / (sm * mhz * 1e6) if mhz else None,
+            "how": "pyjac_measure_peak (csrc/pyjac_peaks.cu): DFMA = 8 independent chains x 2048 threads/SM; HBM = 4 GiB streams, "
+                   "16-byte accesses; L2 = every CTA sweeps one 32 MiB window (ld.global.cg); LDS = conflict-free 16-byte loads; "
+                   "best of 3 x 5 launches, CUDA events"}
+    print(json.dumps(line))
+
+
+def spawn_ranks(n, worker, args, port=None):
+    """`python bench.py --gpus N` outside torchrun: N ranks, one process per GPU (torch.multiprocessing.spawn), the same
+    environment torchrun would give them.  worker(args) runs in every rank and reads RANK / LOCAL_RANK / WORLD_SIZE."""
+    import torch.multiprocessing as mp
+    port = port or 29500 + os.getpid() % 2000
+    mp.spawn(_spawned, nprocs=n, args=(n, port, worker, args), join=True)
+
+
+def _spawned(rank, n, port, worker, args):
+    os.environ.update({"RANK": str(rank), "LOCAL_RANK": str(rank), "WORLD_SIZE": str(n), "MASTER_ADDR": "127.0.0.1",
+                       "MASTER_PORT": str(port)})
+    worker(args)
+
+
+def main(argv=None):
+    args = parse_args(argv)
+    if args.peaks:
+        return run_peaks(args)
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        return spawn_ranks(args.gpus, rank_main, args)
+    return rank_main(args)
+
+
+def rank_main(args):
     rank = int(os.environ.get("RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
     if args.impl == "reference":
@@ -193,11 +279,15 @@ def main():
     cfg = CONFIGS[c]
     mode = cfg["mode"] if args.mode is None else (mg.CONP if args.mode == "conp" else mg.CONV)
     what = "dense" if c in (1, 4) else "sparse"
+    w_id = pj.WHAT_SPARSE if what == "sparse" else pj.WHAT_DENSE
     N = args.states or cfg["n_states"]
     mech = mg.config_mechanism(c)
-    M = pj.Mechanism(mech, local)
-    S, threads, smem = pj.pyjac_launch_info(M.h, pj.WHAT_SPARSE)
-    tile = args.tile or S
+    M = pj.Mechanism(mech, local, pj.PYJAC_PAIR_KERNEL if args.pair_kernel else 0)
+    plan = pj.pyjac_plan_info(M.h)
+    # the library's own launch policy (pyjac_launch_info): states per CTA for this batch; the benchmark layout is
+    # tile = states per CTA of a large batch (a CTA's outputs are then one contiguous range)
+    tile = args.tile or pj.pyjac_launch_info(M.h, w_id, N, 0)[0]
+    S, threads, smem = pj.pyjac_launch_info(M.h, w_id, N, tile)
     ld = (N + tile - 1) // tile * tile
     n_e = M.nnz if what == "sparse" else M.nvar * M.nvar
     # weak scaling: every rank owns its own N states (independent problems, no collective on the data path)
@@ -220,7 +310,8 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
-    for _ in range(max(3, args.warmup)):
+    warm = max(3, args.warmup)
+    for _ in range(warm):
         step()
     barrier()
     evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
@@ -242,34 +333,30 @@ def main():
     total_ms = float(tt.item())
     value = world * N * args.steps / (total_ms * 1e-3)
     kavg_ms = float(np.mean(kern_ms))
-    alg_bytes = (8 * n_e + 8 * (M.ns + 2)) * N            # read phi+param once, write each output once
+    alg_bytes_state = 8 * n_e + 8 * (M.ns + 2)            # read phi+param once, write each output once
     peak, peak_src = measured_peaks()
-    achieved = alg_bytes / (kavg_ms * 1e-3) / 1e9
+    achieved = alg_bytes_state * N / (kavg_ms * 1e-3) / 1e9
+
+    def timed(fn, reps, warm_=2):
+        for _ in range(warm_):
+            fn()
+        torch.cuda.synchronize()
+        a = torch.cuda.Event(enable_timing=True); b = torch.cuda.Event(enable_timing=True)
+        a.record(stream)
+        for _ in range(reps):
+            fn()
+        b.record(stream); torch.cuda.synchronize()
+        return a.elapsed_time(b) / reps
 
     # source terms, timed separately (BASELINE.json configs[4]) in the layout that call prefers: its own states-per-CTA
     # (the source kernel keeps only q_i per reaction on chip, so more states fit a CTA than for the Jacobian)
-    S_src, _, _ = pj.pyjac_launch_info(M.h, pj.WHAT_SOURCE)
-    tile_s = args.tile or S_src
+    tile_s = args.tile or pj.pyjac_launch_info(M.h, pj.WHAT_SOURCE, N, 0)[0]
     ld_s = (N + tile_s - 1) // tile_s * tile_s
-    if tile_s == tile:
-        d_phi_s = d_phi
-    else:
-        d_phi_s = torch.from_numpy(pack_phi(states, mode, ld_s, tile_s)[0]).cuda()
+    d_phi_s = d_phi if tile_s == tile else torch.from_numpy(pack_phi(states, mode, ld_s, tile_s)[0]).cuda()
     d_par_s = torch.zeros(ld_s, dtype=torch.float64, device="cuda"); d_par_s[:N] = d_par[:N]
     d_src = torch.empty(M.nvar * ld_s, dtype=torch.float64, device="cuda")
-
-    def src_step():
-        pj.pyjac_source_terms(M.h, mode, N, ld_s, tile_s, d_phi_s.data_ptr(), d_par_s.data_ptr(), d_src.data_ptr(), stream.cuda_stream)
-
-    for _ in range(3):
-        src_step()
-    torch.cuda.synchronize()
-    a = torch.cuda.Event(enable_timing=True); b = torch.cuda.Event(enable_timing=True)
-    a.record(stream)
-    for _ in range(5):
-        src_step()
-    b.record(stream); torch.cuda.synchronize()
-    src_ms = a.elapsed_time(b) / 5
+    src_ms = timed(lambda: pj.pyjac_source_terms(M.h, mode, N, ld_s, tile_s, d_phi_s.data_ptr(), d_par_s.data_ptr(), d_src.data_ptr(),
+                                                 stream.cuda_stream), 5, 3)
 
     # the paper's comparison (Fig. 12): first-order finite-difference Jacobian in the same output
     # format, same layout, on a bounded sample of the same states (it costs n_var + 1 source evaluations per state)
@@ -277,39 +364,37 @@ def main():
     if not args.no_fd:
         n_fd = min(N, (2048 + tile - 1) // tile * tile)      # one CTA per state: ~14 waves over the 148 SMs
         ffmt = pj.PYJAC_CSR if what == "sparse" else "C"
-
-        def fd_step():
-            pj.pyjac_jacobian_fd(M.h, mode, ffmt, 2.0 ** -26, 1e-14, n_fd, ld, tile, d_phi.data_ptr(), d_par.data_ptr(),
-                                 d_out.data_ptr(), stream.cuda_stream)
-
-        fd_step(); torch.cuda.synchronize()
-        a = torch.cuda.Event(enable_timing=True); b = torch.cuda.Event(enable_timing=True)
-        a.record(stream)
-        for _ in range(3):
-            fd_step()
-        b.record(stream); torch.cuda.synchronize()
-        fd_ms = a.elapsed_time(b) / 3
+        fd_ms = timed(lambda: pj.pyjac_jacobian_fd(M.h, mode, ffmt, 2.0 ** -26, 1e-14, n_fd, ld, tile, d_phi.data_ptr(), d_par.data_ptr(),
+                                                   d_out.data_ptr(), stream.cuda_stream), 3, 1)
         fd = {"states": n_fd, "ns_per_state": 1e6 * fd_ms / n_fd, "states_per_s": n_fd / (fd_ms * 1e-3),
               "columns_per_pass": pj.pyjac_launch_info(M.h, 3)[0], "rel_step": 2.0 ** -26, "abs_step": 1e-14,
               "analytical_speedup": (fd_ms / n_fd) / (kavg_ms / N)}
 
-    # e2e: the C-ABI call on HOST buffers, H2D + kernel + D2H inside the timed region (pinned memory)
+    # machine peaks measured here and now by the library's own microbenchmarks (rank 0 only; after the timed region)
+    here = measure_peaks(pj, local, kinds=(0, 1), reps=3, tries=2) if rank == 0 else None
+
+    # e2e: the C-ABI call on HOST buffers, H2D + kernel + D2H inside the timed region (pinned memory).  The pinned
+    # buffers are capped per rank (28 GiB / world): with more ranks every rank times a prefix of its states.
     e2e = None
     if not args.no_e2e:
-        n2 = N
+        cap = int((28 << 30) / world)
+        n2 = min(N, max(tile, cap // (8 * n_e) // tile * tile))
+        ld2 = (n2 + tile - 1) // tile * tile
+        phi2, par2 = (phi_h, par_h) if n2 == N else pack_phi({k: (v[:n2] if v.ndim == 1 else v[:, :n2]) for k, v in states.items()}, mode, ld2, tile)
+        pinned = True
         try:
-            h_out = torch.empty(n_e * ld, dtype=torch.float64).pin_memory()
+            h_out = torch.empty(n_e * ld2, dtype=torch.float64).pin_memory()
+            h_phi = torch.from_numpy(phi2).pin_memory(); h_par = torch.from_numpy(par2).pin_memory()
         except Exception:
-            n2 = min(N, 1 << 15); h_out = torch.empty(n_e * ld, dtype=torch.float64)
-        h_phi = torch.from_numpy(phi_h).pin_memory(); h_par = torch.from_numpy(par_h).pin_memory()
-        w = pj.WHAT_SPARSE if what == "sparse" else pj.WHAT_DENSE
+            pinned = False
+            h_out = torch.empty(n_e * ld2, dtype=torch.float64); h_phi = torch.from_numpy(phi2); h_par = torch.from_numpy(par2)
         f = pj.PYJAC_CSR if what == "sparse" else "C"
         e_steps = max(1, min(args.steps, 3))
-        pj.pyjac_eval_host(M.h, w, mode, f, n2, ld, tile, h_phi.numpy(), h_par.numpy(), h_out.numpy())
+        pj.pyjac_eval_host(M.h, w_id, mode, f, n2, ld2, tile, h_phi.numpy(), h_par.numpy(), h_out.numpy())     # warm-up: staging buffers
         barrier()
         t_0 = time.perf_counter()
         for _ in range(e_steps):
-            pj.pyjac_eval_host(M.h, w, mode, f, n2, ld, tile, h_phi.numpy(), h_par.numpy(), h_out.numpy())
+            pj.pyjac_eval_host(M.h, w_id, mode, f, n2, ld2, tile, h_phi.numpy(), h_par.numpy(), h_out.numpy())
         torch.cuda.synchronize()
         dt = time.perf_counter() - t_0
         tt = torch.tensor([dt], dtype=torch.float64, device="cuda")
@@ -317,7 +402,8 @@ def main():
             dist.all_reduce(tt, op=dist.ReduceOp.MAX)
         e2e = {"value": world * n2 * e_steps / float(tt.item()), "unit": UNIT,
                "h2d_bytes_per_step": int(8 * (M.nvar + 1) * n2), "d2h_bytes_per_step": int(8 * n_e * n2),
-               "steps": e_steps, "api": "pyjac_eval_host (chunked, double-buffered, pinned host buffers)"}
+               "steps": e_steps, "states_per_gpu": n2, "pinned": pinned,
+               "api": "pyjac_eval_host (chunked, double-buffered, host buffers; staging buffers owned by the handle)"}
         del h_out
 
     if rank == 0:
@@ -326,18 +412,41 @@ def main():
             r, threads_cpu, n_s, dt = oracle_rate(c, mode, what)
             cpu = {"value": r, "unit": UNIT, "cores": threads_cpu, "kind": "oracle",
                    "sample": "%d states of the same workload in %.1f s (oracle/, OpenMP over states)" % (n_s, dt)}
-        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(3, args.warmup),
+        kernel = ("jacobian2_kernel<LS=%d>" % (S // 2)) if args.pair_kernel else ("jacobian_kernel<S=%d,%s>" % (S, "dense" if what == "dense" else "sparse"))
+        ns_state = 1e6 * kavg_ms / N
+        # two bounds (north_star: "the slower of FP64 ops at peak and bytes at peak bandwidth"):
+        #   bytes: algorithmic bytes / the measured HBM peak of MEASURED_PEAKS.json;
+        #   fp64:  a-priori DFMA-equivalent model count / the DFMA rate measured here by pyjac_measure_peak
+        ops_j = fp64_model_ops(mech, what); ops_s = fp64_model_ops(mech, "source")
+        t_hbm = alg_bytes_state / (peak * 1e9) * 1e9
+        t_f64 = ops_j / here["dfma_per_s"] * 1e9
+        bound = "hbm" if t_hbm >= t_f64 else "fp64"
+        traffic = ncu_traffic(c, "pair" if args.pair_kernel else "tile")
+        roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                    "traffic": None if traffic is None else traffic["dram_bytes"] * N / traffic["n_states"],
+                    "traffic_source": None if traffic is None else traffic["source"] + " (a constant scaled to this run's states, not measured by this run)",
+                    "peak_source": peak_src, "kernel": kernel, "algorithmic_bytes_per_state": alg_bytes_state,
+                    "kernel_ms": kavg_ms, "ns_per_state": ns_state,
+                    "binding_bound": bound, "frac_of_binding_bound": max(t_hbm, t_f64) / ns_state,
+                    "hbm": {"bound_ns_per_state": t_hbm, "frac": t_hbm / ns_state,
+                            "frac_of_write_stream_measured_here": alg_bytes_state * N / (kavg_ms * 1e-3) / here["hbm_write_Bps"]},
+                    "fp64": {"model_dfma_per_state": ops_j, "peak_dfma_per_s_measured_here": here["dfma_per_s"],
+                             "bound_ns_per_state": t_f64, "frac": t_f64 / ns_state}}
+        src_ns = 1e6 * src_ms / N
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": warm,
                 "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-                "dtype": "f64", "data": "synthetic", "config": dict(workload_config(c, what, tile, states_per_cta(S, tile, N), N, mode),
-                                                                   l2="l2_flush_between_steps (256 MB written)" if flush is not None
-                                                                   else "inputs+outputs larger than L2 (no flush needed)"),
-                "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                             "traffic": (lambda t: None if t is None else t["dram_bytes"] * N / t["n_states"])(ncu_traffic(c)), "peak_source": peak_src, "kernel": "jacobian_kernel<S=%d>" % states_per_cta(S, tile, N),
-                             "algorithmic_bytes_per_state": 8 * n_e + 8 * (M.ns + 2), "kernel_ms": kavg_ms,
-                             "ns_per_state": 1e6 * kavg_ms / N},
-                "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": args.steps, "clocks": clk.summary(),
+                "dtype": "f64", "data": "synthetic",
+                "config": dict(workload_config(c, what, tile, S, N, mode),
+                               l2="l2_flush_between_steps (256 MB written)" if flush is not None else "inputs+outputs larger than L2 (no flush needed)",
+                               layout="tile = %d: %s" % (tile, "state-major values, one state per tile (not the pure SoA north_star names: pure SoA at this size "
+                                                         "is 2x slower, profiles/r01_sweeps.md)" if tile == 1 else "chunked state-interleaved order (PAPER.md L106)")),
+                "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": args.steps, "clocks": clk.summary(),
                 "extra": {"source_terms_states_per_s": N / (src_ms * 1e-3), "source_terms_ms": src_ms, "source_terms_tile": tile_s,
-                          "nnz": M.nnz, "smem_bytes_per_cta": smem, "threads_per_cta": threads, "fd_jacobian": fd}}
+                          "source_terms_fp64": {"model_dfma_per_state": ops_s, "bound_ns_per_state": ops_s / here["dfma_per_s"] * 1e9,
+                                                "frac": ops_s / here["dfma_per_s"] * 1e9 / src_ns},
+                          "nnz": M.nnz, "smem_bytes_per_cta": smem, "threads_per_cta": threads, "plan": plan,
+                          "peaks_measured_here": {"dfma_per_s": here["dfma_per_s"], "hbm_write_gbs": here["hbm_write_Bps"] / 1e9},
+                          "fd_jacobian": fd}}
         print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()

@@ -63,3 +63,37 @@ def test_two_rank_gloo_sharded_run():
     tmax, total, chk = q.get()
     assert tmax == 11.0 and total == 1001.0
     assert chk == pytest.approx(float(mg.config_states(1, 1001)["T"].sum()), rel=1e-12)
+
+
+def _stub_rank(args):
+    """What bench.rank_main does around its timed region, with the GPU step stubbed: gloo instead of nccl."""
+    import json
+    rank, world = int(os.environ["RANK"]), int(os.environ["WORLD_SIZE"])
+    assert int(os.environ["LOCAL_RANK"]) == rank and os.environ["MASTER_ADDR"] == "127.0.0.1"
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    n_per_rank, steps = 1000, 4
+    off = weak_scaling_offset(n_per_rank, rank)                     # every rank owns its own states (weak scaling)
+    dist.barrier()
+    t = torch.tensor([0.5 + 0.25 * rank], dtype=torch.float64)      # stubbed per-rank elapsed seconds
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    offs = [torch.zeros(1, dtype=torch.int64) for _ in range(world)]
+    dist.all_gather(offs, torch.tensor([off]))
+    if rank == 0:
+        with open(args.out, "w") as f:
+            json.dump({"n_gpus": world, "value": world * n_per_rank * steps / t.item(), "offsets": [int(o) for o in offs]}, f)
+    dist.destroy_process_group()
+
+
+def test_bench_gpus_n_spawns_its_own_ranks(tmp_path):
+    """`python bench.py --gpus N` outside torchrun: bench.spawn_ranks starts N ranks with torchrun's environment."""
+    import json
+    import bench
+    args = bench.parse_args(["--gpus", "2", "--steps", "4"])
+    args.out = str(tmp_path / "line.json")
+    s = socket.socket(); s.bind(("127.0.0.1", 0)); port = s.getsockname()[1]; s.close()
+    bench.spawn_ranks(args.gpus, _stub_rank, args, port=port)
+    line = json.load(open(args.out))
+    assert line["n_gpus"] == 2 and line["offsets"] == [0, 1000]
+    assert line["value"] == pytest.approx(2 * 1000 * 4 / 0.75)
+    # one GPU: no spawn, the rank runs in this process (main() -> rank_main directly)
+    assert bench.parse_args([]).gpus == 1
