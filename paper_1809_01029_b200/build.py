@@ -14,7 +14,7 @@ OBJ = os.path.join(CSRC, "build")
 LIB = os.path.join(HERE, "libpyjac_b200.so")
 SOURCES = ["pyjac_host.cpp", "pyjac_plan.cpp", "pyjac_kernels.cu", "pyjac_jacobian.cu", "pyjac_jacobian_ls1.cu", "pyjac_jacobian_ls2.cu",
            "pyjac_jacobian_ls4.cu", "pyjac_capi.cu", "pyjac_peaks.cu"]
-HEADERS = [os.path.join(CSRC, "pyjac_internal.h"), os.path.join(CSRC, "pyjac_jacobian.cuh"), os.path.join(CSRC, "pyjac_jacobian_launch.cuh"),
+HEADERS = [os.path.join(CSRC, "pyjac_internal.h"), os.path.join(CSRC, "pyjac_jacobian.cuh"), os.path.join(CSRC, "pyjac_jacobian_launch.cuh"), os.path.join(CSRC, "pyjac_math.cuh"),
            os.path.join(ROOT, "include", "pyjac.h")]
 
 

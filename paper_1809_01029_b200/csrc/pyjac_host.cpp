@@ -230,6 +230,21 @@ int build_host_tables(const pyjac_mech_desc* d, bool approx, HostTables& h, std:
   // ---- sort reactions by DESCENDING cost class (type, reversible, non-unit coefficients): warps become
   // type-uniform (the paper's reaction-sorting idea) and the expensive falloff / P-Log / Chebyshev
   // reactions are started first (the kernel hands out 32-reaction chunks dynamically) ---------------------------
+  // fast path of the reaction phase (INFO_FAST): most reactions of a real mechanism
+  auto is_fast = [&](int i) {
+    const int ty = d->type[i];
+    if (ty != PYJAC_ELEMENTARY && ty != PYJAC_THIRD_BODY) return false;
+    if (d->rev_A && d->rev_A[i] > 0.0) return false;
+    const int nre = d->reac_ptr[i + 1] - d->reac_ptr[i], npr = d->prod_ptr[i + 1] - d->prod_ptr[i];
+    if (nre > 2 || npr > 2) return false;
+    for (int j = d->reac_ptr[i]; j < d->reac_ptr[i + 1]; ++j) if (d->reac_nu[j] != 1 || d->reac_species[j] == L) return false;
+    for (int j = d->prod_ptr[i]; j < d->prod_ptr[i + 1]; ++j) if (d->prod_nu[j] != 1 || (d->reversible[i] && d->prod_species[j] == L)) return false;
+    if (ty == PYJAC_THIRD_BODY) {
+      if (d->collider[i] == L) return false;
+      for (int j = d->eff_ptr[i]; j < d->eff_ptr[i + 1]; ++j) if (d->eff_species[j] == L && d->eff_value[j] != 1.0) return false;
+    }
+    return true;
+  };
   h.perm.resize(nr);
   std::iota(h.perm.begin(), h.perm.end(), 0);
   std::stable_sort(h.perm.begin(), h.perm.end(), [&](int a, int b) {
@@ -240,7 +255,7 @@ int build_host_tables(const pyjac_mech_desc* d, bool approx, HostTables& h, std:
     };
     auto cost = [&](int i) {
       static const int rank[7] = {0, 1, 2, 5, 4, 3, 6};   // elementary < third body < Lindemann < P-Log < SRI < Troe < Chebyshev
-      return rank[d->type[i]] * 4 + (d->reversible[i] ? 2 : 0) + (simple(i) ? 0 : 1);
+      return rank[d->type[i]] * 4 + (d->reversible[i] ? 2 : 0) + (simple(i) ? 0 : 1) + (is_fast(i) ? 0 : 64);
     };
     return cost(a) > cost(b);
   });
@@ -256,7 +271,7 @@ int build_host_tables(const pyjac_mech_desc* d, bool approx, HostTables& h, std:
       bool simple = true;
       for (int j = d->reac_ptr[i]; j < d->reac_ptr[i + 1]; ++j) simple &= d->reac_nu[j] == 1;
       for (int j = d->prod_ptr[i]; j < d->prod_ptr[i + 1]; ++j) simple &= d->prod_nu[j] == 1;
-      return rank[d->type[i]] * 4 + (d->reversible[i] ? 2 : 0) + (simple ? 0 : 1);
+      return rank[d->type[i]] * 4 + (d->reversible[i] ? 2 : 0) + (simple ? 0 : 1) + (is_fast(i) ? 0 : 64);
     };
     std::vector<std::array<int, 6>> placed(nr);       // species at each position of the reactions placed so far (ns = dummy)
     auto species_at = [&](int i, const std::array<int, 6>& o, int a) {
@@ -346,6 +361,7 @@ int build_host_tables(const pyjac_mech_desc* d, bool approx, HostTables& h, std:
                (order_f << INFO_OF_SHIFT) | (order_r << INFO_OR_SHIFT);
     if (ty == PYJAC_FALLOFF_TROE && d->troe_has_T2[i]) info |= INFO_T2;
     if (chem) info |= INFO_CHEM;
+    if (is_fast(i)) info |= INFO_FAST;
     if (rev && d->rev_A && d->rev_A[i] > 0.0) {
       info |= INFO_REVX;
       if (h.rev_par.empty()) h.rev_par.assign((size_t)nr * 3, 0.0);

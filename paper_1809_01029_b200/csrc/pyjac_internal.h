@@ -20,6 +20,8 @@ constexpr int INFO_ADEF = 1 << 5;    // default third-body efficiency is 1 (mixt
 constexpr int INFO_SIMPLE = 1 << 6;  // every stoichiometric coefficient is 1 (fast path, no powers)
 constexpr int INFO_CHEM = 1 << 7;    // chemically-activated falloff: Arrhenius columns hold k_0, the falloff record k_inf
 constexpr int INFO_REVX = 1 << 24;   // explicit reverse Arrhenius parameters (rev_par)
+constexpr int INFO_FAST = 1 << 25;   // fast path of the reaction phase: elementary or third body, every coefficient 1, at most two
+                                     // species per side, K_c-based reverse rate, the last species in no role
 constexpr int INFO_SNU_SHIFT = 8;    // bits 8-11: sum(nu) + 8
 constexpr int INFO_NREAC_SHIFT = 12; // bits 12-13: number of reactant entries
 constexpr int INFO_NPROD_SHIFT = 14; // bits 14-15: number of product entries

@@ -17,6 +17,7 @@
 #include <cuda_runtime.h>
 
 #include "pyjac_internal.h"
+#include "pyjac_math.cuh"
 
 namespace pyjac {
 namespace jac2 {
@@ -44,29 +45,6 @@ __device__ __forceinline__ D2 fma2(double x, D2 y, D2 z) { return mk(fma(x, y.a,
 static __device__ __noinline__ double exp_lib(double x) { return exp(x); }
 static __device__ __noinline__ double log_lib(double x) { return log(x); }
 __device__ __forceinline__ D2 exp2_(D2 x) { return mk(exp_lib(x.a), exp_lib(x.b)); }
-// exp(x), |x| < 700 (callers fall back to the library routine otherwise): n = rint(x log2 e), r = x - n ln 2 in two
-// steps, Taylor polynomial of degree 13 (truncation 4e-18) by Estrin's scheme -- a dependency chain of 5 DFMAs instead
-// of Horner's 13, which is what phase 1 waits for with 16 warps per SM -- scaled by 2^n through the exponent field.
-__device__ __forceinline__ double exp_core(double x) {
-  const double t = fma(x, 1.4426950408889634074, 6755399441055744.0);
-  const int n = __double2loint(t);
-  const double nf = t - 6755399441055744.0;
-  double r = fma(nf, -6.93147180559945286227e-01, x);
-  r = fma(nf, -2.31904681384629955842e-17, r);
-  const double r2 = r * r, r4 = r2 * r2, r8 = r4 * r4;
-  const double p01 = 1.0 + r;
-  const double p23 = fma(r, 1.0 / 6.0, 0.5);
-  const double p45 = fma(r, 1.0 / 120.0, 1.0 / 24.0);
-  const double p67 = fma(r, 1.0 / 5040.0, 1.0 / 720.0);
-  const double p89 = fma(r, 1.0 / 362880.0, 1.0 / 40320.0);
-  const double pab = fma(r, 1.0 / 39916800.0, 1.0 / 3628800.0);
-  const double pcd = fma(r, 1.0 / 6227020800.0, 1.0 / 479001600.0);
-  const double q0 = fma(r2, p23, p01), q1 = fma(r2, p67, p45), q2 = fma(r2, pab, p89);
-  const double s0 = fma(r4, q1, q0), s1 = fma(r4, pcd, q2);
-  const double p = fma(r8, s1, s0);
-  return __hiloint2double(__double2hiint(p) + (n << 20), __double2loint(p));
-}
-__device__ __forceinline__ bool exp_in_range(double x) { return fabs(x) < 700.0; }
 __device__ __forceinline__ D2 exp2_fast(D2 x) {
   D2 e = mk(exp_core(x.a), exp_core(x.b));
   if (!(exp_in_range(x.a) && exp_in_range(x.b))) e = exp2_(x);

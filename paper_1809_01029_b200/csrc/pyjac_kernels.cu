@@ -17,6 +17,7 @@
 #include <algorithm>
 
 #include "pyjac_internal.h"
+#include "pyjac_math.cuh"
 
 namespace pyjac {
 
@@ -354,6 +355,74 @@ __device__ __forceinline__ void phases01(const DevMech& m, Tile<S, JAC>& t, int 
                  "r"(w1.x), "r"(w1.y), "r"(rx_base), "r"(e0), "r"(e1), "r"(rx_aux));
     const int type = info & INFO_TYPE_MASK;
     const bool rev = info & INFO_REV;
+    // ---- fast path (INFO_FAST; the reactions are sorted so that whole chunks take it): elementary or third-body
+    // reaction, every coefficient 1, at most two species per side, K_c-based reverse rate, the last species in no role.
+    // One code path without the generic ladder: four species records, both exponentials evaluated together by the
+    // short-chain exp_core, no powers, no P dependence of k_f.
+    if (__all_sync(__activemask(), (info & INFO_FAST) != 0)) {
+      const int k0 = w0.x & 0xffff, k1 = w0.y & 0xffff, k3 = w0.w & 0xffff, k4 = w1.x & 0xffff;   // reactants 0, 1; products 3, 4
+      const double C0 = t.C[k0 * S + s], C1 = t.C[k1 * S + s], C3 = t.C[k3 * S + s], C4 = t.C[k4 * S + s];
+      const double2 g0 = t.gh[k0 * S + s], g1 = t.gh[k1 * S + s], g3 = t.gh[k3 * S + s], g4 = t.gh[k4 * S + s];
+      const double2 e0_ = t.ec[k0 * S + s], e1_ = t.ec[k1 * S + s], e3_ = t.ec[k3 * S + s], e4_ = t.ec[k4 * S + s];
+      const double dg = (g3.x + g4.x) - (g0.x + g1.x), dh = (g3.y + g4.y) - (g0.y + g1.y);
+      const double dEt = (e3_.x + e4_.x) - (e0_.x + e1_.x), dct = (e3_.y + e4_.y) - (e0_.y + e1_.y);
+      const double lnkf = fma(rx_beta, lnT, rx_lnA) - rx_Ta * invT;
+      const double lam_f = fma(rx_Ta, invT, rx_beta) * invT;
+      const double snu = (double)(((info >> INFO_SNU_SHIFT) & 15) - 8);
+      double arg_r = lnkf, lam_r = 0.0;
+      if (rev) { arg_r = lnkf + dg - snu * ln_patm_rt; lam_r = lam_f - (dh - snu) * invT; }   // a4: k_r = k_f / K_c
+      double kf = exp_core(lnkf), kr = exp_core(arg_r);
+      if (!(exp_in_range(lnkf) && exp_in_range(arg_r))) { kf = exp(lnkf); kr = exp(arg_r); }
+      if (!rev) kr = 0.0;
+      const double Rf = kf * (C0 * C1), Rr = kr * (C3 * C4), Rn = Rf - Rr;
+      const double dRdT = lam_f * Rf - lam_r * Rr;
+      const int nre = (info >> INFO_NREAC_SHIFT) & 3, npr = (info >> INFO_NPROD_SHIFT) & 3;
+      double c = 1.0, GT = dRdT, MdcdM_R = 0.0, GL = 0.0;
+      if (type == PYJAC_THIRD_BODY) {                      // a5: c = [M]; dQ/dC_e through [M] = alpha' R_n
+        const double adef = (info & INFO_ADEF) ? 1.0 : 0.0;
+        double M = adef * Ctot;
+        const int sl0 = rx_base + 2 + nre + (rev ? npr : 0);
+        for (int eb = e0; eb < e1; eb += 4) {
+          int esp[4]; double ed[4];
+#pragma unroll
+          for (int q = 0; q < 4; ++q) { esp[q] = eb + q < e1 ? __ldg(m.eff_sp + eb + q) : ns; ed[q] = eb + q < e1 ? __ldg(m.eff_d + eb + q) : 0.0; }
+#pragma unroll
+          for (int q = 0; q < 4; ++q) {
+            M = fma(ed[q], t.C[esp[q] * S + s], M);
+            if (JAC && eb + q < e1) t.P[(sl0 + eb - e0 + q) * S + s] = ed[q] * Rn;
+          }
+        }
+        c = M; GT = M * dRdT; MdcdM_R = M * Rn; GL = adef * Rn;
+      }
+      const double q = c * Rn;
+      acc[0] = fma(dEt, q, acc[0]); acc[1] = fma(rx_dn, q, acc[1]);
+      if (!JAC) {
+        t.P[idx] = q;
+      } else {
+        const double a_ = c * kf, b_ = c * kr;
+        double* __restrict__ Ps = t.P + rx_base * S + s;
+        Ps[2 * S] = a_ * C1;
+        if (nre == 2) Ps[3 * S] = a_ * C0;
+        if (rev) {
+          Ps[(2 + nre) * S] = -(b_ * C4);
+          if (npr == 2) Ps[(3 + nre) * S] = -(b_ * C3);
+        }
+        const double slotT = V * (GT - ctot_T * GL);
+        double slotE;
+        if (mode == PYJAC_CONP) {
+          const double of = (double)((info >> INFO_OF_SHIFT) & 15), orv = (double)((info >> INFO_OR_SHIFT) & 15);
+          slotE = q - c * (of * Rf - orv * Rr) - MdcdM_R + Ctot * GL;
+        } else {
+          slotE = V * (GL / RT);
+        }
+        Ps[0] = slotT;
+        Ps[S] = slotE;
+        t.dE[idx] = dEt;
+        acc[2] = fma(dEt, slotT, acc[2]); acc[3] = fma(rx_dn, slotT, acc[3]); acc[4] = fma(dEt, slotE, acc[4]);
+        acc[5] = fma(rx_dn, slotE, acc[5]); acc[6] = fma(dct, q, acc[6]);
+      }
+      continue;
+    }
     // a3: forward rate constant
     double lnkf, lam_f, dlnk_dP = 0.0;
     if (type <= PYJAC_FALLOFF_SRI) {
