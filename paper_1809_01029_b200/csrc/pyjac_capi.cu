@@ -108,6 +108,10 @@ struct pyjac_mech {
   JacTables j;
   DevMech dm{};
   DevPlan plan[4]{};          // tile kernel (jacobian_kernel, pyjac_kernels.cu)
+  DevPlan xplan[2]{};         // dense 'C' / 'F' by expansion (MODE 2): the sparse CSR / CSC plan + bitmap, ranks, scratch
+  bool has_xplan = false;
+  mutable cudaEvent_t scratch_ev = nullptr;   // launches that share the expansion scratch are ordered behind one another
+  mutable bool scratch_used = false;
   DevJac dj{};                // pair kernel (jacobian2_kernel, pyjac_jacobian.cuh)
   DevJacOut jout[4]{};
   // pyjac_eval_host: two streams and two sets of staging buffers, created on first use and kept (grown when a call needs
@@ -135,6 +139,7 @@ struct pyjac_mech {
   ~pyjac_mech() {
     for (void* p : allocs) cudaFree(p);
     for (cudaEvent_t e : sched_ev) if (e) cudaEventDestroy(e);
+    if (scratch_ev) cudaEventDestroy(scratch_ev);
     for (int b = 0; b < 2; ++b) {
       if (stage.st[b]) cudaStreamDestroy(stage.st[b]);
       cudaFree(stage.phi[b]); cudaFree(stage.param[b]); cudaFree(stage.out[b]);
@@ -239,6 +244,24 @@ int pyjac_mech_create_ex(const pyjac_mech_desc* desc, int cuda_device, uint32_t 
         if (int r_ = m->upload(h.cc_pos[f], &pl.cc_pos)) return r_;
         for (int c = 0; c < 4; ++c) pl.d_pos[c] = h.d_pos[f][c];
         pl.nzmask = f < 2 ? nullptr : mask[f & 1];
+        pl.xpair[0] = pl.xpair[1] = nullptr; pl.scratch = nullptr;
+      }
+      // dense by expansion: mechanisms that leave room for one state per CTA only, with a large dense matrix (C4)
+      const bool one_state = choose_cfg(h, true, (int64_t)1 << 40, (int64_t)1 << 40, m->n_sm).S == 1;
+      if (one_state && (int64_t)h.nvar * h.nvar >= 32768 && h.nnz < (1 << 29)) {
+        void* scr = nullptr;
+        CK(cudaMalloc(&scr, sizeof(double) * 2 * (size_t)m->n_sm * (size_t)h.nnz));   // two buffers (tile parity) per CTA
+        m->allocs.push_back(scr);
+        CK(cudaEventCreateWithFlags(&m->scratch_ev, cudaEventDisableTiming));
+        for (int p = 0; p < 2; ++p) {
+          DevPlan& x = m->xplan[p];
+          x = m->plan[p];                          // positions of the CSR ('C') / CSC ('F') value order
+          x.nzmask = mask[p];
+          for (int sh = 0; sh < 2; ++sh)
+            if (int r_ = m->upload(h.xpair[2 * p + sh], &x.xpair[sh])) return r_;
+          x.scratch = (double*)scr;
+        }
+        m->has_xplan = true;
       }
     }
     // the pair kernel's own tables (block order) and plan
@@ -355,10 +378,16 @@ static int run_jac(const char* fn, const pyjac_mech* mech, int mode, int ofmt, i
     CK(cudaStreamWaitEvent((cudaStream_t)stream, mech->sched_ev[slot], 0));     // the pair's previous launch is still in flight
   (void)cudaGetLastError();                                                       // cudaErrorNotReady is not an error
   unsigned long long* sched = mech->sched + 2 * slot;
+  // dense by expansion (one state per CTA, state-major layout): the launch uses the handle's scratch; it is ordered
+  // behind the previous launch that did (another stream could still be running it)
+  const bool expand = !mech->pair_only && mech->has_xplan && ofmt >= OUT_DENSE_C && cfg.S == 1 && tile == 1;
+  if (expand && mech->scratch_used) CK(cudaStreamWaitEvent((cudaStream_t)stream, mech->scratch_ev, 0));
   const int e = mech->pair_only
                     ? launch_jacobian2(mech->dj, mech->jout[ofmt], cfg, mech->n_sm, mode, n_states, tile, d_phi, d_param, d_out, sched, stream)
-                    : launch_jacobian(mech->dm, mech->plan[ofmt], cfg, mode, n_states, ld, tile, d_phi, d_param, d_out, sched, stream);
+                    : launch_jacobian(mech->dm, expand ? mech->xplan[ofmt - OUT_DENSE_C] : mech->plan[ofmt], cfg, mode, n_states, ld, tile, d_phi,
+                                      d_param, d_out, sched, stream);
   if (e) return cuda_fail((cudaError_t)e, "jacobian kernel launch");
+  if (expand) { CK(cudaEventRecord(mech->scratch_ev, (cudaStream_t)stream)); mech->scratch_used = true; }
   CK(cudaEventRecord(mech->sched_ev[slot], (cudaStream_t)stream));
   mech->sched_used[slot] = true;
   return PYJAC_OK;

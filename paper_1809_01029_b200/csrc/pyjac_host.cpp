@@ -577,6 +577,21 @@ int build_host_tables(const pyjac_mech_desc* d, bool approx, HostTables& h, std:
         const size_t e = p == 0 ? (size_t)r * nvar + h.csr_idx[q] : (size_t)h.csr_idx[q] * nvar + r;
         h.nzmask[p][e >> 5] |= 1u << (e & 31);
       }
+    std::vector<int32_t> rank(h.nzmask[p].size() + 1, 0);       // set bits before every word: the CSR / CSC position
+    for (size_t w = 1; w <= h.nzmask[p].size(); ++w) rank[w] = rank[w - 1] + __builtin_popcount(h.nzmask[p][w - 1]);
+    const int64_t n2 = (int64_t)h.nvar * h.nvar;
+    auto present = [&](int64_t e) { return e >= 0 && e < n2 && ((h.nzmask[p][e >> 5] >> (e & 31)) & 1u); };
+    auto rank_of = [&](int64_t e) { return rank[e >> 5] + __builtin_popcount(h.nzmask[p][e >> 5] & ((1u << (e & 31)) - 1u)); };
+    for (int sh = 0; sh < 2; ++sh) {
+      const int64_t n_pairs = (n2 + sh + 1) / 2;
+      std::vector<int32_t>& x = h.xpair[2 * p + sh];
+      x.assign((size_t)((n_pairs + XPAIR_PAD - 1) / XPAIR_PAD * XPAIR_PAD), 0);
+      for (int64_t q = 0; q < n_pairs; ++q) {
+        const int64_t e1 = 2 * q - sh, e2 = e1 + 1;
+        const bool b1 = present(e1), b2 = present(e2);
+        if (b1 || b2) x[(size_t)q] = (int32_t)(rank_of(b1 ? e1 : e2) << 2) | (b1 ? 1 : 0) | (b2 ? 2 : 0);
+      }
+    }
   }
   return PYJAC_OK;
 }

@@ -29,6 +29,7 @@ constexpr int INFO_OF_SHIFT = 16;    // bits 16-19: forward order  sum nu'
 constexpr int INFO_OR_SHIFT = 20;    // bits 20-23: reverse order  sum nu''
 constexpr uint32_t SIGN_BIT = 0x80000000u;
 constexpr int N_ZERO_SLOTS = 16;             // always-zero slots after the real ones: ELL padding, one per 8-byte bank
+constexpr int XPAIR_PAD = 32 * 16;      // dense by expansion: pairs per batch (32 lanes x XIT warp iterations)
 constexpr int SEG_LEN = 24;           // gather lists longer than this are split into segments
 
 enum OutFmt { OUT_CSR = 0, OUT_CSC = 1, OUT_DENSE_C = 2, OUT_DENSE_F = 3 };
@@ -89,6 +90,10 @@ struct HostTables {
   int n_part_jac = 0, n_part_src = 0;        // doubles of partial-sum scratch per state
   int32_t d_pos[4][4];                       // (T,T) (T,E) (E,T) (E,E)
   std::vector<uint32_t> nzmask[2];           // dense bitmaps, bit e set iff dense element e ('C' / 'F' order) is in the pattern
+  // dense by expansion: per 16-byte-aligned pair of dense elements (pair p = elements 2p - sh, 2p - sh + 1; sh = 0 / 1:
+  // the matrix starts on an even / odd double) rank << 2 | present bits -- rank = CSR ('C') / CSC ('F') position of the
+  // pair's first present element.  Index [2 * layout + sh]; padded with zeros to a multiple of XPAIR_PAD entries.
+  std::vector<int32_t> xpair[4];
   int nslots = 0;                            // total Jacobian slots
   int max_eff = 0;
   // raw gather lists in the slot numbering above, consumed by build_jac_tables (pyjac_plan.cpp)
@@ -196,6 +201,9 @@ struct DevPlan {
   const int32_t *j_pos, *c_pos, *jc_pos, *cc_pos;
   int32_t d_pos[4];
   const uint32_t* nzmask;    // dense only (else nullptr)
+  // dense by expansion (jacobian_kernel MODE 2): set bits before every bitmap word; n_sm x 2 x nnz doubles of scratch
+  const int32_t* xpair[2];   // dense by expansion: the pair tables of this layout for sh = 0 / 1 (HostTables::xpair)
+  double* scratch;
 };
 
 // device view of JacTables (+ the type-specific parameter tables it shares with DevMech)

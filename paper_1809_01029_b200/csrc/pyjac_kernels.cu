@@ -30,6 +30,7 @@ namespace {
 #define PYJAC_UNC 4         // entry-loop unroll of the T/E-row gather
 #define PYJAC_UN1 8         // narrow gather at one state per CTA: segments per thread
 #define PYJAC_UQ 1          // source-term gather: segments per thread
+constexpr int XIT = XPAIR_PAD / 32;   // dense by expansion: warp iterations (of 32 element pairs) per batch
 constexpr int ZERO_WARPS = 1;   // warps that stream the zero fill of large dense matrices
 constexpr int NT = 512;            // threads per CTA
 constexpr int NW = NT / 32;
@@ -232,9 +233,14 @@ struct NoSide { __device__ __forceinline__ bool operator()(const int*, int) cons
 // previous tile there: its second pass needs a barrier after the gathers, and this one serves).
 struct NoMid { __device__ __forceinline__ void operator()() const {} };
 
-template <int S, bool JAC, class PhiF, class SideF, class MidF>
+// step(): called by every warp before each reaction chunk and each gather unit (the dense-by-expansion kernel streams
+// one batch of the PREVIOUS tile's dense matrix out there: different warps are in different kinds of work at any time,
+// so the output stream runs alongside the arithmetic instead of in a phase of its own).
+struct NoStep { __device__ __forceinline__ void operator()() const {} };
+
+template <int S, bool JAC, class PhiF, class SideF, class MidF, class StepF>
 __device__ __forceinline__ void phases01(const DevMech& m, Tile<S, JAC>& t, int mode, PhiF phi_of, double par_,
-                                         int* cnt, SideF side, MidF mid) {
+                                         int* cnt, SideF side, MidF mid, StepF step) {
   const int tid = threadIdx.x;
   const int ns = m.ns, nr = m.nr, L = ns - 1;
   const int s = tid % S;                        // NT % S == 0: a thread keeps its state in every loop
@@ -338,6 +344,7 @@ __device__ __forceinline__ void phases01(const DevMech& m, Tile<S, JAC>& t, int 
   const int n_rx_chunks = (nr * S + 31) / 32;
   if (!side(cnt + CNT_RX, n_rx_chunks))
   for (int chunk = next_chunk(cnt + CNT_RX); chunk < n_rx_chunks; chunk = next_chunk(cnt + CNT_RX)) {
+    step();
     const int idx = chunk * 32 + (tid & 31);
     if (idx >= nr * S) continue;
     const int r = idx / S;
@@ -685,9 +692,9 @@ namespace {
 // ---------------------------------------------------------------------------------------------------
 // EW = segments per super-group (ELL_W, or ELL_W_NARROW for the narrow tail of the species-row plan); metas points at
 // the first of n_groups super-groups, whose first segment has processing slot slot_base.
-template <int S, int STRIDE, int NACC, int U, int UNROLL, int EW, class P, class AccF, class PosF, class StoreF, class SideF>
+template <int S, int STRIDE, int NACC, int U, int UNROLL, int EW, class P, class AccF, class PosF, class StoreF, class SideF, class StepF>
 __device__ __forceinline__ void gather(const int32_t* __restrict__ ell_ent, const int2* __restrict__ metas, int n_groups,
-                                       int slot_base, int* counter, AccF acc, PosF pos_of, StoreF store, SideF side) {
+                                       int slot_base, int* counter, AccF acc, PosF pos_of, StoreF store, SideF side, StepF step) {
   const int lane = threadIdx.x & 31, sub = lane / S;
   constexpr int IPW = 32 / S;                 // segments of one warp per "u"
   // a unit = U * IPW segments of one super-group; a thread owns U segments (U independent loads per step)
@@ -700,6 +707,7 @@ __device__ __forceinline__ void gather(const int32_t* __restrict__ ell_ent, cons
   if (side(counter, n_work)) return;
   int unit = next_chunk(counter);
   while (unit < n_work) {
+    step();
     const int next = next_chunk(counter);
     const int2 meta = metas[unit / UPG];
     const int sg = unit / UPG;
@@ -764,7 +772,7 @@ source_kernel(const DevMech m, int mode, int64_t n_states, int64_t tile, const d
   const bool valid = s0 + s < n_states;
   const int64_t sg = min(s0 + s, n_states - 1);   // ragged tail: recompute the last valid state, never store
   const int64_t pbase = state_base(sg, tile, m.nvar), obase = pbase;
-  phases01<S, false>(m, t, mode, [&](int e) { return phi[pbase + (int64_t)e * tile]; }, param[sg], cnt, NoSide(), NoMid());
+  phases01<S, false>(m, t, mode, [&](int e) { return phi[pbase + (int64_t)e * tile]; }, param[sg], cnt, NoSide(), NoMid(), NoStep());
   const double V = t.sc[SC_V * S + s];
   // a7: omega_k = sum_i nu_ki q_i (Eq. 4), dn_k/dt = V omega_k (Eq. 3)
   const double* __restrict__ P = t.P;
@@ -777,7 +785,7 @@ source_kernel(const DevMech m, int mode, int64_t n_states, int64_t tile, const d
       [&](int, int k, const double (&v)[1]) {
         if (k >= 0) { if (valid) st_out(out + obase + (int64_t)(2 + k) * tile, V * v[0]); }
         else if (k <= -2) t.part[(-2 - k) * S + s] = v[0];
-      }, NoSide());
+      }, NoSide(), NoStep());
   if (m.qplan.n_comb) {
     __syncthreads();
     combine<S, 1>(m.qplan, t.part, [&](int c, const double (&v)[1]) {
@@ -823,7 +831,7 @@ fd_kernel(const DevMech m, int mode, int ofmt, double rel, double ab, int64_t ti
     double x = 0.0, xp = 0.0;
     if (c >= 0) { x = phi[pbase + (int64_t)c * tile]; xp = x + fma(rel, fabs(x), ab); }
     phases01<S, false>(m, t, mode, [&](int e) { const double v = phi[pbase + (int64_t)e * tile]; return e == c ? xp : v; },
-                       par, cnt, NoSide(), NoMid());
+                       par, cnt, NoSide(), NoMid(), NoStep());
     const double V = t.sc[SC_V * S + s];
     const double* __restrict__ P = t.P;
     gather<S, 1, 1, PYJAC_UQ, 4, ELL_W, int>(m.qplan.ell_ent, t.meta, m.qplan.n_sg, 0, cnt + CNT_Q,
@@ -835,7 +843,7 @@ fd_kernel(const DevMech m, int mode, int ofmt, double rel, double ab, int64_t ti
         [&](int, int k, const double (&v)[1]) {
           if (k >= 0) fc[(2 + k) * S + s] = V * v[0];
           else if (k <= -2) t.part[(-2 - k) * S + s] = v[0];
-        }, NoSide());
+        }, NoSide(), NoStep());
     if (m.qplan.n_comb) {
       __syncthreads();
       combine<S, 1>(m.qplan, t.part, [&](int q, const double (&v)[1]) { fc[(2 + __ldg(m.qc_item + q)) * S + s] = V * v[0]; });
@@ -876,10 +884,22 @@ fd_kernel(const DevMech m, int mode, int ofmt, double rel, double ab, int64_t ti
 // ---------------------------------------------------------------------------------------------------
 // Jacobian (sparse CSR / CSC value order or dense 'C' / 'F'), Eq. 9
 // ---------------------------------------------------------------------------------------------------
-template <int S, bool DENSE>
+// MODE 0: sparse values.  MODE 1: dense, nonzeros stored at their dense positions + bitmap-driven zero fill.
+// MODE 2 (one state per CTA, state-major layout, large matrices): dense by EXPANSION -- the gathers write the sparse
+// values (CSR order for 'C', CSC order for 'F': the order of the set bits of the dense bitmap) into the CTA's scratch
+// buffer (L2-resident), and after the tile's gathers every warp streams slices of the dense matrix out: element e =
+// bit set ? scratch[rank(e)] : 0, written with 16-byte coalesced streaming stores.
+// Every 32-byte sector of the output is written exactly once and completely (MODE 1 writes the zeros and the nonzeros
+// of a sector at different times and pays a DRAM read-modify-write for most of them: 1.46 x the algorithmic traffic).
+template <int S, int MODE>
 __global__ void __launch_bounds__(NT, 1)
 jacobian_kernel(const DevMech m, const DevPlan pl, int mode, int64_t n_states, int64_t tile, const double* __restrict__ phi,
                 const double* __restrict__ param, double* __restrict__ out, unsigned long long* __restrict__ sched) {
+  constexpr bool DENSE = MODE == 1, EXPAND = MODE == 2;
+  static_assert(!EXPAND || S == 1, "dense by expansion: one state per CTA");
+  // values of the gathers: streaming stores to the caller's array, but write-back stores to the expansion scratch
+  // (it is read again a tile later and must stay in L2)
+  auto st_g = [](double* q, double v) { if constexpr (MODE == 2) *q = v; else st_out(q, v); };
   extern __shared__ __align__(16) double smem[];
   Tile<S, true> t(smem, m.ns, m.nr, m.nslots, m.n_part_jac, m.cplan.n_sg + pl.jplan.n_sg);
   // PERSISTENT CTA: the grid is one CTA per SM (x occupancy); a CTA starts with tile blockIdx.x and takes further
@@ -913,6 +933,7 @@ jacobian_kernel(const DevMech m, const DevPlan pl, int mode, int64_t n_states, i
   __shared__ long long next_tile;
   int parity = 0;
   // context of the previous tile for its deferred second pass
+  double* prev_gout = out; int64_t prev_tl = 0;
   bool prev_valid = false; int64_t prev_obase = 0; double prev_fT = 0.0, prev_iDV = 0.0, prev_cS = 0.0, prev_cT = 0.0, prev_cL = 0.0;
   const double* prev_ck = t.ck;
   const int nJ2 = pl.jplan.n_comb * S, nC2 = m.cplan.n_comb * S;
@@ -927,7 +948,7 @@ jacobian_kernel(const DevMech m, const DevPlan pl, int mode, int64_t n_states, i
         const int pos = __ldg(pl.jc_pos + c);
         double v = 0.0;
         for (int q = 0; q < n; ++q) v += part[(first + q) * S + s];
-        if (prev_valid) st_out(out + prev_obase + (int64_t)pos * tile, v);
+        if (prev_valid) st_g(prev_gout + prev_obase + (int64_t)pos * tile, v);
       } else {
         const int c = (idx - nJ2) / S;
         const int first = m.cplan.part_base + 2 * __ldg(m.cplan.comb_first + c), n = __ldg(m.cplan.comb_nseg + c);
@@ -937,9 +958,52 @@ jacobian_kernel(const DevMech m, const DevPlan pl, int mode, int64_t n_states, i
         for (int q = 0; q < n; ++q) { v0 += part[(first + 2 * q) * S + s]; v1 += part[(first + 2 * q + 1) * S + s]; }
         if (prev_valid) {
           const double JT = -(v0 + prev_fT * (prev_ck[j * S + s] - prev_cL)) * prev_iDV;
-          st_out(out + prev_obase + (int64_t)pos.x * tile, JT);
-          st_out(out + prev_obase + (int64_t)pos.y * tile, prev_cS * v1 + prev_cT * JT);
+          st_g(prev_gout + prev_obase + (int64_t)pos.x * tile, JT);
+          st_g(prev_gout + prev_obase + (int64_t)pos.y * tile, prev_cS * v1 + prev_cT * JT);
         }
+      }
+    }
+  };
+  const int nn2 = m.nvar * m.nvar;
+  // dense by expansion: the PREVIOUS tile's dense matrix from its sparse values in the scratch buffer, in batches of XIT
+  // warp iterations taken from the work counter CNT_Z by every warp: one before each reaction chunk / gather unit of
+  // the current tile (step), the rest after the tile's gathers.  The matrix's elements are taken in PAIRS that are
+  // 16-byte aligned in the output (pair p = elements 2p - sh, 2p - sh + 1; sh = 1 if the matrix starts on an odd
+  // double); a warp iteration covers 32 consecutive pairs (512 contiguous bytes): a lane loads its pair's table word
+  // (coalesced; rank << 2 | present bits), the values of the present elements from the scratch (L2) and writes one
+  // 16-byte streaming store.  No staging, no intra-warp synchronisation; every 32-byte sector is written once.
+  const int n_xb = EXPAND ? ((nn2 + 2) / 2 + XPAIR_PAD - 1) / XPAIR_PAD : 0;
+  const double* x_scr = nullptr; double* x_dst = nullptr;
+  bool x_more = false;
+  auto expand_batch = [&](int b) {
+    const int sh = (int)((reinterpret_cast<uintptr_t>(x_dst) >> 3) & 1);
+    const int p0 = b * XPAIR_PAD + (tid & 31);
+    const int32_t* __restrict__ xp = pl.xpair[sh] + p0;
+    int32_t c[XIT];
+#pragma unroll
+    for (int q = 0; q < XIT; ++q) c[q] = __ldg(xp + q * 32);        // (the table is padded: no bound)
+    double va[XIT], vb[XIT];
+#pragma unroll
+    for (int q = 0; q < XIT; ++q) {
+      const double* __restrict__ v = x_scr + (c[q] >> 2);
+      va[q] = 0.0; vb[q] = 0.0;
+      if (c[q] & 1) va[q] = __ldcg(v);
+      if (c[q] & 2) vb[q] = __ldcg(v + (c[q] & 1));
+    }
+    double* __restrict__ d = x_dst + 2 * p0 - sh;
+#pragma unroll
+    for (int q = 0; q < XIT; ++q) {
+      const int e1 = 2 * (p0 + q * 32) - sh;
+      if (e1 >= 0 && e1 + 1 < nn2) __stcs(reinterpret_cast<double2*>(d + q * 64), make_double2(va[q], vb[q]));
+      else if (e1 < 0) st_out(x_dst, vb[q]);                      // the odd head element
+      else if (e1 < nn2) st_out(x_dst + e1, va[q]);               // the odd tail element
+    }
+  };
+  auto step = [&]() {
+    if constexpr (EXPAND) {
+      if (x_more) {
+        const int b = next_chunk(cnt + CNT_Z);
+        if (b < n_xb) expand_batch(b); else x_more = false;
       }
     }
   };
@@ -954,7 +1018,9 @@ jacobian_kernel(const DevMech m, const DevPlan pl, int mode, int64_t n_states, i
   const bool valid_a = S == 1 || s0_a + s < n_states;   // one state per tile: every tile is a valid state
   const int64_t sg = min(s0_a + s, n_states - 1);   // ragged tail: recompute the last valid state, never store
   constexpr bool REDERIVE = !DENSE && S > 1;
-  const int64_t obase_a = REDERIVE ? 0 : state_base(sg, tile, pl.n_e);
+  const int64_t obase_a = REDERIVE || EXPAND ? 0 : state_base(sg, tile, pl.n_e);
+  // where the gathers store: the caller's array, or (dense by expansion) this CTA's scratch buffer of the tile's parity
+  double* const gout = EXPAND ? pl.scratch + ((size_t)blockIdx.x * 2 + parity) * (size_t)pl.n_e : out;
   bool valid = valid_a; int64_t obase = obase_a;
   // dense output: structural zeros, each stored once (no memset pass), in slices of 32 bitmap words (1024 elements:
   // one coalesced mask load, then 32 coalesced predicated store instructions at S = 1).  For large matrices the
@@ -980,7 +1046,9 @@ jacobian_kernel(const DevMech m, const DevPlan pl, int mode, int64_t n_states, i
   };
   const bool zero_warp = DENSE && n_zslices >= ZERO_WARP_MIN_SLICES && (tid >> 5) >= NW - ZERO_WARPS;
   auto side = [&](const int* counter, int n) -> bool {
-    if constexpr (!DENSE) {
+    if constexpr (EXPAND) {
+      return false;
+    } else if constexpr (!DENSE) {
       return false;
     } else {
       if (!zero_warp) return false;
@@ -1005,7 +1073,7 @@ jacobian_kernel(const DevMech m, const DevPlan pl, int mode, int64_t n_states, i
         [&]() {
           if (tid == 0) next_tile = (long long)gridDim.x + (long long)ticket;
           if (have_prev && nJ2 + nC2 > 0) second_pass();
-        });
+        }, step);
   }
   tl_next = next_tile;
   if (tl_next < n_tiles) fetch_state(tl_next);
@@ -1047,10 +1115,10 @@ jacobian_kernel(const DevMech m, const DevPlan pl, int mode, int64_t n_states, i
         JET = T * R_GAS * dS_dT + Pp / T * JTT + R_GAS * Ssum - Pp * fT / (T * T);
         JEE = T * R_GAS * dS_dE + Pp / T * JTE + fT / T;
       }
-      out[obase + (int64_t)pl.d_pos[0] * tile] = JTT;
-      out[obase + (int64_t)pl.d_pos[1] * tile] = JTE;
-      out[obase + (int64_t)pl.d_pos[2] * tile] = JET;
-      out[obase + (int64_t)pl.d_pos[3] * tile] = JEE;
+      gout[obase + (int64_t)pl.d_pos[0] * tile] = JTT;
+      gout[obase + (int64_t)pl.d_pos[1] * tile] = JTE;
+      gout[obase + (int64_t)pl.d_pos[2] * tile] = JET;
+      gout[obase + (int64_t)pl.d_pos[3] * tile] = JEE;
     }
   };
   corners();     // before the gathers: that warp joins the dynamically scheduled gather a little late, no serial tail
@@ -1079,14 +1147,14 @@ jacobian_kernel(const DevMech m, const DevPlan pl, int mode, int64_t n_states, i
         if (pp.x >= 0) {
           if (valid) {
             const double JT = -(v[0] + fT * (t.ck[pp.z * S + s] - cL)) * iDV;
-            st_out(out + obase + (int64_t)pp.x * tile, JT);
-            st_out(out + obase + (int64_t)pp.y * tile, cS * v[1] + cT * JT);
+            st_g(gout + obase + (int64_t)pp.x * tile, JT);
+            st_g(gout + obase + (int64_t)pp.y * tile, cS * v[1] + cT * JT);
           }
         } else if (pp.x <= -2) {
           const int pi = m.cplan.part_base + 2 * (-2 - pp.x);
           t.part[pi * S + s] = v[0]; t.part[(pi + 1) * S + s] = v[1];
         }
-      }, side);
+      }, side, step);
   // a9: species rows.  Block entries J[k][j] = sum_i nu_ki (Ghat^j_i - Ghat^Ns_i); T and E columns
   // J[k][T] = sum_i nu_ki slotT_i, J[k][E] = sum_i nu_ki slotE_i.  Every nonzero is finished in a register and
   // stored once.
@@ -1095,30 +1163,42 @@ jacobian_kernel(const DevMech m, const DevPlan pl, int mode, int64_t n_states, i
       const uint32_t ent = (uint32_t)__ldg(e);
       v[0] += apply_sign(P[(ent & ~SIGN_BIT) * S + s], ent);
     };
-    double* __restrict__ out_s = out + obase;
+    double* __restrict__ out_s = gout + obase;
     auto posJ = [&](int slot) { const int p = __ldg(pl.j_pos + slot); return valid || p < 0 ? p : -1; };   // ragged tail: store nothing
     auto storeJ = [&](int, int pos, const double (&v)[1]) {
-      if (pos >= 0) st_out(out_s + (int64_t)pos * tile, v[0]);
+      if (pos >= 0) st_g(out_s + (int64_t)pos * tile, v[0]);
       else if (pos <= -2) t.part[(-2 - pos) * S + s] = v[0];
     };
     auto storeN = [&](int, int pos, const double (&v)[1]) {      // narrow tail: whole lists only (see build_gather)
-      if (pos >= 0) st_out(out_s + (int64_t)pos * tile, v[0]);
+      if (pos >= 0) st_g(out_s + (int64_t)pos * tile, v[0]);
     };
     const int2* metaJ = t.meta + m.cplan.n_sg;
     const int n_wide = pl.jplan.n_wide;
-    gather<S, 1, 1, PYJAC_UJ, PYJAC_UNJ, ELL_W, int>(pl.jplan.ell_ent, metaJ, n_wide, 0, cnt + CNT_J, accJ, posJ, storeJ, side);
+    gather<S, 1, 1, PYJAC_UJ, PYJAC_UNJ, ELL_W, int>(pl.jplan.ell_ent, metaJ, n_wide, 0, cnt + CNT_J, accJ, posJ, storeJ, side, step);
     // the narrow tail (lists of one or two entries: most nonzeros of a sparse mechanism): 16 segments per thread
     gather<S, 1, 1, (S == 1 && !DENSE ? PYJAC_UN1 : ELL_W_NARROW / 32), 1, ELL_W_NARROW, int>(pl.jplan.ell_ent, metaJ + n_wide, pl.jplan.n_sg - n_wide, n_wide * ELL_W,
-                                              cnt + CNT_J2, accJ, posJ, storeN, side);
+                                              cnt + CNT_J2, accJ, posJ, storeN, side, step);
   }
   if (DENSE)                                      // whatever is left of the zero fill
     for (int z = next_chunk(cnt + CNT_Z); z < n_zslices; z = next_chunk(cnt + CNT_Z)) zero_slice(z);
+  prev_gout = gout; prev_tl = tl;
   have_prev = true; prev_valid = valid; prev_obase = obase; prev_fT = fT; prev_iDV = iDV; prev_cS = cS; prev_cT = cT; prev_cL = cL;
   prev_ck = t.ck;
+  if constexpr (EXPAND) {
+    while (x_more) step();                       // what is left of the previous tile's dense matrix
+    x_scr = gout; x_dst = out + tl * (int64_t)nn2;
+    x_more = true;                               // (the counter is reset in the next tile's phase 0, behind a barrier)
+  }
   }  // tiles of this CTA
   if (have_prev && nJ2 + nC2 > 0) {            // the last tile's second pass
     __syncthreads();
     second_pass();
+  }
+  if constexpr (EXPAND) {
+    if (have_prev) {                             // the last tile's dense matrix
+      __syncthreads();
+      for (int b = tid >> 5; b < n_xb; b += NW) expand_batch(b);
+    }
   }
   if (tid == 0 && atomicAdd(sched + 1, 1ull) == (unsigned long long)gridDim.x - 1) { sched[0] = 0; sched[1] = 0; }
 }
@@ -1137,13 +1217,21 @@ template <int S> int launch_jac_S(const DevMech& m, const DevPlan& p, const Laun
   int dev = 0, n_sm = 0, occ = 0;
   cudaError_t e = cudaGetDevice(&dev);
   if (e == cudaSuccess) e = cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
+  const bool expand = p.scratch != nullptr;
+  if constexpr (S == 1) {
+    if (expand) {                                 // dense by expansion: one CTA per SM, two scratch buffers per CTA
+      if (e != cudaSuccess) return (int)e;
+      jacobian_kernel<1, 2><<<(unsigned)std::min<int64_t>(tiles, n_sm), NT, cfg.smem, st>>>(m, p, mode, n, tile, phi, param, out, sched);
+      return (int)cudaGetLastError();
+    }
+  }
   if (e == cudaSuccess)
-    e = p.nzmask != nullptr ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, jacobian_kernel<S, true>, NT, cfg.smem)
-                            : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, jacobian_kernel<S, false>, NT, cfg.smem);
+    e = p.nzmask != nullptr ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, jacobian_kernel<S, 1>, NT, cfg.smem)
+                            : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, jacobian_kernel<S, 0>, NT, cfg.smem);
   if (e != cudaSuccess) return (int)e;
   const int64_t blocks = std::min<int64_t>(tiles, (int64_t)n_sm * (occ > 0 ? occ : 1));
-  if (p.nzmask != nullptr) jacobian_kernel<S, true><<<(unsigned)blocks, NT, cfg.smem, st>>>(m, p, mode, n, tile, phi, param, out, sched);
-  else jacobian_kernel<S, false><<<(unsigned)blocks, NT, cfg.smem, st>>>(m, p, mode, n, tile, phi, param, out, sched);
+  if (p.nzmask != nullptr) jacobian_kernel<S, 1><<<(unsigned)blocks, NT, cfg.smem, st>>>(m, p, mode, n, tile, phi, param, out, sched);
+  else jacobian_kernel<S, 0><<<(unsigned)blocks, NT, cfg.smem, st>>>(m, p, mode, n, tile, phi, param, out, sched);
   return (int)cudaGetLastError();
 }
 
@@ -1227,9 +1315,13 @@ template <int S> static int set_attr_S() {
   if (e != cudaSuccess) return (int)e;
   e = cudaFuncSetAttribute(fd_kernel<S>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_LIMIT);
   if (e != cudaSuccess) return (int)e;
-  e = cudaFuncSetAttribute(jacobian_kernel<S, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_LIMIT);
+  e = cudaFuncSetAttribute(jacobian_kernel<S, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_LIMIT);
   if (e != cudaSuccess) return (int)e;
-  return (int)cudaFuncSetAttribute(jacobian_kernel<S, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_LIMIT);
+  if constexpr (S == 1) {
+    e = cudaFuncSetAttribute(jacobian_kernel<1, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_LIMIT);
+    if (e != cudaSuccess) return (int)e;
+  }
+  return (int)cudaFuncSetAttribute(jacobian_kernel<S, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_LIMIT);
 }
 
 int set_kernel_attributes() {

@@ -326,3 +326,59 @@ def test_many_inert_species(pj):
         got = run_gpu(pj, M, pj.WHAT_SPARSE, mode, mg.CSR, states, 40, 1)
         assert np.isfinite(got).all()
         assert not jac_ok_dense(dense_from_sparse(got, ptr, idx, mg.CSR, M.nvar), Jr).any()
+
+
+# ---- dense by expansion (one state per CTA, state-major layout, n_var^2 >= 32768): more states than SMs, so that a CTA
+# works through several tiles (the expansion of tile k runs inside tile k + 1; both scratch buffers; the last tile's
+# expansion after the loop), both orders, odd and even alignment of a state's matrix (n_var^2 is odd for C4) ----
+@pytest.mark.parametrize("order", ["C", "F"])
+@pytest.mark.parametrize("mode", [mg.CONP, mg.CONV])
+def test_dense_by_expansion_many_tiles(pj, order, mode):
+    m, M, o, st = setup(pj, "c4")
+    n = 3 * 148 + 5
+    states = st(n)
+    fmt = mg.CSR if order == "C" else mg.CSC
+    sparse = run_gpu(pj, M, pj.WHAT_SPARSE, mode, fmt, states, n, 1)          # (its own parity: test_jacobian_sparse)
+    dense = run_gpu(pj, M, pj.WHAT_DENSE, mode, order, states, n, 1)
+    assert np.isfinite(dense).all()
+    ptr, idx = M.sparsity(fmt)
+    # every state, every element: the nonzeros are the sparse path's values (same arithmetic; the sums of a tile depend
+    # on which warp took which chunk, so two launches agree to rounding, not to the bit), everything else is an exact zero
+    expect = dense_from_sparse(sparse, ptr, idx, fmt, M.nvar)                 # [n, row, col]
+    got = dense.reshape(n, M.nvar, M.nvar)
+    if order == "F":
+        got = got.transpose(0, 2, 1)
+    pat = dense_from_sparse(np.ones((1, M.nnz)), ptr, idx, fmt, M.nvar)[0] != 0
+    assert np.all(got[:, ~pat] == 0.0)
+    scale = np.abs(expect).reshape(n, -1).max(axis=1)[:, None, None]
+    assert np.all(np.abs(got - expect) <= 1e-9 * np.abs(expect) + 1e-13 * scale)
+    # and against the oracle on a sample that has neighbours of both alignments, the first and the last state
+    pick = np.array([0, 1, 2, 147, 148, 149, 295, 296, 297, n - 2, n - 1])
+    Jr = o.jacobian_dense(mode, *o.pack(_sub(states, pick), mode))
+    bad = jac_ok_dense(got[pick], Jr)
+    assert not bad.any(), (np.argwhere(bad)[:5], got[pick][bad][:5], Jr[bad][:5])
+
+
+# two dense-by-expansion launches of one handle on two streams share the handle's scratch buffers: the library orders the
+# second behind the first (an event), so both results are those of a launch alone
+def test_dense_by_expansion_two_streams(pj):
+    m, M, o, st = setup(pj, "c4")
+    n = 200
+    sa, sb = st(n), _sub(st(2 * n), np.arange(n, 2 * n))
+    ref_a = run_gpu(pj, M, pj.WHAT_DENSE, mg.CONP, "C", sa, n, 1)
+    ref_b = run_gpu(pj, M, pj.WHAT_DENSE, mg.CONP, "C", sb, n, 1)
+    n_e = M.nvar * M.nvar
+    bufs = []
+    for s_ in (sa, sb):
+        phi, par = pack_phi(s_, mg.CONP, n, 1)
+        bufs.append((torch.from_numpy(phi).cuda(), torch.from_numpy(par).cuda(),
+                     torch.full((n_e * n,), float("nan"), dtype=torch.float64, device="cuda")))
+    torch.cuda.synchronize()
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    for (phi, par, out), s_ in zip(bufs, (s1, s2)):
+        pj.pyjac_jacobian_dense(M.h, mg.CONP, "C", n, n, 1, phi.data_ptr(), par.data_ptr(), out.data_ptr(), s_.cuda_stream)
+    torch.cuda.synchronize()
+    for (_, _, out), ref in zip(bufs, (ref_a, ref_b)):
+        got = out.cpu().numpy().reshape(n, n_e)
+        assert np.array_equal(got == 0.0, ref == 0.0)
+        assert np.all(np.abs(got - ref) <= 1e-9 * np.abs(ref) + 1e-13 * np.abs(ref).max(axis=1, keepdims=True))
