@@ -201,7 +201,7 @@ struct DevPlan {
   const int32_t *j_pos, *c_pos, *jc_pos, *cc_pos;
   int32_t d_pos[4];
   const uint32_t* nzmask;    // dense only (else nullptr)
-  // dense by expansion (jacobian_kernel MODE 2): set bits before every bitmap word; n_sm x 2 x nnz doubles of scratch
+  // dense by expansion (jacobian_kernel MODE 2, else nullptr): pair tables and n_sm x 2 x nnz doubles of scratch
   const int32_t* xpair[2];   // dense by expansion: the pair tables of this layout for sh = 0 / 1 (HostTables::xpair)
   double* scratch;
 };

@@ -887,8 +887,8 @@ fd_kernel(const DevMech m, int mode, int ofmt, double rel, double ab, int64_t ti
 // MODE 0: sparse values.  MODE 1: dense, nonzeros stored at their dense positions + bitmap-driven zero fill.
 // MODE 2 (one state per CTA, state-major layout, large matrices): dense by EXPANSION -- the gathers write the sparse
 // values (CSR order for 'C', CSC order for 'F': the order of the set bits of the dense bitmap) into the CTA's scratch
-// buffer (L2-resident), and after the tile's gathers every warp streams slices of the dense matrix out: element e =
-// bit set ? scratch[rank(e)] : 0, written with 16-byte coalesced streaming stores.
+// buffer of the tile's parity (L2-resident), and the dense matrix is streamed out while the NEXT tile is computed:
+// element e = bit set ? scratch[rank(e)] : 0, in 16-byte pairs with coalesced streaming stores (expand_batch below).
 // Every 32-byte sector of the output is written exactly once and completely (MODE 1 writes the zeros and the nonzeros
 // of a sector at different times and pays a DRAM read-modify-write for most of them: 1.46 x the algorithmic traffic).
 template <int S, int MODE>
@@ -933,7 +933,7 @@ jacobian_kernel(const DevMech m, const DevPlan pl, int mode, int64_t n_states, i
   __shared__ long long next_tile;
   int parity = 0;
   // context of the previous tile for its deferred second pass
-  double* prev_gout = out; int64_t prev_tl = 0;
+  double* prev_gout = out;
   bool prev_valid = false; int64_t prev_obase = 0; double prev_fT = 0.0, prev_iDV = 0.0, prev_cS = 0.0, prev_cT = 0.0, prev_cL = 0.0;
   const double* prev_ck = t.ck;
   const int nJ2 = pl.jplan.n_comb * S, nC2 = m.cplan.n_comb * S;
@@ -1181,7 +1181,7 @@ jacobian_kernel(const DevMech m, const DevPlan pl, int mode, int64_t n_states, i
   }
   if (DENSE)                                      // whatever is left of the zero fill
     for (int z = next_chunk(cnt + CNT_Z); z < n_zslices; z = next_chunk(cnt + CNT_Z)) zero_slice(z);
-  prev_gout = gout; prev_tl = tl;
+  prev_gout = gout;
   have_prev = true; prev_valid = valid; prev_obase = obase; prev_fT = fT; prev_iDV = iDV; prev_cS = cS; prev_cT = cT; prev_cL = cL;
   prev_ck = t.ck;
   if constexpr (EXPAND) {
