@@ -219,6 +219,10 @@ int pyjac_mech_create_ex(const pyjac_mech_desc* desc, int cuda_device, uint32_t 
     UP(slot_base) UP(rev_par) UP(fall) UP(plog_ptr) UP(plog_ent) UP(plog_P) UP(plog_lnP) UP(plog_lnA) UP(plog_b) UP(plog_Ta)
     UP(cheb_meta) UP(cheb_lim) UP(cheb_coef)
 #undef UP
+    for (int ls = 0; ls < 6; ++ls) {
+      if (int r_ = m->upload(h.rxc[ls], &d.rxc[ls])) return r_;
+      d.n_rxc[ls] = (int)h.rxc[ls].size() / 2;
+    }
     if (int r_ = m->upload_plan(h.cplan, h.jplan.n_part, &d.cplan)) return r_;      // C partials follow the J partials
     if (int r_ = m->upload_plan(h.qplan, 0, &d.qplan)) return r_;
     if (int r_ = m->upload(h.q_target, &d.q_target)) return r_;

@@ -318,6 +318,20 @@ int build_host_tables(const pyjac_mech_desc* d, bool approx, HostTables& h, std:
     }
   }
 
+  // ---- reaction chunks of phase 1: a new chunk wherever the cost group changes ----------------------------------
+  for (int ls = 0; ls < 6; ++ls) {
+    static const int rank[7] = {0, 1, 2, 5, 4, 3, 6};
+    auto group = [&](int r) { const int i = h.perm[r]; return is_fast(i) ? 100 : rank[d->type[i]]; };
+    const int cap = 32 >> ls;
+    h.rxc[ls].clear();
+    for (int r = 0; r < nr;) {
+      int e = r + 1;
+      while (e < nr && e - r < cap && group(e) == group(r)) ++e;
+      h.rxc[ls].push_back(r); h.rxc[ls].push_back(e);
+      r = e;
+    }
+  }
+
   h.lnA.resize(nr); h.beta.resize(nr); h.Ta.resize(nr); h.dn.resize(nr);
   h.info.resize(nr); h.aux.assign(nr, -1); h.sp.assign((size_t)nr * 8, (uint32_t)ns);
   h.eff_ptr.assign(1, 0); h.slot_base.assign(1, 0);

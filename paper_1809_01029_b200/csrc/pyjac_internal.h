@@ -56,6 +56,10 @@ struct GatherPlan {
 struct HostTables {
   int ns = 0, nr = 0, nvar = 0;
   std::vector<int32_t> perm;                 // sorted index -> original reaction index
+  // reaction chunks of phase 1 for S = 1, 2, 4, .. 32 states per CTA (index log2 S): chunk c = sorted reactions
+  // [rxc[2c], rxc[2c+1]), at most 32 / S of them, never two cost groups (reaction type / fast path) in one chunk: a warp
+  // that mixes two types runs both code paths one after the other, and the longest chunk bounds the phase
+  std::vector<int32_t> rxc[6];
   // species
   std::vector<double> nasa;                  // [15*ns] coefficient-major: tmid, lo[7], hi[7]
   std::vector<double> wr;                    // [ns] W_k / W_Ns
@@ -184,6 +188,8 @@ struct DevMech {
   const int32_t *eff_ptr, *eff_sp;
   const double* eff_d;
   const int32_t* slot_base;
+  const int32_t* rxc[6];     // reaction chunks (first, end) of phase 1 per log2 S, n_rxc[] of them
+  int n_rxc[6];
   const double* rev_par;
   const double* fall;
   const int32_t *plog_ptr, *plog_ent;

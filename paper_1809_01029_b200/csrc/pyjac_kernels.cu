@@ -341,13 +341,33 @@ __device__ __forceinline__ void phases01(const DevMech& m, Tile<S, JAC>& t, int 
   const double ln_patm_rt = t.sc[SC_LNPRT * S + s];
   const double ctot_T = Ctot * invT;
   double acc[7] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
-  const int n_rx_chunks = (nr * S + 31) / 32;
-  if (!side(cnt + CNT_RX, n_rx_chunks))
-  for (int chunk = next_chunk(cnt + CNT_RX); chunk < n_rx_chunks; chunk = next_chunk(cnt + CNT_RX)) {
+  // One state per CTA: chunks of <= 32 reactions of ONE cost group (table built at create time: HostTables::rxc), in
+  // descending cost -- a warp that mixes two reaction types runs both code paths one after the other, and with 16 warps
+  // for 70 chunks the longest chunk bounds the phase.  The next chunk's number and span are fetched a chunk ahead.
+  // Several states per CTA: chunks of 32 / S reactions are fine-grained enough, plain index arithmetic.
+  constexpr bool RXC = S == 1;
+  const int n_rx_chunks = RXC ? m.n_rxc[0] : (nr * S + 31) / 32;
+  const int2* __restrict__ rxc = reinterpret_cast<const int2*>(m.rxc[0]);
+  if (!side(cnt + CNT_RX, n_rx_chunks)) {
+  int chunk_next = next_chunk(cnt + CNT_RX);
+  int2 span_next = make_int2(0, 0);
+  if (RXC && chunk_next < n_rx_chunks) span_next = __ldg(rxc + chunk_next);
+  while (chunk_next < n_rx_chunks) {
     step();
-    const int idx = chunk * 32 + (tid & 31);
-    if (idx >= nr * S) continue;
-    const int r = idx / S;
+    const int chunk = chunk_next;
+    const int2 span = span_next;
+    chunk_next = next_chunk(cnt + CNT_RX);
+    if (RXC && chunk_next < n_rx_chunks) span_next = __ldg(rxc + chunk_next);
+    int r;
+    if (RXC) {
+      r = span.x + (tid & 31);
+      if (r >= span.y) continue;
+    } else {
+      const int i = chunk * 32 + (tid & 31);
+      if (i >= nr * S) continue;
+      r = i / S;
+    }
+    const int idx = r * S + s;
     // All per-reaction table words are requested back to back at the top of the iteration and pinned (the empty asm
     // makes every one of them live here), so the reaction costs ONE exposed L2 round trip instead of one per first
     // use further down (the compiler otherwise sinks each load to its consumer: ~3 serialized round trips).
@@ -658,6 +678,7 @@ __device__ __forceinline__ void phases01(const DevMech& m, Tile<S, JAC>& t, int 
       t.dE[idx] = dEt;
       acc[2] += dEt * slotT; acc[3] += dn * slotT; acc[4] += dEt * slotE; acc[5] += dn * slotE; acc[6] += dct * q;
     }
+  }
   }
   // reaction sums: only the per-warp partials are written here; the single barrier below also publishes the slots.
   // Consumers add the NW partials themselves (red_sum), which saves the second reduction stage and its barrier.
