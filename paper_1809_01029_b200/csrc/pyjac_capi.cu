@@ -183,7 +183,8 @@ int pyjac_mech_create_ex(const pyjac_mech_desc* desc, int cuda_device, uint32_t 
   if (rc == PYJAC_OK) rc = build_jac_tables(m->h, m->j, err);
   // the tile kernel keeps ALL per-reaction partials of a state on chip; when they do not fit (or on request) the pair
   // kernel, which cuts the reactions into blocks, evaluates the Jacobian
-  m->pair_only = (flags & PYJAC_PAIR_KERNEL) != 0 || choose_cfg(m->h, true, (int64_t)1 << 40, (int64_t)1 << 40, 148).smem > SMEM_LIMIT;
+  m->pair_only = (flags & PYJAC_PAIR_KERNEL) != 0 || choose_cfg(m->h, true, (int64_t)1 << 40, (int64_t)1 << 40, 148).smem > SMEM_LIMIT ||
+                 !m->h.jplan.packable;    // (implied by the shared-memory test: 2^15 slots are 256 KB)
   if (rc != PYJAC_OK) { delete m; return fail(rc, err); }
   if (cuda_device == -1) { m->device = -1; *out = m; return PYJAC_OK; }   // host-only handle: pattern and dims only
   int ndev = 0;

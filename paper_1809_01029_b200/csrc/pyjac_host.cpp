@@ -108,11 +108,21 @@ int validate(const pyjac_mech_desc* d, std::string& err) {
 // consecutive entries and a thread keeps several independent loads in flight.  A list that fits one segment is
 // stored straight to the output; the segments of a split list leave partial sums in shared memory which a short
 // second pass combines.  stride = ints per entry.
+// One-word entries (stride 1) are stored PACKED: two consecutive entries of a segment (steps 2q and 2q + 1) in one
+// 32-bit word, 15 bits of slot index and a sign bit each -- half the plan traffic and half the entry loads of the
+// gathers.  The slots live in shared memory as doubles (<= 227 KB), so an index always fits 15 bits for a mechanism the
+// tile kernels can run; `packable` = false otherwise (the plan is then left unpacked and must not be used by them).
 void build_gather(const std::vector<std::vector<int32_t>>& lists, int stride, int zero_slot, int narrow_len, GatherPlan& g) {
   const int SEG = SEG_LEN;
   const int n = (int)lists.size();
   g = GatherPlan();
   g.stride = stride;
+  g.packed = stride == 1;
+  if (g.packed) {
+    g.packable = zero_slot + N_ZERO_SLOTS <= 0x8000;
+    for (const auto& l : lists) for (int32_t e : l) g.packable &= ((uint32_t)e & ~SIGN_BIT) < 0x8000u;
+    g.packed = g.packable;
+  }
   struct Seg { int item, p0, len, target; };
   std::vector<Seg> segs;
   for (int i = 0; i < n; ++i) {
@@ -188,7 +198,9 @@ void build_gather(const std::vector<std::vector<int32_t>>& lists, int stride, in
     const int i0 = group_first(sg), EW = group_size(sg);
     int width = 0;                                    // the longest segment of the group
     for (int w = 0; w < EW && i0 + w < ns_; ++w) width = std::max(width, segs[i0 + w].len);
-    g.sg_meta.push_back(off); g.sg_meta.push_back(width);
+    if (g.packed) width = (width + 1) & ~1;           // whole words
+    g.sg_meta.push_back(off); g.sg_meta.push_back(g.packed ? width / 2 : width);
+    const size_t first_ent = g.ell_ent.size();
     for (int p = 0; p < width; ++p)
       for (int w0 = 0; w0 < EW; w0 += 16) {
         uint32_t used = 0;                            // banks taken by the real entries of this half-warp step
@@ -205,7 +217,17 @@ void build_gather(const std::vector<std::vector<int32_t>>& lists, int stride, in
             g.ell_ent.push_back(real ? lists[segs[i0 + w].item][(size_t)order[i0 + w][p] * stride + c] : (c == 0 ? zs : 0));
         }
       }
-    off += width * EW;
+    if (g.packed) {                                   // rows 2q and 2q + 1 -> one row of words
+      auto half = [](int32_t e) { return ((uint32_t)e & 0x7fffu) | (((uint32_t)e & SIGN_BIT) ? 0x8000u : 0u); };
+      std::vector<int32_t> rows(g.ell_ent.begin() + first_ent, g.ell_ent.end());
+      g.ell_ent.resize(first_ent);
+      for (int q = 0; q < width / 2; ++q)
+        for (int w = 0; w < EW; ++w)
+          g.ell_ent.push_back((int32_t)(half(rows[(size_t)(2 * q) * EW + w]) | (half(rows[(size_t)(2 * q + 1) * EW + w]) << 16)));
+      off += width / 2 * EW;
+    } else {
+      off += width * EW;
+    }
     for (int w = 0; w < EW; ++w) g.target.push_back(i0 + w < ns_ ? segs[i0 + w].target : -1);
   }
   g.n_padded = off;

@@ -40,10 +40,11 @@ constexpr int NARROW_LEN = 2;
 
 struct GatherPlan {
   int stride = 1;                            // ints per entry
+  bool packed = false, packable = true;      // stride 1: two 16-bit entries per word (see build_gather)
   int n_sg = 0;                              // ELL super-groups: n_wide of ELL_W segments, then n_sg - n_wide of ELL_W_NARROW
   int n_wide = 0;
-  std::vector<int32_t> sg_meta;              // [n_sg*2]: entry offset, padded segment length
-  std::vector<int32_t> ell_ent;              // entry (p, w) of group sg at (off + p*ELL_W + w) * stride
+  std::vector<int32_t> sg_meta;              // [n_sg*2]: entry offset, padded segment length (in words if packed)
+  std::vector<int32_t> ell_ent;              // entry (p, w) of group sg at (off + p*ELL_W + w) * stride; packed: word (q, w) at off + q*ELL_W + w
   // processing slot (n_sg*ELL_W) -> what the segment's sum is: item id >= 0 (the whole list of that item: store
   // the result), -1 padding, <= -2: partial sum number -2 - target of a list that was split into segments
   std::vector<int32_t> target;

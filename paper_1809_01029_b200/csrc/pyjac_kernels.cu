@@ -26,7 +26,7 @@ namespace {
 // unroll factors / segments per thread of the gathers (measured on C5 / C2 / C3, profiles/r01_sweeps.md)
 #define PYJAC_UJ 4          // species-row gather, wide groups: segments per thread
 #define PYJAC_UC 2          // T/E-row gather: segments per thread
-#define PYJAC_UNJ 4         // entry-loop unroll of the species-row gather
+#define PYJAC_UNJ 2         // entry-loop unroll of the species-row gather (in words = pairs of entries)
 #define PYJAC_UNC 4         // entry-loop unroll of the T/E-row gather
 #define PYJAC_UN1 8         // narrow gather at one state per CTA: segments per thread
 #define PYJAC_UQ 1          // source-term gather: segments per thread
@@ -800,7 +800,8 @@ source_kernel(const DevMech m, int mode, int64_t n_states, int64_t tile, const d
   gather<S, 1, 1, PYJAC_UQ, 4, ELL_W, int>(m.qplan.ell_ent, t.meta, m.qplan.n_sg, 0, cnt + CNT_Q,
       [&](const int32_t* e, double (&v)[1]) {
         const uint32_t ent = (uint32_t)__ldg(e);
-        v[0] += apply_sign(P[(ent & ~SIGN_BIT) * S + s], ent);
+        v[0] += apply_sign(P[(ent & 0x7fffu) * S + s], ent << 16);      // packed: two 16-bit entries per word
+        v[0] += apply_sign(P[((ent >> 16) & 0x7fffu) * S + s], ent);
       },
       [&](int slot) { return __ldg(m.q_target + slot); },
       [&](int, int k, const double (&v)[1]) {
@@ -858,7 +859,8 @@ fd_kernel(const DevMech m, int mode, int ofmt, double rel, double ab, int64_t ti
     gather<S, 1, 1, PYJAC_UQ, 4, ELL_W, int>(m.qplan.ell_ent, t.meta, m.qplan.n_sg, 0, cnt + CNT_Q,
         [&](const int32_t* e, double (&v)[1]) {
           const uint32_t ent = (uint32_t)__ldg(e);
-          v[0] += apply_sign(P[(ent & ~SIGN_BIT) * S + s], ent);
+          v[0] += apply_sign(P[(ent & 0x7fffu) * S + s], ent << 16);      // packed: two 16-bit entries per word
+          v[0] += apply_sign(P[((ent >> 16) & 0x7fffu) * S + s], ent);
         },
         [&](int slot) { return __ldg(m.q_target + slot); },
         [&](int, int k, const double (&v)[1]) {
@@ -1182,7 +1184,8 @@ jacobian_kernel(const DevMech m, const DevPlan pl, int mode, int64_t n_states, i
   {
     auto accJ = [&](const int32_t* e, double (&v)[1]) {
       const uint32_t ent = (uint32_t)__ldg(e);
-      v[0] += apply_sign(P[(ent & ~SIGN_BIT) * S + s], ent);
+      v[0] += apply_sign(P[(ent & 0x7fffu) * S + s], ent << 16);      // packed: two 16-bit entries per word
+      v[0] += apply_sign(P[((ent >> 16) & 0x7fffu) * S + s], ent);
     };
     double* __restrict__ out_s = gout + obase;
     auto posJ = [&](int slot) { const int p = __ldg(pl.j_pos + slot); return valid || p < 0 ? p : -1; };   // ragged tail: store nothing
