@@ -24,12 +24,12 @@ namespace pyjac {
 namespace {
 
 // unroll factors / segments per thread of the gathers (measured on C5 / C2 / C3, profiles/r01_sweeps.md)
-#define PYJAC_UJ 4          // species-row gather, wide groups: segments per thread
-#define PYJAC_UC 2          // T/E-row gather: segments per thread
-#define PYJAC_UNJ 2         // entry-loop unroll of the species-row gather (in words = pairs of entries)
-#define PYJAC_UNC 4         // entry-loop unroll of the T/E-row gather
-#define PYJAC_UN1 8         // narrow gather at one state per CTA: segments per thread
-#define PYJAC_UQ 1          // source-term gather: segments per thread
+constexpr int PYJAC_UJ = 4;    // species-row gather, wide groups: segments per thread
+constexpr int PYJAC_UC = 2;    // T/E-row gather: segments per thread
+constexpr int PYJAC_UNJ = 2;   // entry-loop unroll of the species-row gather (in words = pairs of entries)
+constexpr int PYJAC_UNC = 4;   // entry-loop unroll of the T/E-row gather
+constexpr int PYJAC_UN1 = 8;   // narrow gather at one state per CTA: segments per thread
+constexpr int PYJAC_UQ = 1;    // source-term gather: segments per thread
 constexpr int XIT = XPAIR_PAD / 32;   // dense by expansion: warp iterations (of 32 element pairs) per batch
 constexpr int ZERO_WARPS = 1;   // warps that stream the zero fill of large dense matrices
 constexpr int NT = 512;            // threads per CTA
